@@ -1,0 +1,150 @@
+"""fp64 CPU oracle of the RTS hot path -- TEST INFRASTRUCTURE.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline /
+`--impl reference` legs may import this package.  It shares no code with the CUDA
+path (`paper_2107_08145_b200/csrc`); the product path never routes through it.
+
+The arithmetic lives in `rts_oracle.c` (plain C, fp64, one OpenMP loop over the
+independent (band, ray) sweeps); this file only compiles it with gcc and marshals
+numpy arrays through ctypes.  Passages followed: see the header of rts_oracle.c.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "rts_oracle.c")
+_LIB = os.path.join(_HERE, "librts_oracle.so")
+_lib = None
+
+_D = ctypes.c_double
+_I = ctypes.c_int
+_PD = ctypes.POINTER(ctypes.c_double)
+_PF = ctypes.POINTER(ctypes.c_float)
+_PI = ctypes.POINTER(ctypes.c_int)
+
+
+def build(force: bool = False) -> str:
+    """Compile rts_oracle.c -> librts_oracle.so (gcc, -O2, OpenMP, no fast-math)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11",
+           "-o", _LIB, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.oracle_coefficients.restype = _I
+        _lib.oracle_coefficients.argtypes = [_I] * 6 + [_D] * 4 + [_PF] * 5 + [_PD] * 2
+        _lib.oracle_ray_geometry.restype = _I
+        _lib.oracle_ray_geometry.argtypes = [_D, _D, _D, _PD, _PI, _PI, _PD, _PD]
+        _lib.oracle_psi.restype = None
+        _lib.oracle_psi.argtypes = [_D, _PD, _PD, _PD]
+        _lib.oracle_sweep_ray.restype = _I
+        _lib.oracle_sweep_ray.argtypes = [_I, _I, _I, _D, _D, _D, _PD, _I, _PD, _PD, _PD, _I, _PD]
+        _lib.oracle_solve.restype = _I
+        _lib.oracle_solve.argtypes = ([_I, _I, _I, _D, _D, _D, _I, _I, _I, _D, _D, _D, _D,
+                                       _PF, _PF, _I, _I, _PD, _PD, _PF, _PF, _PF,
+                                       _PD, _PD, _PD, _I])
+        _lib.oracle_num_threads.restype = _I
+        _lib.oracle_num_threads.argtypes = []
+    return _lib
+
+
+def _pf(a):
+    return a.ctypes.data_as(_PF)
+
+
+def _pd(a):
+    return a.ctypes.data_as(_PD) if a is not None else None
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def coefficients(inp) -> Tuple[np.ndarray, np.ndarray]:
+    """O-2: (kaprho, S), each float64 [nb][nz][ny][nx]."""
+    lib = _load()
+    N = inp.ncells
+    kap = np.empty((inp.nbands,) + inp.shape, dtype=np.float64)
+    S = np.empty_like(kap)
+    rc = lib.oracle_coefficients(inp.nx, inp.ny, inp.nz, inp.nbands, inp.nT, inp.nP,
+                                 inp.logT_min, inp.logT_max, inp.logP_min, inp.logP_max,
+                                 _pf(inp.logkappa), _pf(inp.bandfrac),
+                                 _pf(inp.rho), _pf(inp.T), _pf(inp.P), _pd(kap), _pd(S))
+    if rc != 0:
+        raise RuntimeError(f"oracle_coefficients failed: {rc}")
+    return kap, S
+
+
+def ray_geometry(dx: float, dy: float, dz: float, mu) -> Tuple[int, Tuple[int, int, int], float, Tuple[float, float, float]]:
+    """O-3: (entry-face axis, signs, ds, fractions f_a)."""
+    lib = _load()
+    mu = np.ascontiguousarray(mu, dtype=np.float64)
+    axis = ctypes.c_int()
+    sg = (ctypes.c_int * 3)()
+    ds = ctypes.c_double()
+    f = (ctypes.c_double * 3)()
+    rc = lib.oracle_ray_geometry(dx, dy, dz, _pd(mu), ctypes.byref(axis), sg, ctypes.byref(ds), f)
+    if rc != 0:
+        raise ValueError("ray has mu_z == 0")
+    return axis.value, tuple(sg), ds.value, tuple(f)
+
+
+def psi(dtau: float) -> Tuple[float, float, float]:
+    """O-6: (E, psi_u, psi_p)."""
+    lib = _load()
+    E, pu, pp = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    lib.oracle_psi(float(dtau), ctypes.byref(E), ctypes.byref(pu), ctypes.byref(pp))
+    return E.value, pu.value, pp.value
+
+
+def sweep_ray(nx, ny, nz, dx, dy, dz, mu, npasses, kaprho, S,
+              inflow: Optional[np.ndarray] = None, form: int = 0) -> np.ndarray:
+    """O-4..O-6 for one band and one ray; returns I^(P) float64 [nz][ny][nx]."""
+    lib = _load()
+    kaprho = np.ascontiguousarray(kaprho, dtype=np.float64)
+    S = np.ascontiguousarray(S, dtype=np.float64)
+    mu = np.ascontiguousarray(mu, dtype=np.float64)
+    if inflow is not None:
+        inflow = np.ascontiguousarray(inflow, dtype=np.float64)
+    I = np.empty((nz, ny, nx), dtype=np.float64)
+    rc = lib.oracle_sweep_ray(nx, ny, nz, dx, dy, dz, _pd(mu), npasses,
+                              _pd(kaprho), _pd(S), _pd(inflow), form, _pd(I))
+    if rc != 0:
+        raise RuntimeError(f"oracle_sweep_ray failed: {rc}")
+    return I
+
+
+def solve(inp, nthreads: int = 0, want_J: bool = False):
+    """O-7: returns (Q [nz][ny][nx], Itop [nb][n_up][ny][nx]) (+ J [nb][nz][ny][nx])."""
+    lib = _load()
+    Q = np.empty(inp.shape, dtype=np.float64)
+    Itop = np.empty((inp.nbands, inp.n_up, inp.ny, inp.nx), dtype=np.float64)
+    J = np.empty((inp.nbands,) + inp.shape, dtype=np.float64) if want_J else None
+    mu = np.ascontiguousarray(inp.mu, dtype=np.float64)
+    wq = np.ascontiguousarray(inp.wq, dtype=np.float64)
+    rc = lib.oracle_solve(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz,
+                          inp.nbands, inp.nT, inp.nP,
+                          inp.logT_min, inp.logT_max, inp.logP_min, inp.logP_max,
+                          _pf(inp.logkappa), _pf(inp.bandfrac),
+                          inp.npasses, inp.nrays, _pd(mu), _pd(wq),
+                          _pf(inp.rho), _pf(inp.T), _pf(inp.P),
+                          _pd(Q), _pd(Itop), _pd(J), nthreads)
+    if rc != 0:
+        raise RuntimeError(f"oracle_solve failed: {rc}")
+    if want_J:
+        return Q, Itop, J
+    return Q, Itop

@@ -1,0 +1,336 @@
+/*
+ * rts_oracle.c -- plain fp64 CPU oracle of the RTS hot path.
+ *
+ * TEST INFRASTRUCTURE.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call this file.  It
+ * shares no code, header, table or helper with the CUDA path under
+ * paper_2107_08145_b200/csrc/ and is never used by the product path.
+ *
+ * What it computes (paper: arxiv 2107.08145, /root/reference/PAPER.md):
+ *   PAPER.md:72  (sec. 2)   short characteristics, 24 Carlson directions, block-local
+ *                           solve started from previous-iteration boundary intensities,
+ *                           iterated 3-4 times
+ *   PAPER.md:78-82 (sec. 2) the four RTS sub-routines Interpolate / Integrate /
+ *                           Exchange / Flux
+ *   PAPER.md:189 (sec. 5.1) "integrating the radiation transfer equation along a ray
+ *                           using values of intensity and opacity interpolated from the
+ *                           neighbouring grid cells", 3 rays per octant
+ *   PAPER.md:195 (sec. 5.1) multi-band opacities; radiative heating per grid point
+ *   PAPER.md:197-217 (Fig. 8) loop nest: rays x { interpol; iterate integrate; flux }
+ *   PAPER.md:231 (Fig. 9)   preloaded boundary layer, each point depends on up to four
+ *                           points of the previous set
+ * The paper prints no formula for the scheme; every numerical choice below is the
+ * reading fixed in SURVEY.md 8(c) (O-1..O-8, R1..R19) and repeated in DESIGN.md.
+ *
+ * The scheme is a discretisation, so the oracle is the scheme itself, step by step,
+ * in the plain node order (k, j, i loops running in the ray's direction): no tiles,
+ * no hyperplanes, no blocking, no fusion.
+ *
+ * Pins (tests/test_oracle_pins.py): exp(-tau) attenuation, linear-in-tau source,
+ * optically thick limit and second moment of the ray set, isothermal exactness,
+ * rotation/mirror symmetry, 1-D reduction against an independent recurrence,
+ * memoised recursive evaluator on tiny grids, pass fixed point, I-form vs D-form,
+ * table stage closed forms, psi check values of SURVEY 8(c) O-6.  Parity: pinned.
+ *
+ * Layout: all fields [nz][ny][nx], x fastest, idx = (k*ny + j)*nx + i; z is up,
+ * k = 0 is the bottom.  cgs units.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <stddef.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define SIGMA_SB 5.670374e-5
+#define ORACLE_PI 3.14159265358979323846
+
+/* ---------------------------------------------------------------------------
+ * O-2  Coefficient stage (paper's interpol() minus the grid staggering,
+ *      PAPER.md:79, 204).  Per node and band:
+ *        x_T = (log10 T - logT_min)/(logT_max - logT_min)*(nT-1), clamped to [0,nT-1]
+ *        i0 = min(floor(x_T), nT-2), t = x_T - i0;   same for P -> j0, u
+ *        log10 kappa_b = bilinear(L_b; i0,t; j0,u);  kaprho_b = 10^(log10 kappa_b)*rho
+ *        f_b = (1-t) f[b][i0] + t f[b][i0+1];        S_b = f_b * sigma T^4 / pi
+ * O-1: inputs are the fp32 arrays, promoted to fp64 on read.
+ * ------------------------------------------------------------------------- */
+int oracle_coefficients(int nx, int ny, int nz, int nb, int nT, int nP,
+                        double logT_min, double logT_max, double logP_min, double logP_max,
+                        const float* logkappa, const float* bandfrac,
+                        const float* rho, const float* T, const float* P,
+                        double* kaprho, double* S)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || nb < 1 || nT < 2 || nP < 2) return -1;
+    const size_t N = (size_t)nx * ny * nz;
+    long n;
+#pragma omp parallel for schedule(static)
+    for (n = 0; n < (long)N; ++n) {
+        double xT = (log10((double)T[n]) - logT_min) / (logT_max - logT_min) * (nT - 1);
+        double xP = (log10((double)P[n]) - logP_min) / (logP_max - logP_min) * (nP - 1);
+        if (xT < 0.0) xT = 0.0;
+        if (xT > nT - 1) xT = nT - 1;
+        if (xP < 0.0) xP = 0.0;
+        if (xP > nP - 1) xP = nP - 1;
+        int i0 = (int)floor(xT); if (i0 > nT - 2) i0 = nT - 2;
+        int j0 = (int)floor(xP); if (j0 > nP - 2) j0 = nP - 2;
+        double t = xT - i0, u = xP - j0;
+        double Tn = (double)T[n];
+        double planck = SIGMA_SB * Tn * Tn * Tn * Tn / ORACLE_PI;
+        for (int b = 0; b < nb; ++b) {
+            const float* L = logkappa + (size_t)b * nT * nP;
+            double lk = (1.0 - t) * (1.0 - u) * (double)L[(size_t)i0 * nP + j0]
+                      + t * (1.0 - u) * (double)L[(size_t)(i0 + 1) * nP + j0]
+                      + (1.0 - t) * u * (double)L[(size_t)i0 * nP + j0 + 1]
+                      + t * u * (double)L[(size_t)(i0 + 1) * nP + j0 + 1];
+            double fb = (1.0 - t) * (double)bandfrac[(size_t)b * nT + i0]
+                      + t * (double)bandfrac[(size_t)b * nT + i0 + 1];
+            kaprho[(size_t)b * N + n] = pow(10.0, lk) * (double)rho[n];
+            S[(size_t)b * N + n] = fb * planck;
+        }
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-3  Ray geometry.  t_a = h_a/|mu_a|; ds = min_a t_a; entry-face axis a* = argmin
+ *      (ties: prefer z, then y, then x); for the two other axes f_c = ds*|mu_c|/h_c.
+ *      sgn[a] = +1 if mu_a >= 0 else -1.
+ * ------------------------------------------------------------------------- */
+int oracle_ray_geometry(double dx, double dy, double dz, const double* mu,
+                        int* axis, int* sgn, double* ds, double* f)
+{
+    const double h[3] = {dx, dy, dz};
+    double t[3];
+    for (int a = 0; a < 3; ++a) {
+        sgn[a] = (mu[a] >= 0.0) ? 1 : -1;
+        t[a] = (mu[a] != 0.0) ? h[a] / fabs(mu[a]) : HUGE_VAL;
+    }
+    if (mu[2] == 0.0) return -1;           /* horizontal rays have no inflow boundary here */
+    int as = 2;                            /* prefer z, then y, then x on ties */
+    if (t[1] < t[as]) as = 1;
+    if (t[0] < t[as]) as = 0;
+    *axis = as;
+    *ds = t[as];
+    for (int a = 0; a < 3; ++a) f[a] = (a == as) ? 1.0 : (*ds) * fabs(mu[a]) / h[a];
+    return 0;
+}
+
+/* O-6 weights of the linear-source-function integration over dtau.
+ *   E = exp(-dtau); w1 = (1-E)/dtau; psi_u = w1 - E; psi_p = 1 - w1.
+ *   Series below dtau < 1e-3 (truncation < 2e-18). */
+void oracle_psi(double dtau, double* E, double* psi_u, double* psi_p)
+{
+    if (dtau < 1e-3) {
+        double d = dtau;
+        *E = exp(-d);
+        *psi_p = d / 2.0 - d * d / 6.0 + d * d * d / 24.0 - d * d * d * d / 120.0;
+        *psi_u = d / 2.0 - d * d / 3.0 + d * d * d / 8.0 - d * d * d * d / 30.0;
+    } else {
+        double e = exp(-dtau);
+        double w1 = (1.0 - e) / dtau;
+        *E = e;
+        *psi_u = w1 - e;
+        *psi_p = 1.0 - w1;
+    }
+}
+
+/* ---------------------------------------------------------------------------
+ * O-4..O-6  Formal solution for ONE band and ONE ray, all passes.
+ *
+ *  kaprho, S : nodal fields of this band [nz][ny][nx] (fp64)
+ *  mu        : direction of photon travel
+ *  I_inflow  : NULL -> the paper's boundary values (bottom I = S for mu_z > 0, top
+ *              I = 0 for mu_z < 0; O-4); else [ny][nx] incoming intensity placed on the
+ *              Dirichlet node plane (test hook for the exp(-tau) pin)
+ *  form      : 0 = carry the intensity I (the scheme as stated);
+ *              1 = carry the departure D = I - S (algebraically identical: S_u is the
+ *                  bilinear interpolant of nodal S); used only to pin the conditioning
+ *  I         : out, I^(P) at every node [nz][ny][nx]
+ *
+ *  Passes (O-5): I^(0) = Dirichlet value on the Dirichlet plane, S elsewhere.  In pass p
+ *  every non-Dirichlet node is updated once in the plain upwind order.  A stencil node
+ *  whose x or y index wraps takes its intensity from I^(p-1) (Jacobi ghosts); stencil
+ *  nodes that do not wrap use I^(p).  Only the faces i = (sx>0 ? nx-1 : 0) and
+ *  j = (sy>0 ? ny-1 : 0) of I^(p-1) are ever read, so only those are kept.
+ * ------------------------------------------------------------------------- */
+int oracle_sweep_ray(int nx, int ny, int nz, double dx, double dy, double dz,
+                     const double* mu, int npasses,
+                     const double* kaprho, const double* S,
+                     const double* I_inflow, int form, double* I)
+{
+    int as, sg[3];
+    double ds, f[3];
+    if (nx < 1 || ny < 1 || nz < 2 || npasses < 1) return -1;
+    if (oracle_ray_geometry(dx, dy, dz, mu, &as, sg, &ds, f) != 0) return -1;
+    const int sx = sg[0], sy = sg[1], sz = sg[2];
+    const size_t N = (size_t)nx * ny * nz;
+    const int kdir = (sz > 0) ? 0 : nz - 1;      /* Dirichlet node plane (O-4) */
+
+    /* the two transverse axes c, d of the entry face and the 4 stencil offsets/weights */
+    int c = (as == 0) ? 1 : 0;
+    int d = (as == 2) ? 1 : 2;
+    int off[4][3];
+    double w[4];
+    for (int ec = 0; ec < 2; ++ec)
+        for (int ed = 0; ed < 2; ++ed) {
+            int q = ec * 2 + ed;
+            off[q][0] = off[q][1] = off[q][2] = 0;
+            off[q][as] = -sg[as];
+            off[q][c] = -ec * sg[c];
+            off[q][d] = -ed * sg[d];
+            w[q] = (ec ? f[c] : 1.0 - f[c]) * (ed ? f[d] : 1.0 - f[d]);
+        }
+
+    /* work array holds the carried quantity X = I (form 0) or D = I - S (form 1) */
+    double* X = I;
+    double* faceX = (double*)malloc(sizeof(double) * (size_t)nz * ny);  /* X^(p-1)(i_face, j, k) */
+    double* faceY = (double*)malloc(sizeof(double) * (size_t)nz * nx);  /* X^(p-1)(i, j_face, k) */
+    if (!faceX || !faceY) { free(faceX); free(faceY); return -2; }
+    const int iface = (sx > 0) ? nx - 1 : 0;
+    const int jface = (sy > 0) ? ny - 1 : 0;
+
+    /* I^(0) */
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t n = ((size_t)k * ny + j) * nx + i;
+                double I0;
+                if (k == kdir) {
+                    if (I_inflow) I0 = I_inflow[(size_t)j * nx + i];
+                    else I0 = (sz > 0) ? S[n] : 0.0;
+                } else I0 = S[n];
+                X[n] = form ? I0 - S[n] : I0;
+            }
+
+    for (int p = 1; p <= npasses; ++p) {
+        /* keep the two faces of pass p-1 */
+        for (int k = 0; k < nz; ++k) {
+            for (int j = 0; j < ny; ++j) faceX[(size_t)k * ny + j] = X[((size_t)k * ny + j) * nx + iface];
+            for (int i = 0; i < nx; ++i) faceY[(size_t)k * nx + i] = X[((size_t)k * ny + jface) * nx + i];
+        }
+        for (int kk = 0; kk < nz; ++kk) {
+            int k = (sz > 0) ? kk : nz - 1 - kk;
+            if (k == kdir) continue;                        /* Dirichlet plane: not updated */
+            for (int jj = 0; jj < ny; ++jj) {
+                int j = (sy > 0) ? jj : ny - 1 - jj;
+                for (int ii = 0; ii < nx; ++ii) {
+                    int i = (sx > 0) ? ii : nx - 1 - ii;
+                    size_t n = ((size_t)k * ny + j) * nx + i;
+                    double Xu = 0.0, ku = 0.0, Su = 0.0;
+                    for (int q = 0; q < 4; ++q) {
+                        int iu = i + off[q][0], ju = j + off[q][1], kq = k + off[q][2];
+                        int wrapx = 0, wrapy = 0;
+                        if (iu < 0) { iu += nx; wrapx = 1; } else if (iu >= nx) { iu -= nx; wrapx = 1; }
+                        if (ju < 0) { ju += ny; wrapy = 1; } else if (ju >= ny) { ju -= ny; wrapy = 1; }
+                        /* kq stays inside [0,nz): the Dirichlet plane is never updated */
+                        size_t m = ((size_t)kq * ny + ju) * nx + iu;
+                        double xv;
+                        if (wrapx) xv = faceX[(size_t)kq * ny + ju];       /* iu == iface */
+                        else if (wrapy) xv = faceY[(size_t)kq * nx + iu];  /* ju == jface */
+                        else xv = X[m];
+                        Xu += w[q] * xv;
+                        ku += w[q] * kaprho[m];
+                        Su += w[q] * S[m];
+                    }
+                    double dtau = 0.5 * (ku + kaprho[n]) * ds;
+                    double E, pu, pp;
+                    oracle_psi(dtau, &E, &pu, &pp);
+                    if (!form) {
+                        X[n] = Xu * E + pu * Su + pp * S[n];
+                    } else {
+                        /* D_p = D_u E - (S_p - S_u)(1-E)/dtau ; (1-E)/dtau = E + psi_u */
+                        X[n] = Xu * E - (S[n] - Su) * (E + pu);
+                    }
+                }
+            }
+        }
+    }
+    if (form) for (size_t n = 0; n < N; ++n) I[n] = X[n] + S[n];
+    free(faceX); free(faceY);
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-7  Full solve: all bands, all rays, J, Q and I_top.
+ *   J_b = sum_r w_r I_{b,r}^(P);  Q = 4 pi sum_b kaprho_b (J_b - S_b) at every node;
+ *   Itop[b][u][j][i] = I_{b,r}^(P)(i,j,nz-1) for the u-th ray with mu_z > 0 (in ray order).
+ *   Optional outputs (may be NULL): Jout [nb][N].
+ *   nthreads <= 0: all OpenMP threads.
+ * ------------------------------------------------------------------------- */
+int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
+                 int nb, int nT, int nP,
+                 double logT_min, double logT_max, double logP_min, double logP_max,
+                 const float* logkappa, const float* bandfrac,
+                 int npasses, int nrays, const double* mu, const double* wq,
+                 const float* rho, const float* T, const float* P,
+                 double* Q, double* Itop, double* Jout, int nthreads)
+{
+    if (nx < 1 || ny < 1 || nz < 2 || nb < 1 || nrays < 1) return -1;
+    const size_t N = (size_t)nx * ny * nz;
+    double* kaprho = (double*)malloc(sizeof(double) * N * nb);
+    double* S = (double*)malloc(sizeof(double) * N * nb);
+    double* J = (double*)calloc(N * nb, sizeof(double));
+    int* upidx = (int*)malloc(sizeof(int) * nrays);
+    if (!kaprho || !S || !J || !upidx) { free(kaprho); free(S); free(J); free(upidx); return -2; }
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+    int rc = oracle_coefficients(nx, ny, nz, nb, nT, nP, logT_min, logT_max, logP_min, logP_max,
+                                 logkappa, bandfrac, rho, T, P, kaprho, S);
+    int nup = 0;
+    for (int r = 0; r < nrays; ++r) upidx[r] = (mu[3 * r + 2] > 0.0) ? nup++ : -1;
+
+    int fail = rc;
+    const int ntask = nb * nrays;
+    int task;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (task = 0; task < ntask; ++task) {
+        int b = task / nrays, r = task % nrays;
+        double* I = (double*)malloc(sizeof(double) * N);
+        if (!I) {
+#pragma omp atomic write
+            fail = -2;
+            continue;
+        }
+        int e = oracle_sweep_ray(nx, ny, nz, dx, dy, dz, mu + 3 * r, npasses,
+                                 kaprho + (size_t)b * N, S + (size_t)b * N, NULL, 0, I);
+        if (e != 0) {
+#pragma omp atomic write
+            fail = e;
+        } else {
+            if (Itop && upidx[r] >= 0) {
+                double* dst = Itop + ((size_t)b * nup + upidx[r]) * ny * nx;
+                memcpy(dst, I + (size_t)(nz - 1) * ny * nx, sizeof(double) * ny * nx);
+            }
+            double* Jb = J + (size_t)b * N;
+#pragma omp critical(oracle_accumulate_J)
+            for (size_t n = 0; n < N; ++n) Jb[n] += wq[r] * I[n];
+        }
+        free(I);
+    }
+    if (fail == 0) {
+        long n;
+#pragma omp parallel for schedule(static)
+        for (n = 0; n < (long)N; ++n) {
+            double q = 0.0;
+            for (int b = 0; b < nb; ++b)
+                q += 4.0 * ORACLE_PI * kaprho[(size_t)b * N + n] * (J[(size_t)b * N + n] - S[(size_t)b * N + n]);
+            Q[n] = q;
+        }
+        if (Jout) memcpy(Jout, J, sizeof(double) * N * nb);
+    }
+    free(kaprho); free(S); free(J); free(upidx);
+    return fail;
+}
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
