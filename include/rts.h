@@ -1,0 +1,130 @@
+/*
+ * rts.h -- C-ABI of the B200-native radiation transport solver (RTS) hot path.
+ *
+ * The operation is MURaM's RTS as described in arxiv 2107.08145:
+ *   PAPER.md:78-82  (sec. 2)    RTS = Interpolate / Integrate / Exchange / Flux
+ *   PAPER.md:189    (sec. 5.1)  short characteristics: integrate the transfer equation
+ *                               along a ray using intensity and opacity interpolated from
+ *                               the neighbouring grid cells, 3 rays per octant (24 rays)
+ *   PAPER.md:195    (sec. 5.1)  multi-band opacities; boundary intensities iterated;
+ *                               radiative heating/cooling at each point
+ *   PAPER.md:197-217 (Fig. 8)   loop nest  rays x { interpol; iterate integrate; flux }
+ * The numerical readings the paper leaves open are fixed in DESIGN.md ("Readings").
+ *
+ * One solve computes, for `nbands` opacity bands and `nrays` directions,
+ *   stage A (interpol):  kaprho_b = 10^(bilinear log10 kappa_b(log10 T, log10 P)) * rho,
+ *                        S_b = f_b(log10 T) * sigma T^4 / pi
+ *   stage B (integrate): per ray and band the short-characteristics formal solution
+ *                        I_p = I_u e^-dtau + psi_u S_u + psi_p S_p (linear source function),
+ *                        upwind values bilinear on the entry face of the upwind cell,
+ *                        dtau = (kaprho_u + kaprho_p)/2 * ds
+ *   stage C:             `npasses` sweeps; a stencil node whose x or y index wraps around the
+ *                        periodic box takes its intensity from the previous pass
+ *                        (pass 0: I = S; inflow planes: bottom I = S, top I = 0)
+ *   stage D (flux):      Q_rad = 4 pi sum_b kaprho_b (J_b - S_b),  J_b = sum_r w_r I_{b,r}
+ *   stage E:             I_top[b][u] = I_{b,r}(.,.,nz-1) for the u-th ray with mu_z > 0
+ *
+ * Conventions
+ *   - extern "C"; every function returns int: 0 = RTS_OK, negative = error.  No exceptions,
+ *     no aborts, nothing printed.  rts_last_error() gives the text of the last failure.
+ *   - Fields are fp32, contiguous [nz][ny][nx] (x fastest), z up, k = 0 is the bottom.  cgs.
+ *   - "host"/"device" is stated per pointer.  The caller owns every buffer it passes in,
+ *     including the device workspace; the library owns only small device copies of the
+ *     tables and its job descriptors (freed by rts_destroy).  Inputs are never modified;
+ *     outputs are fully overwritten (Q_rad is not accumulated into).
+ *   - There is no CPU fallback: without a CUDA device rts_create fails with RTS_ECUDA.
+ *   - Non-finite or non-positive T, P (log10 of <= 0) are the caller's responsibility.
+ */
+#ifndef RTS_H_
+#define RTS_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RTS_OK       0
+#define RTS_EINVAL  -1   /* null pointer, bad size, bad ray, workspace too small or misaligned */
+#define RTS_ESTATE  -2   /* call out of order (solve before tables / workspace) */
+#define RTS_ECUDA   -3   /* CUDA runtime / launch error, or no device */
+#define RTS_ENOMEM  -4   /* host allocation failed */
+#define RTS_ETIMEOUT -5  /* device-side watchdog of the persistent sweep kernel fired */
+
+typedef struct rts_ctx rts_ctx;
+
+/* Create a solver for an nx*ny*nz node grid with spacings dx,dy,dz (cm) and nbands bands.
+ * nx, ny >= 2 (periodic), nz >= 2, nbands >= 1.  Uses the current CUDA device.
+ * Defaults: 24-ray set of BASELINE.json configs[0] (order: r = 3*octant + axis of the large
+ * cosine, octant = bx + 2 by + 4 bz, b = 1 for a negative cosine; weights 1/24), 3 passes. */
+int rts_create(rts_ctx** out, int nx, int ny, int nz,
+               double dx_cm, double dy_cm, double dz_cm, int nbands);
+int rts_destroy(rts_ctx* ctx);
+
+/* Opacity and band-fraction tables; HOST pointers, copied to the device inside the call.
+ *   logkappa[b][iT][iP] (iP fastest) = log10 kappa_b on a uniform nT x nP grid in
+ *   (log10 T, log10 P) spanning [logT_min, logT_max] x [logP_min, logP_max]; lookups are
+ *   bilinear with clamping at the edges.  bandfrac[b][iT] = f_b on the same log10 T grid
+ *   (gray: all 1).  nT, nP >= 2. */
+int rts_set_tables(rts_ctx* ctx, int nT, int nP,
+                   double logT_min, double logT_max, double logP_min, double logP_max,
+                   const float* logkappa_host, const float* bandfrac_host);
+
+/* Number of sweep passes (periodic re-sweeps), >= 1.  Default 3. */
+int rts_set_passes(rts_ctx* ctx, int npasses);
+
+/* Replace the ray set.  mu_xyz: HOST [nrays][3] directions of photon travel (need not be
+ * normalised; mu_z must be non-zero); weights: HOST [nrays] (J = sum_r w_r I_r).
+ * 1 <= nrays <= 256.  Invalidates the workspace size (call rts_workspace_bytes again). */
+int rts_set_rays(rts_ctx* ctx, int nrays, const double* mu_xyz_host, const double* weights_host);
+/* Read back the ray set (HOST out pointers may be NULL). *nrays receives the count. */
+int rts_get_rays(const rts_ctx* ctx, int* nrays, double* mu_xyz_host, double* weights_host);
+/* Number of rays with mu_z > 0 (second extent of I_top). */
+int rts_num_up_rays(const rts_ctx* ctx);
+
+/* Tuning hooks (optional).  march = 0,1,2 selects the sweeps that march along x, y, z;
+ * tile_u is the tile extent along the unit-stride transverse axis (multiple of 4, <= 248),
+ * tile_v along the other transverse axis (<= 254).  0,0 restores the planner's choice.
+ * ctas_per_sm = 0 lets the planner choose.  Invalidates the workspace size. */
+int rts_set_tiling(rts_ctx* ctx, int march, int tile_u, int tile_v);
+int rts_set_ctas_per_sm(rts_ctx* ctx, int ctas_per_sm);
+
+/* Bytes of device workspace the current configuration needs (0 on error). */
+size_t rts_workspace_bytes(rts_ctx* ctx);
+/* Hand over a DEVICE workspace of at least rts_workspace_bytes(), 256-byte aligned.  It must
+ * stay valid until the ctx is destroyed or another workspace is set. */
+int rts_set_workspace(rts_ctx* ctx, void* workspace_dev, size_t bytes);
+
+/* The hot path.  DEVICE pointers: rho, T, P in [nz][ny][nx]; Qrad out [nz][ny][nx];
+ * Itop out [nbands][n_up][ny][nx] or NULL (not wanted).  stream: a cudaStream_t passed as
+ * void* (NULL = default stream).  Asynchronous on that stream; errors of the asynchronous
+ * part surface at the next rts_sync_check / synchronising call. */
+int rts_solve(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const float* P_dev,
+              float* Qrad_dev, float* Itop_dev, void* stream);
+
+/* Same solve with HOST buffers (pinned or pageable): copies rho,T,P to the device, solves,
+ * copies Qrad (and Itop if non-NULL) back, synchronises.  The staging buffers live in the
+ * workspace (rts_workspace_bytes accounts for them). */
+int rts_solve_host(rts_ctx* ctx, const float* rho_host, const float* T_host, const float* P_host,
+                   float* Qrad_host, float* Itop_host, void* stream);
+
+/* Stage A alone, for per-stage parity: DEVICE outputs kaprho, S each [nbands][nz][ny][nx]. */
+int rts_coefficients(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const float* P_dev,
+                     float* kaprho_dev, float* S_dev, void* stream);
+
+/* Synchronise `stream` and report the device-side status of the last solve
+ * (RTS_OK, RTS_ETIMEOUT if the sweep watchdog fired, RTS_ECUDA). */
+int rts_sync_check(rts_ctx* ctx, void* stream);
+
+/* Plan facts for reporting: what[0] = kernels launched per solve, [1] = sweep rounds,
+ * [2] = CTAs per SM of the sweep kernel, [3] = sweep jobs, [4] = threads per CTA,
+ * [5] = dynamic shared memory per CTA (bytes), [6..8] = tile_u of march x,y,z,
+ * [9..11] = tile_v of march x,y,z.  n = number of ints the caller's array holds. */
+int rts_plan_info(rts_ctx* ctx, int* what, int n);
+
+const char* rts_last_error(const rts_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RTS_H_ */

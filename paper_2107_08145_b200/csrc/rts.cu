@@ -1,0 +1,727 @@
+// rts.cu -- host side of the C-ABI in include/rts.h: ray geometry, job list, planner,
+// workspace layout, TMA descriptors, launches.  All arithmetic of the path runs in the
+// kernels of rts_kernels.cuh; nothing here (or anywhere in the product) touches oracle/.
+#include "../../include/rts.h"
+#include "rts_kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace rts;
+
+namespace {
+
+struct HostRay {
+    double mu[3];
+    double w;
+    int march, dir, su, sv, slot, up, itop;
+    double ds, fu, fv;
+};
+
+struct TypePlan {        // per march axis
+    int n_m = 0, n_u = 0, n_v = 0;
+    int TU = 0, TV = 0, ntu = 0, ntv = 0;
+    int userTU = 0, userTV = 0;
+};
+
+struct HostJob {
+    JobDesc d;
+    int nsteps;
+    int round, slot;     // slot = index within its round (selects the exchange buffers)
+};
+
+}  // namespace
+
+struct rts_ctx {
+    int nx = 0, ny = 0, nz = 0, nb = 0;
+    double h[3] = {0, 0, 0};
+    int npass = 3;
+    std::vector<HostRay> rays;
+    int n_up = 0;
+    // tables
+    bool have_tables = false;
+    int nT = 0, nP = 0;
+    double logT_min = 0, logT_max = 0, logP_min = 0, logP_max = 0;
+    float* d_logkappa = nullptr;
+    float* d_bandfrac = nullptr;
+    // device facts
+    int sm_count = 0, max_smem_optin = 0;
+    int user_ctas_per_sm = 0;
+    // plan
+    bool planned = false;
+    TypePlan tp[3];
+    std::vector<HostJob> jobs;
+    std::vector<std::vector<int>> rounds;   // job indices per round
+    int ctas_per_sm = 0, threads = 256, smem_bytes = 0, max_round_jobs = 0;
+    int PX = 0, PY = 0;
+    size_t ws_bytes = 0;
+    // workspace offsets
+    size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_kstar = 0, off_abort = 0,
+           off_jobs = 0, off_slot0 = 0, slot_stride = 0, off_stage_in = 0, off_stage_out = 0;
+    size_t slot_Dg = 0, slot_Gu = 0, slot_Gv = 0, slot_prog = 0;
+    int nblk_a = 0;
+    // workspace
+    unsigned char* ws = nullptr;
+    size_t ws_have = 0;
+    bool maps_ready = false;
+    CUtensorMap mapX, mapY, mapZ;
+    cudaEvent_t ev = nullptr;
+    std::string err;
+};
+
+namespace {
+
+std::string g_create_err = "null context";   // failures of rts_create (no ctx to hold the text)
+
+int fail(rts_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg; else g_create_err = msg;
+    return code;
+}
+#define CUDA_TRY(c, expr)                                                                         \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail((c), RTS_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));      \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// Ray geometry (reading R3): the characteristic leaves the upwind cell through the
+// face reached first; ties prefer z, then y, then x.
+int ray_geometry(const double h[3], HostRay& r)
+{
+    double t[3];
+    for (int a = 0; a < 3; ++a) t[a] = (r.mu[a] != 0.0) ? h[a] / std::fabs(r.mu[a]) : HUGE_VAL;
+    if (r.mu[2] == 0.0) return -1;
+    int as = 2;
+    if (t[1] < t[as]) as = 1;
+    if (t[0] < t[as]) as = 0;
+    r.march = as;
+    r.ds = t[as];
+    r.dir = (r.mu[as] >= 0.0) ? 1 : -1;
+    const int ua = (as == 0) ? 1 : 0;          // unit-stride transverse axis
+    const int va = (as == 2) ? 1 : 2;          // other transverse axis
+    r.su = (r.mu[ua] >= 0.0) ? 1 : -1;
+    r.sv = (r.mu[va] >= 0.0) ? 1 : -1;
+    r.fu = r.ds * std::fabs(r.mu[ua]) / h[ua];
+    r.fv = r.ds * std::fabs(r.mu[va]) / h[va];
+    r.slot = (r.su < 0 ? 1 : 0) + (r.sv < 0 ? 2 : 0);
+    r.up = (r.mu[2] > 0.0) ? 1 : 0;
+    return 0;
+}
+
+// Bilinear weights as fp32 numbers that sum to 1 EXACTLY: the three smaller ones are rounded
+// to multiples of 2^-24, the largest is 1 minus their sum.  A partition of unity that is only
+// accurate to an ulp biases the carried intensity by ~6e-8 per step, which accumulates over
+// hundreds of steps ("precision").
+void make_ray_consts(const HostRay& r, RayC& rc)
+{
+    double w[4] = {(1 - r.fu) * (1 - r.fv), r.fu * (1 - r.fv), (1 - r.fu) * r.fv, r.fu * r.fv};
+    int big = 0;
+    for (int q = 1; q < 4; ++q)
+        if (w[q] > w[big]) big = q;
+    double sum = 0.0;
+    for (int q = 0; q < 4; ++q)
+        if (q != big) { w[q] = std::nearbyint(w[q] * 16777216.0) / 16777216.0; sum += w[q]; }
+    w[big] = 1.0 - sum;
+    for (int q = 0; q < 4; ++q) {
+        rc.wx[q] = (float)w[q];
+        rc.wk[q] = (float)(0.5 * r.ds * w[q]);
+    }
+    rc.kc = (float)(0.5 * r.ds);
+    rc.wq = (float)r.w;
+    rc.active = 1;
+    rc.up = r.up;
+    rc.itop = r.itop;
+}
+
+void default_rays(rts_ctx* c)
+{
+    const double A = 0.2958759, B = 0.9082483;
+    c->rays.clear();
+    for (int o = 0; o < 8; ++o)
+        for (int m = 0; m < 3; ++m) {
+            HostRay r{};
+            for (int a = 0; a < 3; ++a) {
+                const double s = ((o >> a) & 1) ? -1.0 : 1.0;
+                r.mu[a] = s * (a == m ? B : A);
+            }
+            r.w = 1.0 / 24.0;
+            c->rays.push_back(r);
+        }
+}
+
+int box_elems(int TU, int TV) { return (TU + 2 * XPAD) * (TV + 2); }
+int smem_for(int TU, int TV)
+{
+    const int BOX = box_elems(TU, TV);
+    const int stage = (2 * BOX + 31) & ~31, xb = (NSLOT * BOX + 31) & ~31;
+    return (2 * stage + 2 * xb) * (int)sizeof(float);
+}
+
+// --------------------------------------------------------------------------- planner
+// Chooses the tile shape per march axis, the CTAs per SM and the packing of jobs into
+// rounds (one cooperative launch each; all CTAs of a round are co-resident).
+int make_plan(rts_ctx* c)
+{
+    c->planned = false;
+    c->maps_ready = false;
+    const int n[3] = {c->nx, c->ny, c->nz};
+    // --- rays -> geometry, I_top index
+    int nup = 0;
+    for (auto& r : c->rays) {
+        if (ray_geometry(c->h, r) != 0) return fail(c, RTS_EINVAL, "ray with mu_z == 0");
+        r.itop = r.up ? nup++ : -1;
+    }
+    c->n_up = nup;
+    // --- march types
+    for (int a = 0; a < 3; ++a) {
+        TypePlan& t = c->tp[a];
+        t.n_m = n[a];
+        t.n_u = (a == 0) ? n[1] : n[0];
+        t.n_v = (a == 2) ? n[1] : n[2];
+    }
+    c->PX = (int)align_up((size_t)c->nx + 2 * XPAD, 4);
+    c->PY = (int)align_up((size_t)c->ny + 2 * XPAD, 4);
+
+    // --- job skeletons: (march, dir) groups, sub-jobs with <= 1 ray per sign slot, bands
+    struct Group { int march, dir; std::vector<std::vector<int>> sub; };
+    std::vector<Group> groups;
+    for (int ri = 0; ri < (int)c->rays.size(); ++ri) {
+        const HostRay& r = c->rays[ri];
+        Group* g = nullptr;
+        for (auto& gg : groups)
+            if (gg.march == r.march && gg.dir == r.dir) g = &gg;
+        if (!g) { groups.push_back(Group{r.march, r.dir, {}}); g = &groups.back(); }
+        bool placed = false;
+        for (auto& sub : g->sub) {
+            bool freeslot = true;
+            for (int rj : sub) freeslot &= (c->rays[rj].slot != r.slot);
+            if (freeslot) { sub.push_back(ri); placed = true; break; }
+        }
+        if (!placed) g->sub.push_back(std::vector<int>{ri});
+    }
+    int njobs_type[3] = {0, 0, 0};
+    for (auto& g : groups) njobs_type[g.march] += (int)g.sub.size() * c->nb;
+    const int njobs_total = njobs_type[0] + njobs_type[1] + njobs_type[2];
+
+    // --- occupancy limits of the sweep kernel
+    cudaFuncAttributes fa;
+    CUDA_TRY(c, cudaFuncGetAttributes(&fa, rts_sweep_kernel));
+    const int smem_cap_total = c->max_smem_optin;      // per CTA opt-in max (227 KB on sm_100)
+    const int threads = 256;
+    c->threads = threads;
+
+    // --- search CTAs/SM and tile shapes
+    double best_cost = 1e300;
+    int bestR = 0;
+    TypePlan best_tp[3];
+    for (int R = 1; R <= 4; ++R) {
+        if (c->user_ctas_per_sm && R != c->user_ctas_per_sm) continue;
+        // register limit: R CTAs of `threads` threads
+        if ((long long)R * threads * fa.numRegs > 65536) continue;
+        const int smem_cap = std::min(smem_cap_total, (228 * 1024) / R - 1024 - (int)fa.sharedSizeBytes);
+        const int slots = c->sm_count * R;
+        TypePlan tps[3];
+        bool okR = true;
+        double cost = 0.0;
+        for (int a = 0; a < 3 && okR; ++a) {
+            tps[a] = c->tp[a];
+            if (njobs_type[a] == 0) { tps[a].TU = 4; tps[a].TV = 1; tps[a].ntu = tps[a].ntv = 1; continue; }
+            const TypePlan& t = c->tp[a];
+            double bc = 1e300;
+            int bTU = 0, bTV = 0;
+            const int nu4 = (int)align_up((size_t)t.n_u, 4);
+            for (int TU = 4; TU <= std::min(nu4, 248); TU += 4) {
+                if (t.userTU && TU != t.userTU) continue;
+                const int ntu = (t.n_u + TU - 1) / TU;
+                // prefer tile widths that divide the extent evenly
+                if (!t.userTU && (ntu - 1) * TU >= t.n_u) continue;
+                for (int TV = 1; TV <= std::min(t.n_v, 254); ++TV) {
+                    if (t.userTV && TV != t.userTV) continue;
+                    if (smem_for(TU, TV) > smem_cap) break;
+                    const int ntv = (t.n_v + TV - 1) / TV;
+                    const long long T = (long long)ntu * ntv;
+                    if (T > slots) continue;
+                    const int kpr = (int)std::min<long long>(slots / T, njobs_total);   // jobs per round
+                    const int nrounds = (njobs_type[a] + kpr - 1) / kpr;
+                    const int quads = ((TU + 3) / 4) * TV;
+                    const int iters = (quads + threads - 1) / threads;
+                    // SM time per step ~ CTAs on the busiest SM x (thread iterations + fixed step overhead)
+                    const double ctas_sm = std::ceil((double)kpr * T / c->sm_count);
+                    const double step = ctas_sm * (iters * 1.0 + 0.15);
+                    const double cst = nrounds * (double)t.n_m * step;
+                    if (cst < bc * (1 - 1e-9) || (std::fabs(cst - bc) <= 1e-9 * bc && box_elems(TU, TV) < box_elems(bTU, bTV))) {
+                        bc = cst; bTU = TU; bTV = TV;
+                    }
+                }
+            }
+            if (bTU == 0) { okR = false; break; }
+            tps[a].TU = bTU; tps[a].TV = bTV;
+            tps[a].ntu = (t.n_u + bTU - 1) / bTU;
+            tps[a].ntv = (t.n_v + bTV - 1) / bTV;
+            cost += bc;
+        }
+        if (!okR) continue;
+        {
+            int smemR = 0, occ = 0;
+            for (int a = 0; a < 3; ++a)
+                if (njobs_type[a]) smemR = std::max(smemR, smem_for(tps[a].TU, tps[a].TV));
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, threads, (size_t)smemR) != cudaSuccess || occ < R)
+                continue;
+        }
+        if (cost < best_cost) { best_cost = cost; bestR = R; for (int a = 0; a < 3; ++a) best_tp[a] = tps[a]; }
+    }
+    if (bestR == 0) return fail(c, RTS_EINVAL, "planner: no feasible tiling (grid too large for one wave, or bad override)");
+    for (int a = 0; a < 3; ++a) { best_tp[a].userTU = c->tp[a].userTU; best_tp[a].userTV = c->tp[a].userTV; c->tp[a] = best_tp[a]; }
+    c->ctas_per_sm = bestR;
+    const int slots = c->sm_count * bestR;
+
+    // --- materialise jobs
+    c->jobs.clear();
+    for (auto& g : groups)
+        for (auto& sub : g.sub)
+            for (int b = 0; b < c->nb; ++b) {
+                HostJob hj{};
+                JobDesc& d = hj.d;
+                const TypePlan& t = c->tp[g.march];
+                d.march = g.march; d.dir = g.dir; d.band = b;
+                d.n_m = t.n_m; d.n_u = t.n_u; d.n_v = t.n_v;
+                d.TU = t.TU; d.TV = t.TV; d.ntu = t.ntu; d.ntv = t.ntv;
+                d.per_v = (g.march == 2) ? 1 : 0;
+                d.ntiles = t.ntu * t.ntv;
+                d.npass = c->npass;
+                d.nz = c->nz;
+                {
+                    const long long nxy = (long long)c->nx * c->ny;
+                    d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
+                    if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx; }
+                    else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx; }
+                    else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1; }
+                }
+                for (int q = 0; q < NSLOT; ++q) { std::memset(&d.ray[q], 0, sizeof(RayC)); d.ray[q].itop = -1; d.ray[q].dir_row = -1; }
+                for (int ri : sub) {
+                    const HostRay& r = c->rays[ri];
+                    RayC& rc = d.ray[r.slot];
+                    make_ray_consts(r, rc);
+                    rc.dir_row = (g.march == 2) ? -1 : (r.sv > 0 ? 0 : c->nz - 1);
+                }
+                hj.nsteps = t.n_m * c->npass;
+                c->jobs.push_back(hj);
+            }
+    // --- pack into rounds: longest jobs first, fill each round up to `slots` CTAs
+    std::vector<int> order(c->jobs.size());
+    for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return c->jobs[a].nsteps > c->jobs[b].nsteps; });
+    c->rounds.clear();
+    std::vector<int> used;
+    for (int ji : order) {
+        const int T = c->jobs[ji].d.ntiles;
+        int placed = -1;
+        for (size_t r = 0; r < c->rounds.size(); ++r)
+            if (used[r] + T <= slots) { placed = (int)r; break; }
+        if (placed < 0) { c->rounds.emplace_back(); used.push_back(0); placed = (int)c->rounds.size() - 1; }
+        c->jobs[ji].round = placed;
+        c->jobs[ji].slot = (int)c->rounds[placed].size();
+        c->jobs[ji].d.cta_begin = used[placed];
+        c->rounds[placed].push_back(ji);
+        used[placed] += T;
+    }
+    c->max_round_jobs = 0;
+    for (auto& r : c->rounds) c->max_round_jobs = std::max(c->max_round_jobs, (int)r.size());
+    c->smem_bytes = 0;
+    for (int a = 0; a < 3; ++a)
+        if (njobs_type[a]) c->smem_bytes = std::max(c->smem_bytes, smem_for(c->tp[a].TU, c->tp[a].TV));
+
+    // --- workspace layout
+    const size_t N = (size_t)c->nx * c->ny * c->nz;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    const size_t fA = (size_t)c->nz * (c->ny + 2) * c->PX;
+    const size_t fB = (size_t)c->nz * c->nx * c->PY;
+    c->off_coefA = take(sizeof(float) * fA * 2 * c->nb);
+    c->off_coefB = take(sizeof(float) * fB * 2 * c->nb);
+    c->off_QB = take(sizeof(float) * N);
+    c->nblk_a = ((c->nx + 31) / 32) * ((c->ny + 31) / 32);
+    c->off_ksum = take(sizeof(double) * (size_t)c->nb * c->nz * c->nblk_a);
+    c->off_kstar = take(sizeof(int) * c->nb);
+    c->off_abort = take(sizeof(int) * 4);
+    c->off_jobs = take(sizeof(JobDesc) * c->jobs.size());
+    // per round-slot exchange buffers, sized for the largest job type
+    size_t mDg = 0, mGu = 0, mGv = 0, mProg = 0;
+    for (auto& hj : c->jobs) {
+        const JobDesc& d = hj.d;
+        mDg = std::max(mDg, (size_t)2 * NSLOT * d.n_v * d.n_u);
+        mGu = std::max(mGu, (size_t)2 * NSLOT * d.n_m * d.n_v);
+        mGv = std::max(mGv, d.per_v ? (size_t)2 * NSLOT * d.n_m * d.n_u : (size_t)0);
+        mProg = std::max(mProg, (size_t)d.ntiles);
+    }
+    c->slot_Dg = 0;
+    c->slot_Gu = align_up(sizeof(float) * mDg, 256);
+    c->slot_Gv = c->slot_Gu + align_up(sizeof(float) * mGu, 256);
+    c->slot_prog = c->slot_Gv + align_up(sizeof(float) * mGv, 256);
+    c->slot_stride = c->slot_prog + align_up(sizeof(int) * mProg, 256);
+    c->off_slot0 = take(c->slot_stride * c->max_round_jobs);
+    // host-API staging (rts_solve_host)
+    c->off_stage_in = take(sizeof(float) * N * 3);
+    c->off_stage_out = take(sizeof(float) * (N + (size_t)c->nb * c->n_up * c->ny * c->nx));
+    c->ws_bytes = off;
+    c->planned = true;
+    return RTS_OK;
+}
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int encode_map(rts_ctx* c, CUtensorMap* map, void* base, const cuuint64_t dims[4], const cuuint32_t box[4])
+{
+    static PFN_encodeTiled fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr);
+        if (e != cudaSuccess || !p) return fail(c, RTS_ECUDA, "cuTensorMapEncodeTiled entry point not found");
+        fn = (PFN_encodeTiled)p;
+    }
+    cuuint64_t strides[3] = {dims[0] * sizeof(float), dims[0] * dims[1] * sizeof(float),
+                             dims[0] * dims[1] * dims[2] * sizeof(float)};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char buf[96];
+        snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+        return fail(c, RTS_ECUDA, buf);
+    }
+    return RTS_OK;
+}
+
+int bind_workspace(rts_ctx* c)
+{
+    unsigned char* ws = c->ws;
+    // tensor maps
+    float* coefA = (float*)(ws + c->off_coefA);
+    float* coefB = (float*)(ws + c->off_coefB);
+    {
+        const cuuint64_t dA[4] = {(cuuint64_t)c->PX, (cuuint64_t)c->ny + 2, (cuuint64_t)c->nz, (cuuint64_t)2 * c->nb};
+        const cuuint64_t dB[4] = {(cuuint64_t)c->PY, (cuuint64_t)c->nx, (cuuint64_t)c->nz, (cuuint64_t)2 * c->nb};
+        const TypePlan &tx = c->tp[0], &ty = c->tp[1], &tz = c->tp[2];
+        const cuuint32_t bZ[4] = {(cuuint32_t)tz.TU + 2 * XPAD, (cuuint32_t)tz.TV + 2, 1, 2};
+        const cuuint32_t bY[4] = {(cuuint32_t)ty.TU + 2 * XPAD, 1, (cuuint32_t)ty.TV + 2, 2};
+        const cuuint32_t bX[4] = {(cuuint32_t)tx.TU + 2 * XPAD, 1, (cuuint32_t)tx.TV + 2, 2};
+        int rc;
+        if ((rc = encode_map(c, &c->mapZ, coefA, dA, bZ)) != RTS_OK) return rc;
+        if ((rc = encode_map(c, &c->mapY, coefA, dA, bY)) != RTS_OK) return rc;
+        if ((rc = encode_map(c, &c->mapX, coefB, dB, bX)) != RTS_OK) return rc;
+    }
+    // job descriptors with device pointers (output pointers are patched per solve)
+    for (auto& hj : c->jobs) {
+        JobDesc& d = hj.d;
+        unsigned char* sb = ws + c->off_slot0 + c->slot_stride * hj.slot;
+        d.Dg = (float*)(sb + c->slot_Dg);
+        d.Gu = (float*)(sb + c->slot_Gu);
+        d.Gv = (float*)(sb + c->slot_Gv);
+        d.progress = (int*)(sb + c->slot_prog);
+        d.kstar = (const int*)(ws + c->off_kstar) + d.band;
+    }
+    {
+        std::vector<JobDesc> flat;
+        for (auto& r : c->rounds)
+            for (int ji : r) flat.push_back(c->jobs[ji].d);
+        CUDA_TRY(c, cudaMemcpy(ws + c->off_jobs, flat.data(), sizeof(JobDesc) * flat.size(), cudaMemcpyHostToDevice));
+    }
+    c->maps_ready = true;
+    return RTS_OK;
+}
+
+cudaStream_t as_stream(void* s) { return (cudaStream_t)s; }
+
+int launch_stage_a(rts_ctx* c, const float* rho, const float* T, const float* P, float* plain_k, float* plain_s,
+                   cudaStream_t st)
+{
+    CoefParams p{};
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nb = c->nb; p.nT = c->nT; p.nP = c->nP;
+    p.logT_min = c->logT_min; p.inv_dT = (c->nT - 1) / (c->logT_max - c->logT_min);
+    p.logP_min = c->logP_min; p.inv_dP = (c->nP - 1) / (c->logP_max - c->logP_min);
+    p.logkappa = c->d_logkappa; p.bandfrac = c->d_bandfrac;
+    p.rho = rho; p.T = T; p.P = P;
+    p.coefA = (float*)(c->ws + c->off_coefA); p.PX = c->PX; p.strideA_f = (long long)c->nz * (c->ny + 2) * c->PX;
+    p.coefB = (float*)(c->ws + c->off_coefB); p.PY = c->PY; p.strideB_f = (long long)c->nz * c->nx * c->PY;
+    p.ksum = (double*)(c->ws + c->off_ksum);
+    p.plain_k = plain_k; p.plain_s = plain_s;
+    dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, c->nz), block(32, 8);
+    rts_coef_kernel<<<grid, block, 0, st>>>(p);
+    CUDA_TRY(c, cudaGetLastError());
+    return RTS_OK;
+}
+
+}  // namespace
+
+// =========================================================================== C-ABI
+extern "C" {
+
+int rts_create(rts_ctx** out, int nx, int ny, int nz, double dx, double dy, double dz, int nbands)
+{
+    if (!out) return RTS_EINVAL;
+    *out = nullptr;
+    if (nx < 2 || ny < 2 || nz < 2 || nbands < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0))
+        return fail(nullptr, RTS_EINVAL, "rts_create: need nx,ny,nz >= 2, nbands >= 1, positive spacings");
+    if ((long long)nx * ny * nz > (1LL << 31) - 1) return fail(nullptr, RTS_EINVAL, "rts_create: grid too large");
+    rts_ctx* c = new (std::nothrow) rts_ctx();
+    if (!c) return RTS_ENOMEM;
+    auto bail = [&](const std::string& m) { delete c; return fail(nullptr, RTS_ECUDA, "rts_create: " + m); };
+    int dev = 0, ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1) return bail(std::string("no CUDA device: ") + cudaGetErrorString(e));
+    cudaDeviceProp prop;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess || (e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess)
+        return bail(cudaGetErrorString(e));
+    if (prop.major < 10) return bail("device is not sm_100: no other code path exists");
+    int coop = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    if (!coop) return bail("device lacks cooperative launch");
+    c->sm_count = prop.multiProcessorCount;
+    c->nx = nx; c->ny = ny; c->nz = nz; c->nb = nbands;
+    c->h[0] = dx; c->h[1] = dy; c->h[2] = dz;
+    default_rays(c);
+    cudaFuncAttributes fa;
+    if ((e = cudaFuncGetAttributes(&fa, rts_sweep_kernel)) != cudaSuccess) return bail(std::string("sweep kernel not loadable: ") + cudaGetErrorString(e));
+    c->max_smem_optin = (int)prop.sharedMemPerBlockOptin - (int)fa.sharedSizeBytes;
+    if ((e = cudaFuncSetAttribute(rts_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem_optin)) != cudaSuccess)
+        return bail(std::string("cudaFuncSetAttribute(max dynamic smem): ") + cudaGetErrorString(e));
+    if ((e = cudaEventCreateWithFlags(&c->ev, cudaEventDisableTiming)) != cudaSuccess) return bail(cudaGetErrorString(e));
+    *out = c;
+    return RTS_OK;
+}
+
+int rts_destroy(rts_ctx* c)
+{
+    if (!c) return RTS_EINVAL;
+    if (c->d_logkappa) cudaFree(c->d_logkappa);
+    if (c->d_bandfrac) cudaFree(c->d_bandfrac);
+    if (c->ev) cudaEventDestroy(c->ev);
+    delete c;
+    return RTS_OK;
+}
+
+int rts_set_tables(rts_ctx* c, int nT, int nP, double logT_min, double logT_max, double logP_min,
+                   double logP_max, const float* logkappa, const float* bandfrac)
+{
+    if (!c) return RTS_EINVAL;
+    if (!logkappa || !bandfrac || nT < 2 || nP < 2 || !(logT_max > logT_min) || !(logP_max > logP_min))
+        return fail(c, RTS_EINVAL, "rts_set_tables: bad argument");
+    if (c->d_logkappa) { cudaFree(c->d_logkappa); c->d_logkappa = nullptr; }
+    if (c->d_bandfrac) { cudaFree(c->d_bandfrac); c->d_bandfrac = nullptr; }
+    c->have_tables = false;
+    const size_t nk = (size_t)c->nb * nT * nP, nf = (size_t)c->nb * nT;
+    CUDA_TRY(c, cudaMalloc(&c->d_logkappa, nk * sizeof(float)));
+    CUDA_TRY(c, cudaMalloc(&c->d_bandfrac, nf * sizeof(float)));
+    CUDA_TRY(c, cudaMemcpy(c->d_logkappa, logkappa, nk * sizeof(float), cudaMemcpyHostToDevice));
+    CUDA_TRY(c, cudaMemcpy(c->d_bandfrac, bandfrac, nf * sizeof(float), cudaMemcpyHostToDevice));
+    c->nT = nT; c->nP = nP;
+    c->logT_min = logT_min; c->logT_max = logT_max; c->logP_min = logP_min; c->logP_max = logP_max;
+    c->have_tables = true;
+    return RTS_OK;
+}
+
+int rts_set_passes(rts_ctx* c, int npasses)
+{
+    if (!c) return RTS_EINVAL;
+    if (npasses < 1) return fail(c, RTS_EINVAL, "rts_set_passes: npasses < 1");
+    c->npass = npasses;
+    c->planned = false;
+    return RTS_OK;
+}
+
+int rts_set_rays(rts_ctx* c, int nrays, const double* mu, const double* w)
+{
+    if (!c) return RTS_EINVAL;
+    if (!mu || !w || nrays < 1 || nrays > 256) return fail(c, RTS_EINVAL, "rts_set_rays: bad argument");
+    std::vector<HostRay> rr;
+    for (int r = 0; r < nrays; ++r) {
+        HostRay h{};
+        for (int a = 0; a < 3; ++a) h.mu[a] = mu[3 * r + a];
+        if (h.mu[2] == 0.0 || !std::isfinite(h.mu[0]) || !std::isfinite(h.mu[1]) || !std::isfinite(h.mu[2]))
+            return fail(c, RTS_EINVAL, "rts_set_rays: mu_z must be non-zero and finite");
+        h.w = w[r];
+        rr.push_back(h);
+    }
+    c->rays.swap(rr);
+    c->planned = false;
+    return RTS_OK;
+}
+
+int rts_get_rays(const rts_ctx* c, int* nrays, double* mu, double* w)
+{
+    if (!c || !nrays) return RTS_EINVAL;
+    *nrays = (int)c->rays.size();
+    for (size_t r = 0; r < c->rays.size(); ++r) {
+        if (mu) for (int a = 0; a < 3; ++a) mu[3 * r + a] = c->rays[r].mu[a];
+        if (w) w[r] = c->rays[r].w;
+    }
+    return RTS_OK;
+}
+
+int rts_num_up_rays(const rts_ctx* c)
+{
+    if (!c) return RTS_EINVAL;
+    int n = 0;
+    for (auto& r : c->rays) n += (r.mu[2] > 0.0);
+    return n;
+}
+
+int rts_set_tiling(rts_ctx* c, int march, int tile_u, int tile_v)
+{
+    if (!c) return RTS_EINVAL;
+    if (march < 0 || march > 2 || tile_u < 0 || tile_v < 0 || (tile_u % 4) != 0 || tile_u > 248 || tile_v > 254)
+        return fail(c, RTS_EINVAL, "rts_set_tiling: bad argument");
+    c->tp[march].userTU = tile_u;
+    c->tp[march].userTV = tile_v;
+    c->planned = false;
+    return RTS_OK;
+}
+
+int rts_set_ctas_per_sm(rts_ctx* c, int n)
+{
+    if (!c) return RTS_EINVAL;
+    if (n < 0 || n > 4) return fail(c, RTS_EINVAL, "rts_set_ctas_per_sm: 0..4");
+    c->user_ctas_per_sm = n;
+    c->planned = false;
+    return RTS_OK;
+}
+
+size_t rts_workspace_bytes(rts_ctx* c)
+{
+    if (!c) return 0;
+    if (!c->planned && make_plan(c) != RTS_OK) return 0;
+    return c->ws_bytes;
+}
+
+int rts_set_workspace(rts_ctx* c, void* ws, size_t bytes)
+{
+    if (!c) return RTS_EINVAL;
+    if (!c->planned) { int rc = make_plan(c); if (rc != RTS_OK) return rc; }
+    if (!ws || ((uintptr_t)ws & 255u) != 0 || bytes < c->ws_bytes)
+        return fail(c, RTS_EINVAL, "rts_set_workspace: null, misaligned or too small");
+    c->ws = (unsigned char*)ws;
+    c->ws_have = bytes;
+    return bind_workspace(c);
+}
+
+int rts_plan_info(rts_ctx* c, int* what, int n)
+{
+    if (!c || !what) return RTS_EINVAL;
+    if (!c->planned) { int rc = make_plan(c); if (rc != RTS_OK) return rc; }
+    const bool needB = true;
+    int v[12] = {(int)c->rounds.size() + 2 + (needB ? 1 : 0), (int)c->rounds.size(), c->ctas_per_sm, (int)c->jobs.size(),
+                 c->threads, c->smem_bytes, c->tp[0].TU, c->tp[1].TU, c->tp[2].TU, c->tp[0].TV, c->tp[1].TV, c->tp[2].TV};
+    for (int i = 0; i < n && i < 12; ++i) what[i] = v[i];
+    return RTS_OK;
+}
+
+int rts_coefficients(rts_ctx* c, const float* rho, const float* T, const float* P, float* kaprho, float* S, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    if (!rho || !T || !P || !kaprho || !S) return fail(c, RTS_EINVAL, "rts_coefficients: null pointer");
+    if (!c->have_tables || !c->ws || !c->planned || !c->maps_ready) return fail(c, RTS_ESTATE, "rts_coefficients: tables/workspace not set");
+    return launch_stage_a(c, rho, T, P, kaprho, S, as_stream(stream));
+}
+
+int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, float* Q, float* Itop, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    if (!rho || !T || !P || !Q) return fail(c, RTS_EINVAL, "rts_solve: null pointer");
+    if (!c->have_tables) return fail(c, RTS_ESTATE, "rts_solve: tables not set");
+    if (!c->ws || !c->planned || !c->maps_ready) return fail(c, RTS_ESTATE, "rts_solve: workspace not set (or configuration changed since)");
+    cudaStream_t st = as_stream(stream);
+    const size_t N = (size_t)c->nx * c->ny * c->nz;
+    unsigned char* ws = c->ws;
+
+    // stage A + switch heights
+    int rc = launch_stage_a(c, rho, T, P, nullptr, nullptr, st);
+    if (rc != RTS_OK) return rc;
+    rts_kstar_kernel<<<1, 32, 0, st>>>((const double*)(ws + c->off_ksum), c->nb, c->nz, c->nblk_a,
+                                       1.0 / ((double)c->nx * c->ny), c->h[2], 5.0, (int*)(ws + c->off_kstar));
+    CUDA_TRY(c, cudaGetLastError());
+
+    // outputs start from zero; x-march sweeps accumulate into the y-fastest QB
+    float* QB = (float*)(ws + c->off_QB);
+    CUDA_TRY(c, cudaMemsetAsync(Q, 0, N * sizeof(float), st));
+    CUDA_TRY(c, cudaMemsetAsync(QB, 0, N * sizeof(float), st));
+    CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 4, st));
+
+    JobDesc* djobs = (JobDesc*)(ws + c->off_jobs);
+    // sweep rounds
+    int* abortf = (int*)(ws + c->off_abort);
+    size_t jbase = 0;
+    for (auto& r : c->rounds) {
+        int nct = 0;
+        for (int ji : r) nct += c->jobs[ji].d.ntiles;
+        // progress counters of the slots used by this round
+        for (size_t sl = 0; sl < r.size(); ++sl)
+            CUDA_TRY(c, cudaMemsetAsync(ws + c->off_slot0 + c->slot_stride * sl + c->slot_prog, 0,
+                                        sizeof(int) * c->jobs[r[sl]].d.ntiles, st));
+        const JobDesc* jp = djobs + jbase;
+        int nj = (int)r.size();
+        void* args[] = {(void*)&c->mapX, (void*)&c->mapY, (void*)&c->mapZ, (void*)&jp, (void*)&nj,
+                        (void*)&Q, (void*)&QB, (void*)&Itop, (void*)&abortf};
+        CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_sweep_kernel, dim3(nct), dim3(c->threads), args,
+                                                (size_t)c->smem_bytes, st));
+        jbase += r.size();
+    }
+    // finalize
+    {
+        dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, c->nz), block(32, 8);
+        rts_finalize_kernel<<<grid, block, 0, st>>>(Q, QB, c->nx, c->ny, c->nz);
+        CUDA_TRY(c, cudaGetLastError());
+    }
+    return RTS_OK;
+}
+
+int rts_sync_check(rts_ctx* c, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    cudaError_t e = cudaStreamSynchronize(as_stream(stream));
+    if (e != cudaSuccess) return fail(c, RTS_ECUDA, std::string("stream sync: ") + cudaGetErrorString(e));
+    if (c->ws) {
+        int ab = 0;
+        e = cudaMemcpy(&ab, c->ws + c->off_abort, sizeof(int), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return fail(c, RTS_ECUDA, std::string("status read: ") + cudaGetErrorString(e));
+        if (ab) return fail(c, RTS_ETIMEOUT, "sweep kernel watchdog fired (a tile waited too long for a neighbour)");
+    }
+    return RTS_OK;
+}
+
+int rts_solve_host(rts_ctx* c, const float* rho, const float* T, const float* P, float* Q, float* Itop, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    if (!rho || !T || !P || !Q) return fail(c, RTS_EINVAL, "rts_solve_host: null pointer");
+    if (!c->ws || !c->planned || !c->maps_ready) return fail(c, RTS_ESTATE, "rts_solve_host: workspace not set");
+    cudaStream_t st = as_stream(stream);
+    const size_t N = (size_t)c->nx * c->ny * c->nz;
+    const size_t nI = (size_t)c->nb * c->n_up * c->ny * c->nx;
+    float* din = (float*)(c->ws + c->off_stage_in);
+    float* dout = (float*)(c->ws + c->off_stage_out);
+    CUDA_TRY(c, cudaMemcpyAsync(din, rho, N * sizeof(float), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(c, cudaMemcpyAsync(din + N, T, N * sizeof(float), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(c, cudaMemcpyAsync(din + 2 * N, P, N * sizeof(float), cudaMemcpyHostToDevice, st));
+    int rc = rts_solve(c, din, din + N, din + 2 * N, dout, Itop ? dout + N : nullptr, stream);
+    if (rc != RTS_OK) return rc;
+    CUDA_TRY(c, cudaMemcpyAsync(Q, dout, N * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (Itop) CUDA_TRY(c, cudaMemcpyAsync(Itop, dout + N, nI * sizeof(float), cudaMemcpyDeviceToHost, st));
+    return rts_sync_check(c, stream);
+}
+
+const char* rts_last_error(const rts_ctx* c)
+{
+    return c ? c->err.c_str() : g_create_err.c_str();
+}
+
+}  // extern "C"

@@ -1,0 +1,249 @@
+"""Thin Python binding of the C-ABI in include/rts.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of librts.so.  PyTorch is used for
+device memory and the current stream only.  There is no fallback: if librts.so is
+missing (and cannot be built) or no CUDA device is present, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_lib = None
+
+RTS_OK = 0
+_ERR = {-1: "RTS_EINVAL", -2: "RTS_ESTATE", -3: "RTS_ECUDA", -4: "RTS_ENOMEM", -5: "RTS_ETIMEOUT"}
+
+EXPORTS = [
+    "rts_create", "rts_destroy", "rts_set_tables", "rts_set_passes", "rts_set_rays", "rts_get_rays",
+    "rts_num_up_rays", "rts_set_tiling", "rts_set_ctas_per_sm", "rts_workspace_bytes",
+    "rts_set_workspace", "rts_solve", "rts_solve_host", "rts_coefficients", "rts_sync_check",
+    "rts_plan_info", "rts_last_error",
+]
+
+
+def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
+    """dlopen librts.so (building it first if it is missing or stale) and declare prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if build_if_missing and not _build.up_to_date():
+        _build.build()
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: build it with `python -m paper_2107_08145_b200.build`")
+    lib = ctypes.CDLL(path)
+    c_void_p, c_int, c_double, c_size_t = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    PF, PD, PI = ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int)
+    lib.rts_create.restype = c_int
+    lib.rts_create.argtypes = [ctypes.POINTER(c_void_p), c_int, c_int, c_int, c_double, c_double, c_double, c_int]
+    lib.rts_destroy.restype = c_int
+    lib.rts_destroy.argtypes = [c_void_p]
+    lib.rts_set_tables.restype = c_int
+    lib.rts_set_tables.argtypes = [c_void_p, c_int, c_int, c_double, c_double, c_double, c_double, PF, PF]
+    lib.rts_set_passes.restype = c_int
+    lib.rts_set_passes.argtypes = [c_void_p, c_int]
+    lib.rts_set_rays.restype = c_int
+    lib.rts_set_rays.argtypes = [c_void_p, c_int, PD, PD]
+    lib.rts_get_rays.restype = c_int
+    lib.rts_get_rays.argtypes = [c_void_p, PI, PD, PD]
+    lib.rts_num_up_rays.restype = c_int
+    lib.rts_num_up_rays.argtypes = [c_void_p]
+    lib.rts_set_tiling.restype = c_int
+    lib.rts_set_tiling.argtypes = [c_void_p, c_int, c_int, c_int]
+    lib.rts_set_ctas_per_sm.restype = c_int
+    lib.rts_set_ctas_per_sm.argtypes = [c_void_p, c_int]
+    lib.rts_workspace_bytes.restype = c_size_t
+    lib.rts_workspace_bytes.argtypes = [c_void_p]
+    lib.rts_set_workspace.restype = c_int
+    lib.rts_set_workspace.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.rts_solve.restype = c_int
+    lib.rts_solve.argtypes = [c_void_p] + [c_void_p] * 5 + [c_void_p]
+    lib.rts_solve_host.restype = c_int
+    lib.rts_solve_host.argtypes = [c_void_p] + [c_void_p] * 5 + [c_void_p]
+    lib.rts_coefficients.restype = c_int
+    lib.rts_coefficients.argtypes = [c_void_p] + [c_void_p] * 5 + [c_void_p]
+    lib.rts_sync_check.restype = c_int
+    lib.rts_sync_check.argtypes = [c_void_p, c_void_p]
+    lib.rts_plan_info.restype = c_int
+    lib.rts_plan_info.argtypes = [c_void_p, PI, c_int]
+    lib.rts_last_error.restype = ctypes.c_char_p
+    lib.rts_last_error.argtypes = [c_void_p]
+    _lib = lib
+    return lib
+
+
+class RTSError(RuntimeError):
+    pass
+
+
+class RTS:
+    """Handle around rts_ctx.  Names follow include/rts.h."""
+
+    def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, nbands: int):
+        import torch
+        if not torch.cuda.is_available():
+            raise RTSError("no CUDA device: the RTS path has no CPU fallback")
+        self._torch = torch
+        self._lib = load_library()
+        self._ctx = ctypes.c_void_p()
+        self.nx, self.ny, self.nz, self.nbands = nx, ny, nz, nbands
+        torch.cuda.init()
+        torch.zeros(1, device="cuda")          # make sure the primary context exists and is current
+        rc = self._lib.rts_create(ctypes.byref(self._ctx), nx, ny, nz, dx, dy, dz, nbands)
+        if rc != RTS_OK:
+            msg = self._lib.rts_last_error(None)
+            raise RTSError(f"rts_create failed: {_ERR.get(rc, rc)}: {msg.decode() if msg else ''}")
+        self._ws = None
+
+    # -- helpers
+    def _check(self, rc: int, what: str):
+        if rc != RTS_OK:
+            msg = self._lib.rts_last_error(self._ctx)
+            raise RTSError(f"{what}: {_ERR.get(rc, rc)}: {msg.decode() if msg else ''}")
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self._lib.rts_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p()
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- configuration
+    def set_tables(self, nT, nP, logT_min, logT_max, logP_min, logP_max, logkappa, bandfrac):
+        lk = np.ascontiguousarray(logkappa, dtype=np.float32)
+        bf = np.ascontiguousarray(bandfrac, dtype=np.float32)
+        assert lk.shape == (self.nbands, nT, nP) and bf.shape == (self.nbands, nT)
+        PF = ctypes.POINTER(ctypes.c_float)
+        self._check(self._lib.rts_set_tables(self._ctx, nT, nP, logT_min, logT_max, logP_min, logP_max,
+                                             lk.ctypes.data_as(PF), bf.ctypes.data_as(PF)), "rts_set_tables")
+
+    def set_passes(self, n: int):
+        self._check(self._lib.rts_set_passes(self._ctx, n), "rts_set_passes")
+
+    def set_rays(self, mu, w):
+        mu = np.ascontiguousarray(mu, dtype=np.float64)
+        w = np.ascontiguousarray(w, dtype=np.float64)
+        PD = ctypes.POINTER(ctypes.c_double)
+        self._check(self._lib.rts_set_rays(self._ctx, mu.shape[0], mu.ctypes.data_as(PD), w.ctypes.data_as(PD)),
+                    "rts_set_rays")
+
+    def get_rays(self) -> Tuple[np.ndarray, np.ndarray]:
+        n = ctypes.c_int()
+        self._check(self._lib.rts_get_rays(self._ctx, ctypes.byref(n), None, None), "rts_get_rays")
+        mu = np.empty((n.value, 3), dtype=np.float64)
+        w = np.empty(n.value, dtype=np.float64)
+        PD = ctypes.POINTER(ctypes.c_double)
+        self._check(self._lib.rts_get_rays(self._ctx, ctypes.byref(n), mu.ctypes.data_as(PD), w.ctypes.data_as(PD)),
+                    "rts_get_rays")
+        return mu, w
+
+    def num_up_rays(self) -> int:
+        return int(self._lib.rts_num_up_rays(self._ctx))
+
+    def set_tiling(self, march: int, tile_u: int, tile_v: int):
+        self._check(self._lib.rts_set_tiling(self._ctx, march, tile_u, tile_v), "rts_set_tiling")
+
+    def set_ctas_per_sm(self, n: int):
+        self._check(self._lib.rts_set_ctas_per_sm(self._ctx, n), "rts_set_ctas_per_sm")
+
+    def workspace_bytes(self) -> int:
+        n = int(self._lib.rts_workspace_bytes(self._ctx))
+        if n == 0:
+            msg = self._lib.rts_last_error(self._ctx)
+            raise RTSError(f"rts_workspace_bytes: {msg.decode() if msg else 'failed'}")
+        return n
+
+    def allocate_workspace(self):
+        """torch-allocated device workspace handed to rts_set_workspace (caller-owned memory)."""
+        n = self.workspace_bytes()
+        self._ws = self._torch.empty(n + 256, dtype=self._torch.uint8, device="cuda")
+        ptr = (self._ws.data_ptr() + 255) // 256 * 256
+        self._check(self._lib.rts_set_workspace(self._ctx, ctypes.c_void_p(ptr), n), "rts_set_workspace")
+
+    def plan_info(self) -> dict:
+        arr = (ctypes.c_int * 12)()
+        self._check(self._lib.rts_plan_info(self._ctx, arr, 12), "rts_plan_info")
+        keys = ["launches", "rounds", "ctas_per_sm", "jobs", "threads", "smem_bytes",
+                "tile_u_x", "tile_u_y", "tile_u_z", "tile_v_x", "tile_v_y", "tile_v_z"]
+        return dict(zip(keys, [int(v) for v in arr]))
+
+    # -- the hot path
+    def _stream(self):
+        return ctypes.c_void_p(self._torch.cuda.current_stream().cuda_stream)
+
+    def solve(self, rho, T, P, Q=None, Itop=None, want_itop: bool = True):
+        """rho, T, P: float32 CUDA tensors [nz][ny][nx].  Returns (Q, Itop) CUDA tensors."""
+        torch = self._torch
+        for t in (rho, T, P):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+            assert tuple(t.shape) == (self.nz, self.ny, self.nx)
+        if self._ws is None:
+            self.allocate_workspace()
+        if Q is None:
+            Q = torch.empty((self.nz, self.ny, self.nx), dtype=torch.float32, device="cuda")
+        if want_itop and Itop is None:
+            Itop = torch.empty((self.nbands, self.num_up_rays(), self.ny, self.nx), dtype=torch.float32, device="cuda")
+        ip = ctypes.c_void_p(Itop.data_ptr()) if (want_itop and Itop is not None) else None
+        self._check(self._lib.rts_solve(self._ctx, ctypes.c_void_p(rho.data_ptr()), ctypes.c_void_p(T.data_ptr()),
+                                        ctypes.c_void_p(P.data_ptr()), ctypes.c_void_p(Q.data_ptr()), ip,
+                                        self._stream()), "rts_solve")
+        return Q, (Itop if want_itop else None)
+
+    def solve_host(self, rho, T, P, Q, Itop=None):
+        """Host numpy / pinned torch buffers in and out (copies inside the call, synchronous)."""
+        if self._ws is None:
+            self.allocate_workspace()
+
+        def ptr(a):
+            if a is None:
+                return None
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.float32 and a.flags.c_contiguous
+                return ctypes.c_void_p(a.ctypes.data)
+            assert (not a.is_cuda) and a.dtype == self._torch.float32 and a.is_contiguous()
+            return ctypes.c_void_p(a.data_ptr())
+        self._check(self._lib.rts_solve_host(self._ctx, ptr(rho), ptr(T), ptr(P), ptr(Q), ptr(Itop), self._stream()),
+                    "rts_solve_host")
+        return Q, Itop
+
+    def coefficients(self, rho, T, P):
+        """Stage A alone: (kaprho, S) float32 CUDA tensors [nb][nz][ny][nx]."""
+        torch = self._torch
+        if self._ws is None:
+            self.allocate_workspace()
+        k = torch.empty((self.nbands, self.nz, self.ny, self.nx), dtype=torch.float32, device="cuda")
+        s = torch.empty_like(k)
+        self._check(self._lib.rts_coefficients(self._ctx, ctypes.c_void_p(rho.data_ptr()), ctypes.c_void_p(T.data_ptr()),
+                                               ctypes.c_void_p(P.data_ptr()), ctypes.c_void_p(k.data_ptr()),
+                                               ctypes.c_void_p(s.data_ptr()), self._stream()), "rts_coefficients")
+        return k, s
+
+    def sync_check(self):
+        self._check(self._lib.rts_sync_check(self._ctx, self._stream()), "rts_sync_check")
+
+
+def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0) -> "RTS":
+    """Create and configure a solver for an `inputs.RTSInputs` problem."""
+    r = RTS(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.nbands)
+    r.set_tables(inp.nT, inp.nP, inp.logT_min, inp.logT_max, inp.logP_min, inp.logP_max, inp.logkappa, inp.bandfrac)
+    r.set_passes(inp.npasses)
+    r.set_rays(inp.mu, inp.wq)
+    if tiling:
+        for march, (tu, tv) in tiling.items():
+            r.set_tiling(march, tu, tv)
+    if ctas_per_sm:
+        r.set_ctas_per_sm(ctas_per_sm)
+    r.allocate_workspace()
+    return r
