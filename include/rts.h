@@ -116,6 +116,12 @@ int rts_coefficients(rts_ctx* ctx, const float* rho_dev, const float* T_dev, con
  * (RTS_OK, RTS_ETIMEOUT if the sweep watchdog fired, RTS_ECUDA). */
 int rts_sync_check(rts_ctx* ctx, void* stream);
 
+/* Per-stage device timing of the last rts_solve (CUDA events recorded on the solve stream
+ * inside rts_solve).  rts_last_timing waits for the solve and fills ms4 (HOST) with
+ * [0] stage A + switch heights, [1] all sweep launches, [2] finalize, [3] whole solve. */
+int rts_enable_timing(rts_ctx* ctx, int on);
+int rts_last_timing(rts_ctx* ctx, float* ms4_host);
+
 /* Plan facts for reporting: what[0] = kernels launched per solve, [1] = sweep rounds,
  * [2] = CTAs per SM of the sweep kernel, [3] = sweep jobs, [4] = threads per CTA,
  * [5] = dynamic shared memory per CTA (bytes), [6..8] = tile_u of march x,y,z,

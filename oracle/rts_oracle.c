@@ -286,28 +286,25 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
     int fail = rc;
     const int ntask = nb * nrays;
     int task;
-#pragma omp parallel for schedule(dynamic, 1)
+#pragma omp parallel for ordered schedule(dynamic, 1)
     for (task = 0; task < ntask; ++task) {
         int b = task / nrays, r = task % nrays;
         double* I = (double*)malloc(sizeof(double) * N);
-        if (!I) {
-#pragma omp atomic write
-            fail = -2;
-            continue;
+        int e = I ? oracle_sweep_ray(nx, ny, nz, dx, dy, dz, mu + 3 * r, npasses,
+                                     kaprho + (size_t)b * N, S + (size_t)b * N, NULL, 0, I)
+                  : -2;
+        if (e == 0 && Itop && upidx[r] >= 0) {
+            double* dst = Itop + ((size_t)b * nup + upidx[r]) * ny * nx;
+            memcpy(dst, I + (size_t)(nz - 1) * ny * nx, sizeof(double) * ny * nx);
         }
-        int e = oracle_sweep_ray(nx, ny, nz, dx, dy, dz, mu + 3 * r, npasses,
-                                 kaprho + (size_t)b * N, S + (size_t)b * N, NULL, 0, I);
-        if (e != 0) {
-#pragma omp atomic write
-            fail = e;
-        } else {
-            if (Itop && upidx[r] >= 0) {
-                double* dst = Itop + ((size_t)b * nup + upidx[r]) * ny * nx;
-                memcpy(dst, I + (size_t)(nz - 1) * ny * nx, sizeof(double) * ny * nx);
+        /* J_b = sum_r w_r I_r accumulated in ray order (deterministic for any thread count) */
+#pragma omp ordered
+        {
+            if (e != 0) fail = e;
+            else {
+                double* Jb = J + (size_t)b * N;
+                for (size_t n = 0; n < N; ++n) Jb[n] += wq[r] * I[n];
             }
-            double* Jb = J + (size_t)b * N;
-#pragma omp critical(oracle_accumulate_J)
-            for (size_t n = 0; n < N; ++n) Jb[n] += wq[r] * I[n];
         }
         free(I);
     }

@@ -70,6 +70,8 @@ struct rts_ctx {
     bool maps_ready = false;
     CUtensorMap mapX, mapY, mapZ;
     cudaEvent_t ev = nullptr;
+    bool timing = false;
+    cudaEvent_t tev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     std::string err;
 };
 
@@ -249,13 +251,16 @@ int make_plan(rts_ctx* c)
                     const long long T = (long long)ntu * ntv;
                     if (T > slots) continue;
                     const int kpr = (int)std::min<long long>(slots / T, njobs_total);   // jobs per round
-                    const int nrounds = (njobs_type[a] + kpr - 1) / kpr;
                     const int quads = ((TU + 3) / 4) * TV;
                     const int iters = (quads + threads - 1) / threads;
-                    // SM time per step ~ CTAs on the busiest SM x (thread iterations + fixed step overhead)
+                    const int warp_iters = (quads + 31) / 32;
+                    // Step-time model (SM clocks): every step pays a fixed exchange latency on the
+                    // CTA's critical path; the SM time-shares its resident CTAs' warp iterations.
                     const double ctas_sm = std::ceil((double)kpr * T / c->sm_count);
-                    const double step = ctas_sm * (iters * 1.0 + 0.15);
-                    const double cst = nrounds * (double)t.n_m * step;
+                    const double t_crit = 4000.0 + 800.0 * iters;
+                    const double t_sm = ctas_sm * warp_iters * 200.0;
+                    const double step = std::max(t_crit, t_sm);
+                    const double cst = ((double)njobs_type[a] / kpr) * (double)t.n_m * step;
                     if (cst < bc * (1 - 1e-9) || (std::fabs(cst - bc) <= 1e-9 * bc && box_elems(TU, TV) < box_elems(bTU, bTV))) {
                         bc = cst; bTU = TU; bTV = TV;
                     }
@@ -507,6 +512,7 @@ int rts_destroy(rts_ctx* c)
     if (c->d_logkappa) cudaFree(c->d_logkappa);
     if (c->d_bandfrac) cudaFree(c->d_bandfrac);
     if (c->ev) cudaEventDestroy(c->ev);
+    for (auto& e : c->tev) if (e) cudaEventDestroy(e);
     delete c;
     return RTS_OK;
 }
@@ -645,11 +651,13 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     unsigned char* ws = c->ws;
 
     // stage A + switch heights
+    if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[0], st));
     int rc = launch_stage_a(c, rho, T, P, nullptr, nullptr, st);
     if (rc != RTS_OK) return rc;
     rts_kstar_kernel<<<1, 32, 0, st>>>((const double*)(ws + c->off_ksum), c->nb, c->nz, c->nblk_a,
                                        1.0 / ((double)c->nx * c->ny), c->h[2], 5.0, (int*)(ws + c->off_kstar));
     CUDA_TRY(c, cudaGetLastError());
+    if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[1], st));
 
     // outputs start from zero; x-march sweeps accumulate into the y-fastest QB
     float* QB = (float*)(ws + c->off_QB);
@@ -659,6 +667,7 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
 
     JobDesc* djobs = (JobDesc*)(ws + c->off_jobs);
     // sweep rounds
+    if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[2], st));
     int* abortf = (int*)(ws + c->off_abort);
     size_t jbase = 0;
     for (auto& r : c->rounds) {
@@ -677,11 +686,33 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
         jbase += r.size();
     }
     // finalize
+    if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[3], st));
     {
         dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, c->nz), block(32, 8);
         rts_finalize_kernel<<<grid, block, 0, st>>>(Q, QB, c->nx, c->ny, c->nz);
         CUDA_TRY(c, cudaGetLastError());
     }
+    if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[4], st));
+    return RTS_OK;
+}
+
+int rts_enable_timing(rts_ctx* c, int on)
+{
+    if (!c) return RTS_EINVAL;
+    if (on) for (auto& e : c->tev) if (!e) CUDA_TRY(c, cudaEventCreate(&e));
+    c->timing = on != 0;
+    return RTS_OK;
+}
+
+int rts_last_timing(rts_ctx* c, float* ms4)
+{
+    if (!c || !ms4) return RTS_EINVAL;
+    if (!c->timing) return fail(c, RTS_ESTATE, "rts_last_timing: timing not enabled");
+    CUDA_TRY(c, cudaEventSynchronize(c->tev[4]));
+    CUDA_TRY(c, cudaEventElapsedTime(&ms4[0], c->tev[0], c->tev[1]));
+    CUDA_TRY(c, cudaEventElapsedTime(&ms4[1], c->tev[2], c->tev[3]));
+    CUDA_TRY(c, cudaEventElapsedTime(&ms4[2], c->tev[3], c->tev[4]));
+    CUDA_TRY(c, cudaEventElapsedTime(&ms4[3], c->tev[0], c->tev[4]));
     return RTS_OK;
 }
 

@@ -108,28 +108,22 @@ def _box3(g: np.ndarray) -> np.ndarray:
 
 
 def _gauss_periodic_axis(g: np.ndarray, sigma_cells: float, axis: int) -> np.ndarray:
+    """Periodic Gaussian smoothing along one axis (exact circular convolution via FFT)."""
+    import scipy.fft as sfft
     n = g.shape[axis]
-    k = np.fft.rfftfreq(n)  # cycles per cell
+    k = sfft.rfftfreq(n)  # cycles per cell
     resp = np.exp(-2.0 * (np.pi * k * sigma_cells) ** 2)
     shape = [1, 1, 1]
     shape[axis] = resp.shape[0]
-    G = np.fft.rfft(g, axis=axis)
+    G = sfft.rfft(g, axis=axis, workers=-1)
     G *= resp.reshape(shape)
-    return np.fft.irfft(G, n=n, axis=axis)
+    return sfft.irfft(G, n=n, axis=axis, workers=-1)
 
 
 def _gauss_replicate_z(g: np.ndarray, sigma_cells: float) -> np.ndarray:
-    r = int(np.ceil(4.0 * sigma_cells))
-    x = np.arange(-r, r + 1, dtype=np.float64)
-    ker = np.exp(-0.5 * (x / sigma_cells) ** 2)
-    ker /= ker.sum()
-    nz = g.shape[0]
-    idx = np.clip(np.arange(-r, nz + r), 0, nz - 1)
-    gp = g[idx]                      # edge-replicated
-    out = np.zeros_like(g)
-    for t in range(2 * r + 1):
-        out += ker[t] * gp[t:t + nz]
-    return out
+    """Gaussian smoothing along z with edge replication (kernel truncated at 4 sigma)."""
+    from scipy.ndimage import gaussian_filter1d
+    return gaussian_filter1d(g, sigma_cells, axis=0, mode="nearest", truncate=4.0)
 
 
 def _granulation(g: np.ndarray, sig_h_cells_x: float, sig_h_cells_y: float,
@@ -137,7 +131,11 @@ def _granulation(g: np.ndarray, sig_h_cells_x: float, sig_h_cells_y: float,
     g = _gauss_periodic_axis(g, sig_h_cells_x, axis=2)
     g = _gauss_periodic_axis(g, sig_h_cells_y, axis=1)
     g = _gauss_replicate_z(g, sig_v_cells)
-    return g
+    # unit standard deviation on every horizontal level: edge replication in z would
+    # otherwise leave ~4x larger fluctuations on the top and bottom planes
+    g = g - g.mean(axis=(1, 2), keepdims=True)
+    sd = g.std(axis=(1, 2), keepdims=True)
+    return g / np.where(sd > 0, sd, 1.0)
 
 
 def _unit_std(g: np.ndarray) -> np.ndarray:

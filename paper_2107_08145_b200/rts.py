@@ -24,7 +24,7 @@ EXPORTS = [
     "rts_create", "rts_destroy", "rts_set_tables", "rts_set_passes", "rts_set_rays", "rts_get_rays",
     "rts_num_up_rays", "rts_set_tiling", "rts_set_ctas_per_sm", "rts_workspace_bytes",
     "rts_set_workspace", "rts_solve", "rts_solve_host", "rts_coefficients", "rts_sync_check",
-    "rts_plan_info", "rts_last_error",
+    "rts_plan_info", "rts_last_error", "rts_enable_timing", "rts_last_timing",
 ]
 
 
@@ -73,6 +73,10 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_sync_check.argtypes = [c_void_p, c_void_p]
     lib.rts_plan_info.restype = c_int
     lib.rts_plan_info.argtypes = [c_void_p, PI, c_int]
+    lib.rts_enable_timing.restype = c_int
+    lib.rts_enable_timing.argtypes = [c_void_p, c_int]
+    lib.rts_last_timing.restype = c_int
+    lib.rts_last_timing.argtypes = [c_void_p, PF]
     lib.rts_last_error.restype = ctypes.c_char_p
     lib.rts_last_error.argtypes = [c_void_p]
     _lib = lib
@@ -229,6 +233,14 @@ class RTS:
                                                ctypes.c_void_p(P.data_ptr()), ctypes.c_void_p(k.data_ptr()),
                                                ctypes.c_void_p(s.data_ptr()), self._stream()), "rts_coefficients")
         return k, s
+
+    def enable_timing(self, on: bool = True):
+        self._check(self._lib.rts_enable_timing(self._ctx, 1 if on else 0), "rts_enable_timing")
+
+    def last_timing(self) -> dict:
+        arr = (ctypes.c_float * 4)()
+        self._check(self._lib.rts_last_timing(self._ctx, arr), "rts_last_timing")
+        return {"stage_a_ms": arr[0], "sweep_ms": arr[1], "finalize_ms": arr[2], "solve_ms": arr[3]}
 
     def sync_check(self):
         self._check(self._lib.rts_sync_check(self._ctx, self._stream()), "rts_sync_check")

@@ -372,7 +372,9 @@ def _ray_perm(mu, M):
 def test_P5_symmetries():
     inp = _small_problem(nx=9, ny=9, nz=8, nb=2)
     Q, Itop = oracle.solve(inp)
-    tol = 1e-11 * np.abs(Q).max()
+    kap, S = oracle.coefficients(inp)
+    # Q = 4 pi kaprho (J - S) carries the rounding of J (sum order differs under a symmetry)
+    tol = 1e-11 * np.abs(Q).max() + 64 * np.finfo(np.float64).eps * (4 * math.pi * kap * S).max()
     # mirror x
     Qm, Im = oracle.solve(_transform(inp, lambda a: a[:, :, ::-1].copy()))
     assert np.abs(Qm - Q[:, :, ::-1]).max() < tol
@@ -395,7 +397,8 @@ def test_P6_translation_invariance_at_seam_convergence():
     Q, Itop = oracle.solve(inp)
     sh = lambda a: np.roll(np.roll(a, 3, axis=2), -2, axis=1)
     Qs, Is = oracle.solve(_transform(inp, sh))
-    assert np.abs(Qs - sh(Q)).max() < 1e-9 * np.abs(Q).max()
+    kap, S = oracle.coefficients(inp)
+    assert np.abs(Qs - sh(Q)).max() < 1e-9 * np.abs(Q).max() + 64 * np.finfo(np.float64).eps * (4 * math.pi * kap * S).max()
     assert np.allclose(Is, np.roll(np.roll(Itop, 3, axis=3), -2, axis=2), rtol=1e-9)
 
 
