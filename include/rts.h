@@ -82,10 +82,10 @@ int rts_get_rays(const rts_ctx* ctx, int* nrays, double* mu_xyz_host, double* we
 /* Number of rays with mu_z > 0 (second extent of I_top). */
 int rts_num_up_rays(const rts_ctx* ctx);
 
-/* Tuning hooks (optional).  march = 0,1,2 selects the sweeps that march along x, y, z;
- * tile_u is the tile extent along the unit-stride transverse axis (multiple of 4, <= 248),
- * tile_v along the other transverse axis (<= 254).  0,0 restores the planner's choice.
- * ctas_per_sm = 0 lets the planner choose.  Invalidates the workspace size. */
+/* Tuning hooks (optional).  march = 0,1,2 selects the sweeps that march along x, y, z.  A sweep
+ * tile is a row band: the full extent of the unit-stride transverse axis times tile_v nodes of
+ * the other transverse axis (1..254; 0 restores the planner's choice); tile_u is ignored.
+ * ctas_per_sm = 0 lets the planner choose (1 or 2).  Both invalidate the workspace size. */
 int rts_set_tiling(rts_ctx* ctx, int march, int tile_u, int tile_v);
 int rts_set_ctas_per_sm(rts_ctx* ctx, int ctas_per_sm);
 
@@ -122,10 +122,10 @@ int rts_sync_check(rts_ctx* ctx, void* stream);
 int rts_enable_timing(rts_ctx* ctx, int on);
 int rts_last_timing(rts_ctx* ctx, float* ms4_host);
 
-/* Plan facts for reporting: what[0] = kernels launched per solve, [1] = sweep rounds,
- * [2] = CTAs per SM of the sweep kernel, [3] = sweep jobs, [4] = threads per CTA,
- * [5] = dynamic shared memory per CTA (bytes), [6..8] = tile_u of march x,y,z,
- * [9..11] = tile_v of march x,y,z.  n = number of ints the caller's array holds. */
+/* Plan facts for reporting: what[0] = kernels launched per solve, [1] = sweep tasks (tiles of
+ * all jobs), [2] = CTAs per SM of the sweep kernel, [3] = sweep jobs, [4] = threads per CTA,
+ * [5] = dynamic shared memory per CTA (bytes), [6] = sweep grid (persistent CTAs),
+ * [7] = exchange-buffer slots, [8..10] = band height of march x,y,z.  n = ints in `what`. */
 int rts_plan_info(rts_ctx* ctx, int* what, int n);
 
 const char* rts_last_error(const rts_ctx* ctx);

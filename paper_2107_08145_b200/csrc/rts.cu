@@ -24,14 +24,14 @@ struct HostRay {
 
 struct TypePlan {        // per march axis
     int n_m = 0, n_u = 0, n_v = 0;
-    int TU = 0, TV = 0, ntu = 0, ntv = 0;
-    int userTU = 0, userTV = 0;
+    int TV = 0, ntv = 0;
+    int userTV = 0;
 };
 
 struct HostJob {
     JobDesc d;
     int nsteps;
-    int round, slot;     // slot = index within its round (selects the exchange buffers)
+    int buf;             // exchange-buffer slot
 };
 
 }  // namespace
@@ -55,20 +55,19 @@ struct rts_ctx {
     bool planned = false;
     TypePlan tp[3];
     std::vector<HostJob> jobs;
-    std::vector<std::vector<int>> rounds;   // job indices per round
-    int ctas_per_sm = 0, threads = 256, smem_bytes = 0, max_round_jobs = 0;
+    int total_tickets = 0, grid = 0, nbuf = 0;
+    int ctas_per_sm = 0, threads = 256, smem_bytes = 0;
     int PX = 0, PY = 0;
     size_t ws_bytes = 0;
     // workspace offsets
     size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_kstar = 0, off_abort = 0,
-           off_jobs = 0, off_slot0 = 0, slot_stride = 0, off_stage_in = 0, off_stage_out = 0;
-    size_t slot_Dg = 0, slot_Gu = 0, slot_Gv = 0, slot_prog = 0;
+           off_jobs = 0, off_prog = 0, off_buf0 = 0, buf_stride = 0, buf_Gu = 0, off_stage_in = 0, off_stage_out = 0;
+    size_t prog_ints = 0;
     int nblk_a = 0;
     // workspace
     unsigned char* ws = nullptr;
     size_t ws_have = 0;
     bool maps_ready = false;
-    CUtensorMap mapX, mapY, mapZ;
     cudaEvent_t ev = nullptr;
     bool timing = false;
     cudaEvent_t tev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -112,7 +111,7 @@ int ray_geometry(const double h[3], HostRay& r)
     r.sv = (r.mu[va] >= 0.0) ? 1 : -1;
     r.fu = r.ds * std::fabs(r.mu[ua]) / h[ua];
     r.fv = r.ds * std::fabs(r.mu[va]) / h[va];
-    r.slot = (r.su < 0 ? 1 : 0) + (r.sv < 0 ? 2 : 0);
+    r.slot = (r.su < 0) ? 1 : 0;
     r.up = (r.mu[2] > 0.0) ? 1 : 0;
     return 0;
 }
@@ -158,48 +157,47 @@ void default_rays(rts_ctx* c)
         }
 }
 
-int box_elems(int TU, int TV) { return (TU + 2 * XPAD) * (TV + 2); }
-int smem_for(int TU, int TV)
+int smem_for(int n_u, int TV)
 {
-    const int BOX = box_elems(TU, TV);
-    const int stage = (2 * BOX + 31) & ~31, xb = (NSLOT * BOX + 31) & ~31;
-    return (2 * stage + 2 * xb) * (int)sizeof(float);
+    const int n_u4 = (n_u + 3) & ~3;
+    const int BOX = (n_u4 + 2 * XPAD) * (TV + 2);
+    const int stage = (2 * BOX + 31) & ~31;
+    return (NSTAGE * stage + NS * BOX) * (int)sizeof(float);
 }
+int blocks_for(int n_u, int TV) { return (((n_u + 3) & ~3) >> 2) * ((TV + 1) >> 1); }
 
 // --------------------------------------------------------------------------- planner
-// Chooses the tile shape per march axis, the CTAs per SM and the packing of jobs into
-// rounds (one cooperative launch each; all CTAs of a round are co-resident).
+// Chooses the band height TV per march axis, builds the job list (ray pairs x bands), the
+// ticket order and the exchange-buffer pool.
 int make_plan(rts_ctx* c)
 {
     c->planned = false;
     c->maps_ready = false;
     const int n[3] = {c->nx, c->ny, c->nz};
-    // --- rays -> geometry, I_top index
     int nup = 0;
     for (auto& r : c->rays) {
         if (ray_geometry(c->h, r) != 0) return fail(c, RTS_EINVAL, "ray with mu_z == 0");
         r.itop = r.up ? nup++ : -1;
     }
     c->n_up = nup;
-    // --- march types
     for (int a = 0; a < 3; ++a) {
         TypePlan& t = c->tp[a];
         t.n_m = n[a];
         t.n_u = (a == 0) ? n[1] : n[0];
         t.n_v = (a == 2) ? n[1] : n[2];
     }
-    c->PX = (int)align_up((size_t)c->nx + 2 * XPAD, 4);
-    c->PY = (int)align_up((size_t)c->ny + 2 * XPAD, 4);
+    c->PX = (int)align_up((size_t)c->nx, 4) + 2 * XPAD;
+    c->PY = (int)align_up((size_t)c->ny, 4) + 2 * XPAD;
 
-    // --- job skeletons: (march, dir) groups, sub-jobs with <= 1 ray per sign slot, bands
-    struct Group { int march, dir; std::vector<std::vector<int>> sub; };
+    // --- job skeletons: (march, dir, sv) groups, sub-jobs with <= 1 ray per u-sign slot
+    struct Group { int march, dir, sv; std::vector<std::vector<int>> sub; };
     std::vector<Group> groups;
     for (int ri = 0; ri < (int)c->rays.size(); ++ri) {
         const HostRay& r = c->rays[ri];
         Group* g = nullptr;
         for (auto& gg : groups)
-            if (gg.march == r.march && gg.dir == r.dir) g = &gg;
-        if (!g) { groups.push_back(Group{r.march, r.dir, {}}); g = &groups.back(); }
+            if (gg.march == r.march && gg.dir == r.dir && gg.sv == r.sv) g = &gg;
+        if (!g) { groups.push_back(Group{r.march, r.dir, r.sv, {}}); g = &groups.back(); }
         bool placed = false;
         for (auto& sub : g->sub) {
             bool freeslot = true;
@@ -208,140 +206,91 @@ int make_plan(rts_ctx* c)
         }
         if (!placed) g->sub.push_back(std::vector<int>{ri});
     }
-    int njobs_type[3] = {0, 0, 0};
-    for (auto& g : groups) njobs_type[g.march] += (int)g.sub.size() * c->nb;
-    const int njobs_total = njobs_type[0] + njobs_type[1] + njobs_type[2];
+    bool used[3] = {false, false, false};
+    for (auto& g : groups) used[g.march] = true;
 
-    // --- occupancy limits of the sweep kernel
+    // --- band height per march axis: one 4x2 block per thread, 2 CTAs per SM if possible
     cudaFuncAttributes fa;
     CUDA_TRY(c, cudaFuncGetAttributes(&fa, rts_sweep_kernel));
-    const int smem_cap_total = c->max_smem_optin;      // per CTA opt-in max (227 KB on sm_100)
     const int threads = 256;
     c->threads = threads;
-
-    // --- search CTAs/SM and tile shapes
-    double best_cost = 1e300;
     int bestR = 0;
-    TypePlan best_tp[3];
-    for (int R = 1; R <= 4; ++R) {
-        if (c->user_ctas_per_sm && R != c->user_ctas_per_sm) continue;
-        // register limit: R CTAs of `threads` threads
+    for (int R = (c->user_ctas_per_sm ? c->user_ctas_per_sm : 2); R >= 1 && !bestR; --R) {
         if ((long long)R * threads * fa.numRegs > 65536) continue;
-        const int smem_cap = std::min(smem_cap_total, (228 * 1024) / R - 1024 - (int)fa.sharedSizeBytes);
-        const int slots = c->sm_count * R;
-        TypePlan tps[3];
-        bool okR = true;
-        double cost = 0.0;
-        for (int a = 0; a < 3 && okR; ++a) {
-            tps[a] = c->tp[a];
-            if (njobs_type[a] == 0) { tps[a].TU = 4; tps[a].TV = 1; tps[a].ntu = tps[a].ntv = 1; continue; }
-            const TypePlan& t = c->tp[a];
-            double bc = 1e300;
-            int bTU = 0, bTV = 0;
-            const int nu4 = (int)align_up((size_t)t.n_u, 4);
-            for (int TU = 4; TU <= std::min(nu4, 248); TU += 4) {
-                if (t.userTU && TU != t.userTU) continue;
-                const int ntu = (t.n_u + TU - 1) / TU;
-                // prefer tile widths that divide the extent evenly
-                if (!t.userTU && (ntu - 1) * TU >= t.n_u) continue;
-                for (int TV = 1; TV <= std::min(t.n_v, 254); ++TV) {
-                    if (t.userTV && TV != t.userTV) continue;
-                    if (smem_for(TU, TV) > smem_cap) break;
-                    const int ntv = (t.n_v + TV - 1) / TV;
-                    const long long T = (long long)ntu * ntv;
-                    if (T > slots) continue;
-                    const int kpr = (int)std::min<long long>(slots / T, njobs_total);   // jobs per round
-                    const int quads = ((TU + 3) / 4) * TV;
-                    const int iters = (quads + threads - 1) / threads;
-                    const int warp_iters = (quads + 31) / 32;
-                    // Step-time model (SM clocks): every step pays a fixed exchange latency on the
-                    // CTA's critical path; the SM time-shares its resident CTAs' warp iterations.
-                    const double ctas_sm = std::ceil((double)kpr * T / c->sm_count);
-                    const double t_crit = 4000.0 + 800.0 * iters;
-                    const double t_sm = ctas_sm * warp_iters * 200.0;
-                    const double step = std::max(t_crit, t_sm);
-                    const double cst = ((double)njobs_type[a] / kpr) * (double)t.n_m * step;
-                    if (cst < bc * (1 - 1e-9) || (std::fabs(cst - bc) <= 1e-9 * bc && box_elems(TU, TV) < box_elems(bTU, bTV))) {
-                        bc = cst; bTU = TU; bTV = TV;
-                    }
-                }
+        const int smem_cap = std::min(c->max_smem_optin, (228 * 1024) / R - 1024 - (int)fa.sharedSizeBytes);
+        bool ok = true;
+        for (int a = 0; a < 3 && ok; ++a) {
+            if (!used[a]) { c->tp[a].TV = 2; c->tp[a].ntv = (c->tp[a].n_v + 1) / 2; continue; }
+            TypePlan& t = c->tp[a];
+            int best = 0;
+            for (int TV = 1; TV <= std::min(t.n_v, 254); ++TV) {
+                if (t.userTV && TV != t.userTV) continue;
+                if (blocks_for(t.n_u, TV) > threads) break;
+                if (smem_for(t.n_u, TV) > smem_cap) break;
+                if (TV > 1 && (TV & 1) && !t.userTV) continue;      // even heights: full 4x2 blocks
+                best = TV;
             }
-            if (bTU == 0) { okR = false; break; }
-            tps[a].TU = bTU; tps[a].TV = bTV;
-            tps[a].ntu = (t.n_u + bTU - 1) / bTU;
-            tps[a].ntv = (t.n_v + bTV - 1) / bTV;
-            cost += bc;
+            if (!best) { ok = false; break; }
+            t.TV = best;
+            t.ntv = (t.n_v + best - 1) / best;
         }
-        if (!okR) continue;
-        {
-            int smemR = 0, occ = 0;
-            for (int a = 0; a < 3; ++a)
-                if (njobs_type[a]) smemR = std::max(smemR, smem_for(tps[a].TU, tps[a].TV));
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, threads, (size_t)smemR) != cudaSuccess || occ < R)
-                continue;
-        }
-        if (cost < best_cost) { best_cost = cost; bestR = R; for (int a = 0; a < 3; ++a) best_tp[a] = tps[a]; }
+        if (ok) bestR = R;
+        if (c->user_ctas_per_sm) break;
     }
-    if (bestR == 0) return fail(c, RTS_EINVAL, "planner: no feasible tiling (grid too large for one wave, or bad override)");
-    for (int a = 0; a < 3; ++a) { best_tp[a].userTU = c->tp[a].userTU; best_tp[a].userTV = c->tp[a].userTV; c->tp[a] = best_tp[a]; }
+    if (!bestR) return fail(c, RTS_EINVAL, "planner: a row band does not fit (grid too wide: n_u <= 1024, or bad override)");
     c->ctas_per_sm = bestR;
-    const int slots = c->sm_count * bestR;
+    c->smem_bytes = 0;
+    for (int a = 0; a < 3; ++a)
+        if (used[a]) c->smem_bytes = std::max(c->smem_bytes, smem_for(c->tp[a].n_u, c->tp[a].TV));
+    {
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, threads, (size_t)c->smem_bytes) != cudaSuccess || occ < 1)
+            return fail(c, RTS_ECUDA, "planner: sweep kernel does not fit on an SM");
+        c->ctas_per_sm = std::min(bestR, occ);
+    }
 
-    // --- materialise jobs
+    // --- materialise jobs in ticket order
     c->jobs.clear();
+    int ticket = 0;
     for (auto& g : groups)
         for (auto& sub : g.sub)
             for (int b = 0; b < c->nb; ++b) {
                 HostJob hj{};
                 JobDesc& d = hj.d;
+                std::memset(&d, 0, sizeof d);
                 const TypePlan& t = c->tp[g.march];
-                d.march = g.march; d.dir = g.dir; d.band = b;
+                d.march = g.march; d.dir = g.dir; d.sv = g.sv; d.band = b;
                 d.n_m = t.n_m; d.n_u = t.n_u; d.n_v = t.n_v;
-                d.TU = t.TU; d.TV = t.TV; d.ntu = t.ntu; d.ntv = t.ntv;
+                d.TV = t.TV; d.ntv = t.ntv;
                 d.per_v = (g.march == 2) ? 1 : 0;
-                d.ntiles = t.ntu * t.ntv;
+                d.ticket_begin = ticket;
+                ticket += t.ntv;
                 d.npass = c->npass;
                 d.nz = c->nz;
-                {
-                    const long long nxy = (long long)c->nx * c->ny;
-                    d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
-                    if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx; }
-                    else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx; }
-                    else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1; }
-                }
-                for (int q = 0; q < NSLOT; ++q) { std::memset(&d.ray[q], 0, sizeof(RayC)); d.ray[q].itop = -1; d.ray[q].dir_row = -1; }
-                for (int ri : sub) {
-                    const HostRay& r = c->rays[ri];
-                    RayC& rc = d.ray[r.slot];
-                    make_ray_consts(r, rc);
-                    rc.dir_row = (g.march == 2) ? -1 : (r.sv > 0 ? 0 : c->nz - 1);
-                }
+                const long long nxy = (long long)c->nx * c->ny;
+                d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
+                const long long PX = c->PX, PY = c->PY;
+                if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx;
+                                         d.c_field = (long long)c->nz * (c->ny + 2) * PX; d.c_m = (long long)(c->ny + 2) * PX; d.c_v = PX; d.c_off = PX; }
+                else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx;
+                                         d.c_field = (long long)c->nz * (c->ny + 2) * PX; d.c_m = PX; d.c_v = (long long)(c->ny + 2) * PX; d.c_off = PX; }
+                else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1;
+                                         d.c_field = (long long)c->nz * c->nx * PY; d.c_m = PY; d.c_v = (long long)c->nx * PY; d.c_off = 0; }
+                for (int q = 0; q < NS; ++q) d.ray[q].itop = -1;
+                for (int ri : sub) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
                 hj.nsteps = t.n_m * c->npass;
                 c->jobs.push_back(hj);
             }
-    // --- pack into rounds: longest jobs first, fill each round up to `slots` CTAs
-    std::vector<int> order(c->jobs.size());
-    for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
-    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return c->jobs[a].nsteps > c->jobs[b].nsteps; });
-    c->rounds.clear();
-    std::vector<int> used;
-    for (int ji : order) {
-        const int T = c->jobs[ji].d.ntiles;
-        int placed = -1;
-        for (size_t r = 0; r < c->rounds.size(); ++r)
-            if (used[r] + T <= slots) { placed = (int)r; break; }
-        if (placed < 0) { c->rounds.emplace_back(); used.push_back(0); placed = (int)c->rounds.size() - 1; }
-        c->jobs[ji].round = placed;
-        c->jobs[ji].slot = (int)c->rounds[placed].size();
-        c->jobs[ji].d.cta_begin = used[placed];
-        c->rounds[placed].push_back(ji);
-        used[placed] += T;
-    }
-    c->max_round_jobs = 0;
-    for (auto& r : c->rounds) c->max_round_jobs = std::max(c->max_round_jobs, (int)r.size());
-    c->smem_bytes = 0;
-    for (int a = 0; a < 3; ++a)
-        if (njobs_type[a]) c->smem_bytes = std::max(c->smem_bytes, smem_for(c->tp[a].TU, c->tp[a].TV));
+    c->total_tickets = ticket;
+    const int slots = c->sm_count * c->ctas_per_sm;
+    c->grid = std::min(slots, c->total_tickets);
+    int max_ntv = 1, min_ntv = 1 << 30;
+    for (auto& hj : c->jobs) { max_ntv = std::max(max_ntv, hj.d.ntv); min_ntv = std::min(min_ntv, hj.d.ntv); }
+    if (max_ntv > c->grid && c->total_tickets > c->grid)
+        return fail(c, RTS_EINVAL, "planner: more row bands per job than resident CTAs (grid too tall)");
+    // exchange-buffer pool: a slot may be reused once the job that held it must have finished
+    c->nbuf = std::min((int)c->jobs.size(), (slots + min_ntv - 1) / min_ntv + 2);
+    for (size_t j = 0; j < c->jobs.size(); ++j) c->jobs[j].buf = (int)(j % c->nbuf);
 
     // --- workspace layout
     const size_t N = (size_t)c->nx * c->ny * c->nz;
@@ -355,24 +304,20 @@ int make_plan(rts_ctx* c)
     c->nblk_a = ((c->nx + 31) / 32) * ((c->ny + 31) / 32);
     c->off_ksum = take(sizeof(double) * (size_t)c->nb * c->nz * c->nblk_a);
     c->off_kstar = take(sizeof(int) * c->nb);
-    c->off_abort = take(sizeof(int) * 4);
+    c->off_abort = take(sizeof(int) * 8);                    // [0] watchdog, [1] ticket counter
     c->off_jobs = take(sizeof(JobDesc) * c->jobs.size());
-    // per round-slot exchange buffers, sized for the largest job type
-    size_t mDg = 0, mGu = 0, mGv = 0, mProg = 0;
+    c->prog_ints = (size_t)c->total_tickets;
+    c->off_prog = take(sizeof(int) * c->prog_ints);
+    size_t mH = 0, mG = 0;
     for (auto& hj : c->jobs) {
         const JobDesc& d = hj.d;
-        mDg = std::max(mDg, (size_t)2 * NSLOT * d.n_v * d.n_u);
-        mGu = std::max(mGu, (size_t)2 * NSLOT * d.n_m * d.n_v);
-        mGv = std::max(mGv, d.per_v ? (size_t)2 * NSLOT * d.n_m * d.n_u : (size_t)0);
-        mProg = std::max(mProg, (size_t)d.ntiles);
+        const size_t n_u4 = (size_t)((d.n_u + 3) & ~3);
+        mH = std::max(mH, (size_t)d.ntv * hj.nsteps * NS * n_u4);
+        mG = std::max(mG, (size_t)d.ntv * 2 * d.n_m * NS * d.TV);
     }
-    c->slot_Dg = 0;
-    c->slot_Gu = align_up(sizeof(float) * mDg, 256);
-    c->slot_Gv = c->slot_Gu + align_up(sizeof(float) * mGu, 256);
-    c->slot_prog = c->slot_Gv + align_up(sizeof(float) * mGv, 256);
-    c->slot_stride = c->slot_prog + align_up(sizeof(int) * mProg, 256);
-    c->off_slot0 = take(c->slot_stride * c->max_round_jobs);
-    // host-API staging (rts_solve_host)
+    c->buf_Gu = align_up(sizeof(float) * mH, 256);
+    c->buf_stride = c->buf_Gu + align_up(sizeof(float) * mG, 256);
+    c->off_buf0 = take(c->buf_stride * c->nbuf);
     c->off_stage_in = take(sizeof(float) * N * 3);
     c->off_stage_out = take(sizeof(float) * (N + (size_t)c->nb * c->n_up * c->ny * c->nx));
     c->ws_bytes = off;
@@ -380,68 +325,23 @@ int make_plan(rts_ctx* c)
     return RTS_OK;
 }
 
-typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-int encode_map(rts_ctx* c, CUtensorMap* map, void* base, const cuuint64_t dims[4], const cuuint32_t box[4])
-{
-    static PFN_encodeTiled fn = nullptr;
-    if (!fn) {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult qr;
-        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr);
-        if (e != cudaSuccess || !p) return fail(c, RTS_ECUDA, "cuTensorMapEncodeTiled entry point not found");
-        fn = (PFN_encodeTiled)p;
-    }
-    cuuint64_t strides[3] = {dims[0] * sizeof(float), dims[0] * dims[1] * sizeof(float),
-                             dims[0] * dims[1] * dims[2] * sizeof(float)};
-    cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-        char buf[96];
-        snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
-        return fail(c, RTS_ECUDA, buf);
-    }
-    return RTS_OK;
-}
-
 int bind_workspace(rts_ctx* c)
 {
     unsigned char* ws = c->ws;
-    // tensor maps
     float* coefA = (float*)(ws + c->off_coefA);
     float* coefB = (float*)(ws + c->off_coefB);
-    {
-        const cuuint64_t dA[4] = {(cuuint64_t)c->PX, (cuuint64_t)c->ny + 2, (cuuint64_t)c->nz, (cuuint64_t)2 * c->nb};
-        const cuuint64_t dB[4] = {(cuuint64_t)c->PY, (cuuint64_t)c->nx, (cuuint64_t)c->nz, (cuuint64_t)2 * c->nb};
-        const TypePlan &tx = c->tp[0], &ty = c->tp[1], &tz = c->tp[2];
-        const cuuint32_t bZ[4] = {(cuuint32_t)tz.TU + 2 * XPAD, (cuuint32_t)tz.TV + 2, 1, 2};
-        const cuuint32_t bY[4] = {(cuuint32_t)ty.TU + 2 * XPAD, 1, (cuuint32_t)ty.TV + 2, 2};
-        const cuuint32_t bX[4] = {(cuuint32_t)tx.TU + 2 * XPAD, 1, (cuuint32_t)tx.TV + 2, 2};
-        int rc;
-        if ((rc = encode_map(c, &c->mapZ, coefA, dA, bZ)) != RTS_OK) return rc;
-        if ((rc = encode_map(c, &c->mapY, coefA, dA, bY)) != RTS_OK) return rc;
-        if ((rc = encode_map(c, &c->mapX, coefB, dB, bX)) != RTS_OK) return rc;
-    }
-    // job descriptors with device pointers (output pointers are patched per solve)
+    std::vector<JobDesc> flat;
     for (auto& hj : c->jobs) {
         JobDesc& d = hj.d;
-        unsigned char* sb = ws + c->off_slot0 + c->slot_stride * hj.slot;
-        d.Dg = (float*)(sb + c->slot_Dg);
-        d.Gu = (float*)(sb + c->slot_Gu);
-        d.Gv = (float*)(sb + c->slot_Gv);
-        d.progress = (int*)(sb + c->slot_prog);
+        unsigned char* sb = ws + c->off_buf0 + c->buf_stride * hj.buf;
+        d.Hrow = (float*)sb;
+        d.Gu = (float*)(sb + c->buf_Gu);
+        d.progress = (int*)(ws + c->off_prog) + d.ticket_begin;
         d.kstar = (const int*)(ws + c->off_kstar) + d.band;
+        d.cbase = ((d.march == 0) ? coefB : coefA) + (size_t)(2 * d.band) * d.c_field;
+        flat.push_back(d);
     }
-    {
-        std::vector<JobDesc> flat;
-        for (auto& r : c->rounds)
-            for (int ji : r) flat.push_back(c->jobs[ji].d);
-        CUDA_TRY(c, cudaMemcpy(ws + c->off_jobs, flat.data(), sizeof(JobDesc) * flat.size(), cudaMemcpyHostToDevice));
-    }
+    CUDA_TRY(c, cudaMemcpy(ws + c->off_jobs, flat.data(), sizeof(JobDesc) * flat.size(), cudaMemcpyHostToDevice));
     c->maps_ready = true;
     return RTS_OK;
 }
@@ -586,9 +486,9 @@ int rts_num_up_rays(const rts_ctx* c)
 int rts_set_tiling(rts_ctx* c, int march, int tile_u, int tile_v)
 {
     if (!c) return RTS_EINVAL;
-    if (march < 0 || march > 2 || tile_u < 0 || tile_v < 0 || (tile_u % 4) != 0 || tile_u > 248 || tile_v > 254)
+    (void)tile_u;   // tiles always span the full unit-stride extent
+    if (march < 0 || march > 2 || tile_v < 0 || tile_v > 254)
         return fail(c, RTS_EINVAL, "rts_set_tiling: bad argument");
-    c->tp[march].userTU = tile_u;
     c->tp[march].userTV = tile_v;
     c->planned = false;
     return RTS_OK;
@@ -597,7 +497,7 @@ int rts_set_tiling(rts_ctx* c, int march, int tile_u, int tile_v)
 int rts_set_ctas_per_sm(rts_ctx* c, int n)
 {
     if (!c) return RTS_EINVAL;
-    if (n < 0 || n > 4) return fail(c, RTS_EINVAL, "rts_set_ctas_per_sm: 0..4");
+    if (n < 0 || n > 2) return fail(c, RTS_EINVAL, "rts_set_ctas_per_sm: 0..2");
     c->user_ctas_per_sm = n;
     c->planned = false;
     return RTS_OK;
@@ -625,9 +525,8 @@ int rts_plan_info(rts_ctx* c, int* what, int n)
 {
     if (!c || !what) return RTS_EINVAL;
     if (!c->planned) { int rc = make_plan(c); if (rc != RTS_OK) return rc; }
-    const bool needB = true;
-    int v[12] = {(int)c->rounds.size() + 2 + (needB ? 1 : 0), (int)c->rounds.size(), c->ctas_per_sm, (int)c->jobs.size(),
-                 c->threads, c->smem_bytes, c->tp[0].TU, c->tp[1].TU, c->tp[2].TU, c->tp[0].TV, c->tp[1].TV, c->tp[2].TV};
+    int v[12] = {4, c->total_tickets, c->ctas_per_sm, (int)c->jobs.size(), c->threads, c->smem_bytes,
+                 c->grid, c->nbuf, c->tp[0].TV, c->tp[1].TV, c->tp[2].TV, 0};
     for (int i = 0; i < n && i < 12; ++i) what[i] = v[i];
     return RTS_OK;
 }
@@ -663,27 +562,17 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     float* QB = (float*)(ws + c->off_QB);
     CUDA_TRY(c, cudaMemsetAsync(Q, 0, N * sizeof(float), st));
     CUDA_TRY(c, cudaMemsetAsync(QB, 0, N * sizeof(float), st));
-    CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 4, st));
+    CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 8, st));
 
-    JobDesc* djobs = (JobDesc*)(ws + c->off_jobs);
-    // sweep rounds
+    CUDA_TRY(c, cudaMemsetAsync(ws + c->off_prog, 0, sizeof(int) * c->prog_ints, st));
+    // the sweep: one persistent launch, tasks handed out by an in-order ticket counter
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[2], st));
-    int* abortf = (int*)(ws + c->off_abort);
-    size_t jbase = 0;
-    for (auto& r : c->rounds) {
-        int nct = 0;
-        for (int ji : r) nct += c->jobs[ji].d.ntiles;
-        // progress counters of the slots used by this round
-        for (size_t sl = 0; sl < r.size(); ++sl)
-            CUDA_TRY(c, cudaMemsetAsync(ws + c->off_slot0 + c->slot_stride * sl + c->slot_prog, 0,
-                                        sizeof(int) * c->jobs[r[sl]].d.ntiles, st));
-        const JobDesc* jp = djobs + jbase;
-        int nj = (int)r.size();
-        void* args[] = {(void*)&c->mapX, (void*)&c->mapY, (void*)&c->mapZ, (void*)&jp, (void*)&nj,
-                        (void*)&Q, (void*)&QB, (void*)&Itop, (void*)&abortf};
-        CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_sweep_kernel, dim3(nct), dim3(c->threads), args,
-                                                (size_t)c->smem_bytes, st));
-        jbase += r.size();
+    {
+        const JobDesc* djobs = (const JobDesc*)(ws + c->off_jobs);
+        int* abortf = (int*)(ws + c->off_abort);
+        rts_sweep_kernel<<<c->grid, c->threads, (size_t)c->smem_bytes, st>>>(
+            djobs, (int)c->jobs.size(), c->total_tickets, abortf + 1, Q, QB, Itop, abortf);
+        CUDA_TRY(c, cudaGetLastError());
     }
     // finalize
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[3], st));

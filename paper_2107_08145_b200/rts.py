@@ -179,8 +179,8 @@ class RTS:
     def plan_info(self) -> dict:
         arr = (ctypes.c_int * 12)()
         self._check(self._lib.rts_plan_info(self._ctx, arr, 12), "rts_plan_info")
-        keys = ["launches", "rounds", "ctas_per_sm", "jobs", "threads", "smem_bytes",
-                "tile_u_x", "tile_u_y", "tile_u_z", "tile_v_x", "tile_v_y", "tile_v_z"]
+        keys = ["launches", "tasks", "ctas_per_sm", "jobs", "threads", "smem_bytes",
+                "grid", "exchange_slots", "tile_v_x", "tile_v_y", "tile_v_z", "reserved"]
         return dict(zip(keys, [int(v) for v in arr]))
 
     # -- the hot path
