@@ -161,8 +161,8 @@ int smem_for(int n_u, int TV)
 {
     const int n_u4 = (n_u + 3) & ~3;
     const int BOX = (n_u4 + 2 * XPAD) * (TV + 2);
-    const int stage = (2 * BOX + 31) & ~31;
-    return (NSTAGE * stage + NS * BOX) * (int)sizeof(float);
+    const int stage = (2 * BOX + 31) & ~31, xf = (NS * BOX + 31) & ~31;
+    return (NSTAGE * stage + xf + 2 * NS * (n_u4 + 2 * XPAD)) * (int)sizeof(float);
 }
 int blocks_for(int n_u, int TV) { return (((n_u + 3) & ~3) >> 2) * ((TV + 1) >> 1); }
 
@@ -223,9 +223,9 @@ int make_plan(rts_ctx* c)
             if (!used[a]) { c->tp[a].TV = 2; c->tp[a].ntv = (c->tp[a].n_v + 1) / 2; continue; }
             TypePlan& t = c->tp[a];
             int best = 0;
-            for (int TV = 1; TV <= std::min(t.n_v, 254); ++TV) {
+            for (int TV = 1; TV <= std::min(t.n_v, 32 * MAXC / NS - 2); ++TV) {
                 if (t.userTV && TV != t.userTV) continue;
-                if (blocks_for(t.n_u, TV) > threads) break;
+                if (blocks_for(t.n_u, TV) > threads - 32) break;          // the last warp communicates
                 if (smem_for(t.n_u, TV) > smem_cap) break;
                 if (TV > 1 && (TV & 1) && !t.userTV) continue;      // even heights: full 4x2 blocks
                 best = TV;
@@ -487,7 +487,7 @@ int rts_set_tiling(rts_ctx* c, int march, int tile_u, int tile_v)
 {
     if (!c) return RTS_EINVAL;
     (void)tile_u;   // tiles always span the full unit-stride extent
-    if (march < 0 || march > 2 || tile_v < 0 || tile_v > 254)
+    if (march < 0 || march > 2 || tile_v < 0 || tile_v > 32 * MAXC / NS - 2)
         return fail(c, RTS_EINVAL, "rts_set_tiling: bad argument");
     c->tp[march].userTV = tile_v;
     c->planned = false;
@@ -614,7 +614,11 @@ int rts_sync_check(rts_ctx* c, void* stream)
         int ab = 0;
         e = cudaMemcpy(&ab, c->ws + c->off_abort, sizeof(int), cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail(c, RTS_ECUDA, std::string("status read: ") + cudaGetErrorString(e));
-        if (ab) return fail(c, RTS_ETIMEOUT, "sweep kernel watchdog fired (a tile waited too long for a neighbour)");
+        if (ab) {
+            char buf[128];
+            snprintf(buf, sizeof buf, "sweep kernel watchdog fired (code %d, step %d): a wait did not complete", ab & 15, ab >> 4);
+            return fail(c, RTS_ETIMEOUT, buf);
+        }
     }
     return RTS_OK;
 }
@@ -638,6 +642,13 @@ int rts_solve_host(rts_ctx* c, const float* rho, const float* T, const float* P,
     if (Itop) CUDA_TRY(c, cudaMemcpyAsync(Itop, dout + N, nI * sizeof(float), cudaMemcpyDeviceToHost, st));
     return rts_sync_check(c, stream);
 }
+
+#ifdef RTS_TRACE
+int rts_debug_trace(unsigned long long* out, int n)
+{
+    return cudaMemcpyFromSymbol(out, rts::g_trace, sizeof(unsigned long long) * n) == cudaSuccess ? 0 : -3;
+}
+#endif
 
 const char* rts_last_error(const rts_ctx* c)
 {

@@ -17,7 +17,7 @@ namespace rts {
 
 constexpr int   NS = 2;             // rays per sweep job: su = +1 (slot 0) and su = -1 (slot 1)
 constexpr int   XPAD = 4;           // ghost columns on each side of the unit-stride axis
-constexpr int   NSTAGE = 3;         // depth of the coefficient-plane ring in shared memory
+constexpr int   NSTAGE = 4;         // depth of the coefficient-plane ring in shared memory
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float FOUR_PI = 12.566370614359172f;
 constexpr float DTAU_SERIES = 0.05f; // below this the psi weights come from their series
@@ -291,44 +291,44 @@ __device__ __forceinline__ void att_series(float dt, float& em1, float& wl, floa
     em1 = dt * wl;
 }
 
-// One node row (4 consecutive nodes) of one ray with u-sign SU.
-//   ko/so, ku/su_ : opacity / source of the previous plane on the node's own row and on its
-//                   upwind row (6 values: columns ul0-1 .. ul0+4)
-//   xo, xu        : carried quantity on the same two rows (6 values)
+// One node row (4 consecutive nodes) of one ray with u-sign SU, in two phases so that the
+// opacity rows are dead before the source / carried rows are loaded (register pressure).
+//   ko/ku : opacity of the previous plane on the node's own row / upwind row (columns ul0-1..ul0+4)
+template <int SU>
+__device__ __forceinline__ void ray_row_dtau(const float (&ko)[6], const float (&ku)[6], const float (&kp)[4],
+                                             const float4 kv, const float kc, float (&dt)[4])
+{
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int c = j + 1, cs = j + 1 - SU;
+        dt[j] = kc * kp[j] + kv.x * ko[c] + kv.y * ko[cs] + kv.z * ku[c] + kv.w * ku[cs];
+    }
+}
+//   so/su_ : source function on the same two rows; xo/xu: carried quantity
 // REG 0: everything in the departure-carried part (a = 1); 1: all direct (a = 0); 2: mixed.
 template <int SU, int REG>
 __device__ __forceinline__ void ray_row_update(
-    const float (&ko)[6], const float (&ku)[6], const float (&so)[6], const float (&su_)[6],
-    const float (&xo)[6], const float (&xu)[6], const float (&kp)[4], const float (&sp)[4],
-    const float4 wv, const float4 kv, const float kc,
-    const float ap, const float a0, const float a1, const unsigned mask, float (&xp)[4])
+    const float (&dt)[4], const float (&so)[6], const float (&su_)[6],
+    const float (&xo)[6], const float (&xu)[6], const float (&sp)[4],
+    const float4 wv, const float ap, const float a0, const float a1, const bool any_small, float (&xp)[4])
 {
-    float Xu[4], dt[4];
-    bool small = false;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int c = j + 1, cs = j + 1 - SU;
-        Xu[j] = wv.x * xo[c] + wv.y * xo[cs] + wv.z * xu[c] + wv.w * xu[cs];
-        dt[j] = kc * kp[j] + kv.x * ko[c] + kv.y * ko[cs] + kv.z * ku[c] + kv.w * ku[cs];
-        small |= dt[j] < DTAU_SERIES;
-    }
-    const bool any_small = __any_sync(mask, small);
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const int c = j + 1, cs = j + 1 - SU;
-        float em1, wl, pu = 0.f, pp = 0.f;
+        const float Xu = wv.x * xo[c] + wv.y * xo[cs] + wv.z * xu[c] + wv.w * xu[cs];
+        float em1, wl;
         att_closed(dt[j], em1, wl);
-        if (REG != 0) { pp = 1.0f - wl; pu = wl - 1.0f + em1; }
+        float pp = 1.0f - wl;
         if (any_small) {
             float e2, w2, pu2, pp2;
             att_series(dt[j], e2, w2, pu2, pp2);
             const bool sm = dt[j] < DTAU_SERIES;
             pp = sm ? pp2 : pp;
-            pu = sm ? pu2 : pu;
             em1 = sm ? e2 : em1;
             wl = sm ? w2 : wl;
         }
-        float v = fmaf(-Xu[j], em1, Xu[j]);
+        const float pu = em1 - pp;                 // psi_u = (1-E)/dt - E = (1 - E) - psi_p
+        float v = fmaf(-Xu, em1, Xu);
         if (REG == 0) {
             float dS = sp[j];
             dS = fmaf(-wv.x, so[c], dS); dS = fmaf(-wv.y, so[cs], dS);
@@ -353,11 +353,11 @@ __device__ __forceinline__ void ray_row_update(
     }
 }
 
-__device__ __forceinline__ bool spin_abort(const int* abortf, unsigned& spins)
+__device__ __forceinline__ bool spin_abort(const int* abortf, unsigned& spins, int code = 1)
 {
     if ((++spins & 1023u) == 0u) {
         if (*reinterpret_cast<const volatile int*>(abortf) != 0) return true;
-        if (spins > (1u << 26)) { atomicExch(const_cast<int*>(abortf), 1); return true; }
+        if (spins > (1u << 22)) { atomicCAS(const_cast<int*>(abortf), 0, code); return true; }
     }
     return false;
 }
@@ -376,78 +376,94 @@ __device__ __forceinline__ void load_row6(const float* __restrict__ row, bool le
     out[0] = l; out[1] = v.x; out[2] = v.y; out[3] = v.z; out[4] = v.w; out[5] = r;
 }
 
+__device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void named_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
+#ifdef RTS_TRACE
+__device__ unsigned long long g_trace[16384];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TRACE(slot) do { if (trace_on && s >= 200 && s < 264) g_trace[((s - 200) * 16) + (slot)] = gtime(); } while (0)
+#else
+#define TRACE(slot) do { } while (0)
+#endif
+constexpr int MAXC = 8;      // ring-column values per lane of the communication warp (NS * (TV + 2) <= 32 * MAXC)
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 template <int SV>
 __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint64_t* mbar, int* s_flag,
                          float* __restrict__ Qa, float* __restrict__ Qb, float* __restrict__ Itop_all,
                          int* abortf)
 {
-    const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
+    const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
+    const int NCW = (nthr >> 5) - 1;                    // compute warps; the last warp communicates
+    const int ncomp = NCW * 32;
+    const bool is_comm = (warp == NCW);
     const int n_u = J.n_u, n_v = J.n_v, n_m = J.n_m, TV = J.TV;
     const int n_u4 = (n_u + 3) & ~3;
+    const int nq4 = n_u4 >> 2;
     const int BOXU = n_u4 + 2 * XPAD, BOXV = TV + 2, BOX = BOXU * BOXV;
     const int b = (SV > 0) ? t : J.ntv - 1 - t;         // row-band index along v
     const int v0 = b * TV;
     const int tv = min(TV, n_v - v0);
     const bool zmarch = (J.march == 2);
-    const int nsteps = n_m * J.npass;
+    const int npass = J.npass;
+    const int nsteps = n_m * npass;
     const int kstar = *J.kstar;
     float* const Qdst = J.q_in_B ? Qb : Qa;
     float* const Itop_b = Itop_all ? Itop_all + (long long)J.band * J.it_sb : nullptr;
     const RayC* const rays = J.ray;
-    const bool has_up = (t > 0) || (J.per_v && J.ntv >= 1);     // an upwind tile (or the seam) exists
-    const int t_up = (t > 0) ? t - 1 : J.ntv - 1;              // its tile index (seam: previous pass)
+    const bool has_up = (t > 0) || J.per_v;             // an upwind tile (or the periodic seam) exists
+    const int t_up = (t > 0) ? t - 1 : J.ntv - 1;
     const bool seam_up = (t == 0);
+    const int dir_row = (SV > 0) ? 0 : J.nz - 1;        // x/y-march: Dirichlet row of this job's rays
+    const bool up_rays = zmarch ? (J.dir > 0) : (SV > 0);
+    const int vr = (SV > 0) ? -1 : tv;                  // ring row (local v)
+    const int ve = (SV > 0) ? tv - 1 : 0;               // downwind edge row (local v)
+    const bool row_outside = !J.per_v && (v0 + vr < 0 || v0 + vr >= n_v);
 
-    // ---- shared memory: [NSTAGE][2][BOX] coefficient planes, [NS][BOX] carried quantity
+    // ---- shared memory: [NSTAGE][2][BOX] coefficient planes, [NS][BOX] carried quantity,
+    //      [2][NS][BOXU] ring row of the carried quantity (double buffered, filled by TMA)
     float* sm_f = reinterpret_cast<float*>(smem_raw);
     const int stage_floats = (2 * BOX + 31) & ~31;
-    float* coef[NSTAGE];
-#pragma unroll
-    for (int i = 0; i < NSTAGE; ++i) coef[i] = sm_f + i * stage_floats;
+    const int x_floats = (NS * BOX + 31) & ~31;
     float* const X = sm_f + NSTAGE * stage_floats;
-    // rows of the box that exist in memory (x/y-march: v = z is bounded; ghost rows stay zero)
-    const int r_lo = (J.per_v || v0 > 0) ? 0 : 1;
-    const int r_hi = (J.per_v || v0 + tv < n_v) ? tv + 1 : tv;  // inclusive box-row range [r_lo, r_hi]
+    float* const Ring = X + x_floats;                   // [2][NS][BOXU]  ring row (double buffered)
+    uint64_t* const ringbar = mbar + NSTAGE;
+    const int r_lo = (J.per_v || v0 > 0) ? 0 : 1;       // box rows that exist in memory
+    const int r_hi = (J.per_v || v0 + tv < n_v) ? tv + 1 : tv;
     const uint32_t row_bytes = (uint32_t)(BOXU * sizeof(float));
     const uint32_t stage_bytes = 2u * (uint32_t)(r_hi - r_lo + 1) * row_bytes;
 
-    for (int i = tid; i < NSTAGE * stage_floats + NS * BOX; i += nthr) sm_f[i] = 0.f;
+    for (int i = tid; i < NSTAGE * stage_floats + x_floats + 2 * NS * BOXU; i += nthr) sm_f[i] = 0.f;
     if (tid == 0) {
-        for (int i = 0; i < NSTAGE; ++i) mbar_init(&mbar[i], 1);
+        for (int i = 0; i < NSTAGE + 2; ++i) mbar_init(&mbar[i], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        s_flag[1] = 0;
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 
-    auto issue_load = [&](int L) {           // L = load number; -1 is the plane "before" step 0
-        const int m = (L < 0) ? n_m - 1 : (L % n_m);
-        const int pl = (J.dir > 0) ? m : n_m - 1 - m;
-        const int st = (L + NSTAGE) % NSTAGE;
+    const float* const csrc0 = J.cbase + J.c_off + (long long)(v0 + r_lo - 1) * J.c_v;
+    auto issue_load = [&](int pl, int st) {             // one lane: rows r_lo..r_hi of both fields
         uint64_t* bar = &mbar[st];
         mbar_expect_tx(bar, stage_bytes);
-        const float* src0 = J.cbase + J.c_off + (long long)pl * J.c_m;
-        for (int f = 0; f < 2; ++f)
-            for (int r = r_lo; r <= r_hi; ++r)
-                bulk_load(coef[st] + f * BOX + r * BOXU, src0 + f * J.c_field + (long long)(v0 + r - 1) * J.c_v,
-                          row_bytes, bar);
+        float* dst = sm_f + st * stage_floats + r_lo * BOXU;
+        const float* src = csrc0 + (long long)pl * J.c_m;
+        for (int r = r_lo; r <= r_hi; ++r) {
+            bulk_load(dst, src, row_bytes, bar);
+            bulk_load(dst + BOX, src + J.c_field, row_bytes, bar);
+            dst += BOXU; src += J.c_v;
+        }
     };
-    auto wait_load = [&](int L) {
-        const int st = (L + NSTAGE) % NSTAGE;
-        const uint32_t par = (uint32_t)(((L + 1) / NSTAGE) & 1);
-        unsigned spins = 0;
-        while (!mbar_try_wait(&mbar[st], par)) { if (spin_abort(abortf, spins)) break; }
-    };
-    if (tid == 0) {
-        issue_load(-1);
-        issue_load(0);
-        if (nsteps > 1) issue_load(1);
+    auto plane_of = [&](int m) { return (J.dir > 0) ? m : n_m - 1 - m; };
+    if (tid == nthr - 32) {
+        issue_load(plane_of(n_m - 1), NSTAGE - 1);      // load -1: the plane "before" step 0
+        issue_load(plane_of(0), 0);
+        if (nsteps > 1) issue_load(plane_of(1 % n_m), 1);
     }
-
-    // ---- this thread's blocks: 4 nodes x 2 rows; uniform trip count per warp
-    const int quads_u = n_u4 >> 2;
-    const int rpairs = (tv + 1) >> 1;
-    const int nblk = quads_u * rpairs;
-    const int nblk_pad = (nblk + 31) & ~31;
 
     int* const my_progress = J.progress + t;
     const int* const up_progress = J.progress + t_up;
@@ -455,214 +471,290 @@ __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint6
     float* const Hmine = J.Hrow + (size_t)t * hrow_tile;
     const float* const Hup = J.Hrow + (size_t)t_up * hrow_tile;
     float* const Gmine = J.Gu + (size_t)t * 2 * n_m * NS * TV;
-    int known_up = 0;                                    // cached progress of the upwind tile
 
-    const float4 w0 = *reinterpret_cast<const float4*>(rays[0].wx), k0 = *reinterpret_cast<const float4*>(rays[0].wk);
-    const float4 w1 = *reinterpret_cast<const float4*>(rays[1].wx), k1 = *reinterpret_cast<const float4*>(rays[1].wk);
-    const float kc0 = rays[0].kc, kc1 = rays[1].kc;
-    const bool act0 = rays[0].active != 0, act1 = rays[1].active != 0;
-    const int dir_row = (SV > 0) ? 0 : J.nz - 1;        // x/y-march: Dirichlet row of this job's rays
-    const bool up_rays = zmarch ? (J.dir > 0) : (SV > 0);
+    // ---- step-invariant geometry of this thread's 4 x 2 block (compute warps)
+    const int quads_u = nq4;
+    const int nblk = quads_u * ((tv + 1) >> 1);
+    const bool blk_valid = (!is_comm) && (tid < nblk);
+    const int ec = min(tid, nblk - 1);
+    const int rp = ec / quads_u, ql = ec - rp * quads_u;
+    const int vl = rp * 2, ul0 = ql * 4;
+    const int base = (vl + 1) * BOXU + ul0 + XPAD;      // box index of (row vl, node ul0)
+    const bool l_ok = blk_valid && (lane > 0) && (ql > 0);
+    const bool r_ok = blk_valid && (lane < 31) && (ql < quads_u - 1) && (tid + 1 < nblk);
+    const int rA = base + ((SV > 0) ? -BOXU : 0);
+    const int rB = rA + BOXU;
+    const int rC = (SV > 0) ? rA + 2 * BOXU : min(rA + 2 * BOXU, (BOXV - 1) * BOXU + ul0 + XPAD);
+    // rows of the carried quantity that are the ring row live in the Ring buffer
+    const int ring_box_row = vr + 1;
+    const bool ringA = (rA / BOXU == ring_box_row), ringB = (rB / BOXU == ring_box_row), ringC = (rC / BOXU == ring_box_row);
+    const int ring_col = ul0 + XPAD;
+    const bool row1_ok = (vl + 1 < tv);
+    const bool full_u = (ul0 + 4 <= n_u);
+    const int nvalid = min(4, n_u - ul0);
+    float a_pi[2] = {0.f, 0.f}, a_1i[2] = {0.f, 0.f};   // x/y-march: masks depend on the row only
+    if (!zmarch) {
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            a_pi[r] = (v0 + vl + r <= kstar) ? 1.f : 0.f;
+            a_1i[r] = (v0 + vl + r - SV <= kstar) ? 1.f : 0.f;
+        }
+    }
+    float* const qbase = Qdst + (long long)(v0 + vl) * J.q_sv + ul0;
 
+    // ---- communication warp, lanes 0 / 1: the corner of the ring row for ray 0 (u = -1) / ray 1 (u = n_u)
+    const int cq = lane & 1;
+    const int c_ringpos = cq * BOXU + (cq ? n_u : -1) + XPAD;           // position inside one Ring buffer
+    const int c_hidx = cq * n_u4 + (cq ? 0 : n_u - 1);                   // far-u node in an edge-row record
+    int c_gvw = v0 + vr; if (c_gvw < 0) c_gvw += n_v; else if (c_gvw >= n_v) c_gvw -= n_v;
+    // ---- compute threads holding a far-u node store its periodic image (ring column) for the next
+    //      step: the thread with u = n_u-1 writes ray 0's column u = -1, the thread with u = 0 writes
+    //      ray 1's column u = n_u
+    const bool seam_l = blk_valid && (ql == 0);
+    const bool seam_r = blk_valid && (ul0 <= n_u - 1) && (n_u - 1 < ul0 + 4);
+    const int colpos_l = (vl + 1) * BOXU + XPAD - 1;                      // box index of (row vl, u = -1)
+    const int colpos_r = BOX + (vl + 1) * BOXU + n_u + XPAD;              // ray 1 array, (row vl, u = n_u)
+
+    // ---- step 0 start-up (all threads): coefficient planes -1 and 0, X^(0)
+    {
+        unsigned spins = 0;
+        while (!mbar_try_wait(&mbar[0], 0u)) { if (spin_abort(abortf, spins, 4)) break; }
+        spins = 0;
+        while (!mbar_try_wait(&mbar[NSTAGE - 1], 0u)) { if (spin_abort(abortf, spins, 5)) break; }
+    }
+    if (!zmarch) {
+        // X^(0) = I^(0) - a S on the plane "before" step 0; its ring row goes to Ring[0]
+        const float* Sp_prev = sm_f + (NSTAGE - 1) * stage_floats + BOX;
+        for (int row = warp; row < BOXV; row += (nthr >> 5)) {
+            const int gv = v0 + row - 1;
+            const float a = (gv <= kstar) ? 1.f : 0.f;
+            const float f = ((gv == dir_row && !up_rays) ? 0.f : 1.f) - a;
+            for (int c = lane; c < BOXU; c += 32) {
+                const float v = f * Sp_prev[row * BOXU + c];
+                X[row * BOXU + c] = v;
+                X[BOX + row * BOXU + c] = v;
+                if (row == ring_box_row) { Ring[c] = v; Ring[BOXU + c] = v; }
+            }
+        }
+    }
+    __syncthreads();
+
+    int m = 0, pass = 0;
+    int stc = 0, stp = NSTAGE - 1;                      // stages of this step's and the previous plane
+    uint32_t par_c = 0;                                 // parity of this step's stage barrier
+    uint32_t ring_par = 0;                              // bit b: parity of ringbar[b] for its next use
+#ifdef RTS_TRACE
+    const bool trace_on = (J.ticket_begin + t == RTS_TRACE) && (lane == 0) && (warp == 0 || is_comm);
+#endif
     for (int s = 0; s < nsteps; ++s) {
-        const int m = s % n_m;
-        const int pass = s / n_m;
-        const int pl = (J.dir > 0) ? m : n_m - 1 - m;
-        const int plprev = pl - J.dir;
-        const int mprev = (m == 0) ? n_m - 1 : m - 1;
-        const float* const Bc = coef[s % NSTAGE];
-        const float* const Bp = coef[(s + NSTAGE - 1) % NSTAGE];
-        const float* const Sp_prev = Bp + BOX;
-        const bool lastpass = (pass == J.npass - 1);
+        const int pl = plane_of(m);
+        const float* const Bc = sm_f + stc * stage_floats;
+        const float* const Bp = sm_f + stp * stage_floats;
+        const bool lastpass = (pass == npass - 1);
         const bool dirichlet_plane = zmarch && (m == 0);
         const float a_pl = (pl <= kstar) ? 1.f : 0.f;
-        const float a_plprev = (plprev <= kstar) ? 1.f : 0.f;
+        const float a_plprev = (pl - J.dir <= kstar) ? 1.f : 0.f;
+        const int m1 = (m + 1 == n_m) ? 0 : m + 1;
+        const int pass1 = (m + 1 == n_m) ? pass + 1 : pass;
+        const int stn = (stc + 1 == NSTAGE) ? 0 : stc + 1;
+        const int rb = s & 1;                           // ring buffer of this step
 
-        wait_load(s);
-        if (s == 0) {
-            wait_load(-1);
-            if (!zmarch) {
-                __syncthreads();
-                // X^(0) = I^(0) - a S on the plane "before" step 0, ring included
-                for (int idx = tid; idx < NS * BOX; idx += nthr) {
-                    const int q = idx / BOX, pos = idx - q * BOX;
-                    const int gv = v0 + pos / BOXU - 1;
-                    const float Sv = Sp_prev[pos];
-                    const float a = (gv <= kstar) ? 1.f : 0.f;
-                    const float I0 = (gv == dir_row && !up_rays) ? 0.f : Sv;
-                    X[idx] = I0 - a * Sv;
-                }
+        if (is_comm) {
+            // ================= communication warp =================
+            TRACE(8);
+            named_bar_sync(0, nthr);                    // B1(s): X(s-1) is in place
+            TRACE(9);
+            if (s > 0 && lane == 0) {                   // publish step s-1 (its edge row was stored before B1)
+                __threadfence();
+                st_release(my_progress, s);
             }
-        } else if (!dirichlet_plane) {
-            // ---- ring row from the upwind tile (or zero outside a bounded domain)
-            const int need = seam_up ? s - n_m : s;     // steps the upwind tile must have published
-            if (has_up && need > 0) {
-                if (tid < 32 && known_up < need) {
+            TRACE(10);
+            if (lane == 0 && s + 2 < nsteps) {          // coefficient planes two steps ahead
+                const int m2 = (m1 + 1 == n_m) ? 0 : m1 + 1;
+                int st2 = stc + 2; if (st2 >= NSTAGE) st2 -= NSTAGE;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                issue_load(plane_of(m2), st2);          // last read in step s-1
+            }
+            // ---- ring row (+ corners) of step s+1 into the other ring buffer
+            if (s + 1 < nsteps) {
+                const bool ring_used = !(zmarch && m1 == 0);          // a Dirichlet plane reads no ring
+                const bool row_pass0 = seam_up && pass1 == 0;
+                const bool row_up = ring_used && has_up && !row_outside && !row_pass0;   // comes from the upwind tile
+                const bool row_tma = row_up && (n_u4 == n_u);                             // (TMA needs whole float4 rows)
+                const int hs = seam_up ? s - n_m : s;   // upwind step whose edge row feeds step s+1
+                uint64_t* rbar = &ringbar[rb ^ 1];
+                float* rdst = Ring + (rb ^ 1) * NS * BOXU;
+                const float* Sp1 = Bc + BOX;            // source function of the plane before step s+1
+                if (row_up) {
+                    const int need = hs + 1;
                     unsigned spins = 0;
                     int v = 0;
                     while (true) {
                         if (lane == 0) v = ld_acquire(up_progress);
                         v = __shfl_sync(0xffffffffu, v, 0);
                         if (v >= need) break;
-                        if (spin_abort(abortf, spins)) break;
+                        if (spin_abort(abortf, spins, 3 | (s << 4))) { if (lane == 0) s_flag[1] = 1; break; }
                         __nanosleep(40);
                     }
-                    if (lane == 0) *s_flag = v;
+                    TRACE(11);
                 }
-                if (known_up < need) {
-                    __syncthreads();
-                    known_up = *s_flag;
-                }
-            }
-            const int vr = (SV > 0) ? -1 : tv;          // ring row (local v) and its box row
-            const int rowpos = (vr + 1) * BOXU + XPAD;
-            const int gvr = v0 + vr;
-            const bool row_outside = !J.per_v && (gvr < 0 || gvr >= n_v);
-            const bool row_pass0 = seam_up && pass == 0;       // seam in v at pass 0: I^(0)
-            const int hs = seam_up ? s - 1 - n_m : s - 1;      // step whose edge row we need
-            for (int idx = tid; idx < NS * (n_u4 >> 2); idx += nthr) {
-                const int q = idx / (n_u4 >> 2), c4 = idx - q * (n_u4 >> 2);
-                float4 val = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (!row_outside) {
-                    if (row_pass0) {
-                        const float4 Sv = *reinterpret_cast<const float4*>(Sp_prev + rowpos + 4 * c4);
-                        const float a = zmarch ? a_plprev : ((gvr <= kstar) ? 1.f : 0.f);
-                        const bool dn = zmarch ? (mprev == 0) : false;
-                        const float f = ((dn && !up_rays) ? 0.f : 1.f) - a;
-                        val = make_float4(f * Sv.x, f * Sv.y, f * Sv.z, f * Sv.w);
-                    } else {
-                        val = __ldcg(reinterpret_cast<const float4*>(Hup + ((size_t)hs * NS + q) * n_u4) + c4);
-                    }
-                }
-                float* dstp = X + q * BOX + rowpos + 4 * c4;
-                if (4 * c4 + 4 <= n_u) *reinterpret_cast<float4*>(dstp) = val;
-                else { const float vv[4] = {val.x, val.y, val.z, val.w}; for (int j = 0; j < n_u - 4 * c4; ++j) dstp[j] = vv[j]; }
-            }
-            // ---- ring columns (periodic seam in u): own far-column history of the previous pass,
-            //      rows -1 .. tv (the ring-row corner belongs to the upwind tile's history)
-            for (int idx = tid; idx < NS * (tv + 2); idx += nthr) {
-                const int q = idx / (tv + 2), vl = idx - q * (tv + 2) - 1;
-                const int su = q ? -1 : 1;
-                const int ul = (su > 0) ? -1 : n_u;
-                const int pos = (vl + 1) * BOXU + ul + XPAD;
-                const int gv = v0 + vl;
-                float val = 0.f;
-                const bool outside = !J.per_v && (gv < 0 || gv >= n_v);
-                if (!outside) {
-                    if (pass == 0) {
-                        const float Sv = Sp_prev[pos];
-                        int gvw = gv; if (gvw < 0) gvw += n_v; else if (gvw >= n_v) gvw -= n_v;
-                        const float a = zmarch ? a_plprev : ((gvw <= kstar) ? 1.f : 0.f);
-                        const bool dn = zmarch ? (mprev == 0) : (gvw == dir_row);
+                // corners: the periodic image in u of the upwind tile's far node, one pass earlier
+                if (ring_used && !row_outside && lane < NS) {
+                    const int hcs = seam_up ? s - n_m : (m1 == 0 ? s : s - n_m);
+                    float val;
+                    if (pass1 > 0 && has_up && hcs >= 0) val = __ldcg(Hup + (size_t)hcs * NS * n_u4 + c_hidx);
+                    else {
+                        const float Sv = Sp1[ring_box_row * BOXU + (cq ? n_u : -1) + XPAD];
+                        const float a = zmarch ? a_pl : ((c_gvw <= kstar) ? 1.f : 0.f);
+                        const bool dn = zmarch ? (m == 0) : (c_gvw == dir_row);
                         val = ((dn && !up_rays) ? 0.f : Sv) - a * Sv;
-                    } else {
-                        const int pb = (pass - 1) & 1;
-                        const int ufar = (su > 0) ? n_u - 1 : 0;
-                        if (vl >= 0 && vl < tv) {
-                            val = __ldcg(Gmine + (((size_t)pb * n_m + mprev) * NS + q) * TV + vl);
-                        } else if (vl == vr && has_up) {
-                            // corner (u and the row both upwind): far-u node of the upwind tile's edge
-                            // row in pass p-1 -- step s-1 if the march plane itself wrapped (m == 0) or the
-                            // row already is the v-seam (then the ring row is pass p-1 too), else s-1-n_m
-                            const int hcs = seam_up ? s - 1 - n_m : (m == 0 ? s - 1 : s - 1 - n_m);
-                            if (hcs >= 0) val = __ldcg(Hup + ((size_t)hcs * NS + q) * n_u4 + ufar);
-                            else {
-                                const float Sv = Sp_prev[pos];
-                                int gvw = gv; if (gvw < 0) gvw += n_v; else if (gvw >= n_v) gvw -= n_v;
-                                const float a = zmarch ? a_plprev : ((gvw <= kstar) ? 1.f : 0.f);
-                                const bool dn = zmarch ? (mprev == 0) : (gvw == dir_row);
-                                val = ((dn && !up_rays) ? 0.f : Sv) - a * Sv;
-                            }
+                    }
+                    rdst[c_ringpos] = val;
+                }
+                if (row_tma) {
+                    __syncwarp();
+                    if (lane == 0) {
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                        mbar_expect_tx(rbar, (uint32_t)(NS * n_u4 * sizeof(float)));
+                        const float* src = Hup + (size_t)hs * NS * n_u4;
+                        bulk_load(rdst + XPAD, src, (uint32_t)(n_u4 * sizeof(float)), rbar);
+                        bulk_load(rdst + BOXU + XPAD, src + n_u4, (uint32_t)(n_u4 * sizeof(float)), rbar);
+                    }
+                } else {
+                    if (row_up) {                       // ragged width: plain copy of the valid nodes
+                        const float* src = Hup + (size_t)hs * NS * n_u4;
+                        for (int c = lane; c < n_u; c += 32) {
+                            rdst[XPAD + c] = __ldcg(src + c);
+                            rdst[BOXU + XPAD + c] = __ldcg(src + n_u4 + c);
+                        }
+                    } else if (ring_used && row_pass0 && !row_outside) {
+                        // seam in v at pass 0: I^(0) of the plane before step s+1 (= this step's plane)
+                        const float a_r = zmarch ? a_pl : ((c_gvw <= kstar) ? 1.f : 0.f);
+                        const float f0 = ((zmarch && m == 0 && !up_rays) ? 0.f : 1.f) - a_r;
+                        for (int c = lane; c < n_u; c += 32) {
+                            const float v = f0 * Sp1[ring_box_row * BOXU + XPAD + c];
+                            rdst[XPAD + c] = v; rdst[BOXU + XPAD + c] = v;
                         }
                     }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(rbar);
                 }
-                X[q * BOX + pos] = val;
             }
-        }
-        __syncthreads();
-
-        // ---- update: every thread a 4 x 2 block, both rays; results stay in registers
-        float xn[2][NS][4];     // [row of the pair][ray][node]
-        int blk_base = 0, blk_vl = 0, blk_ul0 = 0;
-        bool blk_valid = false;
-        // (one block per thread per iteration; results of the LAST iteration are written after the
-        //  barrier, earlier iterations are written straight away into a spare buffer -- not needed:
-        //  the planner sizes tiles so that nblk <= blockDim.x)
-        {
-            const int e = tid;
-            blk_valid = e < nblk;
-            const int ec = blk_valid ? e : nblk - 1;
-            const int rp = ec / quads_u, ql = ec - rp * quads_u;
-            const int vl = rp * 2;
-            blk_vl = vl; blk_ul0 = ql * 4;
-            const int base = (vl + 1) * BOXU + ql * 4 + XPAD;   // box index of (row vl, node ul0)
-            blk_base = base;
-            const unsigned mask = 0xffffffffu;
-            const bool l_ok = (lane > 0) && (ql > 0) && ((e - 1) / quads_u == rp) && (e < nblk);
-            const bool r_ok = (lane < 31) && (ql < quads_u - 1) && (e + 1 < nblk);
-            // rows of the previous plane: A = upwind row of the first node row, B, C
-            //   SV > 0: node rows (vl, vl+1): A = vl-1, B = vl, C = vl+1 ; row 0 uses (B own, A upwind), row 1 uses (C own, B upwind)
-            //   SV < 0: A = vl, B = vl+1, C = vl+2 ; row 0 uses (A own, B upwind), row 1 uses (B own, C upwind)
-            const int rA = base + ((SV > 0) ? -BOXU : 0);
-            const int rC = (SV > 0) ? rA + 2 * BOXU : min(rA + 2 * BOXU, (BOXV - 1) * BOXU + ql * 4 + XPAD);
-            float kA[6], kB[6], kC[6], sA[6], sB[6], sC[6];
-            if (!dirichlet_plane) {
-                load_row6(Bp + rA, l_ok, r_ok, kA);
-                load_row6(Bp + rA + BOXU, l_ok, r_ok, kB);
-                load_row6(Bp + rC, l_ok, r_ok, kC);
-                load_row6(Bp + BOX + rA, l_ok, r_ok, sA);
-                load_row6(Bp + BOX + rA + BOXU, l_ok, r_ok, sB);
-                load_row6(Bp + BOX + rC, l_ok, r_ok, sC);
+            TRACE(12);
+            TRACE(14);
+        } else {
+            // ================= compute warps =================
+            TRACE(0);
+            {
+                unsigned spins = 0;
+                while (!mbar_try_wait(&mbar[stc], par_c)) { if (spin_abort(abortf, spins, 2 | (s << 4))) break; }
+                if (s > 0) {
+                    spins = 0;
+                    while (!mbar_try_wait(&ringbar[rb], (ring_par >> rb) & 1u)) { if (spin_abort(abortf, spins, 6 | (s << 4))) break; }
+                    ring_par ^= (1u << rb);
+                }
             }
-            const float4 kp0v = *reinterpret_cast<const float4*>(Bc + base);
-            const float4 kp1v = *reinterpret_cast<const float4*>(Bc + base + BOXU);
-            const float4 sp0v = *reinterpret_cast<const float4*>(Bc + BOX + base);
-            const float4 sp1v = *reinterpret_cast<const float4*>(Bc + BOX + base + BOXU);
-            const float kp[2][4] = {{kp0v.x, kp0v.y, kp0v.z, kp0v.w}, {kp1v.x, kp1v.y, kp1v.z, kp1v.w}};
-            const float sp[2][4] = {{sp0v.x, sp0v.y, sp0v.z, sp0v.w}, {sp1v.x, sp1v.y, sp1v.z, sp1v.w}};
-            // regime masks per node row
-            float a_p[2], a_0[2], a_1[2];
+            TRACE(1);
+            named_bar_sync(0, nthr);                    // B1(s)
+            TRACE(2);
+            // u-seam threads: periodic image (previous pass) of the far-u node of their two rows for
+            // step s+1; fetched now, stored in the write phase
+            float gcol[2] = {0.f, 0.f};
+            const bool seam_thr = seam_l || seam_r;
+            const int sq = seam_r ? 0 : 1;               // (a 1-quad-wide band has both; ray 1 handled below)
+            if (seam_thr && pass1 > 0 && m1 != 0 && pass1 < npass) {
+                const float* g = Gmine + ((size_t)((pass1 - 1) & 1) * n_m + m) * NS * TV + vl;
+                gcol[0] = __ldcg(g + sq * TV);
+                if (row1_ok) gcol[1] = __ldcg(g + sq * TV + 1);
+            }
+            float gcol2[2] = {0.f, 0.f};
+            const bool both = seam_l && seam_r;
+            if (both && pass1 > 0 && m1 != 0 && pass1 < npass) {
+                const float* g = Gmine + ((size_t)((pass1 - 1) & 1) * n_m + m) * NS * TV + vl;
+                gcol2[0] = __ldcg(g + TV);
+                if (row1_ok) gcol2[1] = __ldcg(g + TV + 1);
+            }
+            float xn[2][NS][4];
+            float a_p[2], a_1[2];
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
-                if (zmarch) { a_p[r] = a_pl; a_0[r] = a_plprev; a_1[r] = a_plprev; }
-                else {
-                    const int gv = v0 + vl + r;
-                    a_p[r] = (gv <= kstar) ? 1.f : 0.f; a_0[r] = a_p[r];
-                    a_1[r] = (gv - SV <= kstar) ? 1.f : 0.f;
-                }
+                a_p[r] = zmarch ? a_pl : a_pi[r];
+                a_1[r] = zmarch ? a_plprev : a_1i[r];
             }
+            const float4 sp0v = *reinterpret_cast<const float4*>(Bc + BOX + base);
+            const float4 sp1v = *reinterpret_cast<const float4*>(Bc + BOX + base + BOXU);
+            const float sp[2][4] = {{sp0v.x, sp0v.y, sp0v.z, sp0v.w}, {sp1v.x, sp1v.y, sp1v.z, sp1v.w}};
             if (!dirichlet_plane) {
-                const float asum = a_p[0] + a_0[0] + a_1[0] + a_p[1] + a_0[1] + a_1[1];
+                // ---- phase 1: optical path of every (row, ray, node)
+                float dt[2][NS][4];
+                {
+                    const float4 kp0v = *reinterpret_cast<const float4*>(Bc + base);
+                    const float4 kp1v = *reinterpret_cast<const float4*>(Bc + base + BOXU);
+                    const float kp[2][4] = {{kp0v.x, kp0v.y, kp0v.z, kp0v.w}, {kp1v.x, kp1v.y, kp1v.z, kp1v.w}};
+                    float kA[6], kB[6], kC[6];
+                    load_row6(Bp + rA, l_ok, r_ok, kA);
+                    load_row6(Bp + rB, l_ok, r_ok, kB);
+                    load_row6(Bp + rC, l_ok, r_ok, kC);
+                    const float4 kv0 = *reinterpret_cast<const float4*>(rays[0].wk);
+                    const float4 kv1 = *reinterpret_cast<const float4*>(rays[1].wk);
+                    const float kc0 = rays[0].kc, kc1 = rays[1].kc;
+                    if (SV > 0) {
+                        ray_row_dtau<+1>(kB, kA, kp[0], kv0, kc0, dt[0][0]); ray_row_dtau<-1>(kB, kA, kp[0], kv1, kc1, dt[0][1]);
+                        ray_row_dtau<+1>(kC, kB, kp[1], kv0, kc0, dt[1][0]); ray_row_dtau<-1>(kC, kB, kp[1], kv1, kc1, dt[1][1]);
+                    } else {
+                        ray_row_dtau<+1>(kA, kB, kp[0], kv0, kc0, dt[0][0]); ray_row_dtau<-1>(kA, kB, kp[0], kv1, kc1, dt[0][1]);
+                        ray_row_dtau<+1>(kB, kC, kp[1], kv0, kc0, dt[1][0]); ray_row_dtau<-1>(kB, kC, kp[1], kv1, kc1, dt[1][1]);
+                    }
+                }
+                bool small = false;
+#pragma unroll
+                for (int r = 0; r < 2; ++r)
+#pragma unroll
+                    for (int q = 0; q < NS; ++q)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) small |= dt[r][q][j] < DTAU_SERIES;
+                const unsigned mask = 0xffffffffu;
+                const bool any_small = __any_sync(mask, small);
+                // ---- phase 2: source function and carried quantity
+                float sA[6], sB[6], sC[6];
+                load_row6(Bp + BOX + rA, l_ok, r_ok, sA);
+                load_row6(Bp + BOX + rB, l_ok, r_ok, sB);
+                load_row6(Bp + BOX + rC, l_ok, r_ok, sC);
+                const float a00 = zmarch ? a_plprev : a_p[0], a01 = zmarch ? a_plprev : a_p[1];
+                const float asum = a_p[0] + a00 + a_1[0] + a_p[1] + a01 + a_1[1];
                 const int reg = (asum == 6.f) ? 0 : (asum == 0.f) ? 1 : 2;
                 const bool all0 = __all_sync(mask, reg == 0);
                 const bool all1 = __all_sync(mask, reg == 1);
 #pragma unroll
                 for (int q = 0; q < NS; ++q) {
-                    if (!(q ? act1 : act0)) continue;
+                    if (!rays[q].active) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) { xn[0][q][j] = 0.f; xn[1][q][j] = 0.f; }
+                        continue;
+                    }
                     const float* Xq = X + q * BOX;
+                    const float* Rq = Ring + (rb * NS + q) * BOXU + ring_col;
                     float xA[6], xB[6], xC[6];
-                    load_row6(Xq + rA, l_ok, r_ok, xA);
-                    load_row6(Xq + rA + BOXU, l_ok, r_ok, xB);
-                    load_row6(Xq + rC, l_ok, r_ok, xC);
-                    const float4 wv = q ? w1 : w0, kv = q ? k1 : k0;
-                    const float kc = q ? kc1 : kc0;
-                    // row 0: own/upwind = (B, A) for SV > 0, (A, B) for SV < 0;  row 1: (C, B) / (B, C)
-#define RTS_ROW(REG, R, KO, KU, SO, SU_, XO, XU)                                                        \
-    if (q == 0) ray_row_update<+1, REG>(KO, KU, SO, SU_, XO, XU, kp[R], sp[R], wv, kv, kc, a_p[R], a_0[R], a_1[R], mask, xn[R][0]); \
-    else        ray_row_update<-1, REG>(KO, KU, SO, SU_, XO, XU, kp[R], sp[R], wv, kv, kc, a_p[R], a_0[R], a_1[R], mask, xn[R][1]);
+                    load_row6(ringA ? Rq : Xq + rA, l_ok, r_ok, xA);
+                    load_row6(ringB ? Rq : Xq + rB, l_ok, r_ok, xB);
+                    load_row6(ringC ? Rq : Xq + rC, l_ok, r_ok, xC);
+                    const float4 wv = *reinterpret_cast<const float4*>(rays[q].wx);
+#define RTS_ROW(REG, R, SO, SU_, XO, XU, A0)                                                             \
+    if (q == 0) ray_row_update<+1, REG>(dt[R][0], SO, SU_, XO, XU, sp[R], wv, a_p[R], A0, a_1[R], any_small, xn[R][0]); \
+    else        ray_row_update<-1, REG>(dt[R][1], SO, SU_, XO, XU, sp[R], wv, a_p[R], A0, a_1[R], any_small, xn[R][1]);
 #define RTS_BLOCK(REG)                                                                                   \
-    if (SV > 0) { RTS_ROW(REG, 0, kB, kA, sB, sA, xB, xA) RTS_ROW(REG, 1, kC, kB, sC, sB, xC, xB) }     \
-    else        { RTS_ROW(REG, 0, kA, kB, sA, sB, xA, xB) RTS_ROW(REG, 1, kB, kC, sB, sC, xB, xC) }
+    if (SV > 0) { RTS_ROW(REG, 0, sB, sA, xB, xA, a00) RTS_ROW(REG, 1, sC, sB, xC, xB, a01) }           \
+    else        { RTS_ROW(REG, 0, sA, sB, xA, xB, a00) RTS_ROW(REG, 1, sB, sC, xB, xC, a01) }
                     if (all0) { RTS_BLOCK(0) } else if (all1) { RTS_BLOCK(1) } else { RTS_BLOCK(2) }
 #undef RTS_BLOCK
 #undef RTS_ROW
                 }
             }
+            TRACE(3);
             // Dirichlet nodes (not updated): I = S (upward, bottom) or I = 0 (downward, top)
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
-                const int gv = v0 + vl + r;
-                const bool dn = dirichlet_plane || (!zmarch && gv == dir_row);
+                const bool dn = dirichlet_plane || (!zmarch && (v0 + vl + r) == dir_row);
                 if (dn) {
 #pragma unroll
                     for (int q = 0; q < NS; ++q)
@@ -674,14 +766,15 @@ __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint6
             if (lastpass && blk_valid) {
 #pragma unroll
                 for (int r = 0; r < 2; ++r) {
-                    if (vl + r >= tv) continue;
+                    if (r == 1 && !row1_ok) continue;
                     const int gv = v0 + vl + r;
-                    const int nvalid = min(4, n_u - blk_ul0);
+                    const float4 kpv = *reinterpret_cast<const float4*>(Bc + base + r * BOXU);
+                    const float kpq[4] = {kpv.x, kpv.y, kpv.z, kpv.w};
                     float qa[4] = {0.f, 0.f, 0.f, 0.f};
                     const float shs = 1.0f - a_p[r];
 #pragma unroll
                     for (int q = 0; q < NS; ++q) {
-                        if (!(q ? act1 : act0)) continue;
+                        if (!rays[q].active) continue;
                         const float wq = rays[q].wq;
 #pragma unroll
                         for (int j = 0; j < 4; ++j) qa[j] = fmaf(wq, xn[r][q][j] - shs * sp[r][j], qa[j]);   // w_r (I - S)
@@ -689,58 +782,85 @@ __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint6
                             const bool top = zmarch ? (m == n_m - 1) : (gv == J.nz - 1);
                             if (top) {
                                 float* dst = Itop_b + (long long)rays[q].itop * J.it_sr + (zmarch ? (long long)gv : (long long)pl) * J.it_so;
-                                for (int j = 0; j < nvalid; ++j) dst[(long long)(blk_ul0 + j) * J.it_su] = xn[r][q][j] + a_p[r] * sp[r][j];
+                                for (int j = 0; j < nvalid; ++j) dst[(long long)(ul0 + j) * J.it_su] = xn[r][q][j] + a_p[r] * sp[r][j];
                             }
                         }
                     }
-                    float* qd_ = Qdst + (long long)pl * J.q_sm + (long long)gv * J.q_sv + blk_ul0;
-                    for (int j = 0; j < nvalid; ++j) atomicAdd(qd_ + j, FOUR_PI * kp[r][j] * qa[j]);
+                    float* qd_ = qbase + (long long)pl * J.q_sm + (long long)r * J.q_sv;
+                    for (int j = 0; j < nvalid; ++j) atomicAdd(qd_ + j, FOUR_PI * kpq[j] * qa[j]);
                 }
             }
-        }
-        __syncthreads();
-
-        // ---- write the carried plane, append the downwind edge row / far columns to the histories
-        if (blk_valid) {
-            const int ve = (SV > 0) ? tv - 1 : 0;          // downwind edge row (local)
+            TRACE(4);
+            named_bar_sync(1, ncomp);                   // every compute warp is done reading X
+            TRACE(5);
+            // ---- carried plane, edge-row and far-column histories
+            if (blk_valid) {
 #pragma unroll
-            for (int r = 0; r < 2; ++r) {
-                const int vl = blk_vl + r;
-                if (vl >= tv) continue;
+                for (int r = 0; r < 2; ++r) {
+                    if (r == 1 && !row1_ok) continue;
 #pragma unroll
-                for (int q = 0; q < NS; ++q) {
-                    if (!(q ? act1 : act0)) continue;
-                    const float4 v4 = make_float4(xn[r][q][0], xn[r][q][1], xn[r][q][2], xn[r][q][3]);
-                    float* xw = X + q * BOX + blk_base + r * BOXU;
-                    if (blk_ul0 + 4 <= n_u) *reinterpret_cast<float4*>(xw) = v4;
-                    else for (int j = 0; j < n_u - blk_ul0; ++j) xw[j] = xn[r][q][j];
-                    if (vl == ve)
-                        __stcg(reinterpret_cast<float4*>(Hmine + ((size_t)s * NS + q) * n_u4) + (blk_ul0 >> 2), v4);
-                    const int ufar = q ? 0 : n_u - 1;
-                    if (ufar >= blk_ul0 && ufar < blk_ul0 + 4)
-                        __stcg(Gmine + (((size_t)(pass & 1) * n_m + m) * NS + q) * TV + vl, xn[r][q][ufar - blk_ul0]);
+                    for (int q = 0; q < NS; ++q) {
+                        if (!rays[q].active) continue;
+                        const float4 v4 = make_float4(xn[r][q][0], xn[r][q][1], xn[r][q][2], xn[r][q][3]);
+                        float* xw = X + q * BOX + base + r * BOXU;
+                        if (full_u) *reinterpret_cast<float4*>(xw) = v4;
+                        else for (int j = 0; j < nvalid; ++j) xw[j] = xn[r][q][j];
+                        if (vl + r == ve)
+                            __stcg(reinterpret_cast<float4*>(Hmine + ((size_t)s * NS + q) * n_u4) + ql, v4);
+                        const int ufar = q ? 0 : n_u - 1;
+                        if (ufar >= ul0 && ufar < ul0 + 4) {
+                            const float vf = xn[r][q][ufar - ul0];
+                            __stcg(Gmine + (((size_t)(pass & 1) * n_m + m) * NS + q) * TV + vl + r, vf);
+                        }
+                    }
+                }
+                // ring columns for step s+1 (periodic image in u, previous pass)
+                if (seam_thr && s + 1 < nsteps) {
+#pragma unroll
+                    for (int side = 0; side < 2; ++side) {
+                        const bool mine = side ? seam_l : seam_r;
+                        if (!mine) continue;
+                        const int q = side;
+#pragma unroll
+                        for (int r = 0; r < 2; ++r) {
+                            if (r == 1 && !row1_ok) continue;
+                            float val;
+                            if (pass1 == 0) {              // previous pass = I^(0) of this step's plane
+                                const int gv = v0 + vl + r;
+                                const float Sv = Bc[BOX + (side ? colpos_r - BOX : colpos_l) + r * BOXU];
+                                const float a = zmarch ? a_pl : ((gv <= kstar) ? 1.f : 0.f);
+                                const bool dn = zmarch ? (m == 0) : (gv == dir_row);
+                                val = ((dn && !up_rays) ? 0.f : Sv) - a * Sv;
+                            } else if (m1 == 0) {          // pass boundary: this step's own far-u value
+                                val = xn[r][q][(q ? 0 : n_u - 1) - ul0];
+                            } else {
+                                val = (both && side) ? gcol2[r] : gcol[r];
+                            }
+                            X[(side ? colpos_r : colpos_l) + r * BOXU] = val;
+                        }
+                    }
                 }
             }
+            TRACE(6);
         }
-        __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            st_release(my_progress, s + 1);
-            if (s + 2 < nsteps) {
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                issue_load(s + 2);
-            }
-        }
-        if ((s & 63) == 63) {       // uniform watchdog check
-            if (tid == 0) s_flag[1] = *reinterpret_cast<const volatile int*>(abortf);
+        // advance the rotating indices
+        m = m1; pass = pass1;
+        stp = stc; stc = stn;
+        if (stc == NSTAGE - 1) par_c ^= 1u;             // stage NSTAGE-1 already served load -1
+        if ((s & 63) == 63) {                           // uniform watchdog check
+            __syncthreads();
+            if (s_flag[1] != 0 || *reinterpret_cast<const volatile int*>(abortf) != 0) { s_flag[1] = 1; }
             __syncthreads();
             if (s_flag[1] != 0) break;
         }
     }
     __syncthreads();
-    if (tid == 0)
-        for (int i = 0; i < NSTAGE; ++i)
+    if (tid == 0) {
+        __threadfence();
+        st_release(my_progress, nsteps);                // the last step's edge row
+        for (int i = 0; i < NSTAGE + 2; ++i)
             asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&mbar[i])) : "memory");
+    }
 }
 
 __global__ void __launch_bounds__(256, 2)
@@ -749,7 +869,7 @@ rts_sweep_kernel(const JobDesc* __restrict__ jobs, int njobs, int total_tickets,
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ JobDesc J;
-    __shared__ __align__(8) uint64_t mbar[NSTAGE];
+    __shared__ __align__(8) uint64_t mbar[NSTAGE + 2];
     __shared__ int s_ticket;
     __shared__ int s_flag[2];
     while (true) {
