@@ -60,7 +60,7 @@ struct rts_ctx {
     int PX = 0, PY = 0;
     size_t ws_bytes = 0;
     // workspace offsets
-    size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_kstar = 0, off_abort = 0,
+    size_t off_coefZ = 0, off_coefY = 0, off_coefX = 0, off_QB = 0, off_ksum = 0, off_kstar = 0, off_abort = 0,
            off_jobs = 0, off_prog = 0, off_buf0 = 0, buf_stride = 0, buf_Gu = 0, off_stage_in = 0, off_stage_out = 0;
     size_t prog_ints = 0;
     int nblk_a = 0;
@@ -270,12 +270,13 @@ int make_plan(rts_ctx* c)
                 const long long nxy = (long long)c->nx * c->ny;
                 d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
                 const long long PX = c->PX, PY = c->PY;
+                // coefficient layouts (one per march axis): rows v contiguous with pitch = box width
                 if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx;
                                          d.c_field = (long long)c->nz * (c->ny + 2) * PX; d.c_m = (long long)(c->ny + 2) * PX; d.c_v = PX; d.c_off = PX; }
                 else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx;
-                                         d.c_field = (long long)c->nz * (c->ny + 2) * PX; d.c_m = PX; d.c_v = (long long)(c->ny + 2) * PX; d.c_off = PX; }
+                                         d.c_field = (long long)c->ny * (c->nz + 2) * PX; d.c_m = (long long)(c->nz + 2) * PX; d.c_v = PX; d.c_off = PX; }
                 else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1;
-                                         d.c_field = (long long)c->nz * c->nx * PY; d.c_m = PY; d.c_v = (long long)c->nx * PY; d.c_off = 0; }
+                                         d.c_field = (long long)c->nx * (c->nz + 2) * PY; d.c_m = (long long)(c->nz + 2) * PY; d.c_v = PY; d.c_off = PY; }
                 for (int q = 0; q < NS; ++q) d.ray[q].itop = -1;
                 for (int ri : sub) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
                 hj.nsteps = t.n_m * c->npass;
@@ -296,10 +297,12 @@ int make_plan(rts_ctx* c)
     const size_t N = (size_t)c->nx * c->ny * c->nz;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
-    const size_t fA = (size_t)c->nz * (c->ny + 2) * c->PX;
-    const size_t fB = (size_t)c->nz * c->nx * c->PY;
-    c->off_coefA = take(sizeof(float) * fA * 2 * c->nb);
-    c->off_coefB = take(sizeof(float) * fB * 2 * c->nb);
+    const size_t fZ = (size_t)c->nz * (c->ny + 2) * c->PX;
+    const size_t fY = (size_t)c->ny * (c->nz + 2) * c->PX;
+    const size_t fX = (size_t)c->nx * (c->nz + 2) * c->PY;
+    c->off_coefZ = take(sizeof(float) * fZ * 2 * c->nb);
+    c->off_coefY = take(sizeof(float) * fY * 2 * c->nb);
+    c->off_coefX = take(sizeof(float) * fX * 2 * c->nb);
     c->off_QB = take(sizeof(float) * N);
     c->nblk_a = ((c->nx + 31) / 32) * ((c->ny + 31) / 32);
     c->off_ksum = take(sizeof(double) * (size_t)c->nb * c->nz * c->nblk_a);
@@ -328,8 +331,7 @@ int make_plan(rts_ctx* c)
 int bind_workspace(rts_ctx* c)
 {
     unsigned char* ws = c->ws;
-    float* coefA = (float*)(ws + c->off_coefA);
-    float* coefB = (float*)(ws + c->off_coefB);
+    float* coefL[3] = {(float*)(ws + c->off_coefX), (float*)(ws + c->off_coefY), (float*)(ws + c->off_coefZ)};
     std::vector<JobDesc> flat;
     for (auto& hj : c->jobs) {
         JobDesc& d = hj.d;
@@ -338,7 +340,7 @@ int bind_workspace(rts_ctx* c)
         d.Gu = (float*)(sb + c->buf_Gu);
         d.progress = (int*)(ws + c->off_prog) + d.ticket_begin;
         d.kstar = (const int*)(ws + c->off_kstar) + d.band;
-        d.cbase = ((d.march == 0) ? coefB : coefA) + (size_t)(2 * d.band) * d.c_field;
+        d.cbase = coefL[d.march] + (size_t)(2 * d.band) * d.c_field;
         flat.push_back(d);
     }
     CUDA_TRY(c, cudaMemcpy(ws + c->off_jobs, flat.data(), sizeof(JobDesc) * flat.size(), cudaMemcpyHostToDevice));
@@ -357,8 +359,11 @@ int launch_stage_a(rts_ctx* c, const float* rho, const float* T, const float* P,
     p.logP_min = c->logP_min; p.inv_dP = (c->nP - 1) / (c->logP_max - c->logP_min);
     p.logkappa = c->d_logkappa; p.bandfrac = c->d_bandfrac;
     p.rho = rho; p.T = T; p.P = P;
-    p.coefA = (float*)(c->ws + c->off_coefA); p.PX = c->PX; p.strideA_f = (long long)c->nz * (c->ny + 2) * c->PX;
-    p.coefB = (float*)(c->ws + c->off_coefB); p.PY = c->PY; p.strideB_f = (long long)c->nz * c->nx * c->PY;
+    p.coefZ = (float*)(c->ws + c->off_coefZ); p.coefY = (float*)(c->ws + c->off_coefY); p.coefX = (float*)(c->ws + c->off_coefX);
+    p.PX = c->PX; p.PY = c->PY;
+    p.strideZ_f = (long long)c->nz * (c->ny + 2) * c->PX;
+    p.strideY_f = (long long)c->ny * (c->nz + 2) * c->PX;
+    p.strideX_f = (long long)c->nx * (c->nz + 2) * c->PY;
     p.ksum = (double*)(c->ws + c->off_ksum);
     p.plain_k = plain_k; p.plain_s = plain_s;
     dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, c->nz), block(32, 8);

@@ -74,12 +74,14 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+// potentially blocking test: the warp is suspended by the hardware for up to ~`hint_ns`
+// (no issue slots are burnt while the SM's other CTA computes)
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity, uint32_t hint_ns = 4000u) {
     uint32_t ok;
     asm volatile("{\n\t.reg .pred p;\n\t"
-                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
                  "selp.u32 %0, 1, 0, p;\n\t}"
-                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity), "r"(hint_ns) : "memory");
     return ok != 0;
 }
 // TMA engine, non-tensor form: contiguous global -> shared copy completing on an mbarrier
@@ -109,19 +111,21 @@ __device__ __forceinline__ float rcp_approx(float x) {
 // =========================================================================== K_a
 // Stage A.  One thread block = a 32x32 (x,y) patch of one z level; 32x8 threads, 4 nodes each.
 // Evaluates the table coordinates, 10^x and T^4 in fp64 and rounds once to fp32 (DESIGN.md,
-// "precision").  Writes kaprho_b, S_b
-//   layout A  coefA[b][f][nz][ny+2][PX]   x fastest, x index offset XPAD, y offset 1, periodic
-//                                          ghost columns / rows filled here
-//   layout B  coefB[b][f][nz][nx][PY]     y fastest, y index offset XPAD, periodic ghosts in y
-// and per-block partial sums of kaprho for K_k.
+// "precision").  Writes kaprho_b, S_b in one layout per march axis, each with the rows of a
+// sweep tile contiguous in memory (so that a tile's plane is one bulk copy per field):
+//   layout Z  [b][f][nz][ny+2][PX]   x fastest (offset XPAD), rows y (offset 1, periodic ghost rows)
+//   layout Y  [b][f][ny][nz+2][PX]   x fastest (offset XPAD), rows z (offset 1, zero pad rows)
+//   layout X  [b][f][nx][nz+2][PY]   y fastest (offset XPAD), rows z (offset 1, zero pad rows)
+// with periodic ghost columns along the fastest axis, and per-block partial sums of kaprho for K_k.
 struct CoefParams {
     int nx, ny, nz, nb, nT, nP;
     double logT_min, inv_dT, logP_min, inv_dP;   // inv_d = (n-1)/(max-min)
     const float* logkappa;   // device [nb][nT][nP]
     const float* bandfrac;   // device [nb][nT]
     const float *rho, *T, *P;
-    float* coefA; int PX; long long strideA_f;   // field stride = nz*(ny+2)*PX
-    float* coefB; int PY; long long strideB_f;   // field stride = nz*nx*PY
+    float* coefZ; float* coefY; float* coefX;
+    int PX, PY;
+    long long strideZ_f, strideY_f, strideX_f;   // field strides
     double* ksum;            // [nb][nz][nblk] partial sums (nblk = gridDim.x*gridDim.y), or null
     float* plain_k; float* plain_s;              // optional [nb][N] outputs (rts_coefficients)
 };
@@ -160,12 +164,15 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
             rho_[r] = (double)p.rho[n];
         }
     }
+    // periodic images of column i along x (layouts Z, Y)
+    const int icols[3] = {i + XPAD, (i < XPAD) ? i + p.nx + XPAD : -1, (i >= p.nx - XPAD) ? i - p.nx + XPAD : -1};
+    const bool zlo = (k == 0), zhi = (k == p.nz - 1);
 
     for (int b = 0; b < p.nb; ++b) {
         const float* L = p.logkappa + (size_t)b * p.nT * p.nP;
         const float* F = p.bandfrac + (size_t)b * p.nT;
-        float* A0 = p.coefA + (size_t)(2 * b) * p.strideA_f;
-        float* A1 = A0 + p.strideA_f;
+        float* Z0 = p.coefZ + (size_t)(2 * b) * p.strideZ_f;  float* Z1 = Z0 + p.strideZ_f;
+        float* Y0 = p.coefY + (size_t)(2 * b) * p.strideY_f;  float* Y1 = Y0 + p.strideY_f;
         double part = 0.0;
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
@@ -182,20 +189,22 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
                 sr = (float)(fb * planck[r]);
                 part += kd;
                 const int j = j0 + ty + 8 * r;
-                // layout A with periodic images
                 const int jrows[3] = {j + 1, (j == 0) ? p.ny + 1 : -1, (j == p.ny - 1) ? 0 : -1};
-                const int icols[3] = {i + XPAD, (i < XPAD && i + p.nx + XPAD < p.PX) ? i + p.nx + XPAD : -1,
-                                      (i >= p.nx - XPAD && i - p.nx + XPAD >= 0) ? i - p.nx + XPAD : -1};
 #pragma unroll
-                for (int a2 = 0; a2 < 3; ++a2) {
-                    if (jrows[a2] < 0) continue;
-                    const size_t rowoff = ((size_t)k * (p.ny + 2) + jrows[a2]) * p.PX;
+                for (int c2 = 0; c2 < 3; ++c2) {
+                    if (icols[c2] < 0) continue;
+                    // layout Z: periodic ghost rows in y
 #pragma unroll
-                    for (int c2 = 0; c2 < 3; ++c2) {
-                        if (icols[c2] < 0) continue;
-                        A0[rowoff + icols[c2]] = kr;
-                        A1[rowoff + icols[c2]] = sr;
+                    for (int a2 = 0; a2 < 3; ++a2) {
+                        if (jrows[a2] < 0) continue;
+                        const size_t o = ((size_t)k * (p.ny + 2) + jrows[a2]) * p.PX + icols[c2];
+                        Z0[o] = kr; Z1[o] = sr;
                     }
+                    // layout Y: rows z, zero pad rows below / above the box
+                    const size_t oy = ((size_t)j * (p.nz + 2) + (k + 1)) * p.PX + icols[c2];
+                    Y0[oy] = kr; Y1[oy] = sr;
+                    if (zlo) { Y0[oy - p.PX] = 0.f; Y1[oy - p.PX] = 0.f; }
+                    if (zhi) { Y0[oy + p.PX] = 0.f; Y1[oy + p.PX] = 0.f; }
                 }
                 if (p.plain_k) {
                     const long long n = ((long long)k * p.ny + j) * p.nx + i;
@@ -219,22 +228,21 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
             const int nblk = gridDim.x * gridDim.y;
             p.ksum[((size_t)b * p.nz + k) * nblk + blockIdx.y * gridDim.x + blockIdx.x] = s;
         }
-        // layout B: transposed write, coalesced along y
-        float* B0 = p.coefB + (size_t)(2 * b) * p.strideB_f;
-        float* B1 = B0 + p.strideB_f;
+        // layout X: transposed write, coalesced along y
+        float* X0 = p.coefX + (size_t)(2 * b) * p.strideX_f;  float* X1 = X0 + p.strideX_f;
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int ii = i0 + ty + 8 * r, jj = j0 + tx;
             if (ii < p.nx && jj < p.ny) {
                 const float kr = tile[0][tx][ty + 8 * r], sr = tile[1][tx][ty + 8 * r];
-                const size_t rowoff = ((size_t)k * p.nx + ii) * p.PY;
-                const int jc[3] = {jj + XPAD, (jj < XPAD && jj + p.ny + XPAD < p.PY) ? jj + p.ny + XPAD : -1,
-                                   (jj >= p.ny - XPAD && jj - p.ny + XPAD >= 0) ? jj - p.ny + XPAD : -1};
+                const size_t rowoff = ((size_t)ii * (p.nz + 2) + (k + 1)) * p.PY;
+                const int jc[3] = {jj + XPAD, (jj < XPAD) ? jj + p.ny + XPAD : -1, (jj >= p.ny - XPAD) ? jj - p.ny + XPAD : -1};
 #pragma unroll
                 for (int c2 = 0; c2 < 3; ++c2) {
                     if (jc[c2] < 0) continue;
-                    B0[rowoff + jc[c2]] = kr;
-                    B1[rowoff + jc[c2]] = sr;
+                    X0[rowoff + jc[c2]] = kr; X1[rowoff + jc[c2]] = sr;
+                    if (zlo) { X0[rowoff - p.PY + jc[c2]] = 0.f; X1[rowoff - p.PY + jc[c2]] = 0.f; }
+                    if (zhi) { X0[rowoff + p.PY + jc[c2]] = 0.f; X1[rowoff + p.PY + jc[c2]] = 0.f; }
                 }
             }
         }
@@ -353,11 +361,13 @@ __device__ __forceinline__ void ray_row_update(
     }
 }
 
+// watchdog for every wait loop: gives up after ~2^20 unsuccessful probes (seconds) and raises
+// the device-side abort flag so that all CTAs drain instead of hanging the GPU
 __device__ __forceinline__ bool spin_abort(const int* abortf, unsigned& spins, int code = 1)
 {
-    if ((++spins & 1023u) == 0u) {
+    if ((++spins & 255u) == 0u) {
         if (*reinterpret_cast<const volatile int*>(abortf) != 0) return true;
-        if (spins > (1u << 22)) { atomicCAS(const_cast<int*>(abortf), 0, code); return true; }
+        if (spins > (1u << 20)) { atomicCAS(const_cast<int*>(abortf), 0, code); return true; }
     }
     return false;
 }
@@ -432,10 +442,9 @@ __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint6
     float* const X = sm_f + NSTAGE * stage_floats;
     float* const Ring = X + x_floats;                   // [2][NS][BOXU]  ring row (double buffered)
     uint64_t* const ringbar = mbar + NSTAGE;
-    const int r_lo = (J.per_v || v0 > 0) ? 0 : 1;       // box rows that exist in memory
-    const int r_hi = (J.per_v || v0 + tv < n_v) ? tv + 1 : tv;
-    const uint32_t row_bytes = (uint32_t)(BOXU * sizeof(float));
-    const uint32_t stage_bytes = 2u * (uint32_t)(r_hi - r_lo + 1) * row_bytes;
+    // the tile's rows (ring rows included; pad / ghost rows exist in memory) are contiguous
+    const uint32_t field_bytes = (uint32_t)((tv + 2) * BOXU * sizeof(float));
+    const uint32_t stage_bytes = 2u * field_bytes;
 
     for (int i = tid; i < NSTAGE * stage_floats + x_floats + 2 * NS * BOXU; i += nthr) sm_f[i] = 0.f;
     if (tid == 0) {
@@ -446,17 +455,14 @@ __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint6
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 
-    const float* const csrc0 = J.cbase + J.c_off + (long long)(v0 + r_lo - 1) * J.c_v;
-    auto issue_load = [&](int pl, int st) {             // one lane: rows r_lo..r_hi of both fields
+    const float* const csrc0 = J.cbase + J.c_off + (long long)(v0 - 1) * J.c_v;
+    auto issue_load = [&](int pl, int st) {             // one lane: the tile's plane, one copy per field
         uint64_t* bar = &mbar[st];
         mbar_expect_tx(bar, stage_bytes);
-        float* dst = sm_f + st * stage_floats + r_lo * BOXU;
+        float* dst = sm_f + st * stage_floats;
         const float* src = csrc0 + (long long)pl * J.c_m;
-        for (int r = r_lo; r <= r_hi; ++r) {
-            bulk_load(dst, src, row_bytes, bar);
-            bulk_load(dst + BOX, src + J.c_field, row_bytes, bar);
-            dst += BOXU; src += J.c_v;
-        }
+        bulk_load(dst, src, field_bytes, bar);
+        bulk_load(dst + BOX, src + J.c_field, field_bytes, bar);
     };
     auto plane_of = [&](int m) { return (J.dir > 0) ? m : n_m - 1 - m; };
     if (tid == nthr - 32) {
@@ -782,12 +788,12 @@ __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint6
                             const bool top = zmarch ? (m == n_m - 1) : (gv == J.nz - 1);
                             if (top) {
                                 float* dst = Itop_b + (long long)rays[q].itop * J.it_sr + (zmarch ? (long long)gv : (long long)pl) * J.it_so;
-                                for (int j = 0; j < nvalid; ++j) dst[(long long)(ul0 + j) * J.it_su] = xn[r][q][j] + a_p[r] * sp[r][j];
+                                _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j < nvalid) dst[(long long)(ul0 + j) * J.it_su] = xn[r][q][j] + a_p[r] * sp[r][j];
                             }
                         }
                     }
                     float* qd_ = qbase + (long long)pl * J.q_sm + (long long)r * J.q_sv;
-                    for (int j = 0; j < nvalid; ++j) atomicAdd(qd_ + j, FOUR_PI * kpq[j] * qa[j]);
+                    _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j < nvalid) atomicAdd(qd_ + j, FOUR_PI * kpq[j] * qa[j]);
                 }
             }
             TRACE(4);
@@ -804,12 +810,13 @@ __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint6
                         const float4 v4 = make_float4(xn[r][q][0], xn[r][q][1], xn[r][q][2], xn[r][q][3]);
                         float* xw = X + q * BOX + base + r * BOXU;
                         if (full_u) *reinterpret_cast<float4*>(xw) = v4;
-                        else for (int j = 0; j < nvalid; ++j) xw[j] = xn[r][q][j];
+                        else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j < nvalid) xw[j] = xn[r][q][j]; }
                         if (vl + r == ve)
                             __stcg(reinterpret_cast<float4*>(Hmine + ((size_t)s * NS + q) * n_u4) + ql, v4);
-                        const int ufar = q ? 0 : n_u - 1;
-                        if (ufar >= ul0 && ufar < ul0 + 4) {
-                            const float vf = xn[r][q][ufar - ul0];
+                        // far-u node of this ray (u = n_u-1 for ray 0, u = 0 for ray 1), static indexing only
+                        if (q ? seam_l : seam_r) {
+                            const float vf = q ? xn[r][1][0]
+                                               : (nvalid == 4 ? xn[r][0][3] : nvalid == 3 ? xn[r][0][2] : nvalid == 2 ? xn[r][0][1] : xn[r][0][0]);
                             __stcg(Gmine + (((size_t)(pass & 1) * n_m + m) * NS + q) * TV + vl + r, vf);
                         }
                     }
@@ -832,7 +839,8 @@ __device__ void run_task(const JobDesc& J, int t, unsigned char* smem_raw, uint6
                                 const bool dn = zmarch ? (m == 0) : (gv == dir_row);
                                 val = ((dn && !up_rays) ? 0.f : Sv) - a * Sv;
                             } else if (m1 == 0) {          // pass boundary: this step's own far-u value
-                                val = xn[r][q][(q ? 0 : n_u - 1) - ul0];
+                                val = q ? xn[r][1][0]
+                                        : (nvalid == 4 ? xn[r][0][3] : nvalid == 3 ? xn[r][0][2] : nvalid == 2 ? xn[r][0][1] : xn[r][0][0]);
                             } else {
                                 val = (both && side) ? gcol2[r] : gcol[r];
                             }
