@@ -121,8 +121,8 @@ def oracle_sample(inp, sample_bands=1):
 
 def run_reference(args, inputs_mod):
     """--impl reference: the oracle on host cores (rank 0 only)."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    from paper_2107_08145_b200 import multi
+    if not multi.reference_arm_runs_here(multi.env_ranks()[0]):
         return 0
     inp = inputs_mod.make_config(args.config)
     sample_bands = 1
@@ -159,12 +159,6 @@ def workload_name(cfg, inp):
             f"24 rays, {inp.npasses} passes")
 
 
-def aggregate(local_ms: float, local_units: float, world: int, reduce_max=None) -> dict:
-    """Whole-job throughput from per-rank times: units of all ranks / max time (weak scaling)."""
-    t = reduce_max(local_ms) if reduce_max is not None else local_ms
-    return {"ms": t, "value": world * local_units / (t * 1e-3)}
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -185,11 +179,9 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2107_08145_b200 import rts
+    from paper_2107_08145_b200 import multi, rts
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, local_rank, world = multi.env_ranks()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --impl ours needs a CUDA device (no CPU fallback exists)")
     torch.cuda.set_device(local_rank)
@@ -197,7 +189,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     # one independent atmosphere per rank (replicas; no data-path collective)
-    inp = inputs_mod.make_config(args.config, seed_offset=1000 * rank)
+    inp = inputs_mod.make_config(args.config, seed_offset=multi.rank_seed_offset(rank))
     tiling = None
     if args.tile:
         tu, tv = (int(x) for x in args.tile.split(","))
@@ -215,11 +207,7 @@ def main():
         torch.cuda.synchronize()
 
     def reduce_max(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return multi.max_over_ranks(x, world, "cuda")
 
     # ---- device-resident timing
     for _ in range(args.warmup):
@@ -241,7 +229,7 @@ def main():
     solver.sync_check()
     clocks = sampler.stop() if rank == 0 else None
     local_ms = ev0.elapsed_time(ev1) / args.steps
-    agg = aggregate(local_ms, float(inp.updates), world, reduce_max)
+    agg = multi.aggregate(local_ms, float(inp.updates), world, "cuda")
 
     # ---- end to end through the host-buffer entry point (pinned buffers, copies timed)
     e2e = None
