@@ -344,6 +344,7 @@ int bind_workspace(rts_ctx* c)
         flat.push_back(d);
     }
     CUDA_TRY(c, cudaMemcpy(ws + c->off_jobs, flat.data(), sizeof(JobDesc) * flat.size(), cudaMemcpyHostToDevice));
+    CUDA_TRY(c, cudaMemset(ws + c->off_abort, 0, sizeof(int) * 8));   // status word: a fresh workspace holds garbage
     c->maps_ready = true;
     return RTS_OK;
 }
