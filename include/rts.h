@@ -83,10 +83,13 @@ int rts_get_rays(const rts_ctx* ctx, int* nrays, double* mu_xyz_host, double* we
 int rts_num_up_rays(const rts_ctx* ctx);
 
 /* Tuning hooks (optional).  march = 0,1,2 selects the sweeps that march along x, y, z.  A sweep
- * tile is a row band: the full extent of the unit-stride transverse axis times tile_v nodes of
- * the other transverse axis (1..254; 0 restores the planner's choice); tile_u is ignored.
- * ctas_per_sm = 0 lets the planner choose (1 or 2).  Both invalidate the workspace size. */
+ * tile is tile_u nodes of the unit-stride transverse axis (rounded up to a multiple of 4,
+ * <= 248) times tile_v nodes of the other transverse axis (<= 120); 0 = the planner's choice.
+ * Tiles exchange halos every `steps` planes (1..4; 0 = default 4) and recompute a halo of that
+ * depth in between.  ctas_per_sm = 0 lets the planner choose (1 or 2).  All three invalidate
+ * the workspace size (call rts_workspace_bytes / rts_set_workspace again). */
 int rts_set_tiling(rts_ctx* ctx, int march, int tile_u, int tile_v);
+int rts_set_exchange_interval(rts_ctx* ctx, int steps);
 int rts_set_ctas_per_sm(rts_ctx* ctx, int ctas_per_sm);
 
 /* Bytes of device workspace the current configuration needs (0 on error). */
@@ -123,9 +126,10 @@ int rts_enable_timing(rts_ctx* ctx, int on);
 int rts_last_timing(rts_ctx* ctx, float* ms4_host);
 
 /* Plan facts for reporting: what[0] = kernels launched per solve, [1] = sweep tasks (tiles of
- * all jobs), [2] = CTAs per SM of the sweep kernel, [3] = sweep jobs, [4] = threads per CTA,
- * [5] = dynamic shared memory per CTA (bytes), [6] = sweep grid (persistent CTAs),
- * [7] = exchange-buffer slots, [8..10] = band height of march x,y,z.  n = ints in `what`. */
+ * all units), [2] = CTAs per SM of the sweep kernel, [3] = sweep units (march axis x direction
+ * x ray group x band), [4] = threads per CTA, [5] = dynamic shared memory per CTA (bytes),
+ * [6] = sweep grid (persistent CTAs), [7] = exchange interval, [8..10] = tile_v of march x,y,z,
+ * [11..13] = tile_u of march x,y,z.  n = ints in `what` (<= 16). */
 int rts_plan_info(rts_ctx* ctx, int* what, int n);
 
 const char* rts_last_error(const rts_ctx* ctx);

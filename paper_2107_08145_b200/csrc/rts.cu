@@ -1,8 +1,9 @@
-// rts.cu -- host side of the C-ABI in include/rts.h: ray geometry, job list, planner,
-// workspace layout, TMA descriptors, launches.  All arithmetic of the path runs in the
-// kernels of rts_kernels.cuh; nothing here (or anywhere in the product) touches oracle/.
+// rts.cu -- host side of the C-ABI in include/rts.h: ray geometry, sweep units, planner,
+// workspace layout, launches.  All arithmetic of the path runs in the kernels of
+// rts_kernels.cuh / rts_sweep.cuh; nothing here (or anywhere in the product) touches oracle/.
 #include "../../include/rts.h"
 #include "rts_kernels.cuh"
+#include "rts_sweep.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -24,14 +25,14 @@ struct HostRay {
 
 struct TypePlan {        // per march axis
     int n_m = 0, n_u = 0, n_v = 0;
-    int TV = 0, ntv = 0;
-    int userTV = 0;
+    int WU = 0, WV = 0, ntu = 0, ntv = 0;
+    int userWU = 0, userWV = 0;
+    int items = 0;       // 4 x 2 node blocks of a full tile (halo included)
 };
 
-struct HostJob {
-    JobDesc d;
-    int nsteps;
-    int buf;             // exchange-buffer slot
+struct HostUnit {
+    UnitDesc d;
+    size_t off_xex, off_g;   // workspace offsets of its exchange planes and seam histories
 };
 
 }  // namespace
@@ -50,19 +51,18 @@ struct rts_ctx {
     float* d_bandfrac = nullptr;
     // device facts
     int sm_count = 0, max_smem_optin = 0;
-    int user_ctas_per_sm = 0;
+    int user_ctas_per_sm = 0, user_K = 0;
     // plan
     bool planned = false;
     TypePlan tp[3];
-    std::vector<HostJob> jobs;
-    int total_tickets = 0, grid = 0, nbuf = 0;
+    std::vector<HostUnit> units;
+    int total_tickets = 0, grid = 0, K = KMAX;
     int ctas_per_sm = 0, threads = 256, smem_bytes = 0;
-    int PX = 0, PY = 0;
+    int PX = 0, PY = 0, PYR = 0;
     size_t ws_bytes = 0;
     // workspace offsets
-    size_t off_coefZ = 0, off_coefY = 0, off_coefX = 0, off_QB = 0, off_ksum = 0, off_kstar = 0, off_abort = 0,
-           off_jobs = 0, off_prog = 0, off_buf0 = 0, buf_stride = 0, buf_Gu = 0, off_stage_in = 0, off_stage_out = 0;
-    size_t prog_ints = 0;
+    size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_lev = 0, off_kstar = 0, off_abort = 0,
+           off_units = 0, off_bar = 0, off_stage_in = 0, off_stage_out = 0;
     int nblk_a = 0;
     // workspace
     unsigned char* ws = nullptr;
@@ -111,7 +111,7 @@ int ray_geometry(const double h[3], HostRay& r)
     r.sv = (r.mu[va] >= 0.0) ? 1 : -1;
     r.fu = r.ds * std::fabs(r.mu[ua]) / h[ua];
     r.fv = r.ds * std::fabs(r.mu[va]) / h[va];
-    r.slot = (r.su < 0) ? 1 : 0;
+    r.slot = ((r.su < 0) ? 1 : 0) + ((r.sv < 0) ? 2 : 0);
     r.up = (r.mu[2] > 0.0) ? 1 : 0;
     return 0;
 }
@@ -157,18 +157,18 @@ void default_rays(rts_ctx* c)
         }
 }
 
-int smem_for(int n_u, int TV)
+// dynamic shared memory of a CTA whose tiles are WU x WV: guard rows, NSTAGE coefficient planes
+// (2 fields), the double-buffered carried planes of NSLOT rays, the ghost table
+int smem_for(int WU, int WV)
 {
-    const int n_u4 = (n_u + 3) & ~3;
-    const int BOX = (n_u4 + 2 * XPAD) * (TV + 2);
-    const int stage = (2 * BOX + 31) & ~31, xf = (NS * BOX + 31) & ~31;
-    return (NSTAGE * stage + xf + 2 * NS * (n_u4 + 2 * XPAD)) * (int)sizeof(float);
+    const int BU = WU + 2 * HALO, BV = WV + 2 * HALO, BOX = BU * BV;
+    return (2 * BU + (NSTAGE * 2 + 2 * NSLOT) * BOX) * (int)sizeof(float) + NSLOT * (BU + BV) * (int)sizeof(GhostEnt);
 }
-int blocks_for(int n_u, int TV) { return (((n_u + 3) & ~3) >> 2) * ((TV + 1) >> 1); }
+int items_for(int WU, int WV, int K) { return ((WU + HALO) / 4 + 1) * ((WV + K + 2) / 2); }
 
 // --------------------------------------------------------------------------- planner
-// Chooses the band height TV per march axis, builds the job list (ray pairs x bands), the
-// ticket order and the exchange-buffer pool.
+// Groups the rays into sweep units (march axis, direction, one ray per sign pair), chooses the
+// tile shape per march axis and the CTA size, lays out the workspace.
 int make_plan(rts_ctx* c)
 {
     c->planned = false;
@@ -186,18 +186,20 @@ int make_plan(rts_ctx* c)
         t.n_u = (a == 0) ? n[1] : n[0];
         t.n_v = (a == 2) ? n[1] : n[2];
     }
-    c->PX = (int)align_up((size_t)c->nx, 4) + 2 * XPAD;
-    c->PY = (int)align_up((size_t)c->ny, 4) + 2 * XPAD;
+    c->PX = (int)align_up((size_t)c->nx, 4) + 2 * HALO;
+    c->PY = (int)align_up((size_t)c->ny, 4) + 2 * HALO;
+    c->PYR = c->ny + 2 * HALO;
+    c->K = c->user_K ? c->user_K : KMAX;
 
-    // --- job skeletons: (march, dir, sv) groups, sub-jobs with <= 1 ray per u-sign slot
-    struct Group { int march, dir, sv; std::vector<std::vector<int>> sub; };
+    // --- unit skeletons: (march, dir) groups, sub-units with <= 1 ray per slot
+    struct Group { int march, dir; std::vector<std::vector<int>> sub; };
     std::vector<Group> groups;
     for (int ri = 0; ri < (int)c->rays.size(); ++ri) {
         const HostRay& r = c->rays[ri];
         Group* g = nullptr;
         for (auto& gg : groups)
-            if (gg.march == r.march && gg.dir == r.dir && gg.sv == r.sv) g = &gg;
-        if (!g) { groups.push_back(Group{r.march, r.dir, r.sv, {}}); g = &groups.back(); }
+            if (gg.march == r.march && gg.dir == r.dir) g = &gg;
+        if (!g) { groups.push_back(Group{r.march, r.dir, {}}); g = &groups.back(); }
         bool placed = false;
         for (auto& sub : g->sub) {
             bool freeslot = true;
@@ -206,121 +208,115 @@ int make_plan(rts_ctx* c)
         }
         if (!placed) g->sub.push_back(std::vector<int>{ri});
     }
-    bool used[3] = {false, false, false};
-    for (auto& g : groups) used[g.march] = true;
+    int units_of[3] = {0, 0, 0};
+    for (auto& g : groups) units_of[g.march] += (int)g.sub.size() * c->nb;
 
-    // --- band height per march axis: one 4x2 block per thread, 2 CTAs per SM if possible
+    // --- tile shape per march axis: least total 4x2-block work (halo recomputation included)
+    //     among the shapes whose CTA fits R times on an SM
     cudaFuncAttributes fa;
     CUDA_TRY(c, cudaFuncGetAttributes(&fa, rts_sweep_kernel));
-    const int threads = 256;
-    c->threads = threads;
     int bestR = 0;
     for (int R = (c->user_ctas_per_sm ? c->user_ctas_per_sm : 2); R >= 1 && !bestR; --R) {
-        if ((long long)R * threads * fa.numRegs > 65536) continue;
         const int smem_cap = std::min(c->max_smem_optin, (228 * 1024) / R - 1024 - (int)fa.sharedSizeBytes);
+        const int slots = c->sm_count * R;
         bool ok = true;
         for (int a = 0; a < 3 && ok; ++a) {
-            if (!used[a]) { c->tp[a].TV = 2; c->tp[a].ntv = (c->tp[a].n_v + 1) / 2; continue; }
             TypePlan& t = c->tp[a];
-            int best = 0;
-            for (int TV = 1; TV <= std::min(t.n_v, 32 * MAXC / NS - 2); ++TV) {
-                if (t.userTV && TV != t.userTV) continue;
-                if (blocks_for(t.n_u, TV) > threads - 32) break;          // the last warp communicates
-                if (smem_for(t.n_u, TV) > smem_cap) break;
-                if (TV > 1 && (TV & 1) && !t.userTV) continue;      // even heights: full 4x2 blocks
-                best = TV;
+            if (!units_of[a]) { t.WU = 4; t.WV = 2; t.ntu = (t.n_u + 3) / 4; t.ntv = (t.n_v + 1) / 2; t.items = 0; continue; }
+            double best_cost = 0.0;
+            int bu = 0, bv = 0;
+            const int n_u4 = (t.n_u + 3) & ~3;
+            for (int WU = 4; WU <= std::min(n_u4, 248); WU += 4) {
+                if (t.userWU && WU != std::min(n_u4, (t.userWU + 3) & ~3)) continue;
+                for (int WV = 1; WV <= std::min(t.n_v, 120); ++WV) {
+                    if (t.userWV && WV != std::min(t.n_v, t.userWV)) continue;
+                    if (smem_for(WU, WV) > smem_cap) break;
+                    const int ntu = (t.n_u + WU - 1) / WU, ntv = (t.n_v + WV - 1) / WV;
+                    if ((long long)ntu * ntv > slots) continue;          // all tiles of a unit must be resident
+                    const int items = items_for(WU, WV, c->K);
+                    const int warps = (items + 31) / 32;
+                    const int rounds = (warps + 7) / 8;
+                    // work in warp-steps, a mild preference for fewer (larger) tiles
+                    const double cost = (double)ntu * ntv * warps * (1.0 + 0.02 * rounds) + 0.5 * ntu * ntv;
+                    if (!bu || cost < best_cost) { best_cost = cost; bu = WU; bv = WV; }
+                }
             }
-            if (!best) { ok = false; break; }
-            t.TV = best;
-            t.ntv = (t.n_v + best - 1) / best;
+            if (!bu) { ok = false; break; }
+            t.WU = bu; t.WV = bv;
+            t.ntu = (t.n_u + bu - 1) / bu; t.ntv = (t.n_v + bv - 1) / bv;
+            t.items = items_for(bu, bv, c->K);
         }
         if (ok) bestR = R;
         if (c->user_ctas_per_sm) break;
     }
-    if (!bestR) return fail(c, RTS_EINVAL, "planner: a row band does not fit (grid too wide: n_u <= 1024, or bad override)");
-    c->ctas_per_sm = bestR;
+    if (!bestR) return fail(c, RTS_EINVAL, "planner: no tile shape fits (grid too large for one resident unit, or bad override)");
     c->smem_bytes = 0;
+    int max_items = 1;
     for (int a = 0; a < 3; ++a)
-        if (used[a]) c->smem_bytes = std::max(c->smem_bytes, smem_for(c->tp[a].n_u, c->tp[a].TV));
+        if (units_of[a]) {
+            c->smem_bytes = std::max(c->smem_bytes, smem_for(c->tp[a].WU, c->tp[a].WV));
+            max_items = std::max(max_items, c->tp[a].items);
+        }
+    c->threads = std::min(256, std::max(64, (max_items + 31) / 32 * 32));
     {
         int occ = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, threads, (size_t)c->smem_bytes) != cudaSuccess || occ < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, c->threads, (size_t)c->smem_bytes) != cudaSuccess || occ < 1)
             return fail(c, RTS_ECUDA, "planner: sweep kernel does not fit on an SM");
         c->ctas_per_sm = std::min(bestR, occ);
     }
-
-    // --- materialise jobs in ticket order
-    c->jobs.clear();
-    int ticket = 0;
-    for (auto& g : groups)
-        for (auto& sub : g.sub)
-            for (int b = 0; b < c->nb; ++b) {
-                HostJob hj{};
-                JobDesc& d = hj.d;
-                std::memset(&d, 0, sizeof d);
-                const TypePlan& t = c->tp[g.march];
-                d.march = g.march; d.dir = g.dir; d.sv = g.sv; d.band = b;
-                d.n_m = t.n_m; d.n_u = t.n_u; d.n_v = t.n_v;
-                d.TV = t.TV; d.ntv = t.ntv;
-                d.per_v = (g.march == 2) ? 1 : 0;
-                d.ticket_begin = ticket;
-                ticket += t.ntv;
-                d.npass = c->npass;
-                d.nz = c->nz;
-                const long long nxy = (long long)c->nx * c->ny;
-                d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
-                const long long PX = c->PX, PY = c->PY;
-                // coefficient layouts (one per march axis): rows v contiguous with pitch = box width
-                if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx;
-                                         d.c_field = (long long)c->nz * (c->ny + 2) * PX; d.c_m = (long long)(c->ny + 2) * PX; d.c_v = PX; d.c_off = PX; }
-                else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx;
-                                         d.c_field = (long long)c->ny * (c->nz + 2) * PX; d.c_m = (long long)(c->nz + 2) * PX; d.c_v = PX; d.c_off = PX; }
-                else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1;
-                                         d.c_field = (long long)c->nx * (c->nz + 2) * PY; d.c_m = (long long)(c->nz + 2) * PY; d.c_v = PY; d.c_off = PY; }
-                for (int q = 0; q < NS; ++q) d.ray[q].itop = -1;
-                for (int ri : sub) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
-                hj.nsteps = t.n_m * c->npass;
-                c->jobs.push_back(hj);
-            }
-    c->total_tickets = ticket;
     const int slots = c->sm_count * c->ctas_per_sm;
-    c->grid = std::min(slots, c->total_tickets);
-    int max_ntv = 1, min_ntv = 1 << 30;
-    for (auto& hj : c->jobs) { max_ntv = std::max(max_ntv, hj.d.ntv); min_ntv = std::min(min_ntv, hj.d.ntv); }
-    if (max_ntv > c->grid && c->total_tickets > c->grid)
-        return fail(c, RTS_EINVAL, "planner: more row bands per job than resident CTAs (grid too tall)");
-    // exchange-buffer pool: a slot may be reused once the job that held it must have finished
-    c->nbuf = std::min((int)c->jobs.size(), (slots + min_ntv - 1) / min_ntv + 2);
-    for (size_t j = 0; j < c->jobs.size(); ++j) c->jobs[j].buf = (int)(j % c->nbuf);
 
-    // --- workspace layout
+    // --- materialise units in ticket order
+    c->units.clear();
+    int ticket = 0;
     const size_t N = (size_t)c->nx * c->ny * c->nz;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
-    const size_t fZ = (size_t)c->nz * (c->ny + 2) * c->PX;
-    const size_t fY = (size_t)c->ny * (c->nz + 2) * c->PX;
-    const size_t fX = (size_t)c->nx * (c->nz + 2) * c->PY;
-    c->off_coefZ = take(sizeof(float) * fZ * 2 * c->nb);
-    c->off_coefY = take(sizeof(float) * fY * 2 * c->nb);
-    c->off_coefX = take(sizeof(float) * fX * 2 * c->nb);
+    const size_t fA = (size_t)c->nz * c->PYR * c->PX;
+    const size_t fB = (size_t)c->nz * c->nx * c->PY;
+    c->off_coefA = take(sizeof(float) * fA * 2 * c->nb);
+    c->off_coefB = take(sizeof(float) * fB * 2 * c->nb);
     c->off_QB = take(sizeof(float) * N);
     c->nblk_a = ((c->nx + 31) / 32) * ((c->ny + 31) / 32);
     c->off_ksum = take(sizeof(double) * (size_t)c->nb * c->nz * c->nblk_a);
+    c->off_lev = take(sizeof(double) * (size_t)c->nb * c->nz);
     c->off_kstar = take(sizeof(int) * c->nb);
     c->off_abort = take(sizeof(int) * 8);                    // [0] watchdog, [1] ticket counter
-    c->off_jobs = take(sizeof(JobDesc) * c->jobs.size());
-    c->prog_ints = (size_t)c->total_tickets;
-    c->off_prog = take(sizeof(int) * c->prog_ints);
-    size_t mH = 0, mG = 0;
-    for (auto& hj : c->jobs) {
-        const JobDesc& d = hj.d;
-        const size_t n_u4 = (size_t)((d.n_u + 3) & ~3);
-        mH = std::max(mH, (size_t)d.ntv * hj.nsteps * NS * n_u4);
-        mG = std::max(mG, (size_t)d.ntv * 2 * d.n_m * NS * d.TV);
-    }
-    c->buf_Gu = align_up(sizeof(float) * mH, 256);
-    c->buf_stride = c->buf_Gu + align_up(sizeof(float) * mG, 256);
-    c->off_buf0 = take(c->buf_stride * c->nbuf);
+    for (auto& g : groups)
+        for (auto& sub : g.sub)
+            for (int b = 0; b < c->nb; ++b) {
+                HostUnit hu{};
+                UnitDesc& d = hu.d;
+                std::memset(&d, 0, sizeof d);
+                const TypePlan& t = c->tp[g.march];
+                d.march = g.march; d.dir = g.dir; d.band = b;
+                d.per_v = (g.march == 2) ? 1 : 0;
+                d.n_m = t.n_m; d.n_u = t.n_u; d.n_v = t.n_v; d.n_u4 = (t.n_u + 3) & ~3;
+                d.WU = t.WU; d.WV = t.WV; d.ntu = t.ntu; d.ntv = t.ntv;
+                d.K = c->K; d.npass = c->npass;
+                d.ticket_begin = ticket;
+                d.ntiles = t.ntu * t.ntv;
+                ticket += d.ntiles;
+                d.nz = c->nz;
+                const long long nxy = (long long)c->nx * c->ny;
+                d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
+                const long long PX = c->PX, PY = c->PY, PYR = c->PYR;
+                if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx;
+                                         d.c_field = (long long)fA; d.c_m = PYR * PX; d.c_v = PX; d.c_off = HALO * PX; d.P = c->PX; }
+                else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx;
+                                         d.c_field = (long long)fA; d.c_m = PX; d.c_v = PYR * PX; d.c_off = HALO * PX; d.P = c->PX; }
+                else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1;
+                                         d.c_field = (long long)fB; d.c_m = PY; d.c_v = (long long)c->nx * PY; d.c_off = 0; d.P = c->PY; }
+                for (int q = 0; q < NSLOT; ++q) d.ray[q].itop = -1;
+                for (int ri : sub) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
+                hu.off_xex = take(sizeof(float) * 2 * NSLOT * (size_t)d.n_v * d.n_u4);
+                hu.off_g = take(sizeof(float) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u4));
+                c->units.push_back(hu);
+            }
+    c->total_tickets = ticket;
+    c->grid = std::min(slots, c->total_tickets);
+    c->off_units = take(sizeof(UnitDesc) * c->units.size());
+    c->off_bar = take(sizeof(int) * c->units.size());
     c->off_stage_in = take(sizeof(float) * N * 3);
     c->off_stage_out = take(sizeof(float) * (N + (size_t)c->nb * c->n_up * c->ny * c->nx));
     c->ws_bytes = off;
@@ -331,19 +327,19 @@ int make_plan(rts_ctx* c)
 int bind_workspace(rts_ctx* c)
 {
     unsigned char* ws = c->ws;
-    float* coefL[3] = {(float*)(ws + c->off_coefX), (float*)(ws + c->off_coefY), (float*)(ws + c->off_coefZ)};
-    std::vector<JobDesc> flat;
-    for (auto& hj : c->jobs) {
-        JobDesc& d = hj.d;
-        unsigned char* sb = ws + c->off_buf0 + c->buf_stride * hj.buf;
-        d.Hrow = (float*)sb;
-        d.Gu = (float*)(sb + c->buf_Gu);
-        d.progress = (int*)(ws + c->off_prog) + d.ticket_begin;
+    std::vector<UnitDesc> flat;
+    for (size_t i = 0; i < c->units.size(); ++i) {
+        HostUnit& hu = c->units[i];
+        UnitDesc& d = hu.d;
+        d.Xex = (float*)(ws + hu.off_xex);
+        d.Gu = (float*)(ws + hu.off_g);
+        d.barrier = (int*)(ws + c->off_bar) + i;
         d.kstar = (const int*)(ws + c->off_kstar) + d.band;
-        d.cbase = coefL[d.march] + (size_t)(2 * d.band) * d.c_field;
+        const float* base = (const float*)(ws + (d.march == 0 ? c->off_coefB : c->off_coefA));
+        d.cbase = base + (size_t)(2 * d.band) * d.c_field;
         flat.push_back(d);
     }
-    CUDA_TRY(c, cudaMemcpy(ws + c->off_jobs, flat.data(), sizeof(JobDesc) * flat.size(), cudaMemcpyHostToDevice));
+    CUDA_TRY(c, cudaMemcpy(ws + c->off_units, flat.data(), sizeof(UnitDesc) * flat.size(), cudaMemcpyHostToDevice));
     CUDA_TRY(c, cudaMemset(ws + c->off_abort, 0, sizeof(int) * 8));   // status word: a fresh workspace holds garbage
     c->maps_ready = true;
     return RTS_OK;
@@ -360,11 +356,10 @@ int launch_stage_a(rts_ctx* c, const float* rho, const float* T, const float* P,
     p.logP_min = c->logP_min; p.inv_dP = (c->nP - 1) / (c->logP_max - c->logP_min);
     p.logkappa = c->d_logkappa; p.bandfrac = c->d_bandfrac;
     p.rho = rho; p.T = T; p.P = P;
-    p.coefZ = (float*)(c->ws + c->off_coefZ); p.coefY = (float*)(c->ws + c->off_coefY); p.coefX = (float*)(c->ws + c->off_coefX);
-    p.PX = c->PX; p.PY = c->PY;
-    p.strideZ_f = (long long)c->nz * (c->ny + 2) * c->PX;
-    p.strideY_f = (long long)c->ny * (c->nz + 2) * c->PX;
-    p.strideX_f = (long long)c->nx * (c->nz + 2) * c->PY;
+    p.coefA = (float*)(c->ws + c->off_coefA); p.coefB = (float*)(c->ws + c->off_coefB);
+    p.PX = c->PX; p.PY = c->PY; p.PYR = c->PYR;
+    p.strideA_f = (long long)c->nz * c->PYR * c->PX;
+    p.strideB_f = (long long)c->nz * c->nx * c->PY;
     p.ksum = (double*)(c->ws + c->off_ksum);
     p.plain_k = plain_k; p.plain_s = plain_s;
     dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, c->nz), block(32, 8);
@@ -492,10 +487,19 @@ int rts_num_up_rays(const rts_ctx* c)
 int rts_set_tiling(rts_ctx* c, int march, int tile_u, int tile_v)
 {
     if (!c) return RTS_EINVAL;
-    (void)tile_u;   // tiles always span the full unit-stride extent
-    if (march < 0 || march > 2 || tile_v < 0 || tile_v > 32 * MAXC / NS - 2)
+    if (march < 0 || march > 2 || tile_u < 0 || tile_v < 0 || tile_u > 248 || tile_v > 120)
         return fail(c, RTS_EINVAL, "rts_set_tiling: bad argument");
-    c->tp[march].userTV = tile_v;
+    c->tp[march].userWU = tile_u;
+    c->tp[march].userWV = tile_v;
+    c->planned = false;
+    return RTS_OK;
+}
+
+int rts_set_exchange_interval(rts_ctx* c, int k)
+{
+    if (!c) return RTS_EINVAL;
+    if (k < 0 || k > KMAX) return fail(c, RTS_EINVAL, "rts_set_exchange_interval: 0..4");
+    c->user_K = k;
     c->planned = false;
     return RTS_OK;
 }
@@ -531,9 +535,9 @@ int rts_plan_info(rts_ctx* c, int* what, int n)
 {
     if (!c || !what) return RTS_EINVAL;
     if (!c->planned) { int rc = make_plan(c); if (rc != RTS_OK) return rc; }
-    int v[12] = {4, c->total_tickets, c->ctas_per_sm, (int)c->jobs.size(), c->threads, c->smem_bytes,
-                 c->grid, c->nbuf, c->tp[0].TV, c->tp[1].TV, c->tp[2].TV, 0};
-    for (int i = 0; i < n && i < 12; ++i) what[i] = v[i];
+    int v[16] = {4, c->total_tickets, c->ctas_per_sm, (int)c->units.size(), c->threads, c->smem_bytes,
+                 c->grid, c->K, c->tp[0].WV, c->tp[1].WV, c->tp[2].WV, c->tp[0].WU, c->tp[1].WU, c->tp[2].WU, 0, 0};
+    for (int i = 0; i < n && i < 16; ++i) what[i] = v[i];
     return RTS_OK;
 }
 
@@ -559,8 +563,9 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[0], st));
     int rc = launch_stage_a(c, rho, T, P, nullptr, nullptr, st);
     if (rc != RTS_OK) return rc;
-    rts_kstar_kernel<<<1, 32, 0, st>>>((const double*)(ws + c->off_ksum), c->nb, c->nz, c->nblk_a,
-                                       1.0 / ((double)c->nx * c->ny), c->h[2], 5.0, (int*)(ws + c->off_kstar));
+    rts_kstar_kernel<<<c->nb, 256, 0, st>>>((const double*)(ws + c->off_ksum), c->nz, c->nblk_a,
+                                            1.0 / ((double)c->nx * c->ny), c->h[2], 5.0, (int*)(ws + c->off_kstar),
+                                            (double*)(ws + c->off_lev));
     CUDA_TRY(c, cudaGetLastError());
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[1], st));
 
@@ -570,15 +575,18 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     CUDA_TRY(c, cudaMemsetAsync(QB, 0, N * sizeof(float), st));
     CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 8, st));
 
-    CUDA_TRY(c, cudaMemsetAsync(ws + c->off_prog, 0, sizeof(int) * c->prog_ints, st));
+    CUDA_TRY(c, cudaMemsetAsync(ws + c->off_bar, 0, sizeof(int) * c->units.size(), st));
     // the sweep: one persistent launch, tasks handed out by an in-order ticket counter
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[2], st));
     {
-        const JobDesc* djobs = (const JobDesc*)(ws + c->off_jobs);
+        const UnitDesc* dunits = (const UnitDesc*)(ws + c->off_units);
         int* abortf = (int*)(ws + c->off_abort);
-        rts_sweep_kernel<<<c->grid, c->threads, (size_t)c->smem_bytes, st>>>(
-            djobs, (int)c->jobs.size(), c->total_tickets, abortf + 1, Q, QB, Itop, abortf);
-        CUDA_TRY(c, cudaGetLastError());
+        int* ticket = abortf + 1;
+        int nunits = (int)c->units.size(), total = c->total_tickets;
+        void* args[] = {&dunits, &nunits, &total, &ticket, &Q, &QB, &Itop, &abortf};
+        // cooperative launch: every CTA of the grid is resident, which the tile barriers rely on
+        CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_sweep_kernel, dim3(c->grid), dim3(c->threads), args,
+                                                (size_t)c->smem_bytes, st));
     }
     // finalize
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[3], st));

@@ -22,7 +22,7 @@ _ERR = {-1: "RTS_EINVAL", -2: "RTS_ESTATE", -3: "RTS_ECUDA", -4: "RTS_ENOMEM", -
 
 EXPORTS = [
     "rts_create", "rts_destroy", "rts_set_tables", "rts_set_passes", "rts_set_rays", "rts_get_rays",
-    "rts_num_up_rays", "rts_set_tiling", "rts_set_ctas_per_sm", "rts_workspace_bytes",
+    "rts_num_up_rays", "rts_set_tiling", "rts_set_exchange_interval", "rts_set_ctas_per_sm", "rts_workspace_bytes",
     "rts_set_workspace", "rts_solve", "rts_solve_host", "rts_coefficients", "rts_sync_check",
     "rts_plan_info", "rts_last_error", "rts_enable_timing", "rts_last_timing",
 ]
@@ -57,6 +57,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_num_up_rays.argtypes = [c_void_p]
     lib.rts_set_tiling.restype = c_int
     lib.rts_set_tiling.argtypes = [c_void_p, c_int, c_int, c_int]
+    lib.rts_set_exchange_interval.restype = c_int
+    lib.rts_set_exchange_interval.argtypes = [c_void_p, c_int]
     lib.rts_set_ctas_per_sm.restype = c_int
     lib.rts_set_ctas_per_sm.argtypes = [c_void_p, c_int]
     lib.rts_workspace_bytes.restype = c_size_t
@@ -159,6 +161,9 @@ class RTS:
     def set_tiling(self, march: int, tile_u: int, tile_v: int):
         self._check(self._lib.rts_set_tiling(self._ctx, march, tile_u, tile_v), "rts_set_tiling")
 
+    def set_exchange_interval(self, k: int):
+        self._check(self._lib.rts_set_exchange_interval(self._ctx, k), "rts_set_exchange_interval")
+
     def set_ctas_per_sm(self, n: int):
         self._check(self._lib.rts_set_ctas_per_sm(self._ctx, n), "rts_set_ctas_per_sm")
 
@@ -177,10 +182,11 @@ class RTS:
         self._check(self._lib.rts_set_workspace(self._ctx, ctypes.c_void_p(ptr), n), "rts_set_workspace")
 
     def plan_info(self) -> dict:
-        arr = (ctypes.c_int * 12)()
-        self._check(self._lib.rts_plan_info(self._ctx, arr, 12), "rts_plan_info")
-        keys = ["launches", "tasks", "ctas_per_sm", "jobs", "threads", "smem_bytes",
-                "grid", "exchange_slots", "tile_v_x", "tile_v_y", "tile_v_z", "reserved"]
+        arr = (ctypes.c_int * 16)()
+        self._check(self._lib.rts_plan_info(self._ctx, arr, 16), "rts_plan_info")
+        keys = ["launches", "tasks", "ctas_per_sm", "units", "threads", "smem_bytes",
+                "grid", "exchange_interval", "tile_v_x", "tile_v_y", "tile_v_z",
+                "tile_u_x", "tile_u_y", "tile_u_z"]
         return dict(zip(keys, [int(v) for v in arr]))
 
     # -- the hot path
@@ -246,7 +252,7 @@ class RTS:
         self._check(self._lib.rts_sync_check(self._ctx, self._stream()), "rts_sync_check")
 
 
-def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0) -> "RTS":
+def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchange_interval: int = 0) -> "RTS":
     """Create and configure a solver for an `inputs.RTSInputs` problem."""
     r = RTS(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.nbands)
     r.set_tables(inp.nT, inp.nP, inp.logT_min, inp.logT_max, inp.logP_min, inp.logP_max, inp.logkappa, inp.bandfrac)
@@ -257,5 +263,7 @@ def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0) -> "RT
             r.set_tiling(march, tu, tv)
     if ctas_per_sm:
         r.set_ctas_per_sm(ctas_per_sm)
+    if exchange_interval:
+        r.set_exchange_interval(exchange_interval)
     r.allocate_workspace()
     return r

@@ -126,7 +126,7 @@ def test_many_tiles_and_ragged_tail(tv):
     """Row bands of height tv: several tiles per job with a ragged last tile, both parities."""
     inp = inputs.make_config(3, grid=(36, 44, 38), nbands=2)
     _, _, plan = _check(inp, tiling={0: (0, tv), 1: (0, tv), 2: (0, tv)})
-    assert plan["tile_v_x"] == tv and plan["tasks"] > plan["jobs"]
+    assert plan["tile_v_x"] == tv and plan["tasks"] > plan["units"]
 
 
 def test_one_cta_per_sm():
