@@ -51,7 +51,9 @@ struct rts_ctx {
     float* d_bandfrac = nullptr;
     // device facts
     int sm_count = 0, max_smem_optin = 0;
-    int user_ctas_per_sm = 0, user_K = 0;
+    int user_ctas_per_sm = 0, user_K = 0, user_threads = 0;
+    SweepMaps maps;
+    void* encode_fn = nullptr;    // cuTensorMapEncodeTiled
     // plan
     bool planned = false;
     TypePlan tp[3];
@@ -130,9 +132,12 @@ void make_ray_consts(const HostRay& r, RayC& rc)
     for (int q = 0; q < 4; ++q)
         if (q != big) { w[q] = std::nearbyint(w[q] * 16777216.0) / 16777216.0; sum += w[q]; }
     w[big] = 1.0 - sum;
+    // device order: (lower v row, its side neighbour, higher v row, its side neighbour)
+    const int ord_p[4] = {2, 3, 0, 1}, ord_m[4] = {0, 1, 2, 3};
     for (int q = 0; q < 4; ++q) {
-        rc.wx[q] = (float)w[q];
-        rc.wk[q] = (float)(0.5 * r.ds * w[q]);
+        const int src = (r.sv > 0) ? ord_p[q] : ord_m[q];
+        rc.wx[q] = (float)w[src];
+        rc.wk[q] = (float)(0.5 * r.ds * w[src]);
     }
     rc.kc = (float)(0.5 * r.ds);
     rc.wq = (float)r.w;
@@ -157,14 +162,17 @@ void default_rays(rts_ctx* c)
         }
 }
 
-// dynamic shared memory of a CTA whose tiles are WU x WV: guard rows, NSTAGE coefficient planes
-// (2 fields), the double-buffered carried planes of NSLOT rays, the ghost table
-int smem_for(int WU, int WV)
+// dynamic shared memory of a CTA whose tiles are WU x WV (SmemPlan: coefficient ring, carried
+// planes, ghost list, item tables)
+int smem_for(int WU, int WV) { return (int)SmemPlan(WU, WV).bytes(); }
+// items (4 x 2 node blocks of one ray) of a full interior tile per step, halo included, for
+// `nslots` rays; averaged over the steps of a block
+double items_for(int WU, int WV, int K, int nslots)
 {
-    const int BU = WU + 2 * HALO, BV = WV + 2 * HALO, BOX = BU * BV;
-    return (2 * BU + (NSTAGE * 2 + 2 * NSLOT) * BOX) * (int)sizeof(float) + NSLOT * (BU + BV) * (int)sizeof(GhostEnt);
+    double sum = 0.0;
+    for (int hj = 0; hj < K; ++hj) sum += (double)((WU + (hj > 0 ? HALO : 0)) / 4) * ((WV + hj + 1) / 2);
+    return nslots * sum / K;
 }
-int items_for(int WU, int WV, int K) { return ((WU + HALO) / 4 + 1) * ((WV + K + 2) / 2); }
 
 // --------------------------------------------------------------------------- planner
 // Groups the rays into sweep units (march axis, direction, one ray per sign pair), chooses the
@@ -233,18 +241,15 @@ int make_plan(rts_ctx* c)
                     if (smem_for(WU, WV) > smem_cap) break;
                     const int ntu = (t.n_u + WU - 1) / WU, ntv = (t.n_v + WV - 1) / WV;
                     if ((long long)ntu * ntv > slots) continue;          // all tiles of a unit must be resident
-                    const int items = items_for(WU, WV, c->K);
-                    const int warps = (items + 31) / 32;
-                    const int rounds = (warps + 7) / 8;
-                    // work in warp-steps, a mild preference for fewer (larger) tiles
-                    const double cost = (double)ntu * ntv * warps * (1.0 + 0.02 * rounds) + 0.5 * ntu * ntv;
+                    // work in items per step, a mild preference for fewer (larger) tiles
+                    const double cost = (double)ntu * ntv * (items_for(WU, WV, c->K, NSLOT) + 8.0);
                     if (!bu || cost < best_cost) { best_cost = cost; bu = WU; bv = WV; }
                 }
             }
             if (!bu) { ok = false; break; }
             t.WU = bu; t.WV = bv;
             t.ntu = (t.n_u + bu - 1) / bu; t.ntv = (t.n_v + bv - 1) / bv;
-            t.items = items_for(bu, bv, c->K);
+            t.items = NSLOT * ((bu + HALO) / 4) * ((bv + c->K) / 2);   // most items of a step
         }
         if (ok) bestR = R;
         if (c->user_ctas_per_sm) break;
@@ -257,7 +262,11 @@ int make_plan(rts_ctx* c)
             c->smem_bytes = std::max(c->smem_bytes, smem_for(c->tp[a].WU, c->tp[a].WV));
             max_items = std::max(max_items, c->tp[a].items);
         }
-    c->threads = std::min(256, std::max(64, (max_items + 31) / 32 * 32));
+    {   // CTA size: the items of a step in equal rounds
+        const int cap = c->user_threads ? c->user_threads : RTS_SWEEP_THREADS;
+        const int rounds = (max_items + cap - 1) / cap;
+        c->threads = std::min(cap, std::max(64, ((max_items + rounds - 1) / rounds + 31) / 32 * 32));
+    }
     {
         int occ = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, c->threads, (size_t)c->smem_bytes) != cudaSuccess || occ < 1)
@@ -340,6 +349,40 @@ int bind_workspace(rts_ctx* c)
         flat.push_back(d);
     }
     CUDA_TRY(c, cudaMemcpy(ws + c->off_units, flat.data(), sizeof(UnitDesc) * flat.size(), cudaMemcpyHostToDevice));
+    // coefficient tensors for the TMA engine: layout A as (x, y rows, z, field) with the box of the
+    // z-march (x, y) or of the y-march (x, z); layout B as (y, x, z, field) with the x-march box (y, z)
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    EncodeFn enc = (EncodeFn)c->encode_fn;
+    for (int a = 0; a < 3; ++a) {
+        const TypePlan& t = c->tp[a];
+        const cuuint32_t BU = (cuuint32_t)(t.WU + 2 * HALO), BV = (cuuint32_t)(t.WV + 2 * HALO);
+        cuuint64_t dims[4], strides[3];
+        cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
+        void* base;
+        if (a == 0) {
+            base = ws + c->off_coefB;
+            dims[0] = (cuuint64_t)c->PY; dims[1] = (cuuint64_t)c->nx; dims[2] = (cuuint64_t)c->nz; dims[3] = 2ull * c->nb;
+            box[0] = BU; box[1] = 1; box[2] = BV; box[3] = 1;
+        } else {
+            base = ws + c->off_coefA;
+            dims[0] = (cuuint64_t)c->PX; dims[1] = (cuuint64_t)c->PYR; dims[2] = (cuuint64_t)c->nz; dims[3] = 2ull * c->nb;
+            if (a == 2) { box[0] = BU; box[1] = BV; box[2] = 1; box[3] = 1; }
+            else        { box[0] = BU; box[1] = 1; box[2] = BV; box[3] = 1; }
+        }
+        strides[0] = dims[0] * sizeof(float);
+        strides[1] = strides[0] * dims[1];
+        strides[2] = strides[1] * dims[2];
+        CUresult r = enc(&c->maps.m[a], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            char buf[96];
+            snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (march %d, CUresult %d)", a, (int)r);
+            return fail(c, RTS_ECUDA, buf);
+        }
+    }
     CUDA_TRY(c, cudaMemset(ws + c->off_abort, 0, sizeof(int) * 8));   // status word: a fresh workspace holds garbage
     c->maps_ready = true;
     return RTS_OK;
@@ -403,6 +446,12 @@ int rts_create(rts_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     if ((e = cudaFuncSetAttribute(rts_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem_optin)) != cudaSuccess)
         return bail(std::string("cudaFuncSetAttribute(max dynamic smem): ") + cudaGetErrorString(e));
     if ((e = cudaEventCreateWithFlags(&c->ev, cudaEventDisableTiming)) != cudaSuccess) return bail(cudaGetErrorString(e));
+    {
+        cudaDriverEntryPointQueryResult qres;
+        if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &c->encode_fn, cudaEnableDefault, &qres)) != cudaSuccess ||
+            qres != cudaDriverEntryPointSuccess || !c->encode_fn)
+            return bail("cuTensorMapEncodeTiled not available from the driver");
+    }
     *out = c;
     return RTS_OK;
 }
@@ -583,7 +632,7 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
         int* abortf = (int*)(ws + c->off_abort);
         int* ticket = abortf + 1;
         int nunits = (int)c->units.size(), total = c->total_tickets;
-        void* args[] = {&dunits, &nunits, &total, &ticket, &Q, &QB, &Itop, &abortf};
+        void* args[] = {&c->maps, &dunits, &nunits, &total, &ticket, &Q, &QB, &Itop, &abortf};
         // cooperative launch: every CTA of the grid is resident, which the tile barriers rely on
         CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_sweep_kernel, dim3(c->grid), dim3(c->threads), args,
                                                 (size_t)c->smem_bytes, st));

@@ -31,7 +31,9 @@ constexpr double PI_D = 3.14159265358979323846;
 // the ray along them.  Slot s of a unit holds a ray with su = (s & 1 ? -1 : +1),
 // sv = (s & 2 ? -1 : +1).
 struct alignas(16) RayC {
-    float wx[4];      // bilinear weights of (u,v) (u-su,v) (u,v-sv) (u-su,v-sv); sum == 1 exactly
+    float wx[4];      // bilinear weights, sum == 1 exactly, ordered by stencil row: (lower v row, its
+                      // u-side neighbour, higher v row, its u-side neighbour); the node's own row is
+                      // the higher one for sv > 0 and the lower one for sv < 0
     float wk[4];      // 0.5*ds*wx  (opacity -> optical path)
     float kc;         // 0.5*ds
     float wq;         // quadrature weight

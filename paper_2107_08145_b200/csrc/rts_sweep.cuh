@@ -13,24 +13,32 @@
 //   seams = stencil nodes across a periodic boundary come from the previous pass (Jacobi):
 //           far columns / rows of every plane are kept in G (pass parity) and copied into the
 //           ghost column / row of the carried plane before each step.
-// Per step a CTA streams one (kaprho, S) plane box through a 3-stage TMA ring
-// (cp.async.bulk rows completing on mbarriers) and updates, per thread, a 4 x 2 node block for
-// all rays of the unit from registers (opacity / source neighbourhoods are shared by the rays).
+//   item  = a 4 x 2 node block of one ray: the thread-level unit of work.  Items of a step are
+//           listed in a table (per remaining halo depth) and dealt to the threads in order.
+// Per step a CTA streams one (kaprho, S) plane box through a 3-stage TMA ring (one
+// cp.async.bulk.tensor per field, completing on an mbarrier) and updates its items from
+// registers and shared memory.
 // Carried quantity: X = I - a*S with a = 1 at levels k <= kstar (optically thick part, where
 // J - S would cancel) and a = 0 above (thin part, where I << S would cancel).
 #pragma once
 #include "rts_kernels.cuh"
 
+#ifndef RTS_SWEEP_THREADS
+#define RTS_SWEEP_THREADS 512   // most threads of a sweep CTA (two CTAs per SM: <= 64 registers)
+#endif
+
 namespace rts {
 
-struct GhostEnt { int xoff; int goff; int bv; int slot; };   // xoff < 0: unused
+struct GhostEnt { int xoff; int goff; int bv; int slot; };
+
+struct SweepMaps { CUtensorMap m[3]; };      // coefficient tensor of the x-, y-, z-march units
 
 struct TaskShared {
     UnitDesc U;
     int4 reg[KMAX][NSLOT];     // per remaining halo depth hj: rows [x, y), cols [z, w) a slot updates (box coords)
-    int4 uni[KMAX];            // union of the slots: first row (even), row pairs, first quad, quads
+    int  nitems[KMAX];
     uint64_t mbar[NSTAGE];
-    int ticket, flag;
+    int ticket, flag, nghost, pad;
 };
 
 // closed-form attenuation factors: em1 = 1 - e^-dt, wl = (1 - e^-dt)/dt
@@ -46,19 +54,9 @@ __device__ __forceinline__ void att_series(float dt, float& em1, float& wl, floa
     em1 = dt * wl;
 }
 
-// 6 values of one box row around a quad: columns -1 .. 4 relative to the quad.  The centre
-// float4 comes from shared memory; the side values come from the neighbouring lanes' float4 when
-// those lanes hold the adjacent quads of the same row, else from shared memory.
-__device__ __forceinline__ void load_row6(const float* __restrict__ row, bool l_ok, bool r_ok, float (&o)[6])
-{
-    const float4 v = *reinterpret_cast<const float4*>(row);
-    float l = __shfl_up_sync(0xffffffffu, v.w, 1);
-    float r = __shfl_down_sync(0xffffffffu, v.x, 1);
-    if (!l_ok) l = row[-1];
-    if (!r_ok) r = row[4];
-    o[0] = l; o[1] = v.x; o[2] = v.y; o[3] = v.z; o[4] = v.w; o[5] = r;
-}
-// same, only the side the ray looks at (SU > 0: left); result in the 6-layout, other side unset
+// 5 values of one box row around a quad: the quad (o[1..4]) and the side column the ray looks
+// at (SU > 0: left neighbour in o[0]; SU < 0: right neighbour in o[5]).  The side value comes
+// from the neighbouring lane's float4 when that lane holds the adjacent quad of the same row.
 template <int SU>
 __device__ __forceinline__ void load_row5(const float* __restrict__ row, bool l_ok, bool r_ok, float (&o)[6])
 {
@@ -75,34 +73,34 @@ __device__ __forceinline__ void load_row5(const float* __restrict__ row, bool l_
     }
 }
 
-// optical paths of one node row (4 nodes) of a ray with u-sign SU
-//   ko / ku : opacity of the previous plane on the node's own row / upwind row (6-layout)
+// optical paths of one node row (4 nodes).  lo / hi: opacity of the previous plane on the two
+// stencil rows (lower / higher v), kv = 0.5*ds * weights of (lo, lo side, hi, hi side).
 template <int SU>
-__device__ __forceinline__ void row_dtau(const float (&ko)[6], const float (&ku)[6], const float4 kp,
+__device__ __forceinline__ void row_dtau(const float (&lo)[6], const float (&hi)[6], const float4 kp,
                                          const float4 kv, const float kc, float (&dt)[4])
 {
     const float kpa[4] = {kp.x, kp.y, kp.z, kp.w};
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int c = j + 1, cs = j + 1 - SU;
-        dt[j] = kc * kpa[j] + kv.x * ko[c] + kv.y * ko[cs] + kv.z * ku[c] + kv.w * ku[cs];
+        dt[j] = kc * kpa[j] + kv.x * lo[c] + kv.y * lo[cs] + kv.z * hi[c] + kv.w * hi[cs];
     }
 }
 
-// update of one node row.  so/su_: source function on the own / upwind row; xo/xu: carried
-// quantity.  REG 0: everything in the departure-carried part (a = 1); 1: all direct (a = 0);
-// 2: mixed (a_o, a_u, a_p = a on the own row, the upwind row and at the node).
+// update of one node row.  slo/shi: source function on the two stencil rows; xlo/xhi: carried
+// quantity; wv: weights of (lo, lo side, hi, hi side).  REG 0: everything in the departure-carried
+// part (a = 1); 1: all direct (a = 0); 2: mixed (a_lo, a_hi, a_p = a on the two rows and at the node).
 template <int SU, int REG>
 __device__ __forceinline__ void row_update(
-    const float (&dt)[4], const float (&so)[6], const float (&su_)[6],
-    const float (&xo)[6], const float (&xu)[6], const float4 spv,
-    const float4 wv, const float a_o, const float a_u, const float a_p, const bool any_small, float (&xp)[4])
+    const float (&dt)[4], const float (&slo)[6], const float (&shi)[6],
+    const float (&xlo)[6], const float (&xhi)[6], const float4 spv,
+    const float4 wv, const float a_lo, const float a_hi, const float a_p, const bool any_small, float (&xp)[4])
 {
     const float sp[4] = {spv.x, spv.y, spv.z, spv.w};
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int c = j + 1, cs = j + 1 - SU;
-        const float Xu = wv.x * xo[c] + wv.y * xo[cs] + wv.z * xu[c] + wv.w * xu[cs];
+        const float Xu = wv.x * xlo[c] + wv.y * xlo[cs] + wv.z * xhi[c] + wv.w * xhi[cs];
         float em1, wl;
         att_closed(dt[j], em1, wl);
         float pp = 1.0f - wl;
@@ -117,20 +115,20 @@ __device__ __forceinline__ void row_update(
         float v = fmaf(-Xu, em1, Xu);                  // Xu * e^-dt
         if (REG == 0) {
             float dS = sp[j];
-            dS = fmaf(-wv.x, so[c], dS); dS = fmaf(-wv.y, so[cs], dS);
-            dS = fmaf(-wv.z, su_[c], dS); dS = fmaf(-wv.w, su_[cs], dS);
+            dS = fmaf(-wv.x, slo[c], dS); dS = fmaf(-wv.y, slo[cs], dS);
+            dS = fmaf(-wv.z, shi[c], dS); dS = fmaf(-wv.w, shi[cs], dS);
             v = fmaf(-dS, wl, v);
         } else if (REG == 1) {
             const float pu = em1 - pp;                 // psi_u = (1-E)/dt - E = (1 - E) - psi_p
-            float Su = wv.x * so[c];
-            Su = fmaf(wv.y, so[cs], Su); Su = fmaf(wv.z, su_[c], Su); Su = fmaf(wv.w, su_[cs], Su);
+            float Su = wv.x * slo[c];
+            Su = fmaf(wv.y, slo[cs], Su); Su = fmaf(wv.z, shi[c], Su); Su = fmaf(wv.w, shi[cs], Su);
             v = fmaf(pu, Su, v);
             v = fmaf(pp, sp[j], v);
         } else {
             const float pu = em1 - pp;
-            const float R0 = wv.x * so[c] + wv.y * so[cs];
-            const float R1 = wv.z * su_[c] + wv.w * su_[cs];
-            const float St = a_o * R0 + a_u * R1;
+            const float R0 = wv.x * slo[c] + wv.y * slo[cs];
+            const float R1 = wv.z * shi[c] + wv.w * shi[cs];
+            const float St = a_lo * R0 + a_hi * R1;
             const float Sh = (R0 + R1) - St;
             const float Stp = a_p * sp[j];
             v = fmaf(-(Stp - St), wl, v);
@@ -154,8 +152,13 @@ __device__ __forceinline__ bool spin_abort(int* abortf, unsigned& spins, int cod
 
 __device__ __forceinline__ int wrap(int x, int n) { x %= n; return x < 0 ? x + n : x; }
 
-// ------------------------------------------------------------------------------------------
-// Everything a thread needs to finish one slot of its 4 x 2 block (stores, histories, strips).
+// TMA engine, tensor form: one 4-D box (u, ., ., field) of a coefficient layout -> shared memory
+__device__ __forceinline__ void tensor_load4(void* dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
 struct StepCtx {
     int m, pl, pass, hj, par_ex;       // plane counter, plane index, pass, remaining halo depth, exchange parity
     bool dplane;                       // z-march inflow plane: nodes are set, not updated
@@ -164,124 +167,144 @@ struct StepCtx {
 };
 
 struct TileGeo {
-    int u0, v0, wu, wv, BU, BV, BOX;
+    int u0, v0, wu, wv, BU, BV, BOXP;
     int dlo_u, dhi_u, dlo_v, dhi_v;    // domain bounds in box coordinates
     int kstar;
     bool zmarch;
 };
 
-template <int SU, int SV>
-__device__ __forceinline__ void do_slot(
+// ------------------------------------------------------------------------------------------
+// One item: the 4 x 2 node block (rows rowN, rowN+1; columns 4*quad .. 4*quad+3, box coordinates)
+// of slot s.  All lanes of a warp call this together (shuffles); `valid` masks padding lanes.
+template <int SU>
+__device__ __forceinline__ void do_item(
     const int s, const TaskShared& S, const TileGeo& G, const StepCtx& C,
-    const float* __restrict__ Xr, float* __restrict__ Xw,      // carried plane of this slot: read / write box
-    const int boff, const int rowB, const int quad, const bool valid, const bool l_ok, const bool r_ok,
-    const float (&dt)[2][4],
-    const float (&sA)[6], const float (&sB)[6], const float (&sC)[6], const float (&sD)[6],
-    const float4 scB, const float4 scC)
+    const float* __restrict__ Kp, const float* __restrict__ Kc,   // previous / this plane: opacity box, source box at +BOXP
+    const float* __restrict__ Xr, float* __restrict__ Xw,         // carried plane of this slot: read / write box
+    const int rowN, const int quad, const bool valid, const bool l_ok, const bool r_ok)
 {
     const UnitDesc& U = S.U;
+    const int BU = G.BU;
+    const bool svp = !(s & 2);                               // sv > 0
     const int4 rg = S.reg[C.hj][s];
-    const bool actB = rowB >= rg.x && rowB < rg.y;
-    const bool actC = rowB + 1 >= rg.x && rowB + 1 < rg.y;
+    const bool act0 = rowN >= rg.x && rowN < rg.y;
+    const bool act1 = rowN + 1 >= rg.x && rowN + 1 < rg.y;
     const int c0 = max(0, rg.z - 4 * quad), c1 = min(4, rg.w - 4 * quad);
-    const bool act = valid && (c0 < c1) && (actB || actC);
-    if (!__any_sync(0xffffffffu, act)) return;
-
-    const int vB = G.v0 + rowB - HALO;                       // global v of node row B
+    const bool act = valid && (c0 < c1) && (act0 || act1);
+    const int noff = rowN * BU + 4 * quad;                   // node row 0
+    const int off = noff - (svp ? BU : 0);                   // first stencil row: rows (R0, R1, R2)
+    const int vN = G.v0 + rowN - HALO;                       // global v of node row 0
+    const float* const Sp = Kp + G.BOXP;
+    const float* const Sc = Kc + G.BOXP;
+    const float4 sc0 = *reinterpret_cast<const float4*>(Sc + noff);
+    const float4 sc1 = *reinterpret_cast<const float4*>(Sc + noff + BU);
     float o0[4], o1[4];
     if (C.dplane) {
         const float f = (U.ray[s].up ? 1.f : 0.f) - C.a_cur;
-        o0[0] = f * scB.x; o0[1] = f * scB.y; o0[2] = f * scB.z; o0[3] = f * scB.w;
-        o1[0] = f * scC.x; o1[1] = f * scC.y; o1[2] = f * scC.z; o1[3] = f * scC.w;
+        o0[0] = f * sc0.x; o0[1] = f * sc0.y; o0[2] = f * sc0.z; o0[3] = f * sc0.w;
+        o1[0] = f * sc1.x; o1[1] = f * sc1.y; o1[2] = f * sc1.z; o1[3] = f * sc1.w;
     } else {
-        // carried plane: rows (A,B,C) for SV > 0, (B,C,D) for SV < 0
-        float x0[6], x1[6], x2[6];
-        const float* xr = Xr + boff + (SV > 0 ? -G.BU : 0);
-        load_row5<SU>(xr, l_ok, r_ok, x0);
-        load_row5<SU>(xr + G.BU, l_ok, r_ok, x1);
-        load_row5<SU>(xr + 2 * G.BU, l_ok, r_ok, x2);
+        float dt0[4], dt1[4];
+        {
+            float k0[6], k1[6], k2[6];
+            load_row5<SU>(Kp + off, l_ok, r_ok, k0);
+            load_row5<SU>(Kp + off + BU, l_ok, r_ok, k1);
+            load_row5<SU>(Kp + off + 2 * BU, l_ok, r_ok, k2);
+            const float4 kv = *reinterpret_cast<const float4*>(U.ray[s].wk);
+            const float kc = U.ray[s].kc;
+            row_dtau<SU>(k0, k1, *reinterpret_cast<const float4*>(Kc + noff), kv, kc, dt0);
+            row_dtau<SU>(k1, k2, *reinterpret_cast<const float4*>(Kc + noff + BU), kv, kc, dt1);
+        }
         bool small = false;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) small |= (dt[0][j] < DTAU_SERIES) | (dt[1][j] < DTAU_SERIES);
+        for (int j = 0; j < 4; ++j) small |= (dt0[j] < DTAU_SERIES) | (dt1[j] < DTAU_SERIES);
         const bool any_small = __any_sync(0xffffffffu, act && small);
+        float s0[6], s1[6], s2[6], x0[6], x1[6], x2[6];
+        load_row5<SU>(Sp + off, l_ok, r_ok, s0);
+        load_row5<SU>(Sp + off + BU, l_ok, r_ok, s1);
+        load_row5<SU>(Sp + off + 2 * BU, l_ok, r_ok, s2);
+        load_row5<SU>(Xr + off, l_ok, r_ok, x0);
+        load_row5<SU>(Xr + off + BU, l_ok, r_ok, x1);
+        load_row5<SU>(Xr + off + 2 * BU, l_ok, r_ok, x2);
         const float4 wv = *reinterpret_cast<const float4*>(U.ray[s].wx);
-        // regime of the three stencil rows
+        // a on the three stencil rows and at the two node rows
         int reg;
-        float aA, aB, aC;                                    // a on rows (first, second, third) of this slot
+        float a0, a1, a2, ap0, ap1;
         if (G.zmarch) {
-            aA = aB = aC = C.a_prev;
+            a0 = a1 = a2 = C.a_prev; ap0 = ap1 = C.a_cur;
             reg = (C.a_prev != 0.f && C.a_cur != 0.f) ? 0 : ((C.a_prev == 0.f && C.a_cur == 0.f) ? 1 : 2);
         } else {
-            const int v1 = vB + (SV > 0 ? -1 : 0);           // global v of the slot's first row
-            aA = (v1 <= G.kstar) ? 1.f : 0.f;
-            aB = (v1 + 1 <= G.kstar) ? 1.f : 0.f;
-            aC = (v1 + 2 <= G.kstar) ? 1.f : 0.f;
-            reg = (aC != 0.f) ? 0 : ((aA == 0.f) ? 1 : 2);
+            const int v0r = vN - (svp ? 1 : 0);
+            a0 = (v0r <= G.kstar) ? 1.f : 0.f;
+            a1 = (v0r + 1 <= G.kstar) ? 1.f : 0.f;
+            a2 = (v0r + 2 <= G.kstar) ? 1.f : 0.f;
+            ap0 = svp ? a1 : a0; ap1 = svp ? a2 : a1;
+            reg = (a2 != 0.f) ? 0 : ((a0 == 0.f) ? 1 : 2);
         }
-#define RTS_ROWS(REG)                                                                                  \
-    if (SV > 0) {                                                                                      \
-        row_update<SU, REG>(dt[0], sB, sA, x1, x0, scB, wv, aB, aA, G.zmarch ? C.a_cur : aB, any_small, o0); \
-        row_update<SU, REG>(dt[1], sC, sB, x2, x1, scC, wv, aC, aB, G.zmarch ? C.a_cur : aC, any_small, o1); \
-    } else {                                                                                           \
-        row_update<SU, REG>(dt[0], sB, sC, x0, x1, scB, wv, aA, aB, G.zmarch ? C.a_cur : aA, any_small, o0); \
-        row_update<SU, REG>(dt[1], sC, sD, x1, x2, scC, wv, aB, aC, G.zmarch ? C.a_cur : aB, any_small, o1); \
-    }
-        if (reg == 0) { RTS_ROWS(0) } else if (reg == 1) { RTS_ROWS(1) } else { RTS_ROWS(2) }
-#undef RTS_ROWS
+        if (reg == 0) {
+            row_update<SU, 0>(dt0, s0, s1, x0, x1, sc0, wv, a0, a1, ap0, any_small, o0);
+            row_update<SU, 0>(dt1, s1, s2, x1, x2, sc1, wv, a1, a2, ap1, any_small, o1);
+        } else if (reg == 1) {
+            row_update<SU, 1>(dt0, s0, s1, x0, x1, sc0, wv, a0, a1, ap0, any_small, o0);
+            row_update<SU, 1>(dt1, s1, s2, x1, x2, sc1, wv, a1, a2, ap1, any_small, o1);
+        } else {
+            row_update<SU, 2>(dt0, s0, s1, x0, x1, sc0, wv, a0, a1, ap0, any_small, o0);
+            row_update<SU, 2>(dt1, s1, s2, x1, x2, sc1, wv, a1, a2, ap1, any_small, o1);
+        }
         if (!G.zmarch) {
             // inflow row of a bounded v axis (v = z): I = S (upward, bottom row) or 0 (downward, top row)
-            const int drow = (SV > 0) ? 0 : U.n_v - 1;
-            if (vB == drow) {
-                const float f = (SV > 0 ? 1.f : 0.f) - ((vB <= G.kstar) ? 1.f : 0.f);
-                o0[0] = f * scB.x; o0[1] = f * scB.y; o0[2] = f * scB.z; o0[3] = f * scB.w;
+            const int drow = svp ? 0 : U.n_v - 1;
+            const float fu = svp ? 1.f : 0.f;
+            if (vN == drow) {
+                const float f = fu - ap0;
+                o0[0] = f * sc0.x; o0[1] = f * sc0.y; o0[2] = f * sc0.z; o0[3] = f * sc0.w;
             }
-            if (vB + 1 == drow) {
-                const float f = (SV > 0 ? 1.f : 0.f) - ((vB + 1 <= G.kstar) ? 1.f : 0.f);
-                o1[0] = f * scC.x; o1[1] = f * scC.y; o1[2] = f * scC.z; o1[3] = f * scC.w;
+            if (vN + 1 == drow) {
+                const float f = fu - ap1;
+                o1[0] = f * sc1.x; o1[1] = f * sc1.y; o1[2] = f * sc1.z; o1[3] = f * sc1.w;
             }
         }
     }
     if (!act) return;
 
     // ---- carried plane for the next step
-    float* xw = Xw + boff;
+    float* xw = Xw + noff;
     const bool full = (c0 == 0) && (c1 == 4);
-    if (actB) {
+    if (act0) {
         if (full) *reinterpret_cast<float4*>(xw) = make_float4(o0[0], o0[1], o0[2], o0[3]);
         else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) xw[j] = o0[j]; }
     }
-    if (actC) {
-        if (full) *reinterpret_cast<float4*>(xw + G.BU) = make_float4(o1[0], o1[1], o1[2], o1[3]);
-        else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) xw[G.BU + j] = o1[j]; }
+    if (act1) {
+        if (full) *reinterpret_cast<float4*>(xw + BU) = make_float4(o1[0], o1[1], o1[2], o1[3]);
+        else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) xw[BU + j] = o1[j]; }
     }
     if (!(C.hist || C.strips)) return;
 
-    // ---- core nodes only from here on
-    const int cq0 = 4 * quad;                                // box column of the quad
+    // ---- core nodes only from here on: seam histories and exchange strips
+    const int cq0 = 4 * quad;
     const bool core_q = (cq0 >= HALO) && (cq0 < HALO + G.wu);
-    const bool coreB = actB && rowB >= HALO && rowB < HALO + G.wv;
-    const bool coreC = actC && rowB + 1 >= HALO && rowB + 1 < HALO + G.wv;
-    if (!core_q || !(coreB || coreC)) return;
-    const int ug = G.u0 + cq0 - HALO;                        // global u of the quad
+    const bool core0 = act0 && rowN >= HALO && rowN < HALO + G.wv;
+    const bool core1 = act1 && rowN + 1 >= HALO && rowN + 1 < HALO + G.wv;
+    if (!core_q || !(core0 || core1)) return;
+    const int ug = G.u0 + cq0 - HALO;
     if (C.hist) {
         float* Gp = U.Gu + ((size_t)(C.pass & 1) * U.n_m + C.m) * (size_t)(NSLOT * (U.n_v + U.n_u4));
-        // far-u column of this ray: u = n_u-1 (su > 0) or u = 0 (su < 0)
-        const int fj = ((SU > 0) ? G.dhi_u - 1 : G.dlo_u) - cq0;
+        const int fj = ((SU > 0) ? G.dhi_u - 1 : G.dlo_u) - cq0;     // far-u column of this ray inside the quad?
         if (fj >= 0 && fj < 4) {
             const float f0 = fj == 0 ? o0[0] : fj == 1 ? o0[1] : fj == 2 ? o0[2] : o0[3];
             const float f1 = fj == 0 ? o1[0] : fj == 1 ? o1[1] : fj == 2 ? o1[2] : o1[3];
-            if (coreB) __stcg(Gp + s * U.n_v + vB, f0);
-            if (coreC) __stcg(Gp + s * U.n_v + vB + 1, f1);
+            if (core0) __stcg(Gp + s * U.n_v + vN, f0);
+            if (core1) __stcg(Gp + s * U.n_v + vN + 1, f1);
         }
         if (U.per_v) {
-            const int fr = (SV > 0) ? G.dhi_v - 1 : G.dlo_v;  // far-v row (box)
+            const int fr = svp ? G.dhi_v - 1 : G.dlo_v;               // far-v row (box)
             float* gv = Gp + NSLOT * U.n_v + s * U.n_u4 + ug;
             const int nv_ = min(4, HALO + G.wu - cq0);
-            if (coreB && rowB == fr) {
+            if (core0 && rowN == fr) {
                 if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), make_float4(o0[0], o0[1], o0[2], o0[3]));
                 else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j < nv_) __stcg(gv + j, o0[j]); }
             }
-            if (coreC && rowB + 1 == fr) {
+            if (core1 && rowN + 1 == fr) {
                 if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), make_float4(o1[0], o1[1], o1[2], o1[3]));
                 else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j < nv_) __stcg(gv + j, o1[j]); }
             }
@@ -289,55 +312,72 @@ __device__ __forceinline__ void do_slot(
     }
     if (C.strips) {
         const bool su_strip = (SU > 0) ? (cq0 + 4 > HALO + G.wu - U.K) : (cq0 - HALO < U.K);
-        float* xe = U.Xex + (((size_t)C.par_ex * NSLOT + s) * U.n_v + vB) * U.n_u4 + ug;
-        if (coreB) {
-            const bool sv_strip = (SV > 0) ? (HALO + G.wv - 1 - rowB < U.K) : (rowB - HALO < U.K);
+        float* xe = U.Xex + (((size_t)C.par_ex * NSLOT + s) * U.n_v + vN) * U.n_u4 + ug;
+        if (core0) {
+            const bool sv_strip = svp ? (HALO + G.wv - 1 - rowN < U.K) : (rowN - HALO < U.K);
             if (su_strip || sv_strip) __stcg(reinterpret_cast<float4*>(xe), make_float4(o0[0], o0[1], o0[2], o0[3]));
         }
-        if (coreC) {
-            const bool sv_strip = (SV > 0) ? (HALO + G.wv - 2 - rowB < U.K) : (rowB + 1 - HALO < U.K);
+        if (core1) {
+            const bool sv_strip = svp ? (HALO + G.wv - 2 - rowN < U.K) : (rowN + 1 - HALO < U.K);
             if (su_strip || sv_strip) __stcg(reinterpret_cast<float4*>(xe + U.n_u4), make_float4(o1[0], o1[1], o1[2], o1[3]));
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------
-__device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
+// shared-memory carve-up of a CTA (floats unless noted), every part 128-byte aligned
+struct SmemPlan {
+    int BU, BV, BOXP, guardA, guardB, items_max;
+    __host__ __device__ SmemPlan(int WU, int WV) {
+        BU = WU + 2 * HALO; BV = WV + 2 * HALO;
+        BOXP = (BU * BV + 31) & ~31;
+        guardA = (BU + 31) & ~31;
+        guardB = (2 * BU + 31) & ~31;
+        const int per_slot = ((WU + HALO) / 4) * ((WV + KMAX) / 2) + 32;      // one slot's items, padded to a warp
+        items_max = NSLOT * ((per_slot + 31) & ~31);
+    }
+    __host__ __device__ int floats() const { return guardA + (NSTAGE * 2 + 2 * NSLOT) * BOXP + guardB; }
+    __host__ __device__ int nghost_max() const { return NSLOT * (BU + BV); }
+    __host__ __device__ size_t bytes() const {
+        return (size_t)floats() * 4 + (size_t)nghost_max() * sizeof(GhostEnt) + (size_t)KMAX * items_max * 2;
+    }
+};
+
+__device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, float* __restrict__ smf,
                          float* __restrict__ Qa, float* __restrict__ Qb, float* __restrict__ Itop_all,
                          int* abortf)
 {
     const UnitDesc& U = S.U;
     const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31;
+    const SmemPlan SP(U.WU, U.WV);
     TileGeo G;
     const int tu = tile % U.ntu, tv = tile / U.ntu;
     G.u0 = tu * U.WU; G.v0 = tv * U.WV;
     G.wu = min(U.WU, U.n_u - G.u0); G.wv = min(U.WV, U.n_v - G.v0);
-    G.BU = U.WU + 2 * HALO; G.BV = U.WV + 2 * HALO; G.BOX = G.BU * G.BV;
+    G.BU = SP.BU; G.BV = SP.BV; G.BOXP = SP.BOXP;
     G.dlo_u = HALO - G.u0; G.dhi_u = HALO + U.n_u - G.u0;
     G.dlo_v = HALO - G.v0; G.dhi_v = HALO + U.n_v - G.v0;
     G.kstar = *U.kstar;
     G.zmarch = (U.march == 2);
-    const int BU = G.BU, BV = G.BV, BOX = G.BOX;
+    const int BU = G.BU, BV = G.BV, BOXP = G.BOXP;
     const int n_m = U.n_m, npass = U.npass, K = U.K;
     const int nsteps = n_m * npass;
     const bool zmarch = G.zmarch;
     const bool up_z = (U.dir > 0);                           // z-march: the unit's rays point up
 
-    // ---- shared memory: guard row | [NSTAGE][2][BOX] coefficient planes | [2][NSLOT][BOX] carried
-    //      planes (double buffered) | guard row | ghost table
-    float* const stage0 = smf + BU;
-    float* const Xb = stage0 + NSTAGE * 2 * BOX;
-    GhostEnt* const gt = reinterpret_cast<GhostEnt*>(Xb + 2 * NSLOT * BOX + BU);
-    const int ngh = NSLOT * (BV + BU);
+    float* const stage0 = smf + SP.guardA;                   // [NSTAGE][2][BOXP]
+    float* const Xb = stage0 + NSTAGE * 2 * BOXP;            // [2][NSLOT][BOXP]
+    GhostEnt* const gt = reinterpret_cast<GhostEnt*>(smf + SP.floats());
+    unsigned short* const itab = reinterpret_cast<unsigned short*>(gt + SP.nghost_max());   // [KMAX][items_max]
     uint64_t* const mbar = S.mbar;
 
-    for (int i = tid; i < 2 * BU + (NSTAGE * 2 + 2 * NSLOT) * BOX; i += T) smf[i] = 0.f;
+    for (int i = tid; i < SP.floats(); i += T) smf[i] = 0.f;
     if (tid == 0) {
         for (int i = 0; i < NSTAGE; ++i) mbar_init(&mbar[i], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        S.flag = 0;
+        S.flag = 0; S.nghost = 0;
     }
-    // ---- regions per remaining halo depth (threads 0..15), ghost table (all threads)
+    // ---- regions per remaining halo depth
     if (tid < KMAX * NSLOT) {
         const int hj = tid / NSLOT, s = tid % NSLOT;
         const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
@@ -353,75 +393,77 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
         }
         S.reg[hj][s] = r;
     }
-    for (int e = tid; e < ngh; e += T) {
-        const int s = e / (BV + BU), i = e - s * (BV + BU);
-        const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
-        GhostEnt g; g.xoff = -1; g.goff = 0; g.bv = 0; g.slot = s;
-        if (U.ray[s].active) {
-            const int gcol = (su > 0) ? G.dlo_u - 1 : G.dhi_u;
-            const int grow = (sv > 0) ? G.dlo_v - 1 : G.dhi_v;
-            if (i < BV) {                                    // ghost column, box row i
-                int v = G.v0 - HALO + i;
-                const bool okv = U.per_v || (v >= 0 && v < U.n_v);
-                if (gcol >= 0 && gcol < BU && okv) {
-                    v = wrap(v, U.n_v);
-                    g.xoff = s * BOX + i * BU + gcol; g.goff = s * U.n_v + v; g.bv = i;
-                }
-            } else if (U.per_v) {                            // ghost row, box column i - BV
-                const int bu = i - BV;
-                if (grow >= 0 && grow < BV) {
-                    const int u = wrap(G.u0 - HALO + bu, U.n_u);
-                    g.xoff = s * BOX + grow * BU + bu; g.goff = NSLOT * U.n_v + s * U.n_u4 + u; g.bv = grow;
-                }
-            }
-        }
-        gt[e] = g;
-    }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
-    if (tid < KMAX) {
-        int rmin = 1 << 30, rmax = 0, cmin = 1 << 30, cmax = 0;
+    // ---- item tables: slot | first node row << 2 | quad << 9 | padding << 15
+    for (int hj = 0; hj < KMAX; ++hj) {
+        unsigned short* tab = itab + hj * SP.items_max;
+        int cursor = 0;
         for (int s = 0; s < NSLOT; ++s) {
-            const int4 r = S.reg[tid][s];
-            if (r.y > r.x && r.w > r.z) { rmin = min(rmin, r.x); rmax = max(rmax, r.y); cmin = min(cmin, r.z); cmax = max(cmax, r.w); }
+            const int4 r = S.reg[hj][s];
+            if (r.y <= r.x || r.w <= r.z) continue;
+            const int qlo = r.z >> 2, nq = ((r.w + 3) >> 2) - qlo, np = (r.y - r.x + 1) >> 1;
+            const int n = nq * np, npad = (n + 31) & ~31;
+            for (int e = tid; e < npad; e += T) {
+                const int pr = (e < n) ? e / nq : 0, q = (e < n) ? e - pr * nq : 0;
+                tab[cursor + e] = (unsigned short)(s | ((r.x + 2 * pr) << 2) | ((qlo + q) << 9) | ((e < n) ? 0 : 0x8000));
+            }
+            cursor += npad;
         }
-        int4 un = make_int4(0, 0, 0, 0);
-        if (rmax > 0) { un.x = rmin & ~1; un.y = (rmax - un.x + 1) >> 1; un.z = cmin >> 2; un.w = ((cmax + 3) >> 2) - un.z; }
-        S.uni[tid] = un;
+        if (tid == 0) S.nitems[hj] = cursor;
+    }
+    // ---- seam ghosts of this tile (compact list)
+    for (int e = tid; e < SP.nghost_max(); e += T) {
+        const int s = e / (BV + BU), i = e - s * (BV + BU);
+        const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
+        if (!U.ray[s].active) continue;
+        GhostEnt g; g.xoff = -1; g.goff = 0; g.bv = 0; g.slot = s;
+        const int gcol = (su > 0) ? G.dlo_u - 1 : G.dhi_u;
+        const int grow = (sv > 0) ? G.dlo_v - 1 : G.dhi_v;
+        if (i < BV) {                                        // ghost column, box row i
+            int v = G.v0 - HALO + i;
+            const bool okv = U.per_v || (v >= 0 && v < U.n_v);
+            if (gcol >= 0 && gcol < BU && okv) {
+                v = wrap(v, U.n_v);
+                g.xoff = s * BOXP + i * BU + gcol; g.goff = s * U.n_v + v; g.bv = i;
+            }
+        } else if (U.per_v) {                                // ghost row, box column i - BV
+            const int bu = i - BV;
+            if (grow >= 0 && grow < BV) {
+                const int u = wrap(G.u0 - HALO + bu, U.n_u);
+                g.xoff = s * BOXP + grow * BU + bu; g.goff = NSLOT * U.n_v + s * U.n_u4 + u; g.bv = grow;
+            }
+        }
+        if (g.xoff >= 0) gt[atomicAdd(&S.nghost, 1)] = g;
     }
 
-    // ---- coefficient box rows that exist in memory, copy width
-    const int cr_lo = U.per_v ? 0 : max(0, G.dlo_v);
-    const int cr_hi = U.per_v ? min(BV, U.n_v + 2 * HALO - G.v0) : min(BV, G.dhi_v);
-    const int ncr = cr_hi - cr_lo;
-    const int cbw = min(BU, U.P - G.u0);
-    const uint32_t row_bytes = (uint32_t)cbw * 4u;
-    const float* const csrc0 = U.cbase + U.c_off + (long long)(G.v0 - HALO) * U.c_v + G.u0;
+    // ---- coefficient planes through the TMA ring
+    const CUtensorMap* const cmap = &maps.m[U.march];
+    const uint32_t stage_bytes = 2u * (uint32_t)(BU * BV) * 4u;
     auto plane_of = [&](int mm) { return (U.dir > 0) ? mm : n_m - 1 - mm; };
-    auto issue_load = [&](int pl, int st) {                  // warp 0, convergent
+    auto issue_load = [&](int pl, int st) {                  // one thread
         uint64_t* bar = &mbar[st];
-        if (lane == 0) mbar_expect_tx(bar, 2u * (uint32_t)ncr * row_bytes);
-        __syncwarp();
-        float* dst = stage0 + (size_t)st * 2 * BOX;
-        const float* src = csrc0 + (long long)pl * U.c_m;
-        for (int r = lane; r < 2 * ncr; r += 32) {
-            const int f = (r >= ncr) ? 1 : 0, bv = cr_lo + r - f * ncr;
-            bulk_load(dst + f * BOX + bv * BU, src + f * U.c_field + (long long)bv * U.c_v, row_bytes, bar);
-        }
+        mbar_expect_tx(bar, stage_bytes);
+        float* dst = stage0 + (size_t)st * 2 * BOXP;
+        const int c1 = zmarch ? G.v0 : (U.march == 1 ? pl + HALO : pl);
+        const int c2 = zmarch ? pl : G.v0 - HALO;
+        tensor_load4(dst, cmap, G.u0, c1, c2, 2 * U.band, bar);
+        tensor_load4(dst + BOXP, cmap, G.u0, c1, c2, 2 * U.band + 1, bar);
     };
-    if (tid < 32) {
+    if (tid == 0) {
         issue_load(plane_of(n_m - 1), NSTAGE - 1);           // the plane "before" step 0
         issue_load(plane_of(0), 0);
         if (nsteps > 1) issue_load(plane_of(1 % n_m), 1);
     }
     __syncthreads();
+    const int ngh = S.nghost;
 
     auto wait_stage = [&](int st, uint32_t par, int code) {
         unsigned spins = 0;
         while (!mbar_try_wait(&mbar[st], par)) { if (spin_abort(abortf, spins, code)) break; }
     };
     auto a_of = [&](int level) { return (level <= G.kstar) ? 1.f : 0.f; };
-    // value of I^(0) - a S at a box position of plane `msrc` (stage Sbox = its source function)
+    // value of I^(0) - a S at a box position of plane `msrc` (Sbox = its source-function box)
     auto x_initial = [&](const float* Sbox, int s, int bv, int xo_in_box, int msrc) {
         const float Sv = Sbox[xo_in_box];
         float a; bool dn, up;
@@ -433,12 +475,12 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
     // ---- x/y-march: X^(0) on the plane before step 0, whole box (halo and ghosts included)
     wait_stage(NSTAGE - 1, 0u, 5);
     if (!zmarch) {
-        const float* Sp = stage0 + ((NSTAGE - 1) * 2 + 1) * BOX;
-        for (int i = tid; i < BOX; i += T) {
+        const float* Sp = stage0 + ((NSTAGE - 1) * 2 + 1) * BOXP;
+        for (int i = tid; i < BU * BV; i += T) {
             const int bv = i / BU;
 #pragma unroll
             for (int s = 0; s < NSLOT; ++s)
-                if (U.ray[s].active) Xb[s * BOX + i] = x_initial(Sp, s, bv, i, n_m - 1);
+                if (U.ray[s].active) Xb[s * BOXP + i] = x_initial(Sp, s, bv, i, n_m - 1);
         }
     }
     __syncthreads();
@@ -447,9 +489,10 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
     float* const Itop_b = Itop_all ? Itop_all + (long long)U.band * U.it_sb : nullptr;
     const size_t g_plane = (size_t)NSLOT * (U.n_v + U.n_u4);
 
-    // heating and emergent intensity of the plane finished in the previous step (last pass):
-    // reads the new carried plane Xn and that plane's coefficients
-    auto q_pass = [&](const float* Kc, const float* Sc, const float* Xn, int m_done) {
+    // heating and emergent intensity of a finished plane (last pass): reads the new carried
+    // plane Xn and that plane's coefficients
+    auto q_pass = [&](const float* Kc, const float* Xn, int m_done) {
+        const float* Sc = Kc + BOXP;
         const int pl = plane_of(m_done);
         const int nqc = (G.wu + 3) >> 2;
         for (int e = tid; e < nqc * G.wv; e += T) {
@@ -466,7 +509,7 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
 #pragma unroll
             for (int s = 0; s < NSLOT; ++s) {
                 if (!U.ray[s].active) continue;
-                const float4 x = *reinterpret_cast<const float4*>(Xn + s * BOX + bo);
+                const float4 x = *reinterpret_cast<const float4*>(Xn + s * BOXP + bo);
                 const float xa[4] = {x.x, x.y, x.z, x.w};
                 const float wq = U.ray[s].wq;
 #pragma unroll
@@ -486,7 +529,6 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
             for (int j = 0; j < 4; ++j) if (j < nval) atomicAdd(qd + j, FOUR_PI * kpa[j] * acc[j]);
         }
     };
-
     // halo of the carried plane at a block start: K-deep strips of the upwind neighbours' planes
     auto load_halos = [&](float* Xc, int par) {
         for (int s = 0; s < NSLOT; ++s) {
@@ -494,7 +536,7 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
             const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
             const bool up_u = (su > 0) ? (tu > 0) : (tu < U.ntu - 1);
             const bool up_v = (sv > 0) ? (tv > 0) : (tv < U.ntv - 1);
-            // rows / columns of the halo-extended region (depth K), clipped to the domain
+            if (!up_u && !up_v) continue;
             const int rlo = max((sv > 0 && up_v) ? HALO - K : HALO, G.dlo_v);
             const int rhi = min((sv < 0 && up_v) ? HALO + G.wv + K : HALO + G.wv, G.dhi_v);
             const int clo = max((su > 0 && up_u) ? 0 : HALO, G.dlo_u);
@@ -508,7 +550,7 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
                 if (core) continue;
                 const int v = G.v0 - HALO + row, u = G.u0 - HALO + 4 * q;
                 const float4 x = __ldcg(reinterpret_cast<const float4*>(xe + (size_t)v * U.n_u4 + u));
-                float* d = Xc + s * BOX + row * BU + 4 * q;
+                float* d = Xc + s * BOXP + row * BU + 4 * q;
                 const int c0 = max(0, clo - 4 * q), c1 = min(4, chi - 4 * q);
                 if (c0 == 0 && c1 == 4) *reinterpret_cast<float4*>(d) = x;
                 else { const float xa[4] = {x.x, x.y, x.z, x.w};
@@ -517,33 +559,26 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
             }
         }
     };
-    // ghost columns / rows of the carried plane `msrc` (values of the previous pass `psrc`)
+    // seam ghosts: value of ghost entry e for the carried plane `msrc` from pass `psrc`
     auto ghost_fetch = [&](int e, int psrc, int msrc, const float* Sbox) -> float {
         const GhostEnt g = gt[e];
-        if (g.xoff < 0) return 0.f;
-        if (psrc < 0) return x_initial(Sbox, g.slot, g.bv, g.xoff - g.slot * BOX, msrc);
+        if (psrc < 0) return x_initial(Sbox, g.slot, g.bv, g.xoff - g.slot * BOXP, msrc);
         return __ldcg(U.Gu + ((size_t)(psrc & 1) * n_m + msrc) * g_plane + g.goff);
-    };
-    auto ghost_store = [&](int e, float* Xc, float val) {
-        const int xo = gt[e].xoff;
-        if (xo >= 0) Xc[xo] = val;
     };
 
     // ================================================================== the march
     int m = 0, pass = 0, cur = 0, gblk = 0;
+    int stc = 0, stp = NSTAGE - 1;                           // stages of this step's and the previous plane
+    uint32_t par_bits = 1u << (NSTAGE - 1);                  // stage NSTAGE-1 already served the plane before step 0
     for (int s_ = 0; s_ < nsteps; ++s_) {
-        const int stc = s_ % NSTAGE, stp = (s_ + NSTAGE - 1) % NSTAGE;
-        const uint32_t par_c = (uint32_t)((s_ / NSTAGE + (stc == NSTAGE - 1 ? 1 : 0)) & 1);
         const int blk0 = m - m % K, blen = min(K, n_m - blk0);
         const int hj = blen - 1 - (m - blk0);
         const bool blk_first = (m == blk0), blk_last = (hj == 0);
         const int pl = plane_of(m);
-        const float* const Kp = stage0 + (size_t)stp * 2 * BOX;
-        const float* const Sp = Kp + BOX;
-        const float* const Kc = stage0 + (size_t)stc * 2 * BOX;
-        const float* const Sc = Kc + BOX;
-        float* const Xr = Xb + cur * NSLOT * BOX;
-        float* const Xw = Xb + (cur ^ 1) * NSLOT * BOX;
+        const float* const Kp = stage0 + (size_t)stp * 2 * BOXP;
+        const float* const Kc = stage0 + (size_t)stc * 2 * BOXP;
+        float* const Xr = Xb + cur * NSLOT * BOXP;
+        float* const Xw = Xb + (cur ^ 1) * NSLOT * BOXP;
         const int m_prev = (m == 0) ? n_m - 1 : m - 1;
 
         // ---- block start: wait for the unit, fetch halos and seam ghosts of the previous plane
@@ -554,7 +589,7 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
                 unsigned spins = 0;
                 while (ld_acquire(U.barrier) < need) {
                     if (spin_abort(abortf, spins, 3 | (s_ << 4))) { S.flag = 1; break; }
-                    __nanosleep(64);
+                    __nanosleep(100);
                 }
                 if (ab != 0) S.flag = 1;
             }
@@ -562,113 +597,82 @@ __device__ void run_task(TaskShared& S, const int tile, float* __restrict__ smf,
             if (S.flag != 0) break;                          // uniform: the watchdog fired somewhere
             if (!(zmarch && m == 0)) {
                 load_halos(Xr, (gblk - 1) & 1);
-                __syncthreads();                             // halo quads may overlap a ghost column
-                for (int e = tid; e < ngh; e += T) ghost_store(e, Xr, ghost_fetch(e, pass - 1, m_prev, Sp));
+                __syncthreads();                             // a halo quad may overlap a ghost column
+                for (int e = tid; e < ngh; e += T) Xr[gt[e].xoff] = ghost_fetch(e, pass - 1, m_prev, Kp + BOXP);
+                __syncthreads();
             }
-            __syncthreads();
         }
-        wait_stage(stc, par_c, 2 | (s_ << 4));
+        wait_stage(stc, (par_bits >> stc) & 1u, 2 | (s_ << 4));
+        par_bits ^= 1u << stc;
         const bool lastpass = (pass == npass - 1);
         // ---- heating / emergent intensity of the previous step's plane
-        if (lastpass && m > 0) q_pass(Kp, Sp, Xr, m - 1);
+        if (lastpass && m > 0) q_pass(Kp, Xr, m - 1);
 
         // ---- seam ghosts for the next step (previous pass, this plane): fetch now, store after the update
-        const bool ghost_next = !blk_last && (s_ + 1 < nsteps);
+        const bool ghost_next = !blk_last && (s_ + 1 < nsteps) && ngh > 0;
         float gval[2] = {0.f, 0.f};
         if (ghost_next && pass > 0) {
 #pragma unroll
-            for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) gval[i] = ghost_fetch(e, pass - 1, m, Sc); }
+            for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) gval[i] = ghost_fetch(e, pass - 1, m, nullptr); }
         }
 
-        // ---- the update: one 4 x 2 node block per thread and round, all slots
+        // ---- the update
         StepCtx C;
         C.m = m; C.pl = pl; C.pass = pass; C.hj = hj; C.par_ex = gblk & 1;
         C.dplane = zmarch && (m == 0);
         C.hist = !lastpass;
         C.strips = blk_last && (s_ + 1 < nsteps) && !(zmarch && m == n_m - 1);
         C.a_prev = a_of(pl - U.dir); C.a_cur = a_of(pl);
-        const int4 un = S.uni[hj];
-        const int nitems = un.y * un.w;
-        for (int it0 = 0; it0 < nitems; it0 += T) {
-            const int it = it0 + tid;
-            const bool valid = it < nitems;
-            const int idx = min(it, nitems - 1);
-            const int pr = idx / un.w, q = idx - pr * un.w;
-            const int rowB = un.x + 2 * pr, quad = un.z + q;
-            const int boff = rowB * BU + 4 * quad;
-            const bool l_ok = (lane > 0) && (q > 0);
-            const bool r_ok = (lane < 31) && (q < un.w - 1) && (it + 1 < nitems);
-            float dt[NSLOT][2][4];
-            float4 scB, scC;
-            if (!C.dplane) {
-                float kA[6], kB[6], kC[6], kD[6];
-                load_row6(Kp + boff - BU, l_ok, r_ok, kA);
-                load_row6(Kp + boff, l_ok, r_ok, kB);
-                load_row6(Kp + boff + BU, l_ok, r_ok, kC);
-                load_row6(Kp + boff + 2 * BU, l_ok, r_ok, kD);
-                const float4 kcB = *reinterpret_cast<const float4*>(Kc + boff);
-                const float4 kcC = *reinterpret_cast<const float4*>(Kc + boff + BU);
-#define RTS_DT(s, SU, SV)                                                                       \
-    if (U.ray[s].active) {                                                                      \
-        const float4 kv = *reinterpret_cast<const float4*>(U.ray[s].wk);                        \
-        const float kc = U.ray[s].kc;                                                           \
-        row_dtau<SU>(kB, (SV > 0) ? kA : kC, kcB, kv, kc, dt[s][0]);                            \
-        row_dtau<SU>(kC, (SV > 0) ? kB : kD, kcC, kv, kc, dt[s][1]);                            \
-    }
-                RTS_DT(0, +1, +1) RTS_DT(1, -1, +1) RTS_DT(2, +1, -1) RTS_DT(3, -1, -1)
-#undef RTS_DT
+        {
+            const unsigned short* tab = itab + hj * SP.items_max;
+            const int nitems = S.nitems[hj];
+            for (int it = tid; it < nitems; it += T) {       // nitems is a multiple of 32: warps stay whole
+                const unsigned code = tab[it];
+                const int s = code & 3, rowN = (code >> 2) & 127, quad = (code >> 9) & 63;
+                const bool valid = !(code & 0x8000u);
+                const int4 rg = S.reg[hj][s];
+                const bool l_ok = (lane > 0) && (4 * quad > (rg.z & ~3));
+                const bool r_ok = (lane < 31) && (4 * quad + 4 < rg.w);
+                if (s & 1) do_item<-1>(s, S, G, C, Kp, Kc, Xr + s * BOXP, Xw + s * BOXP, rowN, quad, valid, l_ok, r_ok);
+                else       do_item<+1>(s, S, G, C, Kp, Kc, Xr + s * BOXP, Xw + s * BOXP, rowN, quad, valid, l_ok, r_ok);
             }
-            float sA[6], sB[6], sC[6], sD[6];
-            if (!C.dplane) {
-                load_row6(Sp + boff - BU, l_ok, r_ok, sA);
-                load_row6(Sp + boff, l_ok, r_ok, sB);
-                load_row6(Sp + boff + BU, l_ok, r_ok, sC);
-                load_row6(Sp + boff + 2 * BU, l_ok, r_ok, sD);
-            }
-            scB = *reinterpret_cast<const float4*>(Sc + boff);
-            scC = *reinterpret_cast<const float4*>(Sc + boff + BU);
-            if (U.ray[0].active) do_slot<+1, +1>(0, S, G, C, Xr, Xw, boff, rowB, quad, valid, l_ok, r_ok, dt[0], sA, sB, sC, sD, scB, scC);
-            if (U.ray[1].active) do_slot<-1, +1>(1, S, G, C, Xr + BOX, Xw + BOX, boff, rowB, quad, valid, l_ok, r_ok, dt[1], sA, sB, sC, sD, scB, scC);
-            if (U.ray[2].active) do_slot<+1, -1>(2, S, G, C, Xr + 2 * BOX, Xw + 2 * BOX, boff, rowB, quad, valid, l_ok, r_ok, dt[2], sA, sB, sC, sD, scB, scC);
-            if (U.ray[3].active) do_slot<-1, -1>(3, S, G, C, Xr + 3 * BOX, Xw + 3 * BOX, boff, rowB, quad, valid, l_ok, r_ok, dt[3], sA, sB, sC, sD, scB, scC);
         }
         // ---- seam ghosts of this plane into the new carried plane
         if (ghost_next) {
             if (pass > 0) {
 #pragma unroll
-                for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) ghost_store(e, Xw, gval[i]); }
-                for (int e = tid + 2 * T; e < ngh; e += T) ghost_store(e, Xw, ghost_fetch(e, pass - 1, m, Sc));
+                for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) Xw[gt[e].xoff] = gval[i]; }
+                for (int e = tid + 2 * T; e < ngh; e += T) Xw[gt[e].xoff] = ghost_fetch(e, pass - 1, m, nullptr);
             } else {
-                for (int e = tid; e < ngh; e += T) ghost_store(e, Xw, ghost_fetch(e, -1, m, Sc));
+                for (int e = tid; e < ngh; e += T) Xw[gt[e].xoff] = ghost_fetch(e, -1, m, Kc + BOXP);
             }
         }
         // ---- end of step; at a block end publish (release) before anybody waits
         __syncthreads();
-        if (blk_last && s_ + 1 < nsteps) {
-            ++gblk;
-            if (tid == 0) { __threadfence(); atomicAdd(U.barrier, 1); }
+        if (tid == 0) {
+            if (blk_last && s_ + 1 < nsteps) { __threadfence(); atomicAdd(U.barrier, 1); }
+            if (s_ + 2 < nsteps) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                int m2 = m + 2; if (m2 >= n_m) m2 -= n_m; if (m2 >= n_m) m2 %= n_m;
+                issue_load(plane_of(m2), stp);               // the previous plane's stage is free now
+            }
         }
-        if (tid < 32 && s_ + 2 < nsteps) {
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            issue_load(plane_of((m + 2) % n_m), (s_ + 2) % NSTAGE);
-        }
+        if (blk_last && s_ + 1 < nsteps) ++gblk;
         cur ^= 1;
         if (++m == n_m) { m = 0; ++pass; }
+        stp = stc; stc = (stc + 1 == NSTAGE) ? 0 : stc + 1;
     }
     // heating / emergent intensity of the last plane
-    if (S.flag == 0) {
-        const int sl = nsteps - 1;
-        q_pass(stage0 + (size_t)(sl % NSTAGE) * 2 * BOX, stage0 + (size_t)(sl % NSTAGE) * 2 * BOX + BOX,
-               Xb + cur * NSLOT * BOX, n_m - 1);
-    }
+    if (S.flag == 0) q_pass(stage0 + (size_t)stp * 2 * BOXP, Xb + cur * NSLOT * BOXP, n_m - 1);
     __syncthreads();
     if (tid == 0)
         for (int i = 0; i < NSTAGE; ++i)
             asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&mbar[i])) : "memory");
 }
 
-__global__ void __launch_bounds__(256, 2)
-rts_sweep_kernel(const UnitDesc* __restrict__ units, int nunits, int total_tickets, int* ticket_counter,
+__global__ void __launch_bounds__(RTS_SWEEP_THREADS, 2)
+rts_sweep_kernel(const __grid_constant__ SweepMaps maps, const UnitDesc* __restrict__ units, int nunits,
+                 int total_tickets, int* ticket_counter,
                  float* __restrict__ Qa, float* __restrict__ Qb, float* __restrict__ Itop_all, int* abortf)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -694,7 +698,7 @@ rts_sweep_kernel(const UnitDesc* __restrict__ units, int nunits, int total_ticke
             for (int w = threadIdx.x; w < (int)(sizeof(UnitDesc) / sizeof(int)); w += blockDim.x) dst[w] = src[w];
         }
         __syncthreads();
-        run_task(S, ticket - S.U.ticket_begin, reinterpret_cast<float*>(smem_raw), Qa, Qb, Itop_all, abortf);
+        run_task(S, maps, ticket - S.U.ticket_begin, reinterpret_cast<float*>(smem_raw), Qa, Qb, Itop_all, abortf);
     }
 }
 
