@@ -24,22 +24,12 @@
 #include "rts_kernels.cuh"
 
 #ifndef RTS_SWEEP_THREADS
-#define RTS_SWEEP_THREADS 512   // most threads of a sweep CTA (two CTAs per SM: <= 64 registers)
+#define RTS_SWEEP_THREADS 384   // most threads of a sweep CTA (two CTAs per SM: <= 80 registers)
 #endif
 
 namespace rts {
 
-struct GhostEnt { int xoff; int goff; int bv; int slot; };
-
 struct SweepMaps { CUtensorMap m[3]; };      // coefficient tensor of the x-, y-, z-march units
-
-struct TaskShared {
-    UnitDesc U;
-    int4 reg[KMAX][NSLOT];     // per remaining halo depth hj: rows [x, y), cols [z, w) a slot updates (box coords)
-    int  nitems[KMAX];
-    uint64_t mbar[NSTAGE];
-    int ticket, flag, nghost, pad;
-};
 
 // closed-form attenuation factors: em1 = 1 - e^-dt, wl = (1 - e^-dt)/dt
 __device__ __forceinline__ void att_closed(float dt, float& em1, float& wl) {
@@ -159,8 +149,40 @@ __device__ __forceinline__ void tensor_load4(void* dst, const CUtensorMap* map, 
                  ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
 }
 
+
+// Item descriptor (static for a task): x = node offset in the box | first node row << 16 | quad << 24,
+// y = flags.  An item is the 4 x 2 node block (rows rowN, rowN+1; columns 4*quad ..) of one slot.
+enum : unsigned {
+    IT_SLOT = 3u,            // bits 0-1
+    IT_D0_SH = 2,            // bits 2-4   halo depth of node row 0 (0: core side; 7: never active)
+    IT_D1_SH = 5,            // bits 5-7   halo depth of node row 1
+    IT_DQ = 1u << 8,         // halo quad: only active while the remaining halo depth is > 0
+    IT_LOK = 1u << 9,        // lane-1 holds the quad to the left / lane+1 the quad to the right
+    IT_ROK = 1u << 10,
+    IT_REG_SH = 11,          // bits 11-12 regime of the stencil rows (x/y-march; static)
+    IT_DIR0 = 1u << 13,      // node row is the inflow row of a bounded v axis
+    IT_DIR1 = 1u << 14,
+    IT_CORE0 = 1u << 15,     // node row and quad belong to the tile core
+    IT_CORE1 = 1u << 16,
+    IT_C0_SH = 17,           // bits 17-18 first valid column of the quad
+    IT_C1_SH = 19,           // bits 19-21 one past the last valid column (1..4)
+    IT_SPECIAL = 1u << 22,   // core item holding a far-u column or a far-v row: writes the seam history
+    IT_STRIP0 = 1u << 23,    // core node row lies in an exchange strip
+    IT_STRIP1 = 1u << 24,
+    IT_PAD = 1u << 25        // padding entry (keeps warps whole)
+};
+
+struct GhostEnt { unsigned short xoff_lo, bv; int goff; };   // 8 bytes; slot = goff >> 28, xoff = xoff_lo + slot * BOXP
+
+struct TaskShared {
+    UnitDesc U;
+    uint64_t mbar[NSTAGE];
+    int ticket, flag, nghost, nitems, nhalo, pad;
+};
+
 struct StepCtx {
-    int m, pl, pass, hj, par_ex;       // plane counter, plane index, pass, remaining halo depth, exchange parity
+    int m, pass, hj, par_ex;           // plane counter, pass, remaining halo depth, exchange parity
+    int zreg;                          // z-march: regime of this step (0, 1, 2)
     bool dplane;                       // z-march inflow plane: nodes are set, not updated
     bool hist, strips;                 // write seam histories / publish strips this step
     float a_prev, a_cur;               // z-march: a on the previous / this plane
@@ -173,29 +195,74 @@ struct TileGeo {
     bool zmarch;
 };
 
+// seam histories and exchange strips of a core item (rare path)
+struct PubCtx { int v0, u0, wu, far_u, far_v, m, pass, par_ex; bool hist, strips; };   // by value: keeps the callers' state in registers
+
+__device__ __noinline__ void item_publish(const UnitDesc* __restrict__ Up, const PubCtx P, const unsigned fl,
+                                          const int rowN, const int quad, const bool act0, const bool act1,
+                                          const float4 o0, const float4 o1)
+{
+    const UnitDesc& U = *Up;
+    const int s = fl & IT_SLOT;
+    const bool svp = !(s & 2);
+    const bool core0 = act0 && (fl & IT_CORE0), core1 = act1 && (fl & IT_CORE1);
+    if (!(core0 || core1)) return;
+    const int cq0 = 4 * quad;
+    const int vN = P.v0 + rowN - HALO, ug = P.u0 + cq0 - HALO;
+    if (P.hist && (fl & IT_SPECIAL)) {
+        float* Gp = U.Gu + ((size_t)(P.pass & 1) * U.n_m + P.m) * (size_t)(NSLOT * (U.n_v + U.n_u4));
+        const int fj = ((s & 1) ? (P.far_u & 0xffff) : (P.far_u >> 16)) - cq0;   // far-u column of this ray inside the quad?
+        if (fj >= 0 && fj < 4) {
+            const float f0 = fj == 0 ? o0.x : fj == 1 ? o0.y : fj == 2 ? o0.z : o0.w;
+            const float f1 = fj == 0 ? o1.x : fj == 1 ? o1.y : fj == 2 ? o1.z : o1.w;
+            if (core0) __stcg(Gp + s * U.n_v + vN, f0);
+            if (core1) __stcg(Gp + s * U.n_v + vN + 1, f1);
+        }
+        if (U.per_v) {
+            const int fr = svp ? (P.far_v >> 16) : (P.far_v & 0xffff);   // far-v row (box)
+            float* gv = Gp + NSLOT * U.n_v + s * U.n_u4 + ug;
+            const int nv_ = min(4, HALO + P.wu - cq0);
+            if (core0 && rowN == fr) {
+                if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), o0);
+                else { const float a[4] = {o0.x, o0.y, o0.z, o0.w}; for (int j = 0; j < nv_; ++j) __stcg(gv + j, a[j]); }
+            }
+            if (core1 && rowN + 1 == fr) {
+                if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), o1);
+                else { const float a[4] = {o1.x, o1.y, o1.z, o1.w}; for (int j = 0; j < nv_; ++j) __stcg(gv + j, a[j]); }
+            }
+        }
+    }
+    if (P.strips) {
+        float* xe = U.Xex + (((size_t)P.par_ex * NSLOT + s) * U.n_v + vN) * U.n_u4 + ug;
+        if (core0 && (fl & IT_STRIP0)) __stcg(reinterpret_cast<float4*>(xe), o0);
+        if (core1 && (fl & IT_STRIP1)) __stcg(reinterpret_cast<float4*>(xe + U.n_u4), o1);
+    }
+}
+
 // ------------------------------------------------------------------------------------------
-// One item: the 4 x 2 node block (rows rowN, rowN+1; columns 4*quad .. 4*quad+3, box coordinates)
-// of slot s.  All lanes of a warp call this together (shuffles); `valid` masks padding lanes.
+// One item.  All lanes of a warp call this together (shuffles); inactive lanes only load.
 template <int SU>
 __device__ __forceinline__ void do_item(
-    const int s, const TaskShared& S, const TileGeo& G, const StepCtx& C,
+    const uint2 d, const UnitDesc& U, const TileGeo& G, const StepCtx& C,
     const float* __restrict__ Kp, const float* __restrict__ Kc,   // previous / this plane: opacity box, source box at +BOXP
-    const float* __restrict__ Xr, float* __restrict__ Xw,         // carried plane of this slot: read / write box
-    const int rowN, const int quad, const bool valid, const bool l_ok, const bool r_ok)
+    const float* __restrict__ Xr_all, float* __restrict__ Xw_all, const int lane)
 {
-    const UnitDesc& U = S.U;
+    const unsigned fl = d.y;
+    const int s = fl & IT_SLOT;
     const int BU = G.BU;
     const bool svp = !(s & 2);                               // sv > 0
-    const int4 rg = S.reg[C.hj][s];
-    const bool act0 = rowN >= rg.x && rowN < rg.y;
-    const bool act1 = rowN + 1 >= rg.x && rowN + 1 < rg.y;
-    const int c0 = max(0, rg.z - 4 * quad), c1 = min(4, rg.w - 4 * quad);
-    const bool act = valid && (c0 < c1) && (act0 || act1);
-    const int noff = rowN * BU + 4 * quad;                   // node row 0
+    const int hj = C.hj;
+    const bool act0 = (int)((fl >> IT_D0_SH) & 7u) <= hj;
+    const bool act1 = (int)((fl >> IT_D1_SH) & 7u) <= hj;
+    const bool act = !(fl & IT_PAD) && ((fl & IT_DQ) ? hj > 0 : true) && (act0 || act1);
+    if (!__any_sync(0xffffffffu, act)) return;
+    const bool l_ok = (lane > 0) && (fl & IT_LOK);
+    const bool r_ok = (lane < 31) && (fl & IT_ROK);
+    const int noff = (int)(d.x & 0xffffu);                   // node row 0
     const int off = noff - (svp ? BU : 0);                   // first stencil row: rows (R0, R1, R2)
-    const int vN = G.v0 + rowN - HALO;                       // global v of node row 0
     const float* const Sp = Kp + G.BOXP;
     const float* const Sc = Kc + G.BOXP;
+    const float* const Xr = Xr_all + s * G.BOXP;
     const float4 sc0 = *reinterpret_cast<const float4*>(Sc + noff);
     const float4 sc1 = *reinterpret_cast<const float4*>(Sc + noff + BU);
     float o0[4], o1[4];
@@ -227,40 +294,37 @@ __device__ __forceinline__ void do_item(
         load_row5<SU>(Xr + off + BU, l_ok, r_ok, x1);
         load_row5<SU>(Xr + off + 2 * BU, l_ok, r_ok, x2);
         const float4 wv = *reinterpret_cast<const float4*>(U.ray[s].wx);
-        // a on the three stencil rows and at the two node rows
-        int reg;
-        float a0, a1, a2, ap0, ap1;
-        if (G.zmarch) {
-            a0 = a1 = a2 = C.a_prev; ap0 = ap1 = C.a_cur;
-            reg = (C.a_prev != 0.f && C.a_cur != 0.f) ? 0 : ((C.a_prev == 0.f && C.a_cur == 0.f) ? 1 : 2);
-        } else {
-            const int v0r = vN - (svp ? 1 : 0);
-            a0 = (v0r <= G.kstar) ? 1.f : 0.f;
-            a1 = (v0r + 1 <= G.kstar) ? 1.f : 0.f;
-            a2 = (v0r + 2 <= G.kstar) ? 1.f : 0.f;
-            ap0 = svp ? a1 : a0; ap1 = svp ? a2 : a1;
-            reg = (a2 != 0.f) ? 0 : ((a0 == 0.f) ? 1 : 2);
-        }
+        const int reg = G.zmarch ? C.zreg : (int)((fl >> IT_REG_SH) & 3u);
         if (reg == 0) {
-            row_update<SU, 0>(dt0, s0, s1, x0, x1, sc0, wv, a0, a1, ap0, any_small, o0);
-            row_update<SU, 0>(dt1, s1, s2, x1, x2, sc1, wv, a1, a2, ap1, any_small, o1);
+            row_update<SU, 0>(dt0, s0, s1, x0, x1, sc0, wv, 1.f, 1.f, 1.f, any_small, o0);
+            row_update<SU, 0>(dt1, s1, s2, x1, x2, sc1, wv, 1.f, 1.f, 1.f, any_small, o1);
         } else if (reg == 1) {
-            row_update<SU, 1>(dt0, s0, s1, x0, x1, sc0, wv, a0, a1, ap0, any_small, o0);
-            row_update<SU, 1>(dt1, s1, s2, x1, x2, sc1, wv, a1, a2, ap1, any_small, o1);
+            row_update<SU, 1>(dt0, s0, s1, x0, x1, sc0, wv, 0.f, 0.f, 0.f, any_small, o0);
+            row_update<SU, 1>(dt1, s1, s2, x1, x2, sc1, wv, 0.f, 0.f, 0.f, any_small, o1);
         } else {
+            // a on the three stencil rows and at the two node rows
+            float a0, a1, a2, ap0, ap1;
+            if (G.zmarch) { a0 = a1 = a2 = C.a_prev; ap0 = ap1 = C.a_cur; }
+            else {
+                const int v0r = G.v0 + (int)((d.x >> 16) & 0xffu) - HALO - (svp ? 1 : 0);
+                a0 = (v0r <= G.kstar) ? 1.f : 0.f;
+                a1 = (v0r + 1 <= G.kstar) ? 1.f : 0.f;
+                a2 = (v0r + 2 <= G.kstar) ? 1.f : 0.f;
+                ap0 = svp ? a1 : a0; ap1 = svp ? a2 : a1;
+            }
             row_update<SU, 2>(dt0, s0, s1, x0, x1, sc0, wv, a0, a1, ap0, any_small, o0);
             row_update<SU, 2>(dt1, s1, s2, x1, x2, sc1, wv, a1, a2, ap1, any_small, o1);
         }
-        if (!G.zmarch) {
+        if (fl & (IT_DIR0 | IT_DIR1)) {
             // inflow row of a bounded v axis (v = z): I = S (upward, bottom row) or 0 (downward, top row)
-            const int drow = svp ? 0 : U.n_v - 1;
+            const int vN = G.v0 + (int)((d.x >> 16) & 0xffu) - HALO;
             const float fu = svp ? 1.f : 0.f;
-            if (vN == drow) {
-                const float f = fu - ap0;
+            if (fl & IT_DIR0) {
+                const float f = fu - ((vN <= G.kstar) ? 1.f : 0.f);
                 o0[0] = f * sc0.x; o0[1] = f * sc0.y; o0[2] = f * sc0.z; o0[3] = f * sc0.w;
             }
-            if (vN + 1 == drow) {
-                const float f = fu - ap1;
+            if (fl & IT_DIR1) {
+                const float f = fu - ((vN + 1 <= G.kstar) ? 1.f : 0.f);
                 o1[0] = f * sc1.x; o1[1] = f * sc1.y; o1[2] = f * sc1.z; o1[3] = f * sc1.w;
             }
         }
@@ -268,78 +332,47 @@ __device__ __forceinline__ void do_item(
     if (!act) return;
 
     // ---- carried plane for the next step
-    float* xw = Xw + noff;
+    float* xw = Xw_all + s * G.BOXP + noff;
+    const int c0 = (int)((fl >> IT_C0_SH) & 3u), c1 = (int)((fl >> IT_C1_SH) & 7u);
     const bool full = (c0 == 0) && (c1 == 4);
+    const float4 v0_ = make_float4(o0[0], o0[1], o0[2], o0[3]), v1_ = make_float4(o1[0], o1[1], o1[2], o1[3]);
     if (act0) {
-        if (full) *reinterpret_cast<float4*>(xw) = make_float4(o0[0], o0[1], o0[2], o0[3]);
+        if (full) *reinterpret_cast<float4*>(xw) = v0_;
         else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) xw[j] = o0[j]; }
     }
     if (act1) {
-        if (full) *reinterpret_cast<float4*>(xw + BU) = make_float4(o1[0], o1[1], o1[2], o1[3]);
+        if (full) *reinterpret_cast<float4*>(xw + BU) = v1_;
         else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) xw[BU + j] = o1[j]; }
     }
-    if (!(C.hist || C.strips)) return;
-
-    // ---- core nodes only from here on: seam histories and exchange strips
-    const int cq0 = 4 * quad;
-    const bool core_q = (cq0 >= HALO) && (cq0 < HALO + G.wu);
-    const bool core0 = act0 && rowN >= HALO && rowN < HALO + G.wv;
-    const bool core1 = act1 && rowN + 1 >= HALO && rowN + 1 < HALO + G.wv;
-    if (!core_q || !(core0 || core1)) return;
-    const int ug = G.u0 + cq0 - HALO;
-    if (C.hist) {
-        float* Gp = U.Gu + ((size_t)(C.pass & 1) * U.n_m + C.m) * (size_t)(NSLOT * (U.n_v + U.n_u4));
-        const int fj = ((SU > 0) ? G.dhi_u - 1 : G.dlo_u) - cq0;     // far-u column of this ray inside the quad?
-        if (fj >= 0 && fj < 4) {
-            const float f0 = fj == 0 ? o0[0] : fj == 1 ? o0[1] : fj == 2 ? o0[2] : o0[3];
-            const float f1 = fj == 0 ? o1[0] : fj == 1 ? o1[1] : fj == 2 ? o1[2] : o1[3];
-            if (core0) __stcg(Gp + s * U.n_v + vN, f0);
-            if (core1) __stcg(Gp + s * U.n_v + vN + 1, f1);
-        }
-        if (U.per_v) {
-            const int fr = svp ? G.dhi_v - 1 : G.dlo_v;               // far-v row (box)
-            float* gv = Gp + NSLOT * U.n_v + s * U.n_u4 + ug;
-            const int nv_ = min(4, HALO + G.wu - cq0);
-            if (core0 && rowN == fr) {
-                if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), make_float4(o0[0], o0[1], o0[2], o0[3]));
-                else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j < nv_) __stcg(gv + j, o0[j]); }
-            }
-            if (core1 && rowN + 1 == fr) {
-                if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), make_float4(o1[0], o1[1], o1[2], o1[3]));
-                else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j < nv_) __stcg(gv + j, o1[j]); }
-            }
-        }
-    }
-    if (C.strips) {
-        const bool su_strip = (SU > 0) ? (cq0 + 4 > HALO + G.wu - U.K) : (cq0 - HALO < U.K);
-        float* xe = U.Xex + (((size_t)C.par_ex * NSLOT + s) * U.n_v + vN) * U.n_u4 + ug;
-        if (core0) {
-            const bool sv_strip = svp ? (HALO + G.wv - 1 - rowN < U.K) : (rowN - HALO < U.K);
-            if (su_strip || sv_strip) __stcg(reinterpret_cast<float4*>(xe), make_float4(o0[0], o0[1], o0[2], o0[3]));
-        }
-        if (core1) {
-            const bool sv_strip = svp ? (HALO + G.wv - 2 - rowN < U.K) : (rowN + 1 - HALO < U.K);
-            if (su_strip || sv_strip) __stcg(reinterpret_cast<float4*>(xe + U.n_u4), make_float4(o1[0], o1[1], o1[2], o1[3]));
-        }
+    if ((C.hist && (fl & IT_SPECIAL)) || (C.strips && (fl & (IT_STRIP0 | IT_STRIP1)))) {
+        PubCtx P;
+        P.v0 = G.v0; P.u0 = G.u0; P.wu = G.wu;
+        P.far_u = ((G.dhi_u - 1) << 16) | (G.dlo_u & 0xffff);   // far-u column (box) of su > 0 | su < 0 rays
+        P.far_v = ((G.dhi_v - 1) << 16) | (G.dlo_v & 0xffff);
+        P.m = C.m; P.pass = C.pass; P.par_ex = C.par_ex; P.hist = C.hist; P.strips = C.strips;
+        item_publish(&U, P, fl, (int)((d.x >> 16) & 0xffu), (int)(d.x >> 24), act0, act1, v0_, v1_);
     }
 }
 
 // ------------------------------------------------------------------------------------------
-// shared-memory carve-up of a CTA (floats unless noted), every part 128-byte aligned
+// shared-memory carve-up of a CTA, every part 128-byte aligned
+struct HaloEnt { unsigned short xoff_lo; unsigned char slot, mask; int goff; };   // mask = c0 | c1 << 4
+
 struct SmemPlan {
-    int BU, BV, BOXP, guardA, guardB, items_max;
+    int BU, BV, BOXP, guardA, guardB, items_max, nghost_max, nhalo_max;
     __host__ __device__ SmemPlan(int WU, int WV) {
         BU = WU + 2 * HALO; BV = WV + 2 * HALO;
         BOXP = (BU * BV + 31) & ~31;
         guardA = (BU + 31) & ~31;
         guardB = (2 * BU + 31) & ~31;
-        const int per_slot = ((WU + HALO) / 4) * ((WV + KMAX) / 2) + 32;      // one slot's items, padded to a warp
+        const int per_slot = ((WU + HALO) / 4) * ((WV + KMAX) / 2);            // one slot's items (largest region)
         items_max = NSLOT * ((per_slot + 31) & ~31);
+        nghost_max = NSLOT * (BU + BV);
+        nhalo_max = NSLOT * (WV + KMAX + KMAX * ((WU + HALO) / 4));
     }
     __host__ __device__ int floats() const { return guardA + (NSTAGE * 2 + 2 * NSLOT) * BOXP + guardB; }
-    __host__ __device__ int nghost_max() const { return NSLOT * (BU + BV); }
     __host__ __device__ size_t bytes() const {
-        return (size_t)floats() * 4 + (size_t)nghost_max() * sizeof(GhostEnt) + (size_t)KMAX * items_max * 2;
+        return (size_t)floats() * 4 + (size_t)items_max * 8 + (size_t)nghost_max * sizeof(GhostEnt) + (size_t)nhalo_max * sizeof(HaloEnt);
     }
 };
 
@@ -367,77 +400,21 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
 
     float* const stage0 = smf + SP.guardA;                   // [NSTAGE][2][BOXP]
     float* const Xb = stage0 + NSTAGE * 2 * BOXP;            // [2][NSLOT][BOXP]
-    GhostEnt* const gt = reinterpret_cast<GhostEnt*>(smf + SP.floats());
-    unsigned short* const itab = reinterpret_cast<unsigned short*>(gt + SP.nghost_max());   // [KMAX][items_max]
+    uint2* const itab = reinterpret_cast<uint2*>(smf + SP.floats());
+    GhostEnt* const gt = reinterpret_cast<GhostEnt*>(itab + SP.items_max);
+    HaloEnt* const ht = reinterpret_cast<HaloEnt*>(gt + SP.nghost_max);
     uint64_t* const mbar = S.mbar;
 
     for (int i = tid; i < SP.floats(); i += T) smf[i] = 0.f;
     if (tid == 0) {
         for (int i = 0; i < NSTAGE; ++i) mbar_init(&mbar[i], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        S.flag = 0; S.nghost = 0;
-    }
-    // ---- regions per remaining halo depth
-    if (tid < KMAX * NSLOT) {
-        const int hj = tid / NSLOT, s = tid % NSLOT;
-        const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
-        int4 r = make_int4(0, 0, 0, 0);
-        if (U.ray[s].active) {
-            const bool up_u = (su > 0) ? (tu > 0) : (tu < U.ntu - 1);
-            const bool up_v = (sv > 0) ? (tv > 0) : (tv < U.ntv - 1);
-            const int hu = (up_u && hj > 0) ? HALO : 0, hv = up_v ? hj : 0;
-            r.z = max((su > 0) ? HALO - hu : HALO, G.dlo_u);
-            r.w = min((su > 0) ? HALO + G.wu : HALO + G.wu + hu, G.dhi_u);
-            r.x = max((sv > 0) ? HALO - hv : HALO, G.dlo_v);
-            r.y = min((sv > 0) ? HALO + G.wv : HALO + G.wv + hv, G.dhi_v);
-        }
-        S.reg[hj][s] = r;
+        S.flag = 0; S.nghost = 0; S.nhalo = 0;
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
-    // ---- item tables: slot | first node row << 2 | quad << 9 | padding << 15
-    for (int hj = 0; hj < KMAX; ++hj) {
-        unsigned short* tab = itab + hj * SP.items_max;
-        int cursor = 0;
-        for (int s = 0; s < NSLOT; ++s) {
-            const int4 r = S.reg[hj][s];
-            if (r.y <= r.x || r.w <= r.z) continue;
-            const int qlo = r.z >> 2, nq = ((r.w + 3) >> 2) - qlo, np = (r.y - r.x + 1) >> 1;
-            const int n = nq * np, npad = (n + 31) & ~31;
-            for (int e = tid; e < npad; e += T) {
-                const int pr = (e < n) ? e / nq : 0, q = (e < n) ? e - pr * nq : 0;
-                tab[cursor + e] = (unsigned short)(s | ((r.x + 2 * pr) << 2) | ((qlo + q) << 9) | ((e < n) ? 0 : 0x8000));
-            }
-            cursor += npad;
-        }
-        if (tid == 0) S.nitems[hj] = cursor;
-    }
-    // ---- seam ghosts of this tile (compact list)
-    for (int e = tid; e < SP.nghost_max(); e += T) {
-        const int s = e / (BV + BU), i = e - s * (BV + BU);
-        const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
-        if (!U.ray[s].active) continue;
-        GhostEnt g; g.xoff = -1; g.goff = 0; g.bv = 0; g.slot = s;
-        const int gcol = (su > 0) ? G.dlo_u - 1 : G.dhi_u;
-        const int grow = (sv > 0) ? G.dlo_v - 1 : G.dhi_v;
-        if (i < BV) {                                        // ghost column, box row i
-            int v = G.v0 - HALO + i;
-            const bool okv = U.per_v || (v >= 0 && v < U.n_v);
-            if (gcol >= 0 && gcol < BU && okv) {
-                v = wrap(v, U.n_v);
-                g.xoff = s * BOXP + i * BU + gcol; g.goff = s * U.n_v + v; g.bv = i;
-            }
-        } else if (U.per_v) {                                // ghost row, box column i - BV
-            const int bu = i - BV;
-            if (grow >= 0 && grow < BV) {
-                const int u = wrap(G.u0 - HALO + bu, U.n_u);
-                g.xoff = s * BOXP + grow * BU + bu; g.goff = NSLOT * U.n_v + s * U.n_u4 + u; g.bv = grow;
-            }
-        }
-        if (g.xoff >= 0) gt[atomicAdd(&S.nghost, 1)] = g;
-    }
 
-    // ---- coefficient planes through the TMA ring
+    // ---- coefficient planes through the TMA ring (started first: the tables below hide its latency)
     const CUtensorMap* const cmap = &maps.m[U.march];
     const uint32_t stage_bytes = 2u * (uint32_t)(BU * BV) * 4u;
     auto plane_of = [&](int mm) { return (U.dir > 0) ? mm : n_m - 1 - mm; };
@@ -455,8 +432,124 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
         issue_load(plane_of(0), 0);
         if (nsteps > 1) issue_load(plane_of(1 % n_m), 1);
     }
+
+    // ---- item table: per slot the 4 x 2 blocks of its largest region (halo depth K-1)
+    {
+        const int hmax = K - 1;
+        int cursor = 0;
+        for (int s = 0; s < NSLOT; ++s) {
+            if (!U.ray[s].active) continue;
+            const int su = (s & 1) ? -1 : 1;
+            const bool svp = !(s & 2);
+            const bool up_u = (su > 0) ? (tu > 0) : (tu < U.ntu - 1);
+            const bool up_v = svp ? (tv > 0) : (tv < U.ntv - 1);
+            const int hu = (up_u && hmax > 0) ? HALO : 0, hv = up_v ? hmax : 0;
+            const int clo = max((su > 0) ? HALO - hu : HALO, G.dlo_u);
+            const int chi = min((su > 0) ? HALO + G.wu : HALO + G.wu + hu, G.dhi_u);
+            const int rlo = max(svp ? HALO - hv : HALO, G.dlo_v);
+            const int rhi = min(svp ? HALO + G.wv : HALO + G.wv + hv, G.dhi_v);
+            if (rhi <= rlo || chi <= clo) continue;
+            const int qlo = clo >> 2, nq = ((chi + 3) >> 2) - qlo, np = (rhi - rlo + 1) >> 1;
+            const int n = nq * np, npad = (n + 31) & ~31;
+            const int fr = svp ? G.dhi_v - 1 : G.dlo_v;       // far-v row of this slot (box)
+            const int fc = (su > 0) ? G.dhi_u - 1 : G.dlo_u;  // far-u column of this slot (box)
+            const int drow = svp ? 0 : U.n_v - 1;             // inflow row (x/y-march), global v
+            for (int e = tid; e < npad; e += T) {
+                uint2 d = make_uint2(0u, (unsigned)s | IT_PAD | (7u << IT_D0_SH) | (7u << IT_D1_SH));
+                const int pr = (e < n) ? e / nq : 0, q = qlo + ((e < n) ? e - pr * nq : 0);
+                const int rowN = rlo + 2 * pr;
+                d.x = (unsigned)(rowN * BU + 4 * q) | ((unsigned)rowN << 16) | ((unsigned)q << 24);
+                if (e < n) {
+                    unsigned fl = (unsigned)s;
+                    auto depth = [&](int row) {
+                        if (row < rlo || row >= rhi) return 7;
+                        return svp ? max(0, HALO - row) : max(0, row - (HALO + G.wv - 1));
+                    };
+                    fl |= (unsigned)depth(rowN) << IT_D0_SH;
+                    fl |= (unsigned)depth(rowN + 1) << IT_D1_SH;
+                    const int cq0 = 4 * q;
+                    const bool core_q = (cq0 >= HALO) && (cq0 < HALO + G.wu);
+                    if (!core_q) fl |= IT_DQ;
+                    if (q > qlo) fl |= IT_LOK;
+                    if (q < qlo + nq - 1) fl |= IT_ROK;
+                    const int vN = G.v0 + rowN - HALO;
+                    if (!zmarch) {
+                        const int v0r = vN - (svp ? 1 : 0);
+                        const unsigned reg = (v0r + 2 <= G.kstar) ? 0u : ((v0r > G.kstar) ? 1u : 2u);
+                        fl |= reg << IT_REG_SH;
+                        if (vN == drow) fl |= IT_DIR0;
+                        if (vN + 1 == drow) fl |= IT_DIR1;
+                    }
+                    const bool c0r = core_q && rowN >= HALO && rowN < HALO + G.wv;
+                    const bool c1r = core_q && rowN + 1 >= HALO && rowN + 1 < HALO + G.wv;
+                    if (c0r) fl |= IT_CORE0;
+                    if (c1r) fl |= IT_CORE1;
+                    fl |= (unsigned)max(0, clo - cq0) << IT_C0_SH;
+                    fl |= (unsigned)min(4, chi - cq0) << IT_C1_SH;
+                    const bool farc = (fc >= cq0 && fc < cq0 + 4);
+                    const bool farr = U.per_v && ((c0r && rowN == fr) || (c1r && rowN + 1 == fr));
+                    if ((c0r || c1r) && (farc || farr)) fl |= IT_SPECIAL;
+                    const bool su_strip = (su > 0) ? (cq0 + 4 > HALO + G.wu - K) : (cq0 - HALO < K);
+                    if (c0r && (su_strip || (svp ? (HALO + G.wv - 1 - rowN < K) : (rowN - HALO < K)))) fl |= IT_STRIP0;
+                    if (c1r && (su_strip || (svp ? (HALO + G.wv - 2 - rowN < K) : (rowN + 1 - HALO < K)))) fl |= IT_STRIP1;
+                    d.y = fl;
+                }
+                itab[cursor + e] = d;
+            }
+            cursor += npad;
+        }
+        if (tid == 0) S.nitems = cursor;
+    }
+    // ---- seam ghosts of this tile (compact list)
+    for (int e = tid; e < SP.nghost_max; e += T) {
+        const int s = e / (BV + BU), i = e - s * (BV + BU);
+        const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
+        if (!U.ray[s].active) continue;
+        int xoff = -1, goff = 0, bvv = 0;
+        const int gcol = (su > 0) ? G.dlo_u - 1 : G.dhi_u;
+        const int grow = (sv > 0) ? G.dlo_v - 1 : G.dhi_v;
+        if (i < BV) {                                        // ghost column, box row i
+            int v = G.v0 - HALO + i;
+            const bool okv = U.per_v || (v >= 0 && v < U.n_v);
+            if (gcol >= 0 && gcol < BU && okv) { v = wrap(v, U.n_v); xoff = i * BU + gcol; goff = s * U.n_v + v; bvv = i; }
+        } else if (U.per_v) {                                // ghost row, box column i - BV
+            const int bu = i - BV;
+            if (grow >= 0 && grow < BV) {
+                const int u = wrap(G.u0 - HALO + bu, U.n_u);
+                xoff = grow * BU + bu; goff = NSLOT * U.n_v + s * U.n_u4 + u; bvv = grow;
+            }
+        }
+        if (xoff >= 0) {
+            GhostEnt g; g.xoff_lo = (unsigned short)xoff; g.bv = (unsigned short)bvv; g.goff = goff | (s << 28);
+            gt[atomicAdd(&S.nghost, 1)] = g;
+        }
+    }
+    // ---- halo quads fetched at a block start (depth K), compact list
+    for (int s = 0; s < NSLOT; ++s) {
+        if (!U.ray[s].active) continue;
+        const int su = (s & 1) ? -1 : 1;
+        const bool svp = !(s & 2);
+        const bool up_u = (su > 0) ? (tu > 0) : (tu < U.ntu - 1);
+        const bool up_v = svp ? (tv > 0) : (tv < U.ntv - 1);
+        if (!up_u && !up_v) continue;
+        const int rlo = max((svp && up_v) ? HALO - K : HALO, G.dlo_v);
+        const int rhi = min((!svp && up_v) ? HALO + G.wv + K : HALO + G.wv, G.dhi_v);
+        const int clo = max((su > 0 && up_u) ? 0 : HALO, G.dlo_u);
+        const int chi = min((su < 0 && up_u) ? HALO + G.wu + HALO : HALO + G.wu, G.dhi_u);
+        const int q_lo = clo >> 2, nq = ((chi + 3) >> 2) - q_lo, nr = rhi - rlo;
+        for (int e = tid; e < nr * nq; e += T) {
+            const int r = e / nq, row = rlo + r, q = q_lo + (e - r * nq);
+            const bool core = (row >= HALO && row < HALO + G.wv) && (4 * q >= HALO && 4 * q < HALO + G.wu);
+            if (core) continue;
+            HaloEnt h;
+            h.xoff_lo = (unsigned short)(row * BU + 4 * q); h.slot = (unsigned char)s;
+            h.mask = (unsigned char)(max(0, clo - 4 * q) | (min(4, chi - 4 * q) << 4));
+            h.goff = (G.v0 - HALO + row) * U.n_u4 + (G.u0 - HALO + 4 * q);
+            ht[atomicAdd(&S.nhalo, 1)] = h;
+        }
+    }
     __syncthreads();
-    const int ngh = S.nghost;
+    const int ngh = S.nghost, nhalo = S.nhalo, nitems = S.nitems;
 
     auto wait_stage = [&](int st, uint32_t par, int code) {
         unsigned spins = 0;
@@ -531,139 +624,127 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     };
     // halo of the carried plane at a block start: K-deep strips of the upwind neighbours' planes
     auto load_halos = [&](float* Xc, int par) {
-        for (int s = 0; s < NSLOT; ++s) {
-            if (!U.ray[s].active) continue;
-            const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
-            const bool up_u = (su > 0) ? (tu > 0) : (tu < U.ntu - 1);
-            const bool up_v = (sv > 0) ? (tv > 0) : (tv < U.ntv - 1);
-            if (!up_u && !up_v) continue;
-            const int rlo = max((sv > 0 && up_v) ? HALO - K : HALO, G.dlo_v);
-            const int rhi = min((sv < 0 && up_v) ? HALO + G.wv + K : HALO + G.wv, G.dhi_v);
-            const int clo = max((su > 0 && up_u) ? 0 : HALO, G.dlo_u);
-            const int chi = min((su < 0 && up_u) ? HALO + G.wu + HALO : HALO + G.wu, G.dhi_u);
-            const int q_lo = clo >> 2, q_hi = (chi + 3) >> 2, nq = q_hi - q_lo;
-            const int nr = rhi - rlo;
-            const float* xe = U.Xex + ((size_t)par * NSLOT + s) * (size_t)U.n_v * U.n_u4;
-            for (int e = tid; e < nr * nq; e += T) {
-                const int r = e / nq, row = rlo + r, q = q_lo + (e - r * nq);
-                const bool core = (row >= HALO && row < HALO + G.wv) && (4 * q >= HALO && 4 * q < HALO + G.wu);
-                if (core) continue;
-                const int v = G.v0 - HALO + row, u = G.u0 - HALO + 4 * q;
-                const float4 x = __ldcg(reinterpret_cast<const float4*>(xe + (size_t)v * U.n_u4 + u));
-                float* d = Xc + s * BOXP + row * BU + 4 * q;
-                const int c0 = max(0, clo - 4 * q), c1 = min(4, chi - 4 * q);
-                if (c0 == 0 && c1 == 4) *reinterpret_cast<float4*>(d) = x;
-                else { const float xa[4] = {x.x, x.y, x.z, x.w};
+        const float* xe0 = U.Xex + (size_t)par * NSLOT * (size_t)U.n_v * U.n_u4;
+        for (int e = tid; e < nhalo; e += T) {
+            const HaloEnt h = ht[e];
+            const float4 x = __ldcg(reinterpret_cast<const float4*>(xe0 + (size_t)h.slot * U.n_v * U.n_u4 + h.goff));
+            float* d = Xc + h.slot * BOXP + h.xoff_lo;
+            const int c0 = h.mask & 15, c1 = h.mask >> 4;
+            if (c0 == 0 && c1 == 4) *reinterpret_cast<float4*>(d) = x;
+            else { const float xa[4] = {x.x, x.y, x.z, x.w};
 #pragma unroll
-                       for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) d[j] = xa[j]; }
-            }
+                   for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) d[j] = xa[j]; }
         }
     };
-    // seam ghosts: value of ghost entry e for the carried plane `msrc` from pass `psrc`
-    auto ghost_fetch = [&](int e, int psrc, int msrc, const float* Sbox) -> float {
-        const GhostEnt g = gt[e];
-        if (psrc < 0) return x_initial(Sbox, g.slot, g.bv, g.xoff - g.slot * BOXP, msrc);
-        return __ldcg(U.Gu + ((size_t)(psrc & 1) * n_m + msrc) * g_plane + g.goff);
+    // seam ghosts: value of ghost entry g for the carried plane `msrc` from pass `psrc`
+    auto ghost_fetch = [&](const GhostEnt g, int psrc, int msrc, const float* Sbox) -> float {
+        if (psrc < 0) return x_initial(Sbox, g.goff >> 28, g.bv, g.xoff_lo, msrc);
+        return __ldcg(U.Gu + ((size_t)(psrc & 1) * n_m + msrc) * g_plane + (g.goff & 0x0fffffff));
     };
+    auto ghost_off = [&](const GhostEnt g) { return (g.goff >> 28) * BOXP + g.xoff_lo; };
 
     // ================================================================== the march
-    int m = 0, pass = 0, cur = 0, gblk = 0;
+    int cur = 0, gblk = 0, s_ = 0;
     int stc = 0, stp = NSTAGE - 1;                           // stages of this step's and the previous plane
     uint32_t par_bits = 1u << (NSTAGE - 1);                  // stage NSTAGE-1 already served the plane before step 0
-    for (int s_ = 0; s_ < nsteps; ++s_) {
-        const int blk0 = m - m % K, blen = min(K, n_m - blk0);
-        const int hj = blen - 1 - (m - blk0);
-        const bool blk_first = (m == blk0), blk_last = (hj == 0);
-        const int pl = plane_of(m);
-        const float* const Kp = stage0 + (size_t)stp * 2 * BOXP;
-        const float* const Kc = stage0 + (size_t)stc * 2 * BOXP;
-        float* const Xr = Xb + cur * NSLOT * BOXP;
-        float* const Xw = Xb + (cur ^ 1) * NSLOT * BOXP;
-        const int m_prev = (m == 0) ? n_m - 1 : m - 1;
-
-        // ---- block start: wait for the unit, fetch halos and seam ghosts of the previous plane
-        if (blk_first && s_ > 0) {
-            if (tid == 0) {
-                const int need = gblk * U.ntiles;
-                const int ab = *reinterpret_cast<volatile int*>(abortf);
-                unsigned spins = 0;
-                while (ld_acquire(U.barrier) < need) {
-                    if (spin_abort(abortf, spins, 3 | (s_ << 4))) { S.flag = 1; break; }
-                    __nanosleep(100);
-                }
-                if (ab != 0) S.flag = 1;
-            }
-            __syncthreads();
-            if (S.flag != 0) break;                          // uniform: the watchdog fired somewhere
-            if (!(zmarch && m == 0)) {
-                load_halos(Xr, (gblk - 1) & 1);
-                __syncthreads();                             // a halo quad may overlap a ghost column
-                for (int e = tid; e < ngh; e += T) Xr[gt[e].xoff] = ghost_fetch(e, pass - 1, m_prev, Kp + BOXP);
-                __syncthreads();
-            }
-        }
-        wait_stage(stc, (par_bits >> stc) & 1u, 2 | (s_ << 4));
-        par_bits ^= 1u << stc;
+    bool bail = false;
+    for (int pass = 0; pass < npass && !bail; ++pass) {
         const bool lastpass = (pass == npass - 1);
-        // ---- heating / emergent intensity of the previous step's plane
-        if (lastpass && m > 0) q_pass(Kp, Xr, m - 1);
+        for (int blk0 = 0; blk0 < n_m && !bail; blk0 += K) {
+            const int blen = min(K, n_m - blk0);
+            // ---- block start: wait for the unit, fetch halos and seam ghosts of the previous plane
+            if (s_ > 0) {
+                if (tid == 0) {
+                    const int need = gblk * U.ntiles;
+                    const int ab = *reinterpret_cast<volatile int*>(abortf);
+                    unsigned spins = 0, ns = 32;
+                    while (!(U.pad0 & 1) && ld_acquire(U.barrier) < need) {
+                        if (spin_abort(abortf, spins, 3 | (s_ << 4))) { S.flag = 1; break; }
+                        __nanosleep(ns);
+                        if (ns < 2048) ns += ns;             // back off: a unit waiting for residency spins long
+                    }
+                    if (ab != 0) S.flag = 1;
+                }
+                __syncthreads();
+                if (S.flag != 0) { bail = true; break; }     // uniform: the watchdog fired somewhere
+                if (!(zmarch && blk0 == 0)) {
+                    float* const Xr = Xb + cur * NSLOT * BOXP;
+                    const int m_prev = (blk0 == 0) ? n_m - 1 : blk0 - 1;
+                    load_halos(Xr, (gblk - 1) & 1);
+                    if (ngh > 0) {
+                        __syncthreads();                     // a halo quad may overlap a ghost column
+                        const float* Sp = stage0 + (size_t)stp * 2 * BOXP + BOXP;
+                        for (int e = tid; e < ngh; e += T) { const GhostEnt g = gt[e]; Xr[ghost_off(g)] = ghost_fetch(g, pass - 1, m_prev, Sp); }
+                    }
+                    __syncthreads();
+                }
+            }
+            for (int j = 0; j < blen; ++j, ++s_) {
+                const int m = blk0 + j;
+                const int hj = blen - 1 - j;
+                const bool blk_last = (hj == 0);
+                const bool more = (s_ + 1 < nsteps);
+                const int pl = plane_of(m);
+                const float* const Kp = stage0 + (size_t)stp * 2 * BOXP;
+                const float* const Kc = stage0 + (size_t)stc * 2 * BOXP;
+                float* const Xr = Xb + cur * NSLOT * BOXP;
+                float* const Xw = Xb + (cur ^ 1) * NSLOT * BOXP;
 
-        // ---- seam ghosts for the next step (previous pass, this plane): fetch now, store after the update
-        const bool ghost_next = !blk_last && (s_ + 1 < nsteps) && ngh > 0;
-        float gval[2] = {0.f, 0.f};
-        if (ghost_next && pass > 0) {
-#pragma unroll
-            for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) gval[i] = ghost_fetch(e, pass - 1, m, nullptr); }
-        }
+                wait_stage(stc, (par_bits >> stc) & 1u, 2 | (s_ << 4));
+                par_bits ^= 1u << stc;
+                // ---- heating / emergent intensity of the previous step's plane
+                if (lastpass && m > 0) q_pass(Kp, Xr, m - 1);
 
-        // ---- the update
-        StepCtx C;
-        C.m = m; C.pl = pl; C.pass = pass; C.hj = hj; C.par_ex = gblk & 1;
-        C.dplane = zmarch && (m == 0);
-        C.hist = !lastpass;
-        C.strips = blk_last && (s_ + 1 < nsteps) && !(zmarch && m == n_m - 1);
-        C.a_prev = a_of(pl - U.dir); C.a_cur = a_of(pl);
-        {
-            const unsigned short* tab = itab + hj * SP.items_max;
-            const int nitems = S.nitems[hj];
-            for (int it = tid; it < nitems; it += T) {       // nitems is a multiple of 32: warps stay whole
-                const unsigned code = tab[it];
-                const int s = code & 3, rowN = (code >> 2) & 127, quad = (code >> 9) & 63;
-                const bool valid = !(code & 0x8000u);
-                const int4 rg = S.reg[hj][s];
-                const bool l_ok = (lane > 0) && (4 * quad > (rg.z & ~3));
-                const bool r_ok = (lane < 31) && (4 * quad + 4 < rg.w);
-                if (s & 1) do_item<-1>(s, S, G, C, Kp, Kc, Xr + s * BOXP, Xw + s * BOXP, rowN, quad, valid, l_ok, r_ok);
-                else       do_item<+1>(s, S, G, C, Kp, Kc, Xr + s * BOXP, Xw + s * BOXP, rowN, quad, valid, l_ok, r_ok);
-            }
-        }
-        // ---- seam ghosts of this plane into the new carried plane
-        if (ghost_next) {
-            if (pass > 0) {
+                // ---- seam ghosts for the next step (previous pass, this plane): fetch now, store after the update
+                const bool ghost_next = !blk_last && more && ngh > 0;
+                float gval[2] = {0.f, 0.f};
+                if (ghost_next && pass > 0) {
 #pragma unroll
-                for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) Xw[gt[e].xoff] = gval[i]; }
-                for (int e = tid + 2 * T; e < ngh; e += T) Xw[gt[e].xoff] = ghost_fetch(e, pass - 1, m, nullptr);
-            } else {
-                for (int e = tid; e < ngh; e += T) Xw[gt[e].xoff] = ghost_fetch(e, -1, m, Kc + BOXP);
+                    for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) gval[i] = ghost_fetch(gt[e], pass - 1, m, nullptr); }
+                }
+
+                // ---- the update
+                StepCtx C;
+                C.m = m; C.pass = pass; C.hj = hj; C.par_ex = gblk & 1;
+                C.dplane = zmarch && (m == 0);
+                C.hist = !lastpass;
+                C.strips = blk_last && more && !(zmarch && m == n_m - 1);
+                C.a_prev = a_of(pl - U.dir); C.a_cur = a_of(pl);
+                C.zreg = (C.a_prev != 0.f && C.a_cur != 0.f) ? 0 : ((C.a_prev == 0.f && C.a_cur == 0.f) ? 1 : 2);
+                if (!(U.pad0 & 2))
+                for (int it = tid; it < nitems; it += T) {   // nitems is a multiple of 32: warps stay whole
+                    const uint2 d = itab[it];
+                    if (d.y & 1u) do_item<-1>(d, U, G, C, Kp, Kc, Xr, Xw, lane);
+                    else          do_item<+1>(d, U, G, C, Kp, Kc, Xr, Xw, lane);
+                }
+                // ---- seam ghosts of this plane into the new carried plane
+                if (ghost_next) {
+                    if (pass > 0) {
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) Xw[ghost_off(gt[e])] = gval[i]; }
+                        for (int e = tid + 2 * T; e < ngh; e += T) { const GhostEnt g = gt[e]; Xw[ghost_off(g)] = ghost_fetch(g, pass - 1, m, nullptr); }
+                    } else {
+                        for (int e = tid; e < ngh; e += T) { const GhostEnt g = gt[e]; Xw[ghost_off(g)] = ghost_fetch(g, -1, m, Kc + BOXP); }
+                    }
+                }
+                // ---- end of step; at a block end publish (release) before anybody waits
+                __syncthreads();
+                if (tid == 0) {
+                    if (blk_last && more) { __threadfence(); atomicAdd(U.barrier, 1); }
+                    if (s_ + 2 < nsteps) {
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                        int m2 = m + 2; if (m2 >= n_m) m2 -= n_m; if (m2 >= n_m) m2 %= n_m;
+                        issue_load(plane_of(m2), stp);       // the previous plane's stage is free now
+                    }
+                }
+                if (blk_last && more) ++gblk;
+                cur ^= 1;
+                stp = stc; stc = (stc + 1 == NSTAGE) ? 0 : stc + 1;
             }
         }
-        // ---- end of step; at a block end publish (release) before anybody waits
-        __syncthreads();
-        if (tid == 0) {
-            if (blk_last && s_ + 1 < nsteps) { __threadfence(); atomicAdd(U.barrier, 1); }
-            if (s_ + 2 < nsteps) {
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                int m2 = m + 2; if (m2 >= n_m) m2 -= n_m; if (m2 >= n_m) m2 %= n_m;
-                issue_load(plane_of(m2), stp);               // the previous plane's stage is free now
-            }
-        }
-        if (blk_last && s_ + 1 < nsteps) ++gblk;
-        cur ^= 1;
-        if (++m == n_m) { m = 0; ++pass; }
-        stp = stc; stc = (stc + 1 == NSTAGE) ? 0 : stc + 1;
     }
     // heating / emergent intensity of the last plane
-    if (S.flag == 0) q_pass(stage0 + (size_t)stp * 2 * BOXP, Xb + cur * NSLOT * BOXP, n_m - 1);
+    if (!bail) q_pass(stage0 + (size_t)stp * 2 * BOXP, Xb + cur * NSLOT * BOXP, n_m - 1);
     __syncthreads();
     if (tid == 0)
         for (int i = 0; i < NSTAGE; ++i)
