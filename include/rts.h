@@ -99,7 +99,7 @@ size_t rts_workspace_bytes(rts_ctx* ctx);
 int rts_set_workspace(rts_ctx* ctx, void* workspace_dev, size_t bytes);
 
 /* The hot path.  DEVICE pointers: rho, T, P in [nz][ny][nx]; Qrad out [nz][ny][nx];
- * Itop out [nbands][n_up][ny][nx] or NULL (not wanted).  stream: a cudaStream_t passed as
+ * Itop out [nbands][n_up][ny][nx] or NULL (not wanted).  Qrad must be 16-byte aligned.  stream: a cudaStream_t passed as
  * void* (NULL = default stream).  Asynchronous on that stream; errors of the asynchronous
  * part surface at the next rts_sync_check / synchronising call. */
 int rts_solve(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const float* P_dev,

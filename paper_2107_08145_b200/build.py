@@ -12,7 +12,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "rts.cu")
-DEPS = [SRC, os.path.join(HERE, "csrc", "rts_kernels.cuh"),
+DEPS = [SRC, os.path.join(HERE, "csrc", "rts_kernels.cuh"), os.path.join(HERE, "csrc", "rts_sweep.cuh"),
         os.path.join(os.path.dirname(HERE), "include", "rts.h")]
 LIB = os.path.join(HERE, "librts.so")
 

@@ -166,14 +166,9 @@ void default_rays(rts_ctx* c)
 // dynamic shared memory of a CTA whose tiles are WU x WV (SmemPlan: coefficient ring, carried
 // planes, ghost list, item tables)
 int smem_for(int WU, int WV) { return (int)SmemPlan(WU, WV).bytes(); }
-// items (4 x 2 node blocks of one ray) of a full interior tile per step, halo included, for
-// `nslots` rays; averaged over the steps of a block
-double items_for(int WU, int WV, int K, int nslots)
-{
-    double sum = 0.0;
-    for (int hj = 0; hj < K; ++hj) sum += (double)((WU + (hj > 0 ? HALO : 0)) / 4) * ((WV + hj + 1) / 2);
-    return nslots * sum / K;
-}
+// items (4 x 2 node blocks of one ray, halo included, padded to whole warps per ray) of a CTA whose
+// tiles are WU x WV; a thread owns MAXIT of them
+int items_for(int WU, int WV) { return NSLOT * SmemPlan(WU, WV).nitems; }
 
 // --------------------------------------------------------------------------- planner
 // Groups the rays into sweep units (march axis, direction, one ray per sign pair), chooses the
@@ -219,12 +214,14 @@ int make_plan(rts_ctx* c)
     }
     int units_of[3] = {0, 0, 0};
     for (auto& g : groups) units_of[g.march] += (int)g.sub.size() * c->nb;
+    const int units_total = units_of[0] + units_of[1] + units_of[2];
 
     // --- tile shape per march axis: least total 4x2-block work (halo recomputation included)
     //     among the shapes whose CTA fits R times on an SM
     cudaFuncAttributes fa;
     CUDA_TRY(c, cudaFuncGetAttributes(&fa, rts_sweep_kernel));
     int bestR = 0;
+    const int thread_cap = c->user_threads ? std::min(c->user_threads, RTS_SWEEP_THREADS) : RTS_SWEEP_THREADS;
     for (int R = (c->user_ctas_per_sm ? c->user_ctas_per_sm : 2); R >= 1 && !bestR; --R) {
         const int smem_cap = std::min(c->max_smem_optin, (228 * 1024) / R - 1024 - (int)fa.sharedSizeBytes);
         const int slots = c->sm_count * R;
@@ -239,18 +236,21 @@ int make_plan(rts_ctx* c)
                 if (t.userWU && WU != std::min(n_u4, (t.userWU + 3) & ~3)) continue;
                 for (int WV = 1; WV <= std::min(t.n_v, 120); ++WV) {
                     if (t.userWV && WV != std::min(t.n_v, t.userWV)) continue;
-                    if (smem_for(WU, WV) > smem_cap) break;
+                    if (smem_for(WU, WV) > smem_cap || items_for(WU, WV) > MAXIT * thread_cap) break;
                     const int ntu = (t.n_u + WU - 1) / WU, ntv = (t.n_v + WV - 1) / WV;
                     if ((long long)ntu * ntv > slots) continue;          // all tiles of a unit must be resident
-                    // work in items per step, a mild preference for fewer (larger) tiles
-                    const double cost = (double)ntu * ntv * (items_for(WU, WV, c->K, NSLOT) + 8.0);
+                    // time ~ rounds of resident units x work of one tile step (items, whole warps per ray);
+                    // all tiles of a unit are resident together, so slots / ntiles units run at a time
+                    const int uif = std::max(1, slots / (ntu * ntv));
+                    const int rounds = (units_total + uif - 1) / uif;
+                    const double cost = (double)rounds * (items_for(WU, WV) + 64.0 + 0.25 * (WU + WV));   // + exchange perimeter
                     if (!bu || cost < best_cost) { best_cost = cost; bu = WU; bv = WV; }
                 }
             }
             if (!bu) { ok = false; break; }
             t.WU = bu; t.WV = bv;
             t.ntu = (t.n_u + bu - 1) / bu; t.ntv = (t.n_v + bv - 1) / bv;
-            t.items = NSLOT * ((bu + HALO) / 4) * ((bv + c->K) / 2);   // most items of a step
+            t.items = items_for(bu, bv);
         }
         if (ok) bestR = R;
         if (c->user_ctas_per_sm) break;
@@ -263,11 +263,7 @@ int make_plan(rts_ctx* c)
             c->smem_bytes = std::max(c->smem_bytes, smem_for(c->tp[a].WU, c->tp[a].WV));
             max_items = std::max(max_items, c->tp[a].items);
         }
-    {   // CTA size: the items of a step in equal rounds
-        const int cap = c->user_threads ? c->user_threads : RTS_SWEEP_THREADS;
-        const int rounds = (max_items + cap - 1) / cap;
-        c->threads = std::min(cap, std::max(64, ((max_items + rounds - 1) / rounds + 31) / 32 * 32));
-    }
+    c->threads = std::max(64, ((max_items + MAXIT - 1) / MAXIT + 31) / 32 * 32);   // CTA size: MAXIT items per thread
     {
         int occ = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, c->threads, (size_t)c->smem_bytes) != cudaSuccess || occ < 1)
@@ -313,11 +309,11 @@ int make_plan(rts_ctx* c)
                 d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
                 const long long PX = c->PX, PY = c->PY, PYR = c->PYR;
                 if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx;
-                                         d.c_field = (long long)fA; d.c_m = PYR * PX; d.c_v = PX; d.c_off = HALO * PX; d.P = c->PX; }
+                                         d.c_field = (long long)fA; d.c_m = PYR * PX; d.c_v = PX; d.c_off = HALO * PX; d.qvec = (c->nx % 4 == 0); }
                 else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx;
-                                         d.c_field = (long long)fA; d.c_m = PX; d.c_v = PYR * PX; d.c_off = HALO * PX; d.P = c->PX; }
+                                         d.c_field = (long long)fA; d.c_m = PX; d.c_v = PYR * PX; d.c_off = HALO * PX; d.qvec = (c->nx % 4 == 0); }
                 else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1;
-                                         d.c_field = (long long)fB; d.c_m = PY; d.c_v = (long long)c->nx * PY; d.c_off = 0; d.P = c->PY; }
+                                         d.c_field = (long long)fB; d.c_m = PY; d.c_v = (long long)c->nx * PY; d.c_off = 0; d.qvec = (c->ny % 4 == 0); }
                 for (int q = 0; q < NSLOT; ++q) d.ray[q].itop = -1;
                 for (int ri : sub) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
                 hu.off_xex = take(sizeof(float) * 2 * NSLOT * (size_t)d.n_v * d.n_u4);
@@ -606,6 +602,7 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     if (!rho || !T || !P || !Q) return fail(c, RTS_EINVAL, "rts_solve: null pointer");
     if (!c->have_tables) return fail(c, RTS_ESTATE, "rts_solve: tables not set");
     if (!c->ws || !c->planned || !c->maps_ready) return fail(c, RTS_ESTATE, "rts_solve: workspace not set (or configuration changed since)");
+    if (((uintptr_t)Q & 15u) != 0) return fail(c, RTS_EINVAL, "rts_solve: Qrad must be 16-byte aligned");
     cudaStream_t st = as_stream(stream);
     const size_t N = (size_t)c->nx * c->ny * c->nz;
     unsigned char* ws = c->ws;

@@ -55,7 +55,7 @@ struct UnitDesc {
     int n_m, n_u, n_v, n_u4;
     int WU, WV, ntu, ntv;
     int K, npass, ticket_begin, ntiles;
-    int nz, q_in_B, P, pad0;              // P: padded row length of the coefficient layout
+    int nz, q_in_B, qvec, pad0;           // qvec: heating rows are 16-byte aligned (vector reductions)
     RayC ray[NSLOT];
     const float* cbase;                   // coefficient arrays of this band: [2 fields][...]
     long long c_field, c_m, c_v, c_off;   // strides (floats): fields, march planes, v rows; offset of (m=0, v=0, padded col 0)

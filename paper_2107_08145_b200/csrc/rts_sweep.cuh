@@ -13,8 +13,9 @@
 //   seams = stencil nodes across a periodic boundary come from the previous pass (Jacobi):
 //           far columns / rows of every plane are kept in G (pass parity) and copied into the
 //           ghost column / row of the carried plane before each step.
-//   item  = a 4 x 2 node block of one ray: the thread-level unit of work.  Items of a step are
-//           listed in a table (per remaining halo depth) and dealt to the threads in order.
+//   item  = a 4 x 2 node block of one ray: the thread-level unit of work.  Every thread owns the
+//           same (at most two) items for the whole task; their descriptors live in registers.
+//           The items of a slot (ray) fill whole warps, so the ray's signs are warp-uniform.
 // Per step a CTA streams one (kaprho, S) plane box through a 3-stage TMA ring (one
 // cp.async.bulk.tensor per field, completing on an mbarrier) and updates its items from
 // registers and shared memory.
@@ -27,9 +28,23 @@
 #define RTS_SWEEP_THREADS 384   // most threads of a sweep CTA (two CTAs per SM: <= 80 registers)
 #endif
 
+#ifndef RTS_ONE_BODY
+#define RTS_ONE_BODY 0
+#endif
+
 namespace rts {
 
-struct SweepMaps { CUtensorMap m[3]; };      // coefficient tensor of the x-, y-, z-march units
+struct SweepMaps { CUtensorMap m[3]; };
+
+#ifdef RTS_TRACE
+// phase clocks of the sweep (per warp, summed): tuning builds only
+__device__ unsigned long long g_trace[16];
+#define TR_BEGIN() long long tr_t0 = clock64()
+#define TR_MARK(i) do { const long long tr_t1 = clock64(); if ((threadIdx.x & 31) == 0) atomicAdd(&g_trace[i], (unsigned long long)(tr_t1 - tr_t0)); tr_t0 = tr_t1; } while (0)
+#else
+#define TR_BEGIN() do {} while (0)
+#define TR_MARK(i) do {} while (0)
+#endif      // coefficient tensor of the x-, y-, z-march units
 
 // closed-form attenuation factors: em1 = 1 - e^-dt, wl = (1 - e^-dt)/dt
 __device__ __forceinline__ void att_closed(float dt, float& em1, float& wl) {
@@ -44,23 +59,20 @@ __device__ __forceinline__ void att_series(float dt, float& em1, float& wl, floa
     em1 = dt * wl;
 }
 
-// 5 values of one box row around a quad: the quad (o[1..4]) and the side column the ray looks
-// at (SU > 0: left neighbour in o[0]; SU < 0: right neighbour in o[5]).  The side value comes
-// from the neighbouring lane's float4 when that lane holds the adjacent quad of the same row.
+// 6 values of one box row around a quad: left neighbour, the quad, right neighbour
+__device__ __forceinline__ void load_row6(const float* __restrict__ row, float (&o)[6])
+{
+    const float4 v = *reinterpret_cast<const float4*>(row);
+    o[0] = row[-1]; o[1] = v.x; o[2] = v.y; o[3] = v.z; o[4] = v.w; o[5] = row[4];
+}
+// the quad and the side column the ray looks at (SU > 0: left neighbour in o[0]; SU < 0: right in o[5])
 template <int SU>
-__device__ __forceinline__ void load_row5(const float* __restrict__ row, bool l_ok, bool r_ok, float (&o)[6])
+__device__ __forceinline__ void load_row5(const float* __restrict__ row, float (&o)[6])
 {
     const float4 v = *reinterpret_cast<const float4*>(row);
     o[1] = v.x; o[2] = v.y; o[3] = v.z; o[4] = v.w;
-    if (SU > 0) {
-        float l = __shfl_up_sync(0xffffffffu, v.w, 1);
-        if (!l_ok) l = row[-1];
-        o[0] = l; o[5] = 0.f;
-    } else {
-        float r = __shfl_down_sync(0xffffffffu, v.x, 1);
-        if (!r_ok) r = row[4];
-        o[5] = r; o[0] = 0.f;
-    }
+    if (SU > 0) { o[0] = row[-1]; o[5] = 0.f; }
+    else        { o[5] = row[4];  o[0] = 0.f; }
 }
 
 // optical paths of one node row (4 nodes).  lo / hi: opacity of the previous plane on the two
@@ -80,11 +92,13 @@ __device__ __forceinline__ void row_dtau(const float (&lo)[6], const float (&hi)
 // update of one node row.  slo/shi: source function on the two stencil rows; xlo/xhi: carried
 // quantity; wv: weights of (lo, lo side, hi, hi side).  REG 0: everything in the departure-carried
 // part (a = 1); 1: all direct (a = 0); 2: mixed (a_lo, a_hi, a_p = a on the two rows and at the node).
-template <int SU, int REG>
+// SMALL: some optical path of the item is below DTAU_SERIES -> both forms are evaluated and
+// selected per node, branch-free (a branch inside the node loop would serialise the nodes).
+template <int SU, int REG, bool SMALL>
 __device__ __forceinline__ void row_update(
     const float (&dt)[4], const float (&slo)[6], const float (&shi)[6],
     const float (&xlo)[6], const float (&xhi)[6], const float4 spv,
-    const float4 wv, const float a_lo, const float a_hi, const float a_p, const bool any_small, float (&xp)[4])
+    const float4 wv, const float a_lo, const float a_hi, const float a_p, float (&xp)[4])
 {
     const float sp[4] = {spv.x, spv.y, spv.z, spv.w};
 #pragma unroll
@@ -94,7 +108,7 @@ __device__ __forceinline__ void row_update(
         float em1, wl;
         att_closed(dt[j], em1, wl);
         float pp = 1.0f - wl;
-        if (any_small) {
+        if (SMALL) {
             float e2, w2, pp2;
             att_series(dt[j], e2, w2, pp2);
             const bool sm = dt[j] < DTAU_SERIES;
@@ -150,41 +164,40 @@ __device__ __forceinline__ void tensor_load4(void* dst, const CUtensorMap* map, 
 }
 
 
-// Item descriptor (static for a task): x = node offset in the box | first node row << 16 | quad << 24,
-// y = flags.  An item is the 4 x 2 node block (rows rowN, rowN+1; columns 4*quad ..) of one slot.
+// Item descriptor (two registers, static for a task): pos = node offset in the box | first node
+// row << 16 | quad << 24; fl = flags.  The item is the 4 x 2 node block (rows rowN, rowN+1;
+// columns 4*quad ..) of one slot.
 enum : unsigned {
     IT_SLOT = 3u,            // bits 0-1
     IT_D0_SH = 2,            // bits 2-4   halo depth of node row 0 (0: core side; 7: never active)
     IT_D1_SH = 5,            // bits 5-7   halo depth of node row 1
     IT_DQ = 1u << 8,         // halo quad: only active while the remaining halo depth is > 0
-    IT_LOK = 1u << 9,        // lane-1 holds the quad to the left / lane+1 the quad to the right
-    IT_ROK = 1u << 10,
     IT_REG_SH = 11,          // bits 11-12 regime of the stencil rows (x/y-march; static)
     IT_DIR0 = 1u << 13,      // node row is the inflow row of a bounded v axis
     IT_DIR1 = 1u << 14,
     IT_CORE0 = 1u << 15,     // node row and quad belong to the tile core
     IT_CORE1 = 1u << 16,
-    IT_C0_SH = 17,           // bits 17-18 first valid column of the quad
-    IT_C1_SH = 19,           // bits 19-21 one past the last valid column (1..4)
+    IT_C1_SH = 19,           // bits 19-21 one past the last valid column of the quad (1..4)
     IT_SPECIAL = 1u << 22,   // core item holding a far-u column or a far-v row: writes the seam history
     IT_STRIP0 = 1u << 23,    // core node row lies in an exchange strip
-    IT_STRIP1 = 1u << 24,
-    IT_PAD = 1u << 25        // padding entry (keeps warps whole)
+    IT_STRIP1 = 1u << 24
 };
+constexpr unsigned IT_NEVER = (7u << IT_D0_SH) | (7u << IT_D1_SH);
+constexpr int MAXIT = 2;     // items per thread
 
 struct GhostEnt { unsigned short xoff_lo, bv; int goff; };   // 8 bytes; slot = goff >> 28, xoff = xoff_lo + slot * BOXP
 
 struct TaskShared {
     UnitDesc U;
     uint64_t mbar[NSTAGE];
-    int ticket, flag, nghost, nitems, nhalo, pad;
+    int ticket, flag, nghost, nhalo, pad0, pad1;
 };
 
 struct StepCtx {
-    int m, pass, hj, par_ex;           // plane counter, pass, remaining halo depth, exchange parity
+    int m, pl, pass, hj, par_ex;       // plane counter, plane index, pass, remaining halo depth, exchange parity
     int zreg;                          // z-march: regime of this step (0, 1, 2)
     bool dplane;                       // z-march inflow plane: nodes are set, not updated
-    bool hist, strips;                 // write seam histories / publish strips this step
+    bool hist, strips, lastpass;       // write seam histories / publish strips / reduce the heating this step
     float a_prev, a_cur;               // z-march: a on the previous / this plane
 };
 
@@ -198,15 +211,14 @@ struct TileGeo {
 // seam histories and exchange strips of a core item (rare path)
 struct PubCtx { int v0, u0, wu, far_u, far_v, m, pass, par_ex; bool hist, strips; };   // by value: keeps the callers' state in registers
 
-__device__ __noinline__ void item_publish(const UnitDesc* __restrict__ Up, const PubCtx P, const unsigned fl,
-                                          const int rowN, const int quad, const bool act0, const bool act1,
-                                          const float4 o0, const float4 o1)
+// core0 / core1: node row 0 / 1 is a core row and was updated this step
+__device__ __noinline__ void item_publish(const UnitDesc* __restrict__ Up, const PubCtx P, const unsigned fl, const unsigned pos,
+                                          const bool core0, const bool core1, const float4 o0, const float4 o1)
 {
     const UnitDesc& U = *Up;
     const int s = fl & IT_SLOT;
+    const int rowN = (int)((pos >> 16) & 0xffu), quad = (int)(pos >> 24);
     const bool svp = !(s & 2);
-    const bool core0 = act0 && (fl & IT_CORE0), core1 = act1 && (fl & IT_CORE1);
-    if (!(core0 || core1)) return;
     const int cq0 = 4 * quad;
     const int vN = P.v0 + rowN - HALO, ug = P.u0 + cq0 - HALO;
     if (P.hist && (fl & IT_SPECIAL)) {
@@ -240,29 +252,23 @@ __device__ __noinline__ void item_publish(const UnitDesc* __restrict__ Up, const
 }
 
 // ------------------------------------------------------------------------------------------
-// One item.  All lanes of a warp call this together (shuffles); inactive lanes only load.
+// One item (one ray, 4 x 2 nodes).  Kp / Kc: previous / this plane (opacity box, source box at +BOXP).
 template <int SU>
 __device__ __forceinline__ void do_item(
-    const uint2 d, const UnitDesc& U, const TileGeo& G, const StepCtx& C,
-    const float* __restrict__ Kp, const float* __restrict__ Kc,   // previous / this plane: opacity box, source box at +BOXP
-    const float* __restrict__ Xr_all, float* __restrict__ Xw_all, const int lane)
+    const unsigned pos, const unsigned fl, const UnitDesc& U, const TileGeo& G, const StepCtx& C,
+    const float* __restrict__ Kp, const float* __restrict__ Kc,
+    const float* __restrict__ Xr_all, float* __restrict__ Xw_all)
 {
-    const unsigned fl = d.y;
-    const int s = fl & IT_SLOT;
-    const int BU = G.BU;
-    const bool svp = !(s & 2);                               // sv > 0
     const int hj = C.hj;
     const bool act0 = (int)((fl >> IT_D0_SH) & 7u) <= hj;
     const bool act1 = (int)((fl >> IT_D1_SH) & 7u) <= hj;
-    const bool act = !(fl & IT_PAD) && ((fl & IT_DQ) ? hj > 0 : true) && (act0 || act1);
-    if (!__any_sync(0xffffffffu, act)) return;
-    const bool l_ok = (lane > 0) && (fl & IT_LOK);
-    const bool r_ok = (lane < 31) && (fl & IT_ROK);
-    const int noff = (int)(d.x & 0xffffu);                   // node row 0
+    if (!(act0 || act1) || ((fl & IT_DQ) && hj == 0)) return;
+    const int s = fl & IT_SLOT;
+    const bool svp = !(s & 2);                               // sv > 0
+    const int BU = G.BU;
+    const int noff = (int)(pos & 0xffffu);                   // node row 0
     const int off = noff - (svp ? BU : 0);                   // first stencil row: rows (R0, R1, R2)
-    const float* const Sp = Kp + G.BOXP;
     const float* const Sc = Kc + G.BOXP;
-    const float* const Xr = Xr_all + s * G.BOXP;
     const float4 sc0 = *reinterpret_cast<const float4*>(Sc + noff);
     const float4 sc1 = *reinterpret_cast<const float4*>(Sc + noff + BU);
     float o0[4], o1[4];
@@ -274,9 +280,10 @@ __device__ __forceinline__ void do_item(
         float dt0[4], dt1[4];
         {
             float k0[6], k1[6], k2[6];
-            load_row5<SU>(Kp + off, l_ok, r_ok, k0);
-            load_row5<SU>(Kp + off + BU, l_ok, r_ok, k1);
-            load_row5<SU>(Kp + off + 2 * BU, l_ok, r_ok, k2);
+            const float* kp = Kp + off;
+            load_row5<SU>(kp, k0);
+            load_row5<SU>(kp + BU, k1);
+            load_row5<SU>(kp + 2 * BU, k2);
             const float4 kv = *reinterpret_cast<const float4*>(U.ray[s].wk);
             const float kc = U.ray[s].kc;
             row_dtau<SU>(k0, k1, *reinterpret_cast<const float4*>(Kc + noff), kv, kc, dt0);
@@ -285,39 +292,45 @@ __device__ __forceinline__ void do_item(
         bool small = false;
 #pragma unroll
         for (int j = 0; j < 4; ++j) small |= (dt0[j] < DTAU_SERIES) | (dt1[j] < DTAU_SERIES);
-        const bool any_small = __any_sync(0xffffffffu, act && small);
         float s0[6], s1[6], s2[6], x0[6], x1[6], x2[6];
-        load_row5<SU>(Sp + off, l_ok, r_ok, s0);
-        load_row5<SU>(Sp + off + BU, l_ok, r_ok, s1);
-        load_row5<SU>(Sp + off + 2 * BU, l_ok, r_ok, s2);
-        load_row5<SU>(Xr + off, l_ok, r_ok, x0);
-        load_row5<SU>(Xr + off + BU, l_ok, r_ok, x1);
-        load_row5<SU>(Xr + off + 2 * BU, l_ok, r_ok, x2);
+        {
+            const float* sp = Kp + G.BOXP + off;
+            load_row5<SU>(sp, s0);
+            load_row5<SU>(sp + BU, s1);
+            load_row5<SU>(sp + 2 * BU, s2);
+            const float* xr = Xr_all + s * G.BOXP + off;
+            load_row5<SU>(xr, x0);
+            load_row5<SU>(xr + BU, x1);
+            load_row5<SU>(xr + 2 * BU, x2);
+        }
         const float4 wv = *reinterpret_cast<const float4*>(U.ray[s].wx);
         const int reg = G.zmarch ? C.zreg : (int)((fl >> IT_REG_SH) & 3u);
+#define ROWS2(REG, SM, A0, A1, A2, P0, P1)                                                  \
+        do {                                                                                \
+            row_update<SU, REG, SM>(dt0, s0, s1, x0, x1, sc0, wv, A0, A1, P0, o0);          \
+            row_update<SU, REG, SM>(dt1, s1, s2, x1, x2, sc1, wv, A1, A2, P1, o1);          \
+        } while (0)
         if (reg == 0) {
-            row_update<SU, 0>(dt0, s0, s1, x0, x1, sc0, wv, 1.f, 1.f, 1.f, any_small, o0);
-            row_update<SU, 0>(dt1, s1, s2, x1, x2, sc1, wv, 1.f, 1.f, 1.f, any_small, o1);
+            if (small || RTS_ONE_BODY) ROWS2(0, true, 1.f, 1.f, 1.f, 1.f, 1.f); else ROWS2(0, false, 1.f, 1.f, 1.f, 1.f, 1.f);
         } else if (reg == 1) {
-            row_update<SU, 1>(dt0, s0, s1, x0, x1, sc0, wv, 0.f, 0.f, 0.f, any_small, o0);
-            row_update<SU, 1>(dt1, s1, s2, x1, x2, sc1, wv, 0.f, 0.f, 0.f, any_small, o1);
+            if (small || RTS_ONE_BODY) ROWS2(1, true, 0.f, 0.f, 0.f, 0.f, 0.f); else ROWS2(1, false, 0.f, 0.f, 0.f, 0.f, 0.f);
         } else {
             // a on the three stencil rows and at the two node rows
             float a0, a1, a2, ap0, ap1;
             if (G.zmarch) { a0 = a1 = a2 = C.a_prev; ap0 = ap1 = C.a_cur; }
             else {
-                const int v0r = G.v0 + (int)((d.x >> 16) & 0xffu) - HALO - (svp ? 1 : 0);
+                const int v0r = G.v0 + (int)((pos >> 16) & 0xffu) - HALO - (svp ? 1 : 0);
                 a0 = (v0r <= G.kstar) ? 1.f : 0.f;
                 a1 = (v0r + 1 <= G.kstar) ? 1.f : 0.f;
                 a2 = (v0r + 2 <= G.kstar) ? 1.f : 0.f;
                 ap0 = svp ? a1 : a0; ap1 = svp ? a2 : a1;
             }
-            row_update<SU, 2>(dt0, s0, s1, x0, x1, sc0, wv, a0, a1, ap0, any_small, o0);
-            row_update<SU, 2>(dt1, s1, s2, x1, x2, sc1, wv, a1, a2, ap1, any_small, o1);
+            ROWS2(2, true, a0, a1, a2, ap0, ap1);
         }
+#undef ROWS2
         if (fl & (IT_DIR0 | IT_DIR1)) {
             // inflow row of a bounded v axis (v = z): I = S (upward, bottom row) or 0 (downward, top row)
-            const int vN = G.v0 + (int)((d.x >> 16) & 0xffu) - HALO;
+            const int vN = G.v0 + (int)((pos >> 16) & 0xffu) - HALO;
             const float fu = svp ? 1.f : 0.f;
             if (fl & IT_DIR0) {
                 const float f = fu - ((vN <= G.kstar) ? 1.f : 0.f);
@@ -329,20 +342,20 @@ __device__ __forceinline__ void do_item(
             }
         }
     }
-    if (!act) return;
 
     // ---- carried plane for the next step
     float* xw = Xw_all + s * G.BOXP + noff;
-    const int c0 = (int)((fl >> IT_C0_SH) & 3u), c1 = (int)((fl >> IT_C1_SH) & 7u);
-    const bool full = (c0 == 0) && (c1 == 4);
+    const int c1 = (int)((fl >> IT_C1_SH) & 7u);
     const float4 v0_ = make_float4(o0[0], o0[1], o0[2], o0[3]), v1_ = make_float4(o1[0], o1[1], o1[2], o1[3]);
-    if (act0) {
-        if (full) *reinterpret_cast<float4*>(xw) = v0_;
-        else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) xw[j] = o0[j]; }
-    }
-    if (act1) {
-        if (full) *reinterpret_cast<float4*>(xw + BU) = v1_;
-        else { _Pragma("unroll") for (int j = 0; j < 4; ++j) if (j >= c0 && j < c1) xw[BU + j] = o1[j]; }
+    if (c1 == 4) {
+        if (act0) *reinterpret_cast<float4*>(xw) = v0_;
+        if (act1) *reinterpret_cast<float4*>(xw + BU) = v1_;
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (act0 && j < c1) xw[j] = o0[j];
+            if (act1 && j < c1) xw[BU + j] = o1[j];
+        }
     }
     if ((C.hist && (fl & IT_SPECIAL)) || (C.strips && (fl & (IT_STRIP0 | IT_STRIP1)))) {
         PubCtx P;
@@ -350,7 +363,7 @@ __device__ __forceinline__ void do_item(
         P.far_u = ((G.dhi_u - 1) << 16) | (G.dlo_u & 0xffff);   // far-u column (box) of su > 0 | su < 0 rays
         P.far_v = ((G.dhi_v - 1) << 16) | (G.dlo_v & 0xffff);
         P.m = C.m; P.pass = C.pass; P.par_ex = C.par_ex; P.hist = C.hist; P.strips = C.strips;
-        item_publish(&U, P, fl, (int)((d.x >> 16) & 0xffu), (int)(d.x >> 24), act0, act1, v0_, v1_);
+        item_publish(&U, P, fl, pos, act0 && (fl & IT_CORE0), act1 && (fl & IT_CORE1), v0_, v1_);
     }
 }
 
@@ -359,20 +372,19 @@ __device__ __forceinline__ void do_item(
 struct HaloEnt { unsigned short xoff_lo; unsigned char slot, mask; int goff; };   // mask = c0 | c1 << 4
 
 struct SmemPlan {
-    int BU, BV, BOXP, guardA, guardB, items_max, nghost_max, nhalo_max;
+    int BU, BV, BOXP, guardA, guardB, nitems, nghost_max, nhalo_max;
     __host__ __device__ SmemPlan(int WU, int WV) {
         BU = WU + 2 * HALO; BV = WV + 2 * HALO;
         BOXP = (BU * BV + 31) & ~31;
-        guardA = (BU + 31) & ~31;
-        guardB = (2 * BU + 31) & ~31;
-        const int per_slot = ((WU + HALO) / 4) * ((WV + KMAX) / 2);            // one slot's items (largest region)
-        items_max = NSLOT * ((per_slot + 31) & ~31);
+        guardA = (BU + 1 + 31) & ~31;                        // an item reads one row above / below its node rows
+        guardB = (3 * BU + 4 + 31) & ~31;
+        nitems = ((((WU + HALO) / 4) * ((WV + KMAX) / 2)) + 31) & ~31;   // one slot's items (largest region), whole warps
         nghost_max = NSLOT * (BU + BV);
         nhalo_max = NSLOT * (WV + KMAX + KMAX * ((WU + HALO) / 4));
     }
     __host__ __device__ int floats() const { return guardA + (NSTAGE * 2 + 2 * NSLOT) * BOXP + guardB; }
     __host__ __device__ size_t bytes() const {
-        return (size_t)floats() * 4 + (size_t)items_max * 8 + (size_t)nghost_max * sizeof(GhostEnt) + (size_t)nhalo_max * sizeof(HaloEnt);
+        return (size_t)floats() * 4 + (size_t)nghost_max * sizeof(GhostEnt) + (size_t)nhalo_max * sizeof(HaloEnt);
     }
 };
 
@@ -381,7 +393,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                          int* abortf)
 {
     const UnitDesc& U = S.U;
-    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31;
+    const int tid = threadIdx.x, T = blockDim.x;
     const SmemPlan SP(U.WU, U.WV);
     TileGeo G;
     const int tu = tile % U.ntu, tv = tile / U.ntu;
@@ -400,8 +412,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
 
     float* const stage0 = smf + SP.guardA;                   // [NSTAGE][2][BOXP]
     float* const Xb = stage0 + NSTAGE * 2 * BOXP;            // [2][NSLOT][BOXP]
-    uint2* const itab = reinterpret_cast<uint2*>(smf + SP.floats());
-    GhostEnt* const gt = reinterpret_cast<GhostEnt*>(itab + SP.items_max);
+    GhostEnt* const gt = reinterpret_cast<GhostEnt*>(smf + SP.floats());
     HaloEnt* const ht = reinterpret_cast<HaloEnt*>(gt + SP.nghost_max);
     uint64_t* const mbar = S.mbar;
 
@@ -433,12 +444,17 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
         if (nsteps > 1) issue_load(plane_of(1 % n_m), 1);
     }
 
-    // ---- item table: per slot the 4 x 2 blocks of its largest region (halo depth K-1)
-    {
-        const int hmax = K - 1;
-        int cursor = 0;
-        for (int s = 0; s < NSLOT; ++s) {
-            if (!U.ray[s].active) continue;
+    // ---- the items of this thread.  Item index i = tid + r * T; slot = i / nitems (whole warps per
+    //      slot), e = i % nitems enumerates the 4 x 2 blocks of the slot's region (tile core + upwind
+    //      halo of depth K-1, clipped to the domain) row-pair by row-pair.
+    unsigned ipos[MAXIT], ifl[MAXIT];
+#pragma unroll
+    for (int r = 0; r < MAXIT; ++r) {
+        const int idx = tid + r * T;
+        const int s = idx / SP.nitems, e = idx - s * SP.nitems;
+        unsigned fl = IT_NEVER | (unsigned)(s & 3), pos = (unsigned)(HALO * BU + HALO) | ((unsigned)HALO << 16) | (1u << 24);
+        if (s < NSLOT && U.ray[s].active) {
+            const int hmax = K - 1;
             const int su = (s & 1) ? -1 : 1;
             const bool svp = !(s & 2);
             const bool up_u = (su > 0) ? (tu > 0) : (tu < U.ntu - 1);
@@ -448,57 +464,46 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
             const int chi = min((su > 0) ? HALO + G.wu : HALO + G.wu + hu, G.dhi_u);
             const int rlo = max(svp ? HALO - hv : HALO, G.dlo_v);
             const int rhi = min(svp ? HALO + G.wv : HALO + G.wv + hv, G.dhi_v);
-            if (rhi <= rlo || chi <= clo) continue;
             const int qlo = clo >> 2, nq = ((chi + 3) >> 2) - qlo, np = (rhi - rlo + 1) >> 1;
-            const int n = nq * np, npad = (n + 31) & ~31;
-            const int fr = svp ? G.dhi_v - 1 : G.dlo_v;       // far-v row of this slot (box)
-            const int fc = (su > 0) ? G.dhi_u - 1 : G.dlo_u;  // far-u column of this slot (box)
-            const int drow = svp ? 0 : U.n_v - 1;             // inflow row (x/y-march), global v
-            for (int e = tid; e < npad; e += T) {
-                uint2 d = make_uint2(0u, (unsigned)s | IT_PAD | (7u << IT_D0_SH) | (7u << IT_D1_SH));
-                const int pr = (e < n) ? e / nq : 0, q = qlo + ((e < n) ? e - pr * nq : 0);
+            if (rhi > rlo && chi > clo && e < nq * np) {
+                const int pr = e / nq, q = qlo + (e - pr * nq);
                 const int rowN = rlo + 2 * pr;
-                d.x = (unsigned)(rowN * BU + 4 * q) | ((unsigned)rowN << 16) | ((unsigned)q << 24);
-                if (e < n) {
-                    unsigned fl = (unsigned)s;
-                    auto depth = [&](int row) {
-                        if (row < rlo || row >= rhi) return 7;
-                        return svp ? max(0, HALO - row) : max(0, row - (HALO + G.wv - 1));
-                    };
-                    fl |= (unsigned)depth(rowN) << IT_D0_SH;
-                    fl |= (unsigned)depth(rowN + 1) << IT_D1_SH;
-                    const int cq0 = 4 * q;
-                    const bool core_q = (cq0 >= HALO) && (cq0 < HALO + G.wu);
-                    if (!core_q) fl |= IT_DQ;
-                    if (q > qlo) fl |= IT_LOK;
-                    if (q < qlo + nq - 1) fl |= IT_ROK;
-                    const int vN = G.v0 + rowN - HALO;
-                    if (!zmarch) {
-                        const int v0r = vN - (svp ? 1 : 0);
-                        const unsigned reg = (v0r + 2 <= G.kstar) ? 0u : ((v0r > G.kstar) ? 1u : 2u);
-                        fl |= reg << IT_REG_SH;
-                        if (vN == drow) fl |= IT_DIR0;
-                        if (vN + 1 == drow) fl |= IT_DIR1;
-                    }
-                    const bool c0r = core_q && rowN >= HALO && rowN < HALO + G.wv;
-                    const bool c1r = core_q && rowN + 1 >= HALO && rowN + 1 < HALO + G.wv;
-                    if (c0r) fl |= IT_CORE0;
-                    if (c1r) fl |= IT_CORE1;
-                    fl |= (unsigned)max(0, clo - cq0) << IT_C0_SH;
-                    fl |= (unsigned)min(4, chi - cq0) << IT_C1_SH;
-                    const bool farc = (fc >= cq0 && fc < cq0 + 4);
-                    const bool farr = U.per_v && ((c0r && rowN == fr) || (c1r && rowN + 1 == fr));
-                    if ((c0r || c1r) && (farc || farr)) fl |= IT_SPECIAL;
-                    const bool su_strip = (su > 0) ? (cq0 + 4 > HALO + G.wu - K) : (cq0 - HALO < K);
-                    if (c0r && (su_strip || (svp ? (HALO + G.wv - 1 - rowN < K) : (rowN - HALO < K)))) fl |= IT_STRIP0;
-                    if (c1r && (su_strip || (svp ? (HALO + G.wv - 2 - rowN < K) : (rowN + 1 - HALO < K)))) fl |= IT_STRIP1;
-                    d.y = fl;
+                pos = (unsigned)(rowN * BU + 4 * q) | ((unsigned)rowN << 16) | ((unsigned)q << 24);
+                fl = (unsigned)s;
+                auto depth = [&](int row) {
+                    if (row < rlo || row >= rhi) return 7;
+                    return svp ? max(0, HALO - row) : max(0, row - (HALO + G.wv - 1));
+                };
+                fl |= (unsigned)depth(rowN) << IT_D0_SH;
+                fl |= (unsigned)depth(rowN + 1) << IT_D1_SH;
+                const int cq0 = 4 * q;
+                const bool core_q = (cq0 >= HALO) && (cq0 < HALO + G.wu);
+                if (!core_q) fl |= IT_DQ;
+                const int vN = G.v0 + rowN - HALO;
+                if (!zmarch) {
+                    const int v0r = vN - (svp ? 1 : 0);
+                    const unsigned reg = (v0r + 2 <= G.kstar) ? 0u : ((v0r > G.kstar) ? 1u : 2u);
+                    fl |= reg << IT_REG_SH;
+                    const int drow = svp ? 0 : U.n_v - 1;    // inflow row (x/y-march), global v
+                    if (vN == drow) fl |= IT_DIR0;
+                    if (vN + 1 == drow) fl |= IT_DIR1;
                 }
-                itab[cursor + e] = d;
+                const bool c0r = core_q && rowN >= HALO && rowN < HALO + G.wv;
+                const bool c1r = core_q && rowN + 1 >= HALO && rowN + 1 < HALO + G.wv;
+                if (c0r) fl |= IT_CORE0;
+                if (c1r) fl |= IT_CORE1;
+                fl |= (unsigned)min(4, chi - cq0) << IT_C1_SH;
+                const int fr = svp ? G.dhi_v - 1 : G.dlo_v;       // far-v row of this slot (box)
+                const int fc = (su > 0) ? G.dhi_u - 1 : G.dlo_u;  // far-u column of this slot (box)
+                const bool farc = (fc >= cq0 && fc < cq0 + 4);
+                const bool farr = U.per_v && ((c0r && rowN == fr) || (c1r && rowN + 1 == fr));
+                if ((c0r || c1r) && (farc || farr)) fl |= IT_SPECIAL;
+                const bool su_strip = (su > 0) ? (cq0 + 4 > HALO + G.wu - K) : (cq0 - HALO < K);
+                if (c0r && (su_strip || (svp ? (HALO + G.wv - 1 - rowN < K) : (rowN - HALO < K)))) fl |= IT_STRIP0;
+                if (c1r && (su_strip || (svp ? (HALO + G.wv - 2 - rowN < K) : (rowN + 1 - HALO < K)))) fl |= IT_STRIP1;
             }
-            cursor += npad;
         }
-        if (tid == 0) S.nitems = cursor;
+        ipos[r] = pos; ifl[r] = fl;
     }
     // ---- seam ghosts of this tile (compact list)
     for (int e = tid; e < SP.nghost_max; e += T) {
@@ -549,7 +554,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
         }
     }
     __syncthreads();
-    const int ngh = S.nghost, nhalo = S.nhalo, nitems = S.nitems;
+    const int ngh = S.nghost, nhalo = S.nhalo;
 
     auto wait_stage = [&](int st, uint32_t par, int code) {
         unsigned spins = 0;
@@ -653,6 +658,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
         for (int blk0 = 0; blk0 < n_m && !bail; blk0 += K) {
             const int blen = min(K, n_m - blk0);
             // ---- block start: wait for the unit, fetch halos and seam ghosts of the previous plane
+            TR_BEGIN();
             if (s_ > 0) {
                 if (tid == 0) {
                     const int need = gblk * U.ntiles;
@@ -679,6 +685,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                     __syncthreads();
                 }
             }
+            TR_MARK(0);
             for (int j = 0; j < blen; ++j, ++s_) {
                 const int m = blk0 + j;
                 const int hj = blen - 1 - j;
@@ -692,9 +699,9 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
 
                 wait_stage(stc, (par_bits >> stc) & 1u, 2 | (s_ << 4));
                 par_bits ^= 1u << stc;
+                TR_MARK(1);
                 // ---- heating / emergent intensity of the previous step's plane
                 if (lastpass && m > 0) q_pass(Kp, Xr, m - 1);
-
                 // ---- seam ghosts for the next step (previous pass, this plane): fetch now, store after the update
                 const bool ghost_next = !blk_last && more && ngh > 0;
                 float gval[2] = {0.f, 0.f};
@@ -705,18 +712,22 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
 
                 // ---- the update
                 StepCtx C;
-                C.m = m; C.pass = pass; C.hj = hj; C.par_ex = gblk & 1;
+                C.m = m; C.pl = pl; C.pass = pass; C.hj = hj; C.par_ex = gblk & 1;
                 C.dplane = zmarch && (m == 0);
-                C.hist = !lastpass;
+                C.hist = !lastpass; C.lastpass = lastpass;
                 C.strips = blk_last && more && !(zmarch && m == n_m - 1);
                 C.a_prev = a_of(pl - U.dir); C.a_cur = a_of(pl);
                 C.zreg = (C.a_prev != 0.f && C.a_cur != 0.f) ? 0 : ((C.a_prev == 0.f && C.a_cur == 0.f) ? 1 : 2);
-                if (!(U.pad0 & 2))
-                for (int it = tid; it < nitems; it += T) {   // nitems is a multiple of 32: warps stay whole
-                    const uint2 d = itab[it];
-                    if (d.y & 1u) do_item<-1>(d, U, G, C, Kp, Kc, Xr, Xw, lane);
-                    else          do_item<+1>(d, U, G, C, Kp, Kc, Xr, Xw, lane);
+                TR_MARK(2);
+                if (!(U.pad0 & 2)) {
+#pragma unroll 1
+                    for (int r = 0; r < MAXIT; ++r) {        // one copy of the item code; the slot of an item is warp-uniform
+                        const unsigned pos_ = r ? ipos[1] : ipos[0], fl_ = r ? ifl[1] : ifl[0];
+                        if (fl_ & 1u) do_item<-1>(pos_, fl_, U, G, C, Kp, Kc, Xr, Xw);
+                        else          do_item<+1>(pos_, fl_, U, G, C, Kp, Kc, Xr, Xw);
+                    }
                 }
+                TR_MARK(3);
                 // ---- seam ghosts of this plane into the new carried plane
                 if (ghost_next) {
                     if (pass > 0) {
@@ -728,7 +739,9 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                     }
                 }
                 // ---- end of step; at a block end publish (release) before anybody waits
+                TR_MARK(4);
                 __syncthreads();
+                TR_MARK(5);
                 if (tid == 0) {
                     if (blk_last && more) { __threadfence(); atomicAdd(U.barrier, 1); }
                     if (s_ + 2 < nsteps) {
@@ -737,6 +750,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                         issue_load(plane_of(m2), stp);       // the previous plane's stage is free now
                     }
                 }
+                TR_MARK(6);
                 if (blk_last && more) ++gblk;
                 cur ^= 1;
                 stp = stc; stc = (stc + 1 == NSTAGE) ? 0 : stc + 1;
