@@ -86,7 +86,8 @@ int rts_num_up_rays(const rts_ctx* ctx);
  * tile is tile_u nodes of the unit-stride transverse axis (rounded up to a multiple of 4,
  * <= 248) times tile_v nodes of the other transverse axis (<= 120); 0 = the planner's choice.
  * Tiles exchange halos every `steps` planes (1..4; 0 = default 4) and recompute a halo of that
- * depth in between.  ctas_per_sm = 0 lets the planner choose (1 or 2).  All three invalidate
+ * depth in between.  ctas_per_sm = 0 lets the planner choose: two CTAs of <= 384 threads per SM, or
+ * one CTA of <= 768 threads on a larger tile (1 or 2 force it).  All three invalidate
  * the workspace size (call rts_workspace_bytes / rts_set_workspace again). */
 int rts_set_tiling(rts_ctx* ctx, int march, int tile_u, int tile_v);
 int rts_set_exchange_interval(rts_ctx* ctx, int steps);

@@ -220,14 +220,21 @@ int make_plan(rts_ctx* c)
     //     among the shapes whose CTA fits R times on an SM
     cudaFuncAttributes fa;
     CUDA_TRY(c, cudaFuncGetAttributes(&fa, rts_sweep_kernel));
+    // R CTAs share an SM: R = 2 with <= RTS_SWEEP_THREADS / 2 threads each, or one CTA of up to
+    // RTS_SWEEP_THREADS threads on a larger tile (less halo recomputation, half the exchanges).
+    // Both are planned; the cheaper one (rounds of resident units x items an SM updates per step) wins.
     int bestR = 0;
-    const int thread_cap = c->user_threads ? std::min(c->user_threads, RTS_SWEEP_THREADS) : RTS_SWEEP_THREADS;
-    for (int R = (c->user_ctas_per_sm ? c->user_ctas_per_sm : 2); R >= 1 && !bestR; --R) {
+    double bestR_cost = 0.0;
+    TypePlan best_tp[3];
+    for (int R = (c->user_ctas_per_sm ? c->user_ctas_per_sm : 2); R >= 1; --R) {
+        const int thread_cap = std::min(c->user_threads ? c->user_threads : RTS_SWEEP_THREADS, RTS_SWEEP_THREADS / R);
         const int smem_cap = std::min(c->max_smem_optin, (228 * 1024) / R - 1024 - (int)fa.sharedSizeBytes);
         const int slots = c->sm_count * R;
         bool ok = true;
+        double costR = 0.0;
+        TypePlan tp[3] = {c->tp[0], c->tp[1], c->tp[2]};
         for (int a = 0; a < 3 && ok; ++a) {
-            TypePlan& t = c->tp[a];
+            TypePlan& t = tp[a];
             if (!units_of[a]) { t.WU = 4; t.WV = 2; t.ntu = (t.n_u + 3) / 4; t.ntv = (t.n_v + 1) / 2; t.items = 0; continue; }
             double best_cost = 0.0;
             int bu = 0, bv = 0;
@@ -239,11 +246,10 @@ int make_plan(rts_ctx* c)
                     if (smem_for(WU, WV) > smem_cap || items_for(WU, WV) > MAXIT * thread_cap) break;
                     const int ntu = (t.n_u + WU - 1) / WU, ntv = (t.n_v + WV - 1) / WV;
                     if ((long long)ntu * ntv > slots) continue;          // all tiles of a unit must be resident
-                    // time ~ rounds of resident units x work of one tile step (items, whole warps per ray);
                     // all tiles of a unit are resident together, so slots / ntiles units run at a time
                     const int uif = std::max(1, slots / (ntu * ntv));
                     const int rounds = (units_total + uif - 1) / uif;
-                    const double cost = (double)rounds * (items_for(WU, WV) + 64.0 + 0.25 * (WU + WV));   // + exchange perimeter
+                    const double cost = (double)rounds * R * (items_for(WU, WV) + 64.0 + 0.25 * (WU + WV));   // + exchange perimeter
                     if (!bu || cost < best_cost) { best_cost = cost; bu = WU; bv = WV; }
                 }
             }
@@ -251,10 +257,12 @@ int make_plan(rts_ctx* c)
             t.WU = bu; t.WV = bv;
             t.ntu = (t.n_u + bu - 1) / bu; t.ntv = (t.n_v + bv - 1) / bv;
             t.items = items_for(bu, bv);
+            costR += best_cost * units_of[a] / units_total;
         }
-        if (ok) bestR = R;
+        if (ok && (!bestR || costR < bestR_cost)) { bestR = R; bestR_cost = costR; for (int a = 0; a < 3; ++a) best_tp[a] = tp[a]; }
         if (c->user_ctas_per_sm) break;
     }
+    if (bestR) for (int a = 0; a < 3; ++a) c->tp[a] = best_tp[a];
     if (!bestR) return fail(c, RTS_EINVAL, "planner: no tile shape fits (grid too large for one resident unit, or bad override)");
     c->smem_bytes = 0;
     int max_items = 1;

@@ -25,7 +25,7 @@
 #include "rts_kernels.cuh"
 
 #ifndef RTS_SWEEP_THREADS
-#define RTS_SWEEP_THREADS 384   // most threads of a sweep CTA (two CTAs per SM: <= 80 registers)
+#define RTS_SWEEP_THREADS 768   // most threads of a sweep CTA (<= 85 registers): one such CTA per SM, or two of half the size
 #endif
 
 #ifndef RTS_ONE_BODY
@@ -765,7 +765,10 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
             asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&mbar[i])) : "memory");
 }
 
-__global__ void __launch_bounds__(RTS_SWEEP_THREADS, 2)
+#ifndef RTS_SWEEP_MINB
+#define RTS_SWEEP_MINB 1
+#endif
+__global__ void __launch_bounds__(RTS_SWEEP_THREADS, RTS_SWEEP_MINB)
 rts_sweep_kernel(const __grid_constant__ SweepMaps maps, const UnitDesc* __restrict__ units, int nunits,
                  int total_tickets, int* ticket_counter,
                  float* __restrict__ Qa, float* __restrict__ Qb, float* __restrict__ Itop_all, int* abortf)
