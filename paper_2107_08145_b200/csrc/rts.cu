@@ -308,7 +308,6 @@ int make_plan(rts_ctx* c)
                 d.n_m = t.n_m; d.n_u = t.n_u; d.n_v = t.n_v; d.n_u4 = (t.n_u + 3) & ~3;
                 d.WU = t.WU; d.WV = t.WV; d.ntu = t.ntu; d.ntv = t.ntv;
                 d.K = c->K; d.npass = c->npass;
-                d.pad0 = getenv("RTS_DEBUG_BITS") ? atoi(getenv("RTS_DEBUG_BITS")) : 0;   // timing experiments only
                 d.ticket_begin = ticket;
                 d.ntiles = t.ntu * t.ntv;
                 ticket += d.ntiles;

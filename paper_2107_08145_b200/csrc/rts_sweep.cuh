@@ -65,14 +65,30 @@ __device__ __forceinline__ void load_row6(const float* __restrict__ row, float (
     const float4 v = *reinterpret_cast<const float4*>(row);
     o[0] = row[-1]; o[1] = v.x; o[2] = v.y; o[3] = v.z; o[4] = v.w; o[5] = row[4];
 }
+// Loads / stores of the item code on 32-bit shared-window byte addresses: one add per row instead of
+// an index add plus a generic-to-shared conversion per access.
+__device__ __forceinline__ float4 lds128(const uint32_t a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+template <int OFF>
+__device__ __forceinline__ float lds32(const uint32_t a) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(a), "n"(OFF));
+    return v;
+}
+__device__ __forceinline__ void sts128(const uint32_t a, const float4 v) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
 // the quad and the side column the ray looks at (SU > 0: left neighbour in o[0]; SU < 0: right in o[5])
 template <int SU>
-__device__ __forceinline__ void load_row5(const float* __restrict__ row, float (&o)[6])
+__device__ __forceinline__ void load_row5(const uint32_t row, float (&o)[6])
 {
-    const float4 v = *reinterpret_cast<const float4*>(row);
+    const float4 v = lds128(row);
     o[1] = v.x; o[2] = v.y; o[3] = v.z; o[4] = v.w;
-    if (SU > 0) { o[0] = row[-1]; o[5] = 0.f; }
-    else        { o[5] = row[4];  o[0] = 0.f; }
+    if (SU > 0) { o[0] = lds32<-4>(row); o[5] = 0.f; }
+    else        { o[5] = lds32<16>(row); o[0] = 0.f; }
 }
 
 // optical paths of one node row (4 nodes).  lo / hi: opacity of the previous plane on the two
@@ -265,12 +281,12 @@ __device__ __forceinline__ void do_item(
     if (!(act0 || act1) || ((fl & IT_DQ) && hj == 0)) return;
     const int s = fl & IT_SLOT;
     const bool svp = !(s & 2);                               // sv > 0
-    const int BU = G.BU;
-    const int noff = (int)(pos & 0xffffu);                   // node row 0
-    const int off = noff - (svp ? BU : 0);                   // first stencil row: rows (R0, R1, R2)
-    const float* const Sc = Kc + G.BOXP;
-    const float4 sc0 = *reinterpret_cast<const float4*>(Sc + noff);
-    const float4 sc1 = *reinterpret_cast<const float4*>(Sc + noff + BU);
+    const uint32_t BU4 = 4u * (uint32_t)G.BU, BOXP4 = 4u * (uint32_t)G.BOXP;
+    const uint32_t noff4 = 4u * (pos & 0xffffu);             // node row 0 (bytes)
+    const uint32_t off4 = noff4 - (svp ? BU4 : 0u);          // first stencil row: rows (R0, R1, R2)
+    const uint32_t a_c = smem_u32(Kc) + noff4;               // this plane at the node rows
+    const float4 sc0 = lds128(a_c + BOXP4);
+    const float4 sc1 = lds128(a_c + BOXP4 + BU4);
     float o0[4], o1[4];
     if (C.dplane) {
         const float f = (U.ray[s].up ? 1.f : 0.f) - C.a_cur;
@@ -278,30 +294,29 @@ __device__ __forceinline__ void do_item(
         o1[0] = f * sc1.x; o1[1] = f * sc1.y; o1[2] = f * sc1.z; o1[3] = f * sc1.w;
     } else {
         float dt0[4], dt1[4];
+        const uint32_t a_k0 = smem_u32(Kp) + off4, a_k1 = a_k0 + BU4, a_k2 = a_k1 + BU4;
         {
             float k0[6], k1[6], k2[6];
-            const float* kp = Kp + off;
-            load_row5<SU>(kp, k0);
-            load_row5<SU>(kp + BU, k1);
-            load_row5<SU>(kp + 2 * BU, k2);
+            load_row5<SU>(a_k0, k0);
+            load_row5<SU>(a_k1, k1);
+            load_row5<SU>(a_k2, k2);
             const float4 kv = *reinterpret_cast<const float4*>(U.ray[s].wk);
             const float kc = U.ray[s].kc;
-            row_dtau<SU>(k0, k1, *reinterpret_cast<const float4*>(Kc + noff), kv, kc, dt0);
-            row_dtau<SU>(k1, k2, *reinterpret_cast<const float4*>(Kc + noff + BU), kv, kc, dt1);
+            row_dtau<SU>(k0, k1, lds128(a_c), kv, kc, dt0);
+            row_dtau<SU>(k1, k2, lds128(a_c + BU4), kv, kc, dt1);
         }
         bool small = false;
 #pragma unroll
         for (int j = 0; j < 4; ++j) small |= (dt0[j] < DTAU_SERIES) | (dt1[j] < DTAU_SERIES);
         float s0[6], s1[6], s2[6], x0[6], x1[6], x2[6];
         {
-            const float* sp = Kp + G.BOXP + off;
-            load_row5<SU>(sp, s0);
-            load_row5<SU>(sp + BU, s1);
-            load_row5<SU>(sp + 2 * BU, s2);
-            const float* xr = Xr_all + s * G.BOXP + off;
-            load_row5<SU>(xr, x0);
-            load_row5<SU>(xr + BU, x1);
-            load_row5<SU>(xr + 2 * BU, x2);
+            load_row5<SU>(a_k0 + BOXP4, s0);
+            load_row5<SU>(a_k1 + BOXP4, s1);
+            load_row5<SU>(a_k2 + BOXP4, s2);
+            const uint32_t a_x0 = smem_u32(Xr_all) + (uint32_t)s * BOXP4 + off4;
+            load_row5<SU>(a_x0, x0);
+            load_row5<SU>(a_x0 + BU4, x1);
+            load_row5<SU>(a_x0 + 2u * BU4, x2);
         }
         const float4 wv = *reinterpret_cast<const float4*>(U.ray[s].wx);
         const int reg = G.zmarch ? C.zreg : (int)((fl >> IT_REG_SH) & 3u);
@@ -344,17 +359,18 @@ __device__ __forceinline__ void do_item(
     }
 
     // ---- carried plane for the next step
-    float* xw = Xw_all + s * G.BOXP + noff;
     const int c1 = (int)((fl >> IT_C1_SH) & 7u);
     const float4 v0_ = make_float4(o0[0], o0[1], o0[2], o0[3]), v1_ = make_float4(o1[0], o1[1], o1[2], o1[3]);
     if (c1 == 4) {
-        if (act0) *reinterpret_cast<float4*>(xw) = v0_;
-        if (act1) *reinterpret_cast<float4*>(xw + BU) = v1_;
+        const uint32_t a_w = smem_u32(Xw_all) + (uint32_t)s * BOXP4 + noff4;
+        if (act0) sts128(a_w, v0_);
+        if (act1) sts128(a_w + BU4, v1_);
     } else {
+        float* xw = Xw_all + s * G.BOXP + (int)(pos & 0xffffu);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             if (act0 && j < c1) xw[j] = o0[j];
-            if (act1 && j < c1) xw[BU + j] = o1[j];
+            if (act1 && j < c1) xw[G.BU + j] = o1[j];
         }
     }
     if ((C.hist && (fl & IT_SPECIAL)) || (C.strips && (fl & (IT_STRIP0 | IT_STRIP1)))) {
@@ -664,7 +680,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                     const int need = gblk * U.ntiles;
                     const int ab = *reinterpret_cast<volatile int*>(abortf);
                     unsigned spins = 0, ns = 32;
-                    while (!(U.pad0 & 1) && ld_acquire(U.barrier) < need) {
+                    while (ld_acquire(U.barrier) < need) {
                         if (spin_abort(abortf, spins, 3 | (s_ << 4))) { S.flag = 1; break; }
                         __nanosleep(ns);
                         if (ns < 2048) ns += ns;             // back off: a unit waiting for residency spins long
@@ -719,7 +735,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 C.a_prev = a_of(pl - U.dir); C.a_cur = a_of(pl);
                 C.zreg = (C.a_prev != 0.f && C.a_cur != 0.f) ? 0 : ((C.a_prev == 0.f && C.a_cur == 0.f) ? 1 : 2);
                 TR_MARK(2);
-                if (!(U.pad0 & 2)) {
+                {
 #pragma unroll 1
                     for (int r = 0; r < MAXIT; ++r) {        // one copy of the item code; the slot of an item is warp-uniform
                         const unsigned pos_ = r ? ipos[1] : ipos[0], fl_ = r ? ifl[1] : ifl[0];
