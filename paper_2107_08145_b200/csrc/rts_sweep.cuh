@@ -39,11 +39,15 @@ struct SweepMaps { CUtensorMap m[3]; };
 #ifdef RTS_TRACE
 // phase clocks of the sweep (per warp, summed): tuning builds only
 __device__ unsigned long long g_trace[16];
-#define TR_BEGIN() long long tr_t0 = clock64()
-#define TR_MARK(i) do { const long long tr_t1 = clock64(); if ((threadIdx.x & 31) == 0) atomicAdd(&g_trace[i], (unsigned long long)(tr_t1 - tr_t0)); tr_t0 = tr_t1; } while (0)
+#define TR_DECL() unsigned tr_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}; long long tr_t0 = clock64()
+#define TR_BEGIN() tr_t0 = clock64()
+#define TR_MARK(i) do { const long long tr_t1 = clock64(); tr_acc[i] += (unsigned)(tr_t1 - tr_t0); tr_t0 = tr_t1; } while (0)
+#define TR_FLUSH() do { if ((threadIdx.x & 31) == 0) for (int i_ = 0; i_ < 8; ++i_) atomicAdd(&g_trace[i_], (unsigned long long)tr_acc[i_]); } while (0)
 #else
+#define TR_DECL() do {} while (0)
 #define TR_BEGIN() do {} while (0)
 #define TR_MARK(i) do {} while (0)
+#define TR_FLUSH() do {} while (0)
 #endif      // coefficient tensor of the x-, y-, z-march units
 
 // closed-form attenuation factors: em1 = 1 - e^-dt, wl = (1 - e^-dt)/dt
@@ -157,6 +161,11 @@ __device__ __forceinline__ void row_update(
         }
         xp[j] = v;
     }
+}
+
+__device__ __forceinline__ void red_add4(float* p, const float a, const float b, const float c, const float d)
+{
+    asm volatile("red.relaxed.gpu.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
 // watchdog for every wait loop: gives up after ~2^22 unsuccessful probes (seconds) and raises
@@ -640,7 +649,12 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
             float* qd = Qdst + (long long)pl * U.q_sm + (long long)v * U.q_sv + u;
             const float kpa[4] = {kp.x, kp.y, kp.z, kp.w};
 #pragma unroll
-            for (int j = 0; j < 4; ++j) if (j < nval) atomicAdd(qd + j, FOUR_PI * kpa[j] * acc[j]);
+            for (int j = 0; j < 4; ++j) acc[j] *= FOUR_PI * kpa[j];
+            if (U.qvec && nval == 4) red_add4(qd, acc[0], acc[1], acc[2], acc[3]);   // one 16-byte reduction
+            else {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) if (j < nval) atomicAdd(qd + j, acc[j]);
+            }
         }
     };
     // halo of the carried plane at a block start: K-deep strips of the upwind neighbours' planes
@@ -665,6 +679,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     auto ghost_off = [&](const GhostEnt g) { return (g.goff >> 28) * BOXP + g.xoff_lo; };
 
     // ================================================================== the march
+    TR_DECL();
     int cur = 0, gblk = 0, s_ = 0;
     int stc = 0, stp = NSTAGE - 1;                           // stages of this step's and the previous plane
     uint32_t par_bits = 1u << (NSTAGE - 1);                  // stage NSTAGE-1 already served the plane before step 0
@@ -689,6 +704,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 }
                 __syncthreads();
                 if (S.flag != 0) { bail = true; break; }     // uniform: the watchdog fired somewhere
+                TR_MARK(7);
                 if (!(zmarch && blk0 == 0)) {
                     float* const Xr = Xb + cur * NSLOT * BOXP;
                     const int m_prev = (blk0 == 0) ? n_m - 1 : blk0 - 1;
@@ -773,6 +789,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
             }
         }
     }
+    TR_FLUSH();
     // heating / emergent intensity of the last plane
     if (!bail) q_pass(stage0 + (size_t)stp * 2 * BOXP, Xb + cur * NSLOT * BOXP, n_m - 1);
     __syncthreads();
