@@ -47,6 +47,10 @@ def _load():
         _lib = ctypes.CDLL(_LIB)
         _lib.oracle_coefficients.restype = _I
         _lib.oracle_coefficients.argtypes = [_I] * 6 + [_D] * 4 + [_PF] * 5 + [_PD] * 2
+        _lib.oracle_cells_to_nodes.restype = _I
+        _lib.oracle_cells_to_nodes.argtypes = [_I] * 3 + [_PF] * 2
+        _lib.oracle_nodes_to_cells.restype = _I
+        _lib.oracle_nodes_to_cells.argtypes = [_I] * 3 + [_PD] * 2
         _lib.oracle_ray_geometry.restype = _I
         _lib.oracle_ray_geometry.argtypes = [_D, _D, _D, _PD, _PI, _PI, _PD, _PD]
         _lib.oracle_psi.restype = None
@@ -148,3 +152,38 @@ def solve(inp, nthreads: int = 0, want_J: bool = False):
     if want_J:
         return Q, Itop, J
     return Q, Itop
+
+
+def cells_to_nodes(cell: np.ndarray) -> np.ndarray:
+    """O-9: fp32 cell-centred field [ncz][ncy][ncx] -> fp32 corner-node field [ncz+1][ncy][ncx]."""
+    lib = _load()
+    cell = np.ascontiguousarray(cell, dtype=np.float32)
+    ncz, ncy, ncx = cell.shape
+    node = np.empty((ncz + 1, ncy, ncx), dtype=np.float32)
+    rc = lib.oracle_cells_to_nodes(ncx, ncy, ncz, _pf(cell), _pf(node))
+    assert rc == 0, rc
+    return node
+
+
+def nodes_to_cells(qn: np.ndarray) -> np.ndarray:
+    """O-9: fp64 node field [nz][ny][nx] -> fp64 cell field [nz-1][ny][nx] (mean of the 8 corners)."""
+    lib = _load()
+    qn = np.ascontiguousarray(qn, dtype=np.float64)
+    nz, ny, nx = qn.shape
+    qc = np.empty((nz - 1, ny, nx), dtype=np.float64)
+    rc = lib.oracle_nodes_to_cells(nx, ny, nz, _pd(qn), _pd(qc))
+    assert rc == 0, rc
+    return qc
+
+
+def solve_cells(inp_cells, nthreads: int = 0):
+    """Staggered solve: `inp_cells` holds cell-centred rho, T, P [ncz][ncy][ncx]; the RT grid has
+    nz = ncz + 1 levels.  Returns (Q on cells fp64, I_top fp64, node-grid inputs)."""
+    import copy
+    node = copy.copy(inp_cells)
+    node.rho = cells_to_nodes(inp_cells.rho)
+    node.T = cells_to_nodes(inp_cells.T)
+    node.P = cells_to_nodes(inp_cells.P)
+    node.nz = inp_cells.nz + 1
+    Qn, Itop = solve(node, nthreads=nthreads)
+    return nodes_to_cells(Qn), Itop, node

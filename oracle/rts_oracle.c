@@ -30,7 +30,9 @@
  * optically thick limit and second moment of the ray set, isothermal exactness,
  * rotation/mirror symmetry, 1-D reduction against an independent recurrence,
  * memoised recursive evaluator on tiny grids, pass fixed point, I-form vs D-form,
- * table stage closed forms, psi check values of SURVEY 8(c) O-6.  Parity: pinned.
+ * table stage closed forms, psi check values of SURVEY 8(c) O-6; staggering (O-9):
+ * constants, midpoints of linear fields, Fourier-mode attenuation cos(pi m/n),
+ * edge levels, sum rule of the back-averaging.  Parity: pinned.
  *
  * Layout: all fields [nz][ny][nx], x fastest, idx = (k*ny + j)*nx + i; z is up,
  * k = 0 is the bottom.  cgs units.
@@ -321,6 +323,62 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
     }
     free(kaprho); free(S); free(J); free(upidx);
     return fail;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-9  Grid staggering (paper's Interpolate, PAPER.md:79:
+ *      "trilinear interpolation of the MHD variables from the MHD grid to the
+ *      staggered RTS grid").  DESIGN.md reading R20: the MHD variables live at the
+ *      centres of ncx*ncy*ncz cells, the RT nodes are the cell corners.  x and y are
+ *      periodic, so there are nx = ncx, ny = ncy corner columns; there are
+ *      nz = ncz + 1 corner levels, and below the bottom / above the top cell level
+ *      the missing cells are the edge cells again (zero-gradient ghost level).
+ *      Trilinear interpolation at a corner is the mean of its 8 cells:
+ *        node(i,j,k) = 1/8 sum_{a,b,c in {0,1}} cell(wrap(i-a), wrap(j-b), clamp(k-c))
+ *      O-1 holds for the result too: the node fields are fp32 arrays (the mean is
+ *      formed in fp64 -- the sum of 8 floats is exact there -- and rounded once).
+ * ------------------------------------------------------------------------- */
+int oracle_cells_to_nodes(int ncx, int ncy, int ncz, const float* cell, float* node)
+{
+    if (ncx < 2 || ncy < 2 || ncz < 1 || !cell || !node) return -1;
+    const int nz = ncz + 1;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ncy; ++j)
+            for (int i = 0; i < ncx; ++i) {
+                double sum = 0.0;
+                for (int c = 0; c < 2; ++c) {
+                    int kk = k - c;
+                    if (kk < 0) kk = 0;
+                    if (kk > ncz - 1) kk = ncz - 1;
+                    for (int b = 0; b < 2; ++b) {
+                        const int jj = (j - b + ncy) % ncy;
+                        for (int a = 0; a < 2; ++a) {
+                            const int ii = (i - a + ncx) % ncx;
+                            sum += (double)cell[((size_t)kk * ncy + jj) * ncx + ii];
+                        }
+                    }
+                }
+                node[((size_t)k * ncy + j) * ncx + i] = (float)(sum / 8.0);
+            }
+    return 0;
+}
+
+/* Heating back on the MHD grid: the mean of the 8 corner nodes of a cell,
+ *   Qc(i,j,k) = 1/8 sum_{a,b,c in {0,1}} Qn(wrap(i+a), wrap(j+b), k+c),  k = 0..nz-2. */
+int oracle_nodes_to_cells(int nx, int ny, int nz, const double* qn, double* qc)
+{
+    if (nx < 2 || ny < 2 || nz < 2 || !qn || !qc) return -1;
+    for (int k = 0; k < nz - 1; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double sum = 0.0;
+                for (int c = 0; c < 2; ++c)
+                    for (int b = 0; b < 2; ++b)
+                        for (int a = 0; a < 2; ++a)
+                            sum += qn[((size_t)(k + c) * ny + (j + b) % ny) * nx + (i + a) % nx];
+                qc[((size_t)k * ny + j) * nx + i] = sum / 8.0;
+            }
+    return 0;
 }
 
 int oracle_num_threads(void)

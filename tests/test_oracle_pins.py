@@ -466,3 +466,80 @@ def test_P9_energy_balance_trend():
     assert l1 * r1 > 0 and l2 * r2 > 0             # same sign: Q is a cooling where flux leaves
     assert e2 < 0.7 * e1                           # measured 1.5% -> 0.8% (-> 0.4% at n = 32)
     assert e2 < 0.02
+
+
+# ------------------------------------------------------------------ O-9 grid staggering (NEXT #1)
+def test_O9_cells_to_nodes_constant_linear_and_edges():
+    """Trilinear interpolation at a corner = mean of 8 cells: constants are kept, a field linear
+    in z lands on the midpoints, and the bottom / top corner levels repeat the edge cell level
+    (reading R20)."""
+    ncz, ncy, ncx = 6, 4, 5
+    c = np.full((ncz, ncy, ncx), 3.25, dtype=np.float32)
+    assert np.array_equal(oracle.cells_to_nodes(c), np.full((ncz + 1, ncy, ncx), 3.25, dtype=np.float32))
+    z = (np.arange(ncz, dtype=np.float64) + 0.5)                  # cell-centre heights
+    c = np.broadcast_to((2.0 + 0.5 * z)[:, None, None], (ncz, ncy, ncx)).astype(np.float32)
+    n = oracle.cells_to_nodes(c).astype(np.float64)
+    for k in range(1, ncz):
+        assert np.allclose(n[k], 2.0 + 0.5 * k, rtol=0, atol=1e-6)      # corner height k = midpoint
+    assert np.allclose(n[0], c[0]) and np.allclose(n[ncz], c[ncz - 1])  # zero-gradient ghost levels
+
+
+def test_O9_cells_to_nodes_fourier_mode_attenuation():
+    """A horizontal Fourier mode sin(2 pi m (i + 1/2) / n) of the cell centres arrives at the corners
+    x = i as cos(pi m / n) sin(2 pi m i / n): the closed form of the two-point mean, in x and in y."""
+    ncz, ncy, ncx = 3, 12, 16
+    for axis, n_, m in ((2, ncx, 3), (1, ncy, 2)):
+        idx = np.arange(n_, dtype=np.float64)
+        mode = np.sin(2 * np.pi * m * (idx + 0.5) / n_)
+        shape = [1, 1, 1]; shape[axis] = n_
+        c = np.broadcast_to(mode.reshape(shape), (ncz, ncy, ncx)).astype(np.float32)
+        n = oracle.cells_to_nodes(c).astype(np.float64)
+        want = np.cos(np.pi * m / n_) * np.sin(2 * np.pi * m * idx / n_)
+        got = n[1, 0, :] if axis == 2 else n[1, :, 0]
+        assert np.abs(got - want).max() < 2e-7
+
+
+def test_O9_cells_to_nodes_is_the_rounded_exact_mean():
+    """The fp32 node value is the correctly rounded mean of the 8 fp32 cells (brute force in
+    exact rational arithmetic on a tiny grid)."""
+    from fractions import Fraction
+    rng = np.random.default_rng(5)
+    c = (rng.standard_normal((2, 3, 3)) * 10 ** rng.uniform(-3, 3, (2, 3, 3))).astype(np.float32)
+    n = oracle.cells_to_nodes(c)
+    ncz, ncy, ncx = c.shape
+    for k in range(ncz + 1):
+        for j in range(ncy):
+            for i in range(ncx):
+                tot = Fraction(0)
+                for dk in (0, 1):
+                    kk = min(max(k - dk, 0), ncz - 1)
+                    for dj in (0, 1):
+                        for di in (0, 1):
+                            tot += Fraction(float(c[kk, (j - dj) % ncy, (i - di) % ncx]))
+                assert n[k, j, i] == np.float32(float(tot / 8))
+
+
+def test_O9_nodes_to_cells_linear_exact_and_sum_rule():
+    """Back-averaging: exact on a field linear in z; sum over cells = sum over nodes with the
+    trapezoid weights (1/2 on the two boundary levels) -- every node is a corner of 8 cells, or of
+    4 on the bottom / top level."""
+    nz, ny, nx = 7, 5, 6
+    q = np.broadcast_to((1.0 - 0.25 * np.arange(nz))[:, None, None], (nz, ny, nx)).copy()
+    qc = oracle.nodes_to_cells(q)
+    assert qc.shape == (nz - 1, ny, nx)
+    assert np.allclose(qc, (1.0 - 0.25 * (np.arange(nz - 1) + 0.5))[:, None, None], rtol=0, atol=1e-15)
+    rng = np.random.default_rng(9)
+    q = rng.standard_normal((nz, ny, nx))
+    w = np.ones(nz); w[0] = w[-1] = 0.5
+    assert abs(oracle.nodes_to_cells(q).sum() - (w[:, None, None] * q).sum()) < 1e-12
+
+
+def test_O9_solve_cells_of_horizontally_uniform_atmosphere_is_uniform():
+    """A horizontally uniform cell atmosphere stays uniform through staggering, solve and
+    back-averaging (with enough passes for the seams, pin P6)."""
+    inp = inputs.make_config(1, grid=(6, 6, 9), npasses=14)
+    for f in (inp.rho, inp.T, inp.P):
+        f[...] = f[:, :1, :1]
+    Qc, Itop, node = oracle.solve_cells(inp)
+    assert node.nz == inp.nz + 1 and Qc.shape == inp.shape
+    assert np.abs(Qc - Qc[:, :1, :1]).max() <= 1e-9 * np.abs(Qc).max()
