@@ -112,6 +112,22 @@ int rts_solve(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const floa
 int rts_solve_host(rts_ctx* ctx, const float* rho_host, const float* T_host, const float* P_host,
                    float* Qrad_host, float* Itop_host, void* stream);
 
+/* Grid staggering (paper's Interpolate: "trilinear interpolation of the MHD variables from the MHD
+ * grid to the staggered RTS grid"; reading R20).  The MHD variables live at
+ * the centres of nx*ny*(nz-1) cells, the RT nodes of this ctx are the cell corners: x, y periodic,
+ * the corner levels below / above the box repeat the edge cell level.
+ *   rts_cells_to_nodes  node = correctly rounded mean of the 8 cells around a corner;
+ *                       DEVICE cell [nz-1][ny][nx] -> DEVICE node [nz][ny][nx]
+ *   rts_nodes_to_cells  cell = mean of its 8 corner nodes; DEVICE [nz][ny][nx] -> DEVICE [nz-1][ny][nx]
+ *   rts_solve_cells     staggers rho, T, P (DEVICE, cell-centred [nz-1][ny][nx]) into the staging
+ *                       part of the workspace, runs rts_solve on the node grid and averages Q_rad
+ *                       back: Qrad_cells DEVICE out [nz-1][ny][nx]; Itop as in rts_solve.
+ * Asynchronous on `stream`; inputs are not modified; needs tables and workspace like rts_solve. */
+int rts_cells_to_nodes(rts_ctx* ctx, const float* cell_dev, float* node_dev, void* stream);
+int rts_nodes_to_cells(rts_ctx* ctx, const float* node_dev, float* cell_dev, void* stream);
+int rts_solve_cells(rts_ctx* ctx, const float* rho_cells_dev, const float* T_cells_dev, const float* P_cells_dev,
+                    float* Qrad_cells_dev, float* Itop_dev, void* stream);
+
 /* Stage A alone, for per-stage parity: DEVICE outputs kaprho, S each [nbands][nz][ny][nx]. */
 int rts_coefficients(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const float* P_dev,
                      float* kaprho_dev, float* S_dev, void* stream);

@@ -712,6 +712,58 @@ int rts_solve_host(rts_ctx* c, const float* rho, const float* T, const float* P,
     return rts_sync_check(c, stream);
 }
 
+namespace {
+int launch_c2n(rts_ctx* c, int nf, const float* const* cell, float* const* node, cudaStream_t st)
+{
+    StaggerParams p{};
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nf = nf; p.zchunk = 32;
+    for (int f = 0; f < nf; ++f) { p.cell[f] = cell[f]; p.node[f] = node[f]; }
+    dim3 block(64, 4), grid((c->nx + 63) / 64, (c->ny + 3) / 4, (c->nz + p.zchunk - 1) / p.zchunk);
+    rts_cells_to_nodes_kernel<<<grid, block, 0, st>>>(p);
+    CUDA_TRY(c, cudaGetLastError());
+    return RTS_OK;
+}
+int launch_n2c(rts_ctx* c, const float* qn, float* qc, cudaStream_t st)
+{
+    const int zchunk = 32;
+    dim3 block(64, 4), grid((c->nx + 63) / 64, (c->ny + 3) / 4, (c->nz - 1 + zchunk - 1) / zchunk);
+    rts_nodes_to_cells_kernel<<<grid, block, 0, st>>>(qn, qc, c->nx, c->ny, c->nz, zchunk);
+    CUDA_TRY(c, cudaGetLastError());
+    return RTS_OK;
+}
+}  // namespace
+
+int rts_cells_to_nodes(rts_ctx* c, const float* cell, float* node, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    if (!cell || !node) return fail(c, RTS_EINVAL, "rts_cells_to_nodes: null pointer");
+    return launch_c2n(c, 1, &cell, &node, as_stream(stream));
+}
+
+int rts_nodes_to_cells(rts_ctx* c, const float* qn, float* qc, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    if (!qn || !qc) return fail(c, RTS_EINVAL, "rts_nodes_to_cells: null pointer");
+    return launch_n2c(c, qn, qc, as_stream(stream));
+}
+
+int rts_solve_cells(rts_ctx* c, const float* rho_c, const float* T_c, const float* P_c, float* Qc, float* Itop, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    if (!rho_c || !T_c || !P_c || !Qc) return fail(c, RTS_EINVAL, "rts_solve_cells: null pointer");
+    if (!c->ws || !c->planned || !c->maps_ready) return fail(c, RTS_ESTATE, "rts_solve_cells: workspace not set");
+    const size_t N = (size_t)c->nx * c->ny * c->nz;
+    float* din = (float*)(c->ws + c->off_stage_in);      // node fields rho, T, P
+    float* qn = (float*)(c->ws + c->off_stage_out);      // node heating
+    const float* cell[3] = {rho_c, T_c, P_c};
+    float* node[3] = {din, din + N, din + 2 * N};
+    int rc = launch_c2n(c, 3, cell, node, as_stream(stream));
+    if (rc != RTS_OK) return rc;
+    rc = rts_solve(c, din, din + N, din + 2 * N, qn, Itop, stream);
+    if (rc != RTS_OK) return rc;
+    return launch_n2c(c, qn, Qc, as_stream(stream));
+}
+
 #ifdef RTS_TRACE
 int rts_debug_trace(unsigned long long* out, int n)
 {

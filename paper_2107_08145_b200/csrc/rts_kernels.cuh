@@ -7,6 +7,7 @@
 //   K_b  rts_sweep_kernel   stages B-E (paper's integrate() + readbuf/writebuf/exchange with
 //                           the box as its own neighbour + flux())
 //   K_f  rts_finalize_kernel adds the x-march partial heating (stored y-fastest) into Q_rad
+//   K_s  rts_cells_to_nodes_kernel / rts_nodes_to_cells_kernel   grid staggering
 //
 // Shares nothing with oracle/.
 #pragma once
@@ -278,6 +279,69 @@ __global__ void __launch_bounds__(256) rts_finalize_kernel(float* Q, const float
     for (int r = 0; r < 4; ++r) {
         const int j = j0 + ty + 8 * r, i = i0 + tx;
         if (i < nx && j < ny) Q[((size_t)k * ny + j) * nx + i] += tile[tx][ty + 8 * r];
+    }
+}
+
+// =========================================================================== K_s (NEXT #1)
+// Grid staggering (paper's Interpolate; reading R20).  The MHD variables
+// live at the centres of nx * ny * (nz-1) cells, the RT nodes are the cell corners: x and y are
+// periodic, the corner levels below / above the box repeat the edge cell level.
+// One thread owns a corner column (i, j) of a z chunk and marches up: the 4-cell horizontal sum of a
+// level is formed once (fp64: exact) and used by the two corner levels that touch it, so a node
+// costs 4 coalesced loads per field instead of 8.  node = (float)((h_below + h_above) / 8): the
+// correctly rounded mean, bit-identical to the oracle.  Up to 3 fields per launch.
+struct StaggerParams {
+    int nx, ny, nz;          // RT node grid (nz = cell levels + 1)
+    int nf, zchunk;
+    const float* cell[3];    // [nz-1][ny][nx]
+    float* node[3];          // [nz][ny][nx]
+};
+
+__global__ void __launch_bounds__(256) rts_cells_to_nodes_kernel(const StaggerParams p)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= p.nx || j >= p.ny) return;
+    const int k0 = blockIdx.z * p.zchunk, k1 = min(p.nz, k0 + p.zchunk);
+    const int im = (i == 0) ? p.nx - 1 : i - 1, jm = (j == 0) ? p.ny - 1 : j - 1;
+    const size_t r0 = (size_t)j * p.nx, r1 = (size_t)jm * p.nx, plane = (size_t)p.nx * p.ny;
+    const int ncz = p.nz - 1;
+    for (int f = 0; f < p.nf; ++f) {
+        const float* __restrict__ c = p.cell[f];
+        float* __restrict__ n = p.node[f];
+        auto hsum = [&](int kc) {
+            const float* q = c + (size_t)kc * plane;
+            return ((double)__ldg(q + r0 + i) + (double)__ldg(q + r0 + im)) + ((double)__ldg(q + r1 + i) + (double)__ldg(q + r1 + im));
+        };
+        double below = hsum(min(max(k0 - 1, 0), ncz - 1));
+        for (int k = k0; k < k1; ++k) {
+            const double above = (k <= ncz - 1) ? hsum(k) : below;   // top corner level: edge cells again
+            if (k == 0) below = above;                               // bottom corner level
+            n[(size_t)k * plane + r0 + i] = (float)((below + above) * 0.125);
+            below = above;
+        }
+    }
+}
+
+// Qc(i,j,k) = mean of the 8 corner nodes of cell (i,j,k), k = 0..nz-2 (fp32; the heating goes back to
+// the MHD grid).  Same marching scheme.
+__global__ void __launch_bounds__(256) rts_nodes_to_cells_kernel(const float* __restrict__ qn, float* __restrict__ qc,
+                                                                  int nx, int ny, int nz, int zchunk)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= nx || j >= ny) return;
+    const int k0 = blockIdx.z * zchunk, k1 = min(nz - 1, k0 + zchunk);
+    const int ip = (i == nx - 1) ? 0 : i + 1, jp = (j == ny - 1) ? 0 : j + 1;
+    const size_t r0 = (size_t)j * nx, r1 = (size_t)jp * nx, plane = (size_t)nx * ny;
+    auto hsum = [&](int k) {
+        const float* q = qn + (size_t)k * plane;
+        return (__ldg(q + r0 + i) + __ldg(q + r0 + ip)) + (__ldg(q + r1 + i) + __ldg(q + r1 + ip));
+    };
+    if (k0 >= k1) return;
+    float below = hsum(k0);
+    for (int k = k0; k < k1; ++k) {
+        const float above = hsum(k + 1);
+        qc[(size_t)k * plane + r0 + i] = 0.125f * (below + above);
+        below = above;
     }
 }
 

@@ -25,6 +25,7 @@ EXPORTS = [
     "rts_num_up_rays", "rts_set_tiling", "rts_set_exchange_interval", "rts_set_ctas_per_sm", "rts_workspace_bytes",
     "rts_set_workspace", "rts_solve", "rts_solve_host", "rts_coefficients", "rts_sync_check",
     "rts_plan_info", "rts_last_error", "rts_enable_timing", "rts_last_timing",
+    "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells",
 ]
 
 
@@ -79,6 +80,12 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_enable_timing.argtypes = [c_void_p, c_int]
     lib.rts_last_timing.restype = c_int
     lib.rts_last_timing.argtypes = [c_void_p, PF]
+    lib.rts_cells_to_nodes.restype = c_int
+    lib.rts_cells_to_nodes.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.rts_nodes_to_cells.restype = c_int
+    lib.rts_nodes_to_cells.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.rts_solve_cells.restype = c_int
+    lib.rts_solve_cells.argtypes = [c_void_p] + [c_void_p] * 5 + [c_void_p]
     lib.rts_last_error.restype = ctypes.c_char_p
     lib.rts_last_error.argtypes = [c_void_p]
     _lib = lib
@@ -240,6 +247,44 @@ class RTS:
                                                ctypes.c_void_p(s.data_ptr()), self._stream()), "rts_coefficients")
         return k, s
 
+    # ---- grid staggering (cells of the MHD grid <-> corner nodes of the RT grid)
+    def _cell_check(self, t, nz):
+        torch = self._torch
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == (nz, self.ny, self.nx)
+        return ctypes.c_void_p(t.data_ptr())
+
+    def cells_to_nodes(self, cell, node=None):
+        """float32 CUDA [nz-1][ny][nx] -> [nz][ny][nx]."""
+        if node is None:
+            node = self._torch.empty((self.nz, self.ny, self.nx), dtype=self._torch.float32, device="cuda")
+        self._check(self._lib.rts_cells_to_nodes(self._ctx, self._cell_check(cell, self.nz - 1), self._cell_check(node, self.nz),
+                                                 self._stream()), "rts_cells_to_nodes")
+        return node
+
+    def nodes_to_cells(self, qn, qc=None):
+        """float32 CUDA [nz][ny][nx] -> [nz-1][ny][nx]."""
+        if qc is None:
+            qc = self._torch.empty((self.nz - 1, self.ny, self.nx), dtype=self._torch.float32, device="cuda")
+        self._check(self._lib.rts_nodes_to_cells(self._ctx, self._cell_check(qn, self.nz), self._cell_check(qc, self.nz - 1),
+                                                 self._stream()), "rts_nodes_to_cells")
+        return qc
+
+    def solve_cells(self, rho_c, T_c, P_c, Qc=None, Itop=None, want_itop: bool = True):
+        """Cell-centred rho, T, P (float32 CUDA [nz-1][ny][nx]) -> (Q_rad on the cells, I_top)."""
+        torch = self._torch
+        if self._ws is None:
+            self.allocate_workspace()
+        if Qc is None:
+            Qc = torch.empty((self.nz - 1, self.ny, self.nx), dtype=torch.float32, device="cuda")
+        if want_itop and Itop is None:
+            Itop = torch.empty((self.nbands, self.num_up_rays(), self.ny, self.nx), dtype=torch.float32, device="cuda")
+        ip = ctypes.c_void_p(Itop.data_ptr()) if (want_itop and Itop is not None) else None
+        ncz = self.nz - 1
+        self._check(self._lib.rts_solve_cells(self._ctx, self._cell_check(rho_c, ncz), self._cell_check(T_c, ncz),
+                                              self._cell_check(P_c, ncz), self._cell_check(Qc, ncz), ip, self._stream()),
+                    "rts_solve_cells")
+        return Qc, (Itop if want_itop else None)
+
     def enable_timing(self, on: bool = True):
         self._check(self._lib.rts_enable_timing(self._ctx, 1 if on else 0), "rts_enable_timing")
 
@@ -252,9 +297,11 @@ class RTS:
         self._check(self._lib.rts_sync_check(self._ctx, self._stream()), "rts_sync_check")
 
 
-def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchange_interval: int = 0) -> "RTS":
-    """Create and configure a solver for an `inputs.RTSInputs` problem."""
-    r = RTS(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.nbands)
+def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchange_interval: int = 0,
+                cells: bool = False) -> "RTS":
+    """Create and configure a solver for an `inputs.RTSInputs` problem.  cells=True: the fields of
+    `inp` are cell-centred (solve_cells); the RT node grid then has one level more."""
+    r = RTS(inp.nx, inp.ny, inp.nz + (1 if cells else 0), inp.dx, inp.dy, inp.dz, inp.nbands)
     r.set_tables(inp.nT, inp.nP, inp.logT_min, inp.logT_max, inp.logP_min, inp.logP_max, inp.logkappa, inp.bandfrac)
     r.set_passes(inp.npasses)
     r.set_rays(inp.mu, inp.wq)
