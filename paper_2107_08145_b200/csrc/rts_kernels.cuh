@@ -313,6 +313,7 @@ __global__ void __launch_bounds__(256) rts_cells_to_nodes_kernel(const StaggerPa
             return ((double)__ldg(q + r0 + i) + (double)__ldg(q + r0 + im)) + ((double)__ldg(q + r1 + i) + (double)__ldg(q + r1 + im));
         };
         double below = hsum(min(max(k0 - 1, 0), ncz - 1));
+#pragma unroll 4
         for (int k = k0; k < k1; ++k) {
             const double above = (k <= ncz - 1) ? hsum(k) : below;   // top corner level: edge cells again
             if (k == 0) below = above;                               // bottom corner level
@@ -338,6 +339,7 @@ __global__ void __launch_bounds__(256) rts_nodes_to_cells_kernel(const float* __
     };
     if (k0 >= k1) return;
     float below = hsum(k0);
+#pragma unroll 4
     for (int k = k0; k < k1; ++k) {
         const float above = hsum(k + 1);
         qc[(size_t)k * plane + r0 + i] = 0.125f * (below + above);
