@@ -691,6 +691,16 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
             // ---- block start: wait for the unit, fetch halos and seam ghosts of the previous plane
             TR_BEGIN();
             if (s_ > 0) {
+                const bool exch = !(zmarch && blk0 == 0);
+                const int m_prev = (blk0 == 0) ? n_m - 1 : blk0 - 1;
+                // seam ghosts of the previous plane come from the previous pass: inside a pass (blk0 > 0)
+                // they were written more than one block ago, i.e. before the arrival counter this tile
+                // has already seen, so they are fetched before the wait and only stored after it (one
+                // L2 round trip and one barrier less per block); at a pass start they belong to the
+                // block the wait is for
+                const bool pre = exch && pass > 0 && blk0 > 0 && ngh > 0;
+                float gpre = 0.f;
+                if (pre && tid < ngh) gpre = ghost_fetch(gt[tid], pass - 1, m_prev, nullptr);
                 if (tid == 0) {
                     const int need = gblk * U.ntiles;
                     const int ab = *reinterpret_cast<volatile int*>(abortf);
@@ -705,14 +715,14 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 __syncthreads();
                 if (S.flag != 0) { bail = true; break; }     // uniform: the watchdog fired somewhere
                 TR_MARK(7);
-                if (!(zmarch && blk0 == 0)) {
+                if (exch) {
+                    // halo quads lie inside the domain, ghost columns / rows outside it: disjoint stores
                     float* const Xr = Xb + cur * NSLOT * BOXP;
-                    const int m_prev = (blk0 == 0) ? n_m - 1 : blk0 - 1;
                     load_halos(Xr, (gblk - 1) & 1);
                     if (ngh > 0) {
-                        __syncthreads();                     // a halo quad may overlap a ghost column
                         const float* Sp = stage0 + (size_t)stp * 2 * BOXP + BOXP;
-                        for (int e = tid; e < ngh; e += T) { const GhostEnt g = gt[e]; Xr[ghost_off(g)] = ghost_fetch(g, pass - 1, m_prev, Sp); }
+                        if (pre && tid < ngh) Xr[ghost_off(gt[tid])] = gpre;
+                        for (int e = pre ? tid + T : tid; e < ngh; e += T) { const GhostEnt g = gt[e]; Xr[ghost_off(g)] = ghost_fetch(g, pass - 1, m_prev, Sp); }
                     }
                     __syncthreads();
                 }
