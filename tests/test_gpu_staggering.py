@@ -55,3 +55,9 @@ def test_staggered_solve_matches_oracle(cfg, grid):
     Qc2 = s.nodes_to_cells(Qn)
     assert (Qc2 - Qc).abs().max().item() <= 4e-6 * Qc.abs().max().item()        # atomics: summation order
     s.close()
+
+
+@pytest.mark.slow
+def test_staggered_solve_full_size_config3():
+    """BASELINE.json configs[2] at full size through rts_solve_cells (planner defaults)."""
+    test_staggered_solve_matches_oracle(3, None)
