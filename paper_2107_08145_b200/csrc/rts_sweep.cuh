@@ -203,7 +203,8 @@ enum : unsigned {
     IT_CORE0 = 1u << 15,     // node row and quad belong to the tile core
     IT_CORE1 = 1u << 16,
     IT_C1_SH = 19,           // bits 19-21 one past the last valid column of the quad (1..4)
-    IT_SPECIAL = 1u << 22,   // core item holding a far-u column or a far-v row: writes the seam history
+    IT_SPECIAL = 1u << 22,   // core item holding a far-v row of a periodic v axis: writes the seam history (out of line)
+    IT_FARC = 1u << 26,      // core item holding the far-u column of its ray: writes the seam history (in line)
     IT_STRIP0 = 1u << 23,    // core node row lies in an exchange strip
     IT_STRIP1 = 1u << 24
 };
@@ -224,6 +225,7 @@ struct StepCtx {
     bool dplane;                       // z-march inflow plane: nodes are set, not updated
     bool hist, strips, lastpass;       // write seam histories / publish strips / reduce the heating this step
     float a_prev, a_cur;               // z-march: a on the previous / this plane
+    float* Ghist;                      // seam history of this plane and pass (far columns, then far rows)
 };
 
 struct TileGeo {
@@ -248,13 +250,6 @@ __device__ __noinline__ void item_publish(const UnitDesc* __restrict__ Up, const
     const int vN = P.v0 + rowN - HALO, ug = P.u0 + cq0 - HALO;
     if (P.hist && (fl & IT_SPECIAL)) {
         float* Gp = U.Gu + ((size_t)(P.pass & 1) * U.n_m + P.m) * (size_t)(NSLOT * (U.n_v + U.n_u4));
-        const int fj = ((s & 1) ? (P.far_u & 0xffff) : (P.far_u >> 16)) - cq0;   // far-u column of this ray inside the quad?
-        if (fj >= 0 && fj < 4) {
-            const float f0 = fj == 0 ? o0.x : fj == 1 ? o0.y : fj == 2 ? o0.z : o0.w;
-            const float f1 = fj == 0 ? o1.x : fj == 1 ? o1.y : fj == 2 ? o1.z : o1.w;
-            if (core0) __stcg(Gp + s * U.n_v + vN, f0);
-            if (core1) __stcg(Gp + s * U.n_v + vN + 1, f1);
-        }
         if (U.per_v) {
             const int fr = svp ? (P.far_v >> 16) : (P.far_v & 0xffff);   // far-v row (box)
             float* gv = Gp + NSLOT * U.n_v + s * U.n_u4 + ug;
@@ -381,6 +376,15 @@ __device__ __forceinline__ void do_item(
             if (act0 && j < c1) xw[j] = o0[j];
             if (act1 && j < c1) xw[G.BU + j] = o1[j];
         }
+    }
+    if (C.hist && (fl & IT_FARC)) {
+        // far-u column of this ray: its values are the next pass's seam ghosts of this plane
+        const int rowN = (int)((pos >> 16) & 0xffu), fj = ((s & 1) ? G.dlo_u : G.dhi_u - 1) - 4 * (int)(pos >> 24);
+        const float f0 = fj == 0 ? o0[0] : fj == 1 ? o0[1] : fj == 2 ? o0[2] : o0[3];
+        const float f1 = fj == 0 ? o1[0] : fj == 1 ? o1[1] : fj == 2 ? o1[2] : o1[3];
+        float* g = C.Ghist + s * U.n_v + (G.v0 + rowN - HALO);
+        if (act0 && (fl & IT_CORE0)) __stcg(g, f0);
+        if (act1 && (fl & IT_CORE1)) __stcg(g + 1, f1);
     }
     if ((C.hist && (fl & IT_SPECIAL)) || (C.strips && (fl & (IT_STRIP0 | IT_STRIP1)))) {
         PubCtx P;
@@ -522,7 +526,8 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 const int fc = (su > 0) ? G.dhi_u - 1 : G.dlo_u;  // far-u column of this slot (box)
                 const bool farc = (fc >= cq0 && fc < cq0 + 4);
                 const bool farr = U.per_v && ((c0r && rowN == fr) || (c1r && rowN + 1 == fr));
-                if ((c0r || c1r) && (farc || farr)) fl |= IT_SPECIAL;
+                if ((c0r || c1r) && farc) fl |= IT_FARC;
+                if ((c0r || c1r) && farr) fl |= IT_SPECIAL;
                 const bool su_strip = (su > 0) ? (cq0 + 4 > HALO + G.wu - K) : (cq0 - HALO < K);
                 if (c0r && (su_strip || (svp ? (HALO + G.wv - 1 - rowN < K) : (rowN - HALO < K)))) fl |= IT_STRIP0;
                 if (c1r && (su_strip || (svp ? (HALO + G.wv - 2 - rowN < K) : (rowN + 1 - HALO < K)))) fl |= IT_STRIP1;
@@ -757,6 +762,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 C.m = m; C.pl = pl; C.pass = pass; C.hj = hj; C.par_ex = gblk & 1;
                 C.dplane = zmarch && (m == 0);
                 C.hist = !lastpass; C.lastpass = lastpass;
+                C.Ghist = U.Gu + ((size_t)(pass & 1) * n_m + m) * g_plane;
                 C.strips = blk_last && more && !(zmarch && m == n_m - 1);
                 C.a_prev = a_of(pl - U.dir); C.a_cur = a_of(pl);
                 C.zreg = (C.a_prev != 0.f && C.a_cur != 0.f) ? 0 : ((C.a_prev == 0.f && C.a_cur == 0.f) ? 1 : 2);
