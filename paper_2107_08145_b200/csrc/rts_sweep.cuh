@@ -203,7 +203,7 @@ enum : unsigned {
     IT_CORE0 = 1u << 15,     // node row and quad belong to the tile core
     IT_CORE1 = 1u << 16,
     IT_C1_SH = 19,           // bits 19-21 one past the last valid column of the quad (1..4)
-    IT_SPECIAL = 1u << 22,   // core item holding a far-v row of a periodic v axis: writes the seam history (out of line)
+    IT_SPECIAL = 1u << 22,   // core item holding a far-v row of a periodic v axis: writes the seam history (in line)
     IT_FARC = 1u << 26,      // core item holding the far-u column of its ray: writes the seam history (in line)
     IT_STRIP0 = 1u << 23,    // core node row lies in an exchange strip
     IT_STRIP1 = 1u << 24
@@ -235,40 +235,19 @@ struct TileGeo {
     bool zmarch;
 };
 
-// seam histories and exchange strips of a core item (rare path)
-struct PubCtx { int v0, u0, wu, far_u, far_v, m, pass, par_ex; bool hist, strips; };   // by value: keeps the callers' state in registers
-
+// exchange strips of a core item at a block end (out of line: one step in K)
 // core0 / core1: node row 0 / 1 is a core row and was updated this step
-__device__ __noinline__ void item_publish(const UnitDesc* __restrict__ Up, const PubCtx P, const unsigned fl, const unsigned pos,
+__device__ __noinline__ void item_publish(const UnitDesc* __restrict__ Up, const int v0, const int u0, const int par_ex,
+                                          const unsigned fl, const unsigned pos,
                                           const bool core0, const bool core1, const float4 o0, const float4 o1)
 {
     const UnitDesc& U = *Up;
     const int s = fl & IT_SLOT;
-    const int rowN = (int)((pos >> 16) & 0xffu), quad = (int)(pos >> 24);
-    const bool svp = !(s & 2);
-    const int cq0 = 4 * quad;
-    const int vN = P.v0 + rowN - HALO, ug = P.u0 + cq0 - HALO;
-    if (P.hist && (fl & IT_SPECIAL)) {
-        float* Gp = U.Gu + ((size_t)(P.pass & 1) * U.n_m + P.m) * (size_t)(NSLOT * (U.n_v + U.n_u4));
-        if (U.per_v) {
-            const int fr = svp ? (P.far_v >> 16) : (P.far_v & 0xffff);   // far-v row (box)
-            float* gv = Gp + NSLOT * U.n_v + s * U.n_u4 + ug;
-            const int nv_ = min(4, HALO + P.wu - cq0);
-            if (core0 && rowN == fr) {
-                if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), o0);
-                else { const float a[4] = {o0.x, o0.y, o0.z, o0.w}; for (int j = 0; j < nv_; ++j) __stcg(gv + j, a[j]); }
-            }
-            if (core1 && rowN + 1 == fr) {
-                if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), o1);
-                else { const float a[4] = {o1.x, o1.y, o1.z, o1.w}; for (int j = 0; j < nv_; ++j) __stcg(gv + j, a[j]); }
-            }
-        }
-    }
-    if (P.strips) {
-        float* xe = U.Xex + (((size_t)P.par_ex * NSLOT + s) * U.n_v + vN) * U.n_u4 + ug;
-        if (core0 && (fl & IT_STRIP0)) __stcg(reinterpret_cast<float4*>(xe), o0);
-        if (core1 && (fl & IT_STRIP1)) __stcg(reinterpret_cast<float4*>(xe + U.n_u4), o1);
-    }
+    const int rowN = (int)((pos >> 16) & 0xffu), cq0 = 4 * (int)(pos >> 24);
+    const int vN = v0 + rowN - HALO, ug = u0 + cq0 - HALO;
+    float* xe = U.Xex + (((size_t)par_ex * NSLOT + s) * U.n_v + vN) * U.n_u4 + ug;
+    if (core0 && (fl & IT_STRIP0)) __stcg(reinterpret_cast<float4*>(xe), o0);
+    if (core1 && (fl & IT_STRIP1)) __stcg(reinterpret_cast<float4*>(xe + U.n_u4), o1);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -386,14 +365,21 @@ __device__ __forceinline__ void do_item(
         if (act0 && (fl & IT_CORE0)) __stcg(g, f0);
         if (act1 && (fl & IT_CORE1)) __stcg(g + 1, f1);
     }
-    if ((C.hist && (fl & IT_SPECIAL)) || (C.strips && (fl & (IT_STRIP0 | IT_STRIP1)))) {
-        PubCtx P;
-        P.v0 = G.v0; P.u0 = G.u0; P.wu = G.wu;
-        P.far_u = ((G.dhi_u - 1) << 16) | (G.dlo_u & 0xffff);   // far-u column (box) of su > 0 | su < 0 rays
-        P.far_v = ((G.dhi_v - 1) << 16) | (G.dlo_v & 0xffff);
-        P.m = C.m; P.pass = C.pass; P.par_ex = C.par_ex; P.hist = C.hist; P.strips = C.strips;
-        item_publish(&U, P, fl, pos, act0 && (fl & IT_CORE0), act1 && (fl & IT_CORE1), v0_, v1_);
+    if (C.hist && (fl & IT_SPECIAL)) {
+        // far-v row of this ray (periodic v axis): the next pass's seam ghost row of this plane
+        const int rowN = (int)((pos >> 16) & 0xffu), cq0 = 4 * (int)(pos >> 24);
+        const bool r1 = (rowN + 1 == (svp ? G.dhi_v - 1 : G.dlo_v));         // the far row is node row 1 (else row 0)
+        const float4 fv = r1 ? v1_ : v0_;
+        const bool okr = r1 ? (act1 && (fl & IT_CORE1)) : (act0 && (fl & IT_CORE0));
+        float* gv = C.Ghist + NSLOT * U.n_v + s * U.n_u4 + (G.u0 + cq0 - HALO);
+        const int nv_ = min(4, HALO + G.wu - cq0);
+        if (okr) {
+            if (nv_ == 4) __stcg(reinterpret_cast<float4*>(gv), fv);
+            else { const float a[4] = {fv.x, fv.y, fv.z, fv.w}; for (int j = 0; j < nv_; ++j) __stcg(gv + j, a[j]); }
+        }
     }
+    if (C.strips && (fl & (IT_STRIP0 | IT_STRIP1)))
+        item_publish(&U, G.v0, G.u0, C.par_ex, fl, pos, act0 && (fl & IT_CORE0), act1 && (fl & IT_CORE1), v0_, v1_);
 }
 
 // ------------------------------------------------------------------------------------------
