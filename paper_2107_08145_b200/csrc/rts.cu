@@ -249,8 +249,14 @@ int make_plan(rts_ctx* c)
                     // all tiles of a unit are resident together, so slots / ntiles units run at a time
                     const int uif = std::max(1, slots / (ntu * ntv));
                     const int rounds = (units_total + uif - 1) / uif;
-                    const double cost = (double)rounds * R * (items_for(WU, WV) + 64.0 + 0.25 * (WU + WV));   // + exchange perimeter
-                    if (!bu || cost < best_cost) { best_cost = cost; bu = WU; bv = WV; }
+                    // ragged last tiles run at the pace of the full ones: charge the covered area
+                    const double cover = ((double)ntu * WU * ntv * WV) / ((double)t.n_u * t.n_v);
+                    // items updated per step, averaged over a block: the u halo is a whole quad column while
+                    // the v halo shrinks from K-1 rows to none (wide tiles along the unit-stride axis win)
+                    const double work = NSLOT * ((WU + HALO) / 4) * (WV + 0.5 * (c->K - 1)) * 0.5;
+                    const double cost = (double)rounds * R * cover * (work + 64.0 + 0.25 * (WU + WV));   // + exchange perimeter
+                    // within the model's accuracy (1.5 %) the squarer tile (less exchange) is taken
+                    if (!bu || cost < 0.985 * best_cost || (cost < 1.015 * best_cost && WU + WV < bu + bv)) { best_cost = cost; bu = WU; bv = WV; }
                 }
             }
             if (!bu) { ok = false; break; }
