@@ -256,6 +256,9 @@ def test_error_codes():
     assert lib.rts_set_workspace(ctx, ctypes.c_void_p(base), n - 1) == -1            # too small
     assert lib.rts_set_workspace(ctx, ctypes.c_void_p(base), n) == 0
     assert lib.rts_solve(ctx, None, p, p, p, None, None) == -1                       # null field
+    assert lib.rts_solve(ctx, p, p, p, ctypes.c_void_p(buf.data_ptr() + 4), None, None) == -1   # Qrad not 16-byte aligned
+    assert b"aligned" in lib.rts_last_error(ctx)
+    assert lib.rts_solve_cells(ctx, p, p, p, None, None, None) == -1                  # null output
     assert lib.rts_set_passes(ctx, 2) == 0
     assert lib.rts_solve(ctx, p, p, p, p, None, None) == -2                          # plan changed
     assert lib.rts_destroy(ctx) == 0
