@@ -95,6 +95,20 @@ __device__ __forceinline__ void load_row5(const uint32_t row, float (&o)[6])
     else        { o[5] = lds32<16>(row); o[0] = 0.f; }
 }
 
+// packed fp32 pairs (Blackwell FFMA2 / FMUL2): one issue slot for two nodes
+__device__ __forceinline__ float2 fma2(const float2 a, const float2 b, const float2 c) {
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(*reinterpret_cast<const unsigned long long*>(&a)),
+        "l"(*reinterpret_cast<const unsigned long long*>(&b)), "l"(*reinterpret_cast<const unsigned long long*>(&c)));
+    return *reinterpret_cast<float2*>(&r);
+}
+__device__ __forceinline__ float2 mul2(const float2 a, const float2 b) {
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(*reinterpret_cast<const unsigned long long*>(&a)),
+        "l"(*reinterpret_cast<const unsigned long long*>(&b)));
+    return *reinterpret_cast<float2*>(&r);
+}
+
 // optical paths of one node row (4 nodes).  lo / hi: opacity of the previous plane on the two
 // stencil rows (lower / higher v), kv = 0.5*ds * weights of (lo, lo side, hi, hi side).
 template <int SU>
@@ -121,6 +135,39 @@ __device__ __forceinline__ void row_update(
     const float4 wv, const float a_lo, const float a_hi, const float a_p, float (&xp)[4])
 {
     const float sp[4] = {spv.x, spv.y, spv.z, spv.w};
+    if (REG != 2 && !SMALL) {
+        // the common bodies: the bilinear sums per node (their side-column operands are not
+        // pair-aligned), the attenuation factors and the final combination for two nodes per
+        // instruction (fma.rn.f32x2); same operations, same order, same rounding as the scalar form
+#pragma unroll
+        for (int j = 0; j < 4; j += 2) {
+            const int c = j + 1, cs = j + 1 - SU;
+            const float2 Xu = make_float2(wv.x * xlo[c] + wv.y * xlo[cs] + wv.z * xhi[c] + wv.w * xhi[cs],
+                                          wv.x * xlo[c + 1] + wv.y * xlo[cs + 1] + wv.z * xhi[c + 1] + wv.w * xhi[cs + 1]);
+            const float2 dt2 = make_float2(dt[j], dt[j + 1]);
+            const float2 t2 = mul2(dt2, make_float2(-LOG2E, -LOG2E));
+            const float2 E2 = make_float2(ex2_approx(t2.x), ex2_approx(t2.y));
+            const float2 em1 = fma2(E2, make_float2(-1.f, -1.f), make_float2(1.f, 1.f));
+            const float2 wl = mul2(em1, make_float2(rcp_approx(dt2.x), rcp_approx(dt2.y)));
+            float2 v = fma2(make_float2(-Xu.x, -Xu.y), em1, Xu);                  // Xu * e^-dt
+            if (REG == 0) {
+                float d0 = sp[j], d1 = sp[j + 1];
+                d0 = fmaf(-wv.x, slo[c], d0); d0 = fmaf(-wv.y, slo[cs], d0); d0 = fmaf(-wv.z, shi[c], d0); d0 = fmaf(-wv.w, shi[cs], d0);
+                d1 = fmaf(-wv.x, slo[c + 1], d1); d1 = fmaf(-wv.y, slo[cs + 1], d1); d1 = fmaf(-wv.z, shi[c + 1], d1); d1 = fmaf(-wv.w, shi[cs + 1], d1);
+                v = fma2(make_float2(-d0, -d1), wl, v);
+            } else {
+                const float2 pp = fma2(wl, make_float2(-1.f, -1.f), make_float2(1.f, 1.f));   // psi_p = 1 - (1-E)/dt
+                const float2 pu = fma2(pp, make_float2(-1.f, -1.f), em1);                    // psi_u = (1 - E) - psi_p
+                float s0_ = wv.x * slo[c], s1_ = wv.x * slo[c + 1];
+                s0_ = fmaf(wv.y, slo[cs], s0_); s0_ = fmaf(wv.z, shi[c], s0_); s0_ = fmaf(wv.w, shi[cs], s0_);
+                s1_ = fmaf(wv.y, slo[cs + 1], s1_); s1_ = fmaf(wv.z, shi[c + 1], s1_); s1_ = fmaf(wv.w, shi[cs + 1], s1_);
+                v = fma2(pu, make_float2(s0_, s1_), v);
+                v = fma2(pp, make_float2(sp[j], sp[j + 1]), v);
+            }
+            xp[j] = v.x; xp[j + 1] = v.y;
+        }
+        return;
+    }
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int c = j + 1, cs = j + 1 - SU;
