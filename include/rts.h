@@ -136,6 +136,15 @@ int rts_coefficients(rts_ctx* ctx, const float* rho_dev, const float* T_dev, con
  * (RTS_OK, RTS_ETIMEOUT if the sweep watchdog fired, RTS_ECUDA). */
 int rts_sync_check(rts_ctx* ctx, void* stream);
 
+/* Thick-plane shortcut (default on).  Where every optical path of a z-march ray on a level pair
+ * exceeds 88.5 the fp32 exp underflows to exactly 0 and the update does not depend on the carried
+ * intensity; the sweeps along z skip those planes in the non-final passes.  Results are bit-identical
+ * for I_top and identical up to the summation order of the heating atomics.
+ * rts_thick_levels: after a solve, HOST out [nbands] = number of level pairs from the bottom that were
+ * found thick (synchronises `stream`); skipped updates = levels * nx * ny * (z-march rays) * (passes-1). */
+int rts_set_thick_skip(rts_ctx* ctx, int on);
+int rts_thick_levels(rts_ctx* ctx, int* levels_host, void* stream);
+
 /* Per-stage device timing of the last rts_solve (CUDA events recorded on the solve stream
  * inside rts_solve).  rts_last_timing waits for the solve and fills ms4 (HOST) with
  * [0] stage A + switch heights, [1] all sweep launches, [2] finalize, [3] whole solve. */

@@ -42,6 +42,7 @@ struct rts_ctx {
     int nx = 0, ny = 0, nz = 0, nb = 0;
     double h[3] = {0, 0, 0};
     int npass = 3;
+    bool thick_skip = true;
     std::vector<HostRay> rays;
     int n_up = 0;
     // tables
@@ -64,7 +65,7 @@ struct rts_ctx {
     int PX = 0, PY = 0, PYR = 0;
     size_t ws_bytes = 0;
     // workspace offsets
-    size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_lev = 0, off_kstar = 0, off_abort = 0,
+    size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_kmin = 0, off_lev = 0, off_kstar = 0, off_mthick = 0, off_abort = 0,
            off_units = 0, off_bar = 0, off_stage_in = 0, off_stage_out = 0;
     int nblk_a = 0;
     // workspace
@@ -299,8 +300,10 @@ int make_plan(rts_ctx* c)
     c->off_QB = take(sizeof(float) * N);
     c->nblk_a = ((c->nx + 31) / 32) * ((c->ny + 31) / 32);
     c->off_ksum = take(sizeof(double) * (size_t)c->nb * c->nz * c->nblk_a);
-    c->off_lev = take(sizeof(double) * (size_t)c->nb * c->nz);
+    c->off_kmin = take(sizeof(float) * (size_t)c->nb * c->nz * c->nblk_a);
+    c->off_lev = take(sizeof(double) * (size_t)c->nb * c->nz * 2);
     c->off_kstar = take(sizeof(int) * c->nb);
+    c->off_mthick = take(sizeof(int) * c->nb);
     c->off_abort = take(sizeof(int) * 8);                    // [0] watchdog, [1] ticket counter
     for (auto& g : groups)
         for (auto& sub : g.sub)
@@ -355,6 +358,11 @@ int bind_workspace(rts_ctx* c)
         d.Gu = (float*)(ws + hu.off_g);
         d.barrier = (int*)(ws + c->off_bar) + i;
         d.kstar = (const int*)(ws + c->off_kstar) + d.band;
+        d.mthick = (const int*)(ws + c->off_mthick) + d.band;
+        // carried strips and seam histories must hold finite numbers from the start: planes that are
+        // skipped as optically thick leave their entries untouched, and readers multiply them by exactly 0
+        CUDA_TRY(c, cudaMemset(ws + hu.off_xex, 0, sizeof(float) * 2 * NSLOT * (size_t)d.n_v * d.n_u4));
+        CUDA_TRY(c, cudaMemset(ws + hu.off_g, 0, sizeof(float) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u4)));
         const float* base = (const float*)(ws + (d.march == 0 ? c->off_coefB : c->off_coefA));
         d.cbase = base + (size_t)(2 * d.band) * d.c_field;
         flat.push_back(d);
@@ -415,6 +423,7 @@ int launch_stage_a(rts_ctx* c, const float* rho, const float* T, const float* P,
     p.strideA_f = (long long)c->nz * c->PYR * c->PX;
     p.strideB_f = (long long)c->nz * c->nx * c->PY;
     p.ksum = (double*)(c->ws + c->off_ksum);
+    p.kmin = (float*)(c->ws + c->off_kmin);
     p.plain_k = plain_k; p.plain_s = plain_s;
     dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, c->nz), block(32, 8);
     rts_coef_kernel<<<grid, block, 0, st>>>(p);
@@ -624,9 +633,11 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[0], st));
     int rc = launch_stage_a(c, rho, T, P, nullptr, nullptr, st);
     if (rc != RTS_OK) return rc;
-    rts_kstar_kernel<<<c->nb, 256, 0, st>>>((const double*)(ws + c->off_ksum), c->nz, c->nblk_a,
-                                            1.0 / ((double)c->nx * c->ny), c->h[2], 5.0, (int*)(ws + c->off_kstar),
-                                            (double*)(ws + c->off_lev));
+    double kc_z = 0.0;                                      // smallest half path of a z-march ray (0: none)
+    if (c->thick_skip) for (auto& r : c->rays) if (r.march == 2) kc_z = (kc_z == 0.0) ? (double)(float)(0.5 * r.ds) : std::min(kc_z, (double)(float)(0.5 * r.ds));
+    rts_kstar_kernel<<<c->nb, 256, 0, st>>>((const double*)(ws + c->off_ksum), (const float*)(ws + c->off_kmin), c->nz, c->nblk_a,
+                                            1.0 / ((double)c->nx * c->ny), c->h[2], 5.0, kc_z, (int*)(ws + c->off_kstar),
+                                            (int*)(ws + c->off_mthick), (double*)(ws + c->off_lev));
     CUDA_TRY(c, cudaGetLastError());
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[1], st));
 
@@ -657,6 +668,22 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
         CUDA_TRY(c, cudaGetLastError());
     }
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[4], st));
+    return RTS_OK;
+}
+
+int rts_set_thick_skip(rts_ctx* c, int on)
+{
+    if (!c) return RTS_EINVAL;
+    c->thick_skip = on != 0;
+    return RTS_OK;
+}
+
+int rts_thick_levels(rts_ctx* c, int* levels_host, void* stream)
+{
+    if (!c || !levels_host) return RTS_EINVAL;
+    if (!c->ws || !c->planned) return fail(c, RTS_ESTATE, "rts_thick_levels: workspace not set");
+    CUDA_TRY(c, cudaStreamSynchronize(as_stream(stream)));
+    CUDA_TRY(c, cudaMemcpy(levels_host, c->ws + c->off_mthick, sizeof(int) * c->nb, cudaMemcpyDeviceToHost));
     return RTS_OK;
 }
 

@@ -65,6 +65,7 @@ struct UnitDesc {
                       //                            every slot, then (per_v only) far-v row of every slot
     int*   barrier;   // arrivals of this unit's tiles (monotonic)
     const int* kstar; // device: switch height of this band
+    const int* mthick;// device: thick level pairs from the bottom of this band (z-march plane skipping)
     long long q_sm, q_sv;                 // heating strides along (march, v); u stride 1
     long long it_su, it_so, it_sr, it_sb; // I_top strides along u, march-or-v axis, ray, band
 };
@@ -132,6 +133,7 @@ struct CoefParams {
     int PX, PY, PYR;
     long long strideA_f, strideB_f;              // field strides
     double* ksum;            // [nb][nz][nblk] partial sums (nblk = gridDim.x*gridDim.y), or null
+    float* kmin;             // [nb][nz][nblk] partial minima of kaprho (with ksum)
     float* plain_k; float* plain_s;              // optional [nb][N] outputs (rts_coefficients)
 };
 
@@ -139,6 +141,7 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
 {
     __shared__ float tile[2][32][33];
     __shared__ double red[8];
+    __shared__ float redm[8];
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32, k = blockIdx.z;
     const int i = i0 + tx;
@@ -176,6 +179,7 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
         const float* F = p.bandfrac + (size_t)b * p.nT;
         float* A0 = p.coefA + (size_t)(2 * b) * p.strideA_f;  float* A1 = A0 + p.strideA_f;
         double part = 0.0;
+        float pmin = 3.0e38f;
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             float kr = 0.f, sr = 0.f;
@@ -190,6 +194,7 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
                 kr = (float)kd;
                 sr = (float)(fb * planck[r]);
                 part += kd;
+                pmin = fminf(pmin, kr);
                 const int j = j0 + ty + 8 * r;
                 // layout A: every periodic image of (i, j) inside the padded plane
                 for (int row = (j + HALO) % p.ny; row < p.PYR; row += p.ny) {
@@ -208,15 +213,17 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
         // block sum of kaprho (deterministic order)
         if (p.ksum) {
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-            if (tx == 0) red[ty] = part;
+            for (int o = 16; o > 0; o >>= 1) { part += __shfl_xor_sync(0xffffffffu, part, o); pmin = fminf(pmin, __shfl_xor_sync(0xffffffffu, pmin, o)); }
+            if (tx == 0) { red[ty] = part; redm[ty] = pmin; }
         }
         __syncthreads();
         if (p.ksum && tx == 0 && ty == 0) {
             double s = 0.0;
-            for (int w = 0; w < 8; ++w) s += red[w];
+            float mn = 3.0e38f;
+            for (int w = 0; w < 8; ++w) { s += red[w]; mn = fminf(mn, redm[w]); }
             const int nblk = gridDim.x * gridDim.y;
             p.ksum[((size_t)b * p.nz + k) * nblk + blockIdx.y * gridDim.x + blockIdx.x] = s;
+            p.kmin[((size_t)b * p.nz + k) * nblk + blockIdx.y * gridDim.x + blockIdx.x] = mn;
         }
         // layout B: transposed write, coalesced along y
         float* B0 = p.coefB + (size_t)(2 * b) * p.strideB_f;  float* B1 = B0 + p.strideB_f;
@@ -236,19 +243,28 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
 // =========================================================================== K_k
 // kstar[b] = highest level k whose horizontally averaged optical depth from the top,
 // tau(k) = sum_{k' >= k} <kaprho_b>(k') dz, is >= tau_switch; -1 if none.  One block per band.
-__global__ void __launch_bounds__(256) rts_kstar_kernel(const double* ksum, int nz, int nblk, double inv_nxy,
-                                                        double dz, double tau_switch, int* kstar, double* lev)
+// mthick[b] = number of consecutive level pairs (k-1, k), k = 1, 2, ..., from the bottom on which every
+// optical path of a z-march ray exceeds DTAU_SKIP: kc_z * (min kaprho(k-1) + min kaprho(k)) > DTAU_SKIP
+// bounds dtau = kc*kaprho_p + sum_n wk_n*kaprho_n from below (sum_n wk_n = kc).  There the approximate
+// exp underflows to exactly 0 and the update does not depend on the carried plane (rts_sweep.cuh).
+constexpr float DTAU_SKIP = 88.5f;
+__global__ void __launch_bounds__(256) rts_kstar_kernel(const double* ksum, const float* kmin, int nz, int nblk, double inv_nxy,
+                                                        double dz, double tau_switch, double kc_z, int* kstar, int* mthick,
+                                                        double* lev)
 {
     const int b = blockIdx.x;
-    double* L = lev + (size_t)b * nz;
+    double* L = lev + (size_t)b * 2 * nz;
+    double* M = L + nz;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (int k = warp; k < nz; k += nw) {             // level sums, fixed order
+    for (int k = warp; k < nz; k += nw) {             // level sums (fixed order) and level minima
         const double* q = ksum + ((size_t)b * nz + k) * nblk;
+        const float* qm = kmin + ((size_t)b * nz + k) * nblk;
         double s = 0.0;
-        for (int w = lane; w < nblk; w += 32) s += q[w];
+        float mn = 3.0e38f;
+        for (int w = lane; w < nblk; w += 32) { s += q[w]; mn = fminf(mn, qm[w]); }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0) L[k] = s;
+        for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o)); }
+        if (lane == 0) { L[k] = s; M[k] = (double)mn; }
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -259,6 +275,11 @@ __global__ void __launch_bounds__(256) rts_kstar_kernel(const double* ksum, int 
             if (tau >= tau_switch) { ks = k; break; }
         }
         kstar[b] = ks;
+        int m = 0;
+        for (int k = 1; k < nz; ++k) {
+            if (kc_z * (M[k - 1] + M[k]) > (double)DTAU_SKIP) m = k; else break;
+        }
+        mthick[b] = m;
     }
 }
 

@@ -465,6 +465,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     G.dlo_u = HALO - G.u0; G.dhi_u = HALO + U.n_u - G.u0;
     G.dlo_v = HALO - G.v0; G.dhi_v = HALO + U.n_v - G.v0;
     G.kstar = *U.kstar;
+    const int mthick = (U.march == 2) ? *U.mthick : 0;   // z-march: planes below this level are optically thick
     G.zmarch = (U.march == 2);
     const int BU = G.BU, BV = G.BV, BOXP = G.BOXP;
     const int n_m = U.n_m, npass = U.npass, K = U.K;
@@ -800,7 +801,11 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 C.a_prev = a_of(pl - U.dir); C.a_cur = a_of(pl);
                 C.zreg = (C.a_prev != 0.f && C.a_cur != 0.f) ? 0 : ((C.a_prev == 0.f && C.a_cur == 0.f) ? 1 : 2);
                 TR_MARK(2);
-                {
+                // Thick-plane shortcut (z-march, non-final passes): on planes pl <= mthick every optical path
+                // exceeds DTAU_SKIP, e^-dtau is exactly 0 and the new plane does not depend on the carried one.
+                // The planes pl < mthick only feed such planes (and seam ghosts that are multiplied by 0), so
+                // their updates are skipped; plane mthick restarts from whatever finite values the buffers hold.
+                if (!(zmarch && !lastpass && pl < mthick)) {
 #pragma unroll 1
                     for (int r = 0; r < MAXIT; ++r) {        // one copy of the item code; the slot of an item is warp-uniform
                         const unsigned pos_ = r ? ipos[1] : ipos[0], fl_ = r ? ifl[1] : ifl[0];

@@ -25,7 +25,7 @@ EXPORTS = [
     "rts_num_up_rays", "rts_set_tiling", "rts_set_exchange_interval", "rts_set_ctas_per_sm", "rts_workspace_bytes",
     "rts_set_workspace", "rts_solve", "rts_solve_host", "rts_coefficients", "rts_sync_check",
     "rts_plan_info", "rts_last_error", "rts_enable_timing", "rts_last_timing",
-    "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells",
+    "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells", "rts_set_thick_skip", "rts_thick_levels",
 ]
 
 
@@ -86,6 +86,10 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_nodes_to_cells.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
     lib.rts_solve_cells.restype = c_int
     lib.rts_solve_cells.argtypes = [c_void_p] + [c_void_p] * 5 + [c_void_p]
+    lib.rts_set_thick_skip.restype = c_int
+    lib.rts_set_thick_skip.argtypes = [c_void_p, c_int]
+    lib.rts_thick_levels.restype = c_int
+    lib.rts_thick_levels.argtypes = [c_void_p, PI, c_void_p]
     lib.rts_last_error.restype = ctypes.c_char_p
     lib.rts_last_error.argtypes = [c_void_p]
     _lib = lib
@@ -284,6 +288,15 @@ class RTS:
                                               self._cell_check(P_c, ncz), self._cell_check(Qc, ncz), ip, self._stream()),
                     "rts_solve_cells")
         return Qc, (Itop if want_itop else None)
+
+    def set_thick_skip(self, on: bool):
+        self._check(self._lib.rts_set_thick_skip(self._ctx, 1 if on else 0), "rts_set_thick_skip")
+
+    def thick_levels(self):
+        """Level pairs from the bottom found optically thick in the last solve, per band."""
+        arr = (ctypes.c_int * self.nbands)()
+        self._check(self._lib.rts_thick_levels(self._ctx, arr, self._stream()), "rts_thick_levels")
+        return [int(v) for v in arr]
 
     def enable_timing(self, on: bool = True):
         self._check(self._lib.rts_enable_timing(self._ctx, 1 if on else 0), "rts_enable_timing")

@@ -191,6 +191,26 @@ def test_isothermal_closed_form_on_gpu():
     assert (Q <= 1e-6 * np.abs(Q).max()).all()          # only cooling (downward rays see I < S)
 
 
+# ------------------------------------------------------------------ thick-plane shortcut
+def test_thick_plane_shortcut_is_bit_exact_on_itop():
+    """The z sweeps skip optically thick planes in the non-final passes: I_top (no atomics) must be
+    bit-identical with the shortcut off, Q_rad identical up to the summation order of its atomics."""
+    torch, rts = _gpu()
+    inp = inputs.make_config(4, grid=(44, 40, 60), nbands=6)      # bands up to x1e5: many thick levels
+    rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
+    s = rts.from_inputs(inp, tiling={0: (16, 12), 1: (16, 12), 2: (16, 12)})
+    Q1, I1 = s.solve(rho, T, P); s.sync_check()
+    levels = s.thick_levels()
+    Q1 = Q1.clone(); I1 = I1.clone()
+    s.set_thick_skip(False)
+    Q0, I0 = s.solve(rho, T, P); s.sync_check()
+    assert s.thick_levels() == [0] * inp.nbands
+    s.close()
+    assert max(levels) >= 4 and levels == sorted(levels), levels    # opacity scale grows with the band index
+    assert torch.equal(I0, I1)
+    assert (Q0 - Q1).abs().max().item() <= 2e-6 * Q0.abs().max().item()
+
+
 # ------------------------------------------------------------------ API behaviour
 def test_solve_host_matches_device_solve_and_itop_optional():
     torch, rts = _gpu()
