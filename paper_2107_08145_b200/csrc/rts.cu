@@ -28,7 +28,9 @@ struct TypePlan {        // per march axis
     int n_m = 0, n_u = 0, n_v = 0;
     int WU = 0, WV = 0, ntu = 0, ntv = 0;
     int userWU = 0, userWV = 0;
-    int items = 0;       // 4 x 2 node blocks of a full tile (halo included)
+    int ng = 2;          // ray groups (same su) per unit: 2, or 1 where a plane with all four rays does not fit
+    int nstage = 3;      // depth of the coefficient ring
+    int items = 0;       // 2 x 2 node blocks of one group of a full tile (halo included)
 };
 
 struct HostUnit {
@@ -39,7 +41,7 @@ struct HostUnit {
 }  // namespace
 
 struct rts_ctx {
-    int nx = 0, ny = 0, nz = 0, nb = 0;
+    int nx = 0, ny = 0, nz = 0, nb = 0, nbp = 0;   // nbp = band pairs
     double h[3] = {0, 0, 0};
     int npass = 3;
     bool thick_skip = true;
@@ -53,7 +55,7 @@ struct rts_ctx {
     float* d_bandfrac = nullptr;
     // device facts
     int sm_count = 0, max_smem_optin = 0;
-    int user_ctas_per_sm = 0, user_K = 0, user_threads = 0;
+    int user_ctas_per_sm = 0, user_K = 0, user_threads = 0, user_nstage = 0, user_ng = 0;
     SweepMaps maps;
     void* encode_fn = nullptr;    // cuTensorMapEncodeTiled
     // plan
@@ -65,7 +67,7 @@ struct rts_ctx {
     int PX = 0, PY = 0, PYR = 0;
     size_t ws_bytes = 0;
     // workspace offsets
-    size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_kmin = 0, off_lev = 0, off_kstar = 0, off_mthick = 0, off_abort = 0,
+    size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_kmin = 0, off_lev = 0, off_kstar = 0, off_mthick = 0, off_mthick_b = 0, off_abort = 0,
            off_units = 0, off_bar = 0, off_stage_in = 0, off_stage_out = 0;
     int nblk_a = 0;
     // workspace
@@ -138,8 +140,7 @@ void make_ray_consts(const HostRay& r, RayC& rc)
     const int ord_p[4] = {2, 3, 0, 1}, ord_m[4] = {0, 1, 2, 3};
     for (int q = 0; q < 4; ++q) {
         const int src = (r.sv > 0) ? ord_p[q] : ord_m[q];
-        rc.wx[q] = (float)w[src];
-        rc.wk[q] = (float)(0.5 * r.ds * w[src]);
+        rc.w[q] = (float)w[src];
     }
     rc.kc = (float)(0.5 * r.ds);
     rc.wq = (float)r.w;
@@ -165,15 +166,16 @@ void default_rays(rts_ctx* c)
 }
 
 // dynamic shared memory of a CTA whose tiles are WU x WV (SmemPlan: coefficient ring, carried
-// planes, ghost list, item tables)
-int smem_for(int WU, int WV) { return (int)SmemPlan(WU, WV).bytes(); }
-// items (4 x 2 node blocks of one ray, halo included, padded to whole warps per ray) of a CTA whose
+// planes, ghost list, halo list)
+int smem_for(int WU, int WV, int ng, int nstage) { return (int)SmemPlan(WU, WV, ng, nstage).bytes(); }
+// items (2 x 2 node blocks, halo included, padded to whole warps) of ONE ray group of a CTA whose
 // tiles are WU x WV; a thread owns MAXIT of them
-int items_for(int WU, int WV) { return NSLOT * SmemPlan(WU, WV).nitems; }
+int items_for(int WU, int WV, int ng, int nstage) { return SmemPlan(WU, WV, ng, nstage).nitems; }
 
 // --------------------------------------------------------------------------- planner
-// Groups the rays into sweep units (march axis, direction, one ray per sign pair), chooses the
-// tile shape per march axis and the CTA size, lays out the workspace.
+// Groups the rays into sweep units (march axis, direction, one ray per sign pair, band pair), chooses the
+// tile shape, the ray groups per unit and the ring depth per march axis and the CTA size, lays out
+// the workspace.
 int make_plan(rts_ctx* c)
 {
     c->planned = false;
@@ -185,6 +187,7 @@ int make_plan(rts_ctx* c)
         r.itop = r.up ? nup++ : -1;
     }
     c->n_up = nup;
+    c->nbp = (c->nb + 1) / 2;
     for (int a = 0; a < 3; ++a) {
         TypePlan& t = c->tp[a];
         t.n_m = n[a];
@@ -213,22 +216,19 @@ int make_plan(rts_ctx* c)
         }
         if (!placed) g->sub.push_back(std::vector<int>{ri});
     }
-    int units_of[3] = {0, 0, 0};
-    for (auto& g : groups) units_of[g.march] += (int)g.sub.size() * c->nb;
-    const int units_total = units_of[0] + units_of[1] + units_of[2];
+    int skel_of[3] = {0, 0, 0};                  // (march, dir, sub) skeletons x band pairs
+    for (auto& g : groups) skel_of[g.march] += (int)g.sub.size() * c->nbp;
 
-    // --- tile shape per march axis: least total 4x2-block work (halo recomputation included)
-    //     among the shapes whose CTA fits R times on an SM
+    // --- per march axis: tile shape, ray groups per unit (2: all four rays of a plane in one CTA; 1: the
+    //     su = +1 and su = -1 rays as separate units, for planes too large to be resident otherwise) and ring
+    //     depth, by least modelled time among the shapes whose CTA fits R times on an SM
     cudaFuncAttributes fa;
     CUDA_TRY(c, cudaFuncGetAttributes(&fa, rts_sweep_kernel));
-    // R CTAs share an SM: R = 2 with <= RTS_SWEEP_THREADS / 2 threads each, or one CTA of up to
-    // RTS_SWEEP_THREADS threads on a larger tile (less halo recomputation, half the exchanges).
-    // Both are planned; the cheaper one (rounds of resident units x items an SM updates per step) wins.
     int bestR = 0;
     double bestR_cost = 0.0;
     TypePlan best_tp[3];
     for (int R = (c->user_ctas_per_sm ? c->user_ctas_per_sm : 2); R >= 1; --R) {
-        const int thread_cap = std::min(c->user_threads ? c->user_threads : RTS_SWEEP_THREADS, RTS_SWEEP_THREADS / R);
+        const int thread_cap = std::min(c->user_threads ? c->user_threads : RTS_SWEEP_THREADS, RTS_SWEEP_THREADS / R) / 64 * 64;
         const int smem_cap = std::min(c->max_smem_optin, (228 * 1024) / R - 1024 - (int)fa.sharedSizeBytes);
         const int slots = c->sm_count * R;
         bool ok = true;
@@ -236,36 +236,46 @@ int make_plan(rts_ctx* c)
         TypePlan tp[3] = {c->tp[0], c->tp[1], c->tp[2]};
         for (int a = 0; a < 3 && ok; ++a) {
             TypePlan& t = tp[a];
-            if (!units_of[a]) { t.WU = 4; t.WV = 2; t.ntu = (t.n_u + 3) / 4; t.ntv = (t.n_v + 1) / 2; t.items = 0; continue; }
+            if (!skel_of[a]) { t.WU = 2; t.WV = 2; t.ntu = (t.n_u + 1) / 2; t.ntv = (t.n_v + 1) / 2; t.items = 0; t.ng = 2; t.nstage = 3; continue; }
             double best_cost = 0.0;
-            int bu = 0, bv = 0;
-            const int n_u4 = (t.n_u + 3) & ~3;
-            for (int WU = 4; WU <= std::min(n_u4, 248); WU += 4) {
-                if (t.userWU && WU != std::min(n_u4, (t.userWU + 3) & ~3)) continue;
-                for (int WV = 1; WV <= std::min(t.n_v, 120); ++WV) {
-                    if (t.userWV && WV != std::min(t.n_v, t.userWV)) continue;
-                    if (smem_for(WU, WV) > smem_cap || items_for(WU, WV) > MAXIT * thread_cap) break;
-                    const int ntu = (t.n_u + WU - 1) / WU, ntv = (t.n_v + WV - 1) / WV;
-                    if ((long long)ntu * ntv > slots) continue;          // all tiles of a unit must be resident
-                    // all tiles of a unit are resident together, so slots / ntiles units run at a time
-                    const int uif = std::max(1, slots / (ntu * ntv));
-                    const int rounds = (units_total + uif - 1) / uif;
-                    // ragged last tiles run at the pace of the full ones: charge the covered area
-                    const double cover = ((double)ntu * WU * ntv * WV) / ((double)t.n_u * t.n_v);
-                    // items updated per step, averaged over a block: the u halo is a whole quad column while
-                    // the v halo shrinks from K-1 rows to none (wide tiles along the unit-stride axis win)
-                    const double work = NSLOT * ((WU + HALO) / 4) * (WV + 0.5 * (c->K - 1)) * 0.5;
-                    const double cost = (double)rounds * R * cover * (work + 64.0 + 0.25 * (WU + WV));   // + exchange perimeter
-                    // within the model's accuracy (1.5 %) the tile that is wider along the unit-stride axis is
-                    // taken (measured: 96 x 24 beats 48 x 48 by 2 % at 288^3, 128 x 14 beats 32 x 57 by 3 % at 512^2)
-                    if (!bu || cost < 0.985 * best_cost || (cost < 1.015 * best_cost && WU > bu)) { best_cost = cost; bu = WU; bv = WV; }
+            int bu = 0, bv = 0, bng = 0, bns = 0;
+            const int n_u2 = (t.n_u + 1) & ~1;
+            for (int ng = 2; ng >= 1; --ng) {
+                if (c->user_ng && ng != c->user_ng) continue;
+                for (int nst = 3; nst >= 2; --nst) {
+                    if (c->user_nstage && nst != c->user_nstage) continue;
+                    for (int WU = 2; WU <= std::min(n_u2, 120); WU += 2) {
+                        if (t.userWU && WU != std::min(std::min(n_u2, 120), (t.userWU + 1) & ~1)) continue;
+                        for (int WV = 1; WV <= std::min(t.n_v, 120); ++WV) {
+                            if (t.userWV && WV != std::min(t.n_v, t.userWV)) continue;
+                            if (smem_for(WU, WV, ng, nst) > smem_cap) break;
+                            if (ng * (((items_for(WU, WV, ng, nst) + MAXIT - 1) / MAXIT + 31) / 32 * 32) > thread_cap) break;
+                            const int ntu = (t.n_u + WU - 1) / WU, ntv = (t.n_v + WV - 1) / WV;
+                            if ((long long)ntu * ntv > slots) continue;          // all tiles of a unit must be resident
+                            // all tiles of a unit are resident together, so slots / ntiles units run at a time
+                            const int uif = std::max(1, slots / (ntu * ntv));
+                            const double units = (double)skel_of[a] * (2 / ng);
+                            // ragged last tiles run at the pace of the full ones: charge the covered area
+                            const double cover = ((double)ntu * WU * ntv * WV) / ((double)t.n_u * t.n_v);
+                            // node-rays updated per step, averaged over a block: the u halo is a fixed strip while the
+                            // v halo shrinks from K-1 rows to none; plus the per-step and per-block fixed costs
+                            const double work = 2.0 * ng * (WU + 0.75 * HALO) * (WV + 0.5 * (c->K - 1));
+                            const double fixed = 700.0 + 6.0 * (WU + WV);
+                            double cost = units / uif * R * cover * (work + fixed);
+                            if (nst == 2) cost *= 1.12;                          // the next plane's load is not hidden
+                            // within the model's accuracy the tile that is wider along the unit-stride axis is taken
+                            if (!bu || cost < 0.985 * best_cost || (cost < 1.015 * best_cost && ng == bng && nst == bns && WU > bu)) {
+                                best_cost = cost; bu = WU; bv = WV; bng = ng; bns = nst;
+                            }
+                        }
+                    }
                 }
             }
             if (!bu) { ok = false; break; }
-            t.WU = bu; t.WV = bv;
+            t.WU = bu; t.WV = bv; t.ng = bng; t.nstage = bns;
             t.ntu = (t.n_u + bu - 1) / bu; t.ntv = (t.n_v + bv - 1) / bv;
-            t.items = items_for(bu, bv);
-            costR += best_cost * units_of[a] / units_total;
+            t.items = items_for(bu, bv, bng, bns);
+            costR += best_cost;
         }
         if (ok && (!bestR || costR < bestR_cost)) { bestR = R; bestR_cost = costR; for (int a = 0; a < 3; ++a) best_tp[a] = tp[a]; }
         if (c->user_ctas_per_sm) break;
@@ -273,13 +283,14 @@ int make_plan(rts_ctx* c)
     if (bestR) for (int a = 0; a < 3; ++a) c->tp[a] = best_tp[a];
     if (!bestR) return fail(c, RTS_EINVAL, "planner: no tile shape fits (grid too large for one resident unit, or bad override)");
     c->smem_bytes = 0;
-    int max_items = 1;
+    c->threads = 64;
     for (int a = 0; a < 3; ++a)
-        if (units_of[a]) {
-            c->smem_bytes = std::max(c->smem_bytes, smem_for(c->tp[a].WU, c->tp[a].WV));
-            max_items = std::max(max_items, c->tp[a].items);
+        if (skel_of[a]) {
+            const TypePlan& t = c->tp[a];
+            c->smem_bytes = std::max(c->smem_bytes, smem_for(t.WU, t.WV, t.ng, t.nstage));
+            c->threads = std::max(c->threads, t.ng * (((t.items + MAXIT - 1) / MAXIT + 31) / 32 * 32));
         }
-    c->threads = std::max(64, ((max_items + MAXIT - 1) / MAXIT + 31) / 32 * 32);   // CTA size: MAXIT items per thread
+    c->threads = (c->threads + 63) / 64 * 64;                  // both group counts split the CTA into whole warps
     {
         int occ = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, c->threads, (size_t)c->smem_bytes) != cudaSuccess || occ < 1)
@@ -287,6 +298,9 @@ int make_plan(rts_ctx* c)
         c->ctas_per_sm = std::min(bestR, occ);
     }
     const int slots = c->sm_count * c->ctas_per_sm;
+    for (int a = 0; a < 3; ++a)
+        if (skel_of[a] && c->tp[a].ntu * c->tp[a].ntv > slots)
+            return fail(c, RTS_EINVAL, "planner: a sweep unit has more tiles than resident CTAs at the achieved occupancy");
 
     // --- materialise units in ticket order
     c->units.clear();
@@ -294,48 +308,54 @@ int make_plan(rts_ctx* c)
     const size_t N = (size_t)c->nx * c->ny * c->nz;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
-    const size_t fA = (size_t)c->nz * c->PYR * c->PX;
+    const size_t fA = (size_t)c->nz * c->PYR * c->PX;          // nodes per field of layout A
     const size_t fB = (size_t)c->nz * c->nx * c->PY;
-    c->off_coefA = take(sizeof(float) * fA * 2 * c->nb);
-    c->off_coefB = take(sizeof(float) * fB * 2 * c->nb);
+    c->off_coefA = take(sizeof(float2) * fA * 2 * c->nbp);
+    c->off_coefB = take(sizeof(float2) * fB * 2 * c->nbp);
     c->off_QB = take(sizeof(float) * N);
     c->nblk_a = ((c->nx + 31) / 32) * ((c->ny + 31) / 32);
     c->off_ksum = take(sizeof(double) * (size_t)c->nb * c->nz * c->nblk_a);
     c->off_kmin = take(sizeof(float) * (size_t)c->nb * c->nz * c->nblk_a);
     c->off_lev = take(sizeof(double) * (size_t)c->nb * c->nz * 2);
-    c->off_kstar = take(sizeof(int) * c->nb);
-    c->off_mthick = take(sizeof(int) * c->nb);
+    c->off_kstar = take(sizeof(int) * c->nbp);
+    c->off_mthick = take(sizeof(int) * c->nbp * 3);
+    c->off_mthick_b = take(sizeof(int) * c->nb * 3);
     c->off_abort = take(sizeof(int) * 8);                    // [0] watchdog, [1] ticket counter
     for (auto& g : groups)
         for (auto& sub : g.sub)
-            for (int b = 0; b < c->nb; ++b) {
-                HostUnit hu{};
-                UnitDesc& d = hu.d;
-                std::memset(&d, 0, sizeof d);
+            for (int b = 0; b < c->nbp; ++b) {
                 const TypePlan& t = c->tp[g.march];
-                d.march = g.march; d.dir = g.dir; d.band = b;
-                d.per_v = (g.march == 2) ? 1 : 0;
-                d.n_m = t.n_m; d.n_u = t.n_u; d.n_v = t.n_v; d.n_u4 = (t.n_u + 3) & ~3;
-                d.WU = t.WU; d.WV = t.WV; d.ntu = t.ntu; d.ntv = t.ntv;
-                d.K = c->K; d.npass = c->npass;
-                d.ticket_begin = ticket;
-                d.ntiles = t.ntu * t.ntv;
-                ticket += d.ntiles;
-                d.nz = c->nz;
-                const long long nxy = (long long)c->nx * c->ny;
-                d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
-                const long long PX = c->PX, PY = c->PY, PYR = c->PYR;
-                if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx;
-                                         d.c_field = (long long)fA; d.c_m = PYR * PX; d.c_v = PX; d.c_off = HALO * PX; d.qvec = (c->nx % 4 == 0); }
-                else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx;
-                                         d.c_field = (long long)fA; d.c_m = PX; d.c_v = PYR * PX; d.c_off = HALO * PX; d.qvec = (c->nx % 4 == 0); }
-                else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1;
-                                         d.c_field = (long long)fB; d.c_m = PY; d.c_v = (long long)c->nx * PY; d.c_off = 0; d.qvec = (c->ny % 4 == 0); }
-                for (int q = 0; q < NSLOT; ++q) d.ray[q].itop = -1;
-                for (int ri : sub) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
-                hu.off_xex = take(sizeof(float) * 2 * NSLOT * (size_t)d.n_v * d.n_u4);
-                hu.off_g = take(sizeof(float) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u4));
-                c->units.push_back(hu);
+                for (int gi = 0; gi < (t.ng == 2 ? 1 : 2); ++gi) {     // one unit, or one per su
+                    const int only_su = (t.ng == 2) ? 0 : (gi == 0 ? 1 : -1);
+                    bool any = false;
+                    for (int ri : sub) any |= (only_su == 0 || c->rays[ri].su == only_su);
+                    if (!any) continue;
+                    HostUnit hu{};
+                    UnitDesc& d = hu.d;
+                    std::memset(&d, 0, sizeof d);
+                    d.march = g.march; d.dir = g.dir; d.pair = b;
+                    d.per_v = (g.march == 2) ? 1 : 0;
+                    d.n_m = t.n_m; d.n_u = t.n_u; d.n_v = t.n_v; d.n_u2 = (t.n_u + 1) & ~1;
+                    d.WU = t.WU; d.WV = t.WV; d.ntu = t.ntu; d.ntv = t.ntv;
+                    d.K = c->K; d.npass = c->npass;
+                    d.ticket_begin = ticket;
+                    d.ntiles = t.ntu * t.ntv;
+                    ticket += d.ntiles;
+                    d.nz = c->nz;
+                    d.nstage = t.nstage; d.ng = t.ng; d.gsu0 = only_su ? only_su : 1;
+                    d.nband_ok = (2 * b + 1 < c->nb) ? 2 : 1;
+                    const long long nxy = (long long)c->nx * c->ny;
+                    d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
+                    if (g.march == 2)      { d.q_in_B = 0; d.q_sm = nxy;   d.q_sv = c->nx; d.it_su = 1;     d.it_so = c->nx; d.qvec = (c->nx % 2 == 0); }
+                    else if (g.march == 1) { d.q_in_B = 0; d.q_sm = c->nx; d.q_sv = nxy;   d.it_su = 1;     d.it_so = c->nx; d.qvec = (c->nx % 2 == 0); }
+                    else                   { d.q_in_B = 1; d.q_sm = c->ny; d.q_sv = nxy;   d.it_su = c->nx; d.it_so = 1;     d.qvec = (c->ny % 2 == 0); }
+                    for (int q = 0; q < NSLOT; ++q) d.ray[q].itop = -1;
+                    for (int ri : sub)
+                        if (only_su == 0 || c->rays[ri].su == only_su) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
+                    hu.off_xex = take(sizeof(float2) * 2 * NSLOT * (size_t)d.n_v * d.n_u2);
+                    hu.off_g = take(sizeof(float2) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u2));
+                    c->units.push_back(hu);
+                }
             }
     c->total_tickets = ticket;
     c->grid = std::min(slots, c->total_tickets);
@@ -358,19 +378,18 @@ int bind_workspace(rts_ctx* c)
         d.Xex = (float*)(ws + hu.off_xex);
         d.Gu = (float*)(ws + hu.off_g);
         d.barrier = (int*)(ws + c->off_bar) + i;
-        d.kstar = (const int*)(ws + c->off_kstar) + d.band;
-        d.mthick = (const int*)(ws + c->off_mthick) + d.band;
+        d.kstar = (const int*)(ws + c->off_kstar) + d.pair;
+        d.mthick = (const int*)(ws + c->off_mthick) + 3 * d.pair;
         // carried strips and seam histories must hold finite numbers from the start: planes that are
         // skipped as optically thick leave their entries untouched, and readers multiply them by exactly 0
-        CUDA_TRY(c, cudaMemset(ws + hu.off_xex, 0, sizeof(float) * 2 * NSLOT * (size_t)d.n_v * d.n_u4));
-        CUDA_TRY(c, cudaMemset(ws + hu.off_g, 0, sizeof(float) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u4)));
-        const float* base = (const float*)(ws + (d.march == 0 ? c->off_coefB : c->off_coefA));
-        d.cbase = base + (size_t)(2 * d.band) * d.c_field;
+        CUDA_TRY(c, cudaMemset(ws + hu.off_xex, 0, sizeof(float2) * 2 * NSLOT * (size_t)d.n_v * d.n_u2));
+        CUDA_TRY(c, cudaMemset(ws + hu.off_g, 0, sizeof(float2) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u2)));
         flat.push_back(d);
     }
     CUDA_TRY(c, cudaMemcpy(ws + c->off_units, flat.data(), sizeof(UnitDesc) * flat.size(), cudaMemcpyHostToDevice));
-    // coefficient tensors for the TMA engine: layout A as (x, y rows, z, field) with the box of the
-    // z-march (x, y) or of the y-march (x, z); layout B as (y, x, z, field) with the x-march box (y, z)
+    // coefficient tensors for the TMA engine (fp32 elements, two per node): layout A as (x, y rows, z, field)
+    // with the box of the z-march (x, y) or of the y-march (x, z); layout B as (y, x, z, field) with the
+    // x-march box (y, z)
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -383,13 +402,13 @@ int bind_workspace(rts_ctx* c)
         void* base;
         if (a == 0) {
             base = ws + c->off_coefB;
-            dims[0] = (cuuint64_t)c->PY; dims[1] = (cuuint64_t)c->nx; dims[2] = (cuuint64_t)c->nz; dims[3] = 2ull * c->nb;
-            box[0] = BU; box[1] = 1; box[2] = BV; box[3] = 1;
+            dims[0] = 2ull * c->PY; dims[1] = (cuuint64_t)c->nx; dims[2] = (cuuint64_t)c->nz; dims[3] = 2ull * c->nbp;
+            box[0] = 2 * BU; box[1] = 1; box[2] = BV; box[3] = 1;
         } else {
             base = ws + c->off_coefA;
-            dims[0] = (cuuint64_t)c->PX; dims[1] = (cuuint64_t)c->PYR; dims[2] = (cuuint64_t)c->nz; dims[3] = 2ull * c->nb;
-            if (a == 2) { box[0] = BU; box[1] = BV; box[2] = 1; box[3] = 1; }
-            else        { box[0] = BU; box[1] = 1; box[2] = BV; box[3] = 1; }
+            dims[0] = 2ull * c->PX; dims[1] = (cuuint64_t)c->PYR; dims[2] = (cuuint64_t)c->nz; dims[3] = 2ull * c->nbp;
+            if (a == 2) { box[0] = 2 * BU; box[1] = BV; box[2] = 1; box[3] = 1; }
+            else        { box[0] = 2 * BU; box[1] = 1; box[2] = BV; box[3] = 1; }
         }
         strides[0] = dims[0] * sizeof(float);
         strides[1] = strides[0] * dims[1];
@@ -421,8 +440,8 @@ int launch_stage_a(rts_ctx* c, const float* rho, const float* T, const float* P,
     p.rho = rho; p.T = T; p.P = P;
     p.coefA = (float*)(c->ws + c->off_coefA); p.coefB = (float*)(c->ws + c->off_coefB);
     p.PX = c->PX; p.PY = c->PY; p.PYR = c->PYR;
-    p.strideA_f = (long long)c->nz * c->PYR * c->PX;
-    p.strideB_f = (long long)c->nz * c->nx * c->PY;
+    p.strideA_n = (long long)c->nz * c->PYR * c->PX;
+    p.strideB_n = (long long)c->nz * c->nx * c->PY;
     p.ksum = (double*)(c->ws + c->off_ksum);
     p.kmin = (float*)(c->ws + c->off_kmin);
     p.plain_k = plain_k; p.plain_s = plain_s;
@@ -557,7 +576,7 @@ int rts_num_up_rays(const rts_ctx* c)
 int rts_set_tiling(rts_ctx* c, int march, int tile_u, int tile_v)
 {
     if (!c) return RTS_EINVAL;
-    if (march < 0 || march > 2 || tile_u < 0 || tile_v < 0 || tile_u > 248 || tile_v > 120)
+    if (march < 0 || march > 2 || tile_u < 0 || tile_v < 0 || tile_u > 120 || tile_v > 120)
         return fail(c, RTS_EINVAL, "rts_set_tiling: bad argument");
     c->tp[march].userWU = tile_u;
     c->tp[march].userWV = tile_v;
@@ -634,11 +653,21 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[0], st));
     int rc = launch_stage_a(c, rho, T, P, nullptr, nullptr, st);
     if (rc != RTS_OK) return rc;
-    double kc_z = 0.0;                                      // smallest half path of a z-march ray (0: none)
-    if (c->thick_skip) for (auto& r : c->rays) if (r.march == 2) kc_z = (kc_z == 0.0) ? (double)(float)(0.5 * r.ds) : std::min(kc_z, (double)(float)(0.5 * r.ds));
-    rts_kstar_kernel<<<c->nb, 256, 0, st>>>((const double*)(ws + c->off_ksum), (const float*)(ws + c->off_kmin), c->nz, c->nblk_a,
-                                            1.0 / ((double)c->nx * c->ny), c->h[2], 5.0, kc_z, (int*)(ws + c->off_kstar),
-                                            (int*)(ws + c->off_mthick), (double*)(ws + c->off_lev));
+    {
+        KstarParams kp{};
+        kp.ksum = (const double*)(ws + c->off_ksum); kp.kmin = (const float*)(ws + c->off_kmin);
+        kp.nb = c->nb; kp.nz = c->nz; kp.nblk = c->nblk_a;
+        kp.inv_nxy = 1.0 / ((double)c->nx * c->ny); kp.dz = c->h[2]; kp.tau_switch = 5.0;
+        for (int a = 0; a < 3; ++a) kp.kc[a] = 0.0;             // smallest half path of the rays marching along a (0: none)
+        if (c->thick_skip)
+            for (auto& r : c->rays) {
+                const double k = (double)(float)(0.5 * r.ds);
+                kp.kc[r.march] = (kp.kc[r.march] == 0.0) ? k : std::min(kp.kc[r.march], k);
+            }
+        kp.kstar_pair = (int*)(ws + c->off_kstar); kp.mthick_pair = (int*)(ws + c->off_mthick);
+        kp.mthick_band = (int*)(ws + c->off_mthick_b); kp.lev = (double*)(ws + c->off_lev);
+        rts_kstar_kernel<<<c->nbp, 256, 0, st>>>(kp);
+    }
     CUDA_TRY(c, cudaGetLastError());
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[1], st));
 
@@ -684,7 +713,9 @@ int rts_thick_levels(rts_ctx* c, int* levels_host, void* stream)
     if (!c || !levels_host) return RTS_EINVAL;
     if (!c->ws || !c->planned) return fail(c, RTS_ESTATE, "rts_thick_levels: workspace not set");
     CUDA_TRY(c, cudaStreamSynchronize(as_stream(stream)));
-    CUDA_TRY(c, cudaMemcpy(levels_host, c->ws + c->off_mthick, sizeof(int) * c->nb, cudaMemcpyDeviceToHost));
+    std::vector<int> lv((size_t)c->nb * 3);
+    CUDA_TRY(c, cudaMemcpy(lv.data(), c->ws + c->off_mthick_b, sizeof(int) * lv.size(), cudaMemcpyDeviceToHost));
+    for (int b = 0; b < c->nb; ++b) levels_host[b] = lv[(size_t)b * 3 + 2];
     return RTS_OK;
 }
 
@@ -798,12 +829,6 @@ int rts_solve_cells(rts_ctx* c, const float* rho_c, const float* T_c, const floa
     return launch_n2c(c, qn, Qc, as_stream(stream));
 }
 
-#ifdef RTS_TRACE
-int rts_debug_trace(unsigned long long* out, int n)
-{
-    return cudaMemcpyFromSymbol(out, rts::g_trace, sizeof(unsigned long long) * n) == cudaSuccess ? 0 : -3;
-}
-#endif
 
 const char* rts_last_error(const rts_ctx* c)
 {

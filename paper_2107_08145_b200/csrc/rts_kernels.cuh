@@ -2,12 +2,18 @@
 // stage A and the small helper kernels.  The sweep kernel is in rts_sweep.cuh.
 //
 //   K_a  rts_coef_kernel    stage A  (paper's interpol())
-//   K_k  rts_kstar_kernel   picks, per band, the height below which the sweep carries the
-//                           departure I - S instead of I (precision device)
+//   K_k  rts_kstar_kernel   picks, per band pair, the height below which the sweep carries the
+//                           departure I - S instead of I (precision device) and the
+//                           optically thick levels the non-final passes may skip
 //   K_b  rts_sweep_kernel   stages B-E (paper's integrate() + readbuf/writebuf/exchange with
 //                           the box as its own neighbour + flux())
 //   K_f  rts_finalize_kernel adds the x-march partial heating (stored y-fastest) into Q_rad
 //   K_s  rts_cells_to_nodes_kernel / rts_nodes_to_cells_kernel   grid staggering
+//
+// Bands travel in PAIRS: every coefficient and every carried intensity is a float2 holding
+// bands (2p, 2p+1) of one node, so that the whole update runs on packed fp32 pairs
+// (fma.rn.f32x2: one issue slot for two bands).  An odd band count repeats the last band in
+// the second half of the last pair; its results are never written.
 //
 // Shares nothing with oracle/.
 #pragma once
@@ -20,7 +26,7 @@ namespace rts {
 constexpr int   HALO = 4;           // ghost columns / rows around the periodic axes of the coefficient
                                     // layouts = halo allocation around a sweep tile
 constexpr int   NSLOT = 4;          // rays per sweep unit: one per sign pair (su, sv)
-constexpr int   NSTAGE = 3;         // depth of the coefficient-plane ring in shared memory
+constexpr int   NSTAGE_MAX = 3;     // deepest coefficient-plane ring in shared memory
 constexpr int   KMAX = 4;           // most steps between two halo exchanges (<= HALO)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float FOUR_PI = 12.566370614359172f;
@@ -32,11 +38,10 @@ constexpr double PI_D = 3.14159265358979323846;
 // the ray along them.  Slot s of a unit holds a ray with su = (s & 1 ? -1 : +1),
 // sv = (s & 2 ? -1 : +1).
 struct alignas(16) RayC {
-    float wx[4];      // bilinear weights, sum == 1 exactly, ordered by stencil row: (lower v row, its
+    float w[4];       // bilinear weights, sum == 1 exactly, ordered by stencil row: (lower v row, its
                       // u-side neighbour, higher v row, its u-side neighbour); the node's own row is
                       // the higher one for sv > 0 and the lower one for sv < 0
-    float wk[4];      // 0.5*ds*wx  (opacity -> optical path)
-    float kc;         // 0.5*ds
+    float kc;         // 0.5*ds  (opacity sum -> optical path)
     float wq;         // quadrature weight
     int   active;
     int   up;         // mu_z > 0
@@ -45,27 +50,27 @@ struct alignas(16) RayC {
 };
 
 // One sweep unit: the (at most four) rays that march along `march` in direction `dir`, for one
-// band.  The transverse plane is cut into ntu x ntv tiles of WU x WV nodes; one CTA owns one tile
-// for the whole march (all planes, all passes).  Tiles exchange K-deep halos every K steps
+// band pair.  The transverse plane is cut into ntu x ntv tiles of WU x WV nodes; one CTA owns one
+// tile for the whole march (all planes, all passes).  Tiles exchange K-deep halos every K steps
 // through Xex and meet at `barrier`; the periodic seams read the previous pass from Gu.
 struct UnitDesc {
     int march;        // 0: x, 1: y, 2: z  (axis the sweep marches along)
     int dir;          // +1 / -1 along the march axis
-    int band;
+    int pair;         // band pair: bands 2*pair, 2*pair + 1
     int per_v;        // v periodic (z-march: v = y) or bounded (x/y-march: v = z)
-    int n_m, n_u, n_v, n_u4;
+    int n_m, n_u, n_v, n_u2;               // n_u2 = n_u rounded up to even (row pitch of Xex / Gu, nodes)
     int WU, WV, ntu, ntv;
     int K, npass, ticket_begin, ntiles;
-    int nz, q_in_B, qvec, pad0;           // qvec: heating rows are 16-byte aligned (vector reductions)
+    int nz, q_in_B, qvec, nstage;          // qvec: heating rows are 16-byte aligned (vector reductions)
+    int ng, gsu0, nband_ok, pad0;          // ray groups (same su) of this unit: 2 (su = +1, -1) or 1 (su = gsu0);
+                                           // nband_ok: bands of the pair that exist (1 or 2)
     RayC ray[NSLOT];
-    const float* cbase;                   // coefficient arrays of this band: [2 fields][...]
-    long long c_field, c_m, c_v, c_off;   // strides (floats): fields, march planes, v rows; offset of (m=0, v=0, padded col 0)
-    float* Xex;       // [2][NSLOT][n_v][n_u4]      carried planes at block ends (strips only)
-    float* Gu;        // [2][n_m][NSLOT*n_v + NSLOT*n_u4]  per pass parity and plane: far-u column of
-                      //                            every slot, then (per_v only) far-v row of every slot
+    float* Xex;       // float2 [2][NSLOT][n_v][n_u2]   carried planes at block ends (strips only)
+    float* Gu;        // float2 [2][n_m][NSLOT*n_v + NSLOT*n_u2]  per pass parity and plane: far-u column
+                      //                                of every slot, then (per_v only) far-v row of every slot
     int*   barrier;   // arrivals of this unit's tiles (monotonic)
-    const int* kstar; // device: switch height of this band
-    const int* mthick;// device: thick level pairs from the bottom of this band (z-march plane skipping)
+    const int* kstar; // device: switch height of this band pair
+    const int* mthick;// device: thick level pairs from the bottom of this band pair (z-march plane skipping)
     long long q_sm, q_sv;                 // heating strides along (march, v); u stride 1
     long long it_su, it_so, it_sr, it_sb; // I_top strides along u, march-or-v axis, ray, band
 };
@@ -118,11 +123,11 @@ __device__ __forceinline__ float rcp_approx(float x) {
 // =========================================================================== K_a
 // Stage A.  One thread block = a 32x32 (x,y) patch of one z level; 32x8 threads, 4 nodes each.
 // Evaluates the table coordinates, 10^x and T^4 in fp64 and rounds once to fp32 (DESIGN.md,
-// "precision").  Writes kaprho_b, S_b in two layouts, both with HALO periodic images on each
-// side of every periodic axis that a sweep tile can reach across:
-//   layout A  [b][f][nz][ny+2H][PX]   x fastest (offset H), rows y (offset H)   z- and y-march
-//   layout B  [b][f][nz][nx][PY]      y fastest (offset H)                       x-march
-// plus per-block partial sums of kaprho for K_k.
+// "precision").  Writes (kaprho, S) of every band pair as float2 per node in two layouts, both
+// with HALO periodic images on each side of every periodic axis that a sweep tile can reach across:
+//   layout A  [pair][f][nz][ny+2H][PX] float2   x fastest (offset H), rows y (offset H)   z- and y-march
+//   layout B  [pair][f][nz][nx][PY]    float2   y fastest (offset H)                       x-march
+// plus per-block partial sums / minima of kaprho per band for K_k.
 struct CoefParams {
     int nx, ny, nz, nb, nT, nP;
     double logT_min, inv_dT, logP_min, inv_dP;   // inv_d = (n-1)/(max-min)
@@ -130,8 +135,8 @@ struct CoefParams {
     const float* bandfrac;   // device [nb][nT]
     const float *rho, *T, *P;
     float* coefA; float* coefB;
-    int PX, PY, PYR;
-    long long strideA_f, strideB_f;              // field strides
+    int PX, PY, PYR;                             // padded row lengths / row count (nodes)
+    long long strideA_n, strideB_n;              // field strides (nodes)
     double* ksum;            // [nb][nz][nblk] partial sums (nblk = gridDim.x*gridDim.y), or null
     float* kmin;             // [nb][nz][nblk] partial minima of kaprho (with ksum)
     float* plain_k; float* plain_s;              // optional [nb][N] outputs (rts_coefficients)
@@ -139,9 +144,9 @@ struct CoefParams {
 
 __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
 {
-    __shared__ float tile[2][32][33];
-    __shared__ double red[8];
-    __shared__ float redm[8];
+    __shared__ float2 tile[2][32][33];
+    __shared__ double red[2][8];
+    __shared__ float redm[2][8];
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32, k = blockIdx.z;
     const int i = i0 + tx;
@@ -173,67 +178,83 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
         }
     }
     const int cA0 = (i + HALO) % p.nx;            // first padded column of layout A congruent to i
+    const int npair = (p.nb + 1) >> 1;
 
-    for (int b = 0; b < p.nb; ++b) {
-        const float* L = p.logkappa + (size_t)b * p.nT * p.nP;
-        const float* F = p.bandfrac + (size_t)b * p.nT;
-        float* A0 = p.coefA + (size_t)(2 * b) * p.strideA_f;  float* A1 = A0 + p.strideA_f;
-        double part = 0.0;
-        float pmin = 3.0e38f;
+    for (int pr = 0; pr < npair; ++pr) {
+        float2* A0 = reinterpret_cast<float2*>(p.coefA) + (size_t)(2 * pr) * p.strideA_n;
+        float2* A1 = A0 + p.strideA_n;
+        double part[2] = {0.0, 0.0};
+        float pmin[2] = {3.0e38f, 3.0e38f};
+        const int nbe = (2 * pr + 1 < p.nb) ? 2 : 1;
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
-            float kr = 0.f, sr = 0.f;
+            float kr[2] = {0.f, 0.f}, sr[2] = {0.f, 0.f};
             if (ok[r]) {
                 const int a = it_[r], c = ip_[r];
                 const double t = t_[r], u = u_[r];
-                const double l00 = (double)L[(size_t)a * p.nP + c], l10 = (double)L[(size_t)(a + 1) * p.nP + c];
-                const double l01 = (double)L[(size_t)a * p.nP + c + 1], l11 = (double)L[(size_t)(a + 1) * p.nP + c + 1];
-                const double lk = (1.0 - t) * (1.0 - u) * l00 + t * (1.0 - u) * l10 + (1.0 - t) * u * l01 + t * u * l11;
-                const double fb = (1.0 - t) * (double)F[a] + t * (double)F[a + 1];
-                const double kd = exp10(lk) * rho_[r];
-                kr = (float)kd;
-                sr = (float)(fb * planck[r]);
-                part += kd;
-                pmin = fminf(pmin, kr);
                 const int j = j0 + ty + 8 * r;
+                for (int e = 0; e < nbe; ++e) {
+                    const int b = 2 * pr + e;
+                    const float* L = p.logkappa + (size_t)b * p.nT * p.nP;
+                    const float* F = p.bandfrac + (size_t)b * p.nT;
+                    const double l00 = (double)L[(size_t)a * p.nP + c], l10 = (double)L[(size_t)(a + 1) * p.nP + c];
+                    const double l01 = (double)L[(size_t)a * p.nP + c + 1], l11 = (double)L[(size_t)(a + 1) * p.nP + c + 1];
+                    const double lk = (1.0 - t) * (1.0 - u) * l00 + t * (1.0 - u) * l10 + (1.0 - t) * u * l01 + t * u * l11;
+                    const double fb = (1.0 - t) * (double)F[a] + t * (double)F[a + 1];
+                    const double kd = exp10(lk) * rho_[r];
+                    kr[e] = (float)kd;
+                    sr[e] = (float)(fb * planck[r]);
+                    part[e] += kd;
+                    pmin[e] = fminf(pmin[e], kr[e]);
+                    if (p.plain_k) {
+                        const long long n = ((long long)k * p.ny + j) * p.nx + i;
+                        p.plain_k[(size_t)b * N + n] = kr[e];
+                        p.plain_s[(size_t)b * N + n] = sr[e];
+                    }
+                }
+                if (nbe == 1) { kr[1] = kr[0]; sr[1] = sr[0]; }     // odd band count: the last band twice
                 // layout A: every periodic image of (i, j) inside the padded plane
+                const float2 kv = make_float2(kr[0], kr[1]), sv = make_float2(sr[0], sr[1]);
                 for (int row = (j + HALO) % p.ny; row < p.PYR; row += p.ny) {
                     const size_t ro = ((size_t)k * p.PYR + row) * p.PX;
-                    for (int col = cA0; col < p.PX; col += p.nx) { A0[ro + col] = kr; A1[ro + col] = sr; }
-                }
-                if (p.plain_k) {
-                    const long long n = ((long long)k * p.ny + j) * p.nx + i;
-                    p.plain_k[(size_t)b * N + n] = kr;
-                    p.plain_s[(size_t)b * N + n] = sr;
+                    for (int col = cA0; col < p.PX; col += p.nx) { A0[ro + col] = kv; A1[ro + col] = sv; }
                 }
             }
-            tile[0][ty + 8 * r][tx] = kr;
-            tile[1][ty + 8 * r][tx] = sr;
+            tile[0][ty + 8 * r][tx] = make_float2(kr[0], kr[1]);
+            tile[1][ty + 8 * r][tx] = make_float2(sr[0], sr[1]);
         }
-        // block sum of kaprho (deterministic order)
+        // block sums / minima of kaprho per band (deterministic order)
         if (p.ksum) {
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) { part += __shfl_xor_sync(0xffffffffu, part, o); pmin = fminf(pmin, __shfl_xor_sync(0xffffffffu, pmin, o)); }
-            if (tx == 0) { red[ty] = part; redm[ty] = pmin; }
+            for (int e = 0; e < 2; ++e) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    part[e] += __shfl_xor_sync(0xffffffffu, part[e], o);
+                    pmin[e] = fminf(pmin[e], __shfl_xor_sync(0xffffffffu, pmin[e], o));
+                }
+                if (tx == 0) { red[e][ty] = part[e]; redm[e][ty] = pmin[e]; }
+            }
         }
         __syncthreads();
-        if (p.ksum && tx == 0 && ty == 0) {
+        if (p.ksum && tx == 0 && ty < nbe) {
             double s = 0.0;
             float mn = 3.0e38f;
-            for (int w = 0; w < 8; ++w) { s += red[w]; mn = fminf(mn, redm[w]); }
+            for (int w = 0; w < 8; ++w) { s += red[ty][w]; mn = fminf(mn, redm[ty][w]); }
             const int nblk = gridDim.x * gridDim.y;
-            p.ksum[((size_t)b * p.nz + k) * nblk + blockIdx.y * gridDim.x + blockIdx.x] = s;
-            p.kmin[((size_t)b * p.nz + k) * nblk + blockIdx.y * gridDim.x + blockIdx.x] = mn;
+            const size_t o = ((size_t)(2 * pr + ty) * p.nz + k) * nblk + blockIdx.y * gridDim.x + blockIdx.x;
+            p.ksum[o] = s;
+            p.kmin[o] = mn;
         }
         // layout B: transposed write, coalesced along y
-        float* B0 = p.coefB + (size_t)(2 * b) * p.strideB_f;  float* B1 = B0 + p.strideB_f;
+        float2* B0 = reinterpret_cast<float2*>(p.coefB) + (size_t)(2 * pr) * p.strideB_n;
+        float2* B1 = B0 + p.strideB_n;
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int ii = i0 + ty + 8 * r, jj = j0 + tx;
             if (ii < p.nx && jj < p.ny) {
-                const float kr = tile[0][tx][ty + 8 * r], sr = tile[1][tx][ty + 8 * r];
+                const float2 kv = tile[0][tx][ty + 8 * r], sv = tile[1][tx][ty + 8 * r];
                 const size_t ro = ((size_t)k * p.nx + ii) * p.PY;
-                for (int col = (jj + HALO) % p.ny; col < p.PY; col += p.ny) { B0[ro + col] = kr; B1[ro + col] = sr; }
+                for (int col = (jj + HALO) % p.ny; col < p.PY; col += p.ny) { B0[ro + col] = kv; B1[ro + col] = sv; }
             }
         }
         __syncthreads();
@@ -241,45 +262,82 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
 }
 
 // =========================================================================== K_k
-// kstar[b] = highest level k whose horizontally averaged optical depth from the top,
-// tau(k) = sum_{k' >= k} <kaprho_b>(k') dz, is >= tau_switch; -1 if none.  One block per band.
-// mthick[b] = number of consecutive level pairs (k-1, k), k = 1, 2, ..., from the bottom on which every
-// optical path of a z-march ray exceeds DTAU_SKIP: kc_z * (min kaprho(k-1) + min kaprho(k)) > DTAU_SKIP
-// bounds dtau = kc*kaprho_p + sum_n wk_n*kaprho_n from below (sum_n wk_n = kc).  There the approximate
-// exp underflows to exactly 0 and the update does not depend on the carried plane (rts_sweep.cuh).
+// Per band: kstar_b = highest level k whose horizontally averaged optical depth from the top,
+// tau(k) = sum_{k' >= k} <kaprho_b>(k') dz, is >= tau_switch (-1 if none).
+// mthick_b[2] = number of consecutive level pairs (k-1, k), k = 1, 2, ..., from the bottom on which every
+// optical path of a z-march ray exceeds DTAU_SKIP: kc * (min kaprho(k-1) + min kaprho(k)) > DTAU_SKIP bounds
+// dtau = kc*(kaprho_p + sum_n w_n*kaprho_n) from below (kc = smallest half path of the z-march rays).
+// mthick_b[0], [1] = number of consecutive levels from the bottom on which every optical path of an x- / y-march
+// ray exceeds DTAU_SKIP (the stencil of such a node lies on its own level and the one below or above:
+// 2*kc*min over the three levels bounds dtau).  There the approximate exp underflows to exactly 0 and the
+// update does not depend on the carried intensity (rts_sweep.cuh).  One block per band pair; the pair takes the higher switch height and the
+// smaller thick counts of its two bands (both bands ride in one float2).
 constexpr float DTAU_SKIP = 88.5f;
-__global__ void __launch_bounds__(256) rts_kstar_kernel(const double* ksum, const float* kmin, int nz, int nblk, double inv_nxy,
-                                                        double dz, double tau_switch, double kc_z, int* kstar, int* mthick,
-                                                        double* lev)
+struct KstarParams {
+    const double* ksum; const float* kmin;
+    int nb, nz, nblk;
+    double inv_nxy, dz, tau_switch;
+    double kc[3];            // per march axis (0: no such ray / shortcut off)
+    int* kstar_pair;         // [npair]
+    int* mthick_pair;        // [npair][3]
+    int* mthick_band;        // [nb][3]    (reporting)
+    double* lev;             // scratch [nb][2][nz]
+};
+__global__ void __launch_bounds__(256) rts_kstar_kernel(const KstarParams p)
 {
-    const int b = blockIdx.x;
-    double* L = lev + (size_t)b * 2 * nz;
-    double* M = L + nz;
+    __shared__ int sh_ks[2], sh_mt[2][3];
+    const int pr = blockIdx.x;
+    const int nz = p.nz, nblk = p.nblk;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (int k = warp; k < nz; k += nw) {             // level sums (fixed order) and level minima
-        const double* q = ksum + ((size_t)b * nz + k) * nblk;
-        const float* qm = kmin + ((size_t)b * nz + k) * nblk;
-        double s = 0.0;
-        float mn = 3.0e38f;
-        for (int w = lane; w < nblk; w += 32) { s += q[w]; mn = fminf(mn, qm[w]); }
+    const int nbe = (2 * pr + 1 < p.nb) ? 2 : 1;
+    for (int e = 0; e < nbe; ++e) {
+        const int b = 2 * pr + e;
+        double* L = p.lev + (size_t)b * 2 * nz;
+        double* M = L + nz;
+        for (int k = warp; k < nz; k += nw) {             // level sums (fixed order) and level minima
+            const double* q = p.ksum + ((size_t)b * nz + k) * nblk;
+            const float* qm = p.kmin + ((size_t)b * nz + k) * nblk;
+            double s = 0.0;
+            float mn = 3.0e38f;
+            for (int w = lane; w < nblk; w += 32) { s += q[w]; mn = fminf(mn, qm[w]); }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o)); }
-        if (lane == 0) { L[k] = s; M[k] = (double)mn; }
+            for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o)); }
+            if (lane == 0) { L[k] = s; M[k] = (double)mn; }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double tau = 0.0;
+            int ks = -1;
+            for (int k = nz - 1; k >= 0; --k) {
+                tau += L[k] * p.inv_nxy * p.dz;
+                if (tau >= p.tau_switch) { ks = k; break; }
+            }
+            sh_ks[e] = ks;
+            for (int a = 0; a < 3; ++a) {
+                int m = 0;
+                if (p.kc[a] > 0.0) {
+                    if (a == 2) {
+                        for (int k = 1; k < nz; ++k) {
+                            if (p.kc[a] * (M[k - 1] + M[k]) > (double)DTAU_SKIP) m = k; else break;
+                        }
+                    } else {
+                        // x- / y-march: levels 0 .. m-1 are thick for upward and downward rays alike
+                        for (int k = 0; k < nz; ++k) {
+                            const double mn = fmin(M[k], fmin(M[max(k - 1, 0)], M[min(k + 1, nz - 1)]));
+                            if (2.0 * p.kc[a] * mn > (double)DTAU_SKIP) m = k + 1; else break;
+                        }
+                    }
+                }
+                sh_mt[e][a] = m;
+                p.mthick_band[b * 3 + a] = m;
+            }
+        }
+        __syncthreads();
     }
-    __syncthreads();
     if (threadIdx.x == 0) {
-        double tau = 0.0;
-        int ks = -1;
-        for (int k = nz - 1; k >= 0; --k) {
-            tau += L[k] * inv_nxy * dz;
-            if (tau >= tau_switch) { ks = k; break; }
-        }
-        kstar[b] = ks;
-        int m = 0;
-        for (int k = 1; k < nz; ++k) {
-            if (kc_z * (M[k - 1] + M[k]) > (double)DTAU_SKIP) m = k; else break;
-        }
-        mthick[b] = m;
+        p.kstar_pair[pr] = (nbe == 2) ? max(sh_ks[0], sh_ks[1]) : sh_ks[0];
+        for (int a = 0; a < 3; ++a)
+            p.mthick_pair[pr * 3 + a] = (nbe == 2) ? min(sh_mt[0][a], sh_mt[1][a]) : sh_mt[0][a];
     }
 }
 
