@@ -92,6 +92,9 @@ int rts_num_up_rays(const rts_ctx* ctx);
 int rts_set_tiling(rts_ctx* ctx, int march, int tile_u, int tile_v);
 int rts_set_exchange_interval(rts_ctx* ctx, int steps);
 int rts_set_ctas_per_sm(rts_ctx* ctx, int ctas_per_sm);
+/* Depth of the shared-memory ring the coefficient planes stream through: 3 (the load of the next plane
+ * overlaps the current step), 2 (smaller footprint: larger tiles or two CTAs per SM), 0 = planner's choice. */
+int rts_set_ring_depth(rts_ctx* ctx, int stages);
 
 /* Bytes of device workspace the current configuration needs (0 on error). */
 size_t rts_workspace_bytes(rts_ctx* ctx);

@@ -30,7 +30,8 @@ struct TypePlan {        // per march axis
     int userWU = 0, userWV = 0;
     int ng = 2;          // ray groups (same su) per unit: 2, or 1 where a plane with all four rays does not fit
     int nstage = 3;      // depth of the coefficient ring
-    int items = 0;       // 2 x 2 node blocks of one group of a full tile (halo included)
+    int rc = 4;          // rows per strip
+    int items = 0;       // strips of one ray of a full tile (halo included)
 };
 
 struct HostUnit {
@@ -55,14 +56,14 @@ struct rts_ctx {
     float* d_bandfrac = nullptr;
     // device facts
     int sm_count = 0, max_smem_optin = 0;
-    int user_ctas_per_sm = 0, user_K = 0, user_threads = 0, user_nstage = 0, user_ng = 0;
+    int user_ctas_per_sm = 0, user_K = 0, user_threads = 0, user_nstage = 0, user_ng = 0, user_rc = 0;
     SweepMaps maps;
     void* encode_fn = nullptr;    // cuTensorMapEncodeTiled
     // plan
     bool planned = false;
     TypePlan tp[3];
     std::vector<HostUnit> units;
-    int total_tickets = 0, grid = 0, K = KMAX;
+    int total_tickets = 0, grid = 0, K = KMAX, pitch = 56;
     int ctas_per_sm = 0, threads = 256, smem_bytes = 0;
     int PX = 0, PY = 0, PYR = 0;
     size_t ws_bytes = 0;
@@ -136,12 +137,9 @@ void make_ray_consts(const HostRay& r, RayC& rc)
     for (int q = 0; q < 4; ++q)
         if (q != big) { w[q] = std::nearbyint(w[q] * 16777216.0) / 16777216.0; sum += w[q]; }
     w[big] = 1.0 - sum;
-    // device order: (lower v row, its side neighbour, higher v row, its side neighbour)
-    const int ord_p[4] = {2, 3, 0, 1}, ord_m[4] = {0, 1, 2, 3};
-    for (int q = 0; q < 4; ++q) {
-        const int src = (r.sv > 0) ? ord_p[q] : ord_m[q];
-        rc.w[q] = (float)w[src];
-    }
+    // device order: (upwind v row, its side neighbour, own v row, its side neighbour)
+    const int ord[4] = {2, 3, 0, 1};
+    for (int q = 0; q < 4; ++q) rc.w[q] = (float)w[ord[q]];
     rc.kc = (float)(0.5 * r.ds);
     rc.wq = (float)r.w;
     rc.active = 1;
@@ -165,12 +163,24 @@ void default_rays(rts_ctx* c)
         }
 }
 
+// The sweep kernel is compiled for a few shared-memory row pitches (nodes per box row); a plan uses one.
+constexpr int NPITCH = 4;
+const int kPitch[NPITCH] = {24, 56, 72, 128};
+const void* sweep_fn(int pitch)
+{
+    switch (pitch) {
+        case 24: return (const void*)rts_sweep_kernel<24>;
+        case 56: return (const void*)rts_sweep_kernel<56>;
+        case 72: return (const void*)rts_sweep_kernel<72>;
+        default: return (const void*)rts_sweep_kernel<128>;
+    }
+}
 // dynamic shared memory of a CTA whose tiles are WU x WV (SmemPlan: coefficient ring, carried
 // planes, ghost list, halo list)
-int smem_for(int WU, int WV, int ng, int nstage) { return (int)SmemPlan(WU, WV, ng, nstage).bytes(); }
-// items (2 x 2 node blocks, halo included, padded to whole warps) of ONE ray group of a CTA whose
-// tiles are WU x WV; a thread owns MAXIT of them
-int items_for(int WU, int WV, int ng, int nstage) { return SmemPlan(WU, WV, ng, nstage).nitems; }
+int smem_for(int pitch, int WU, int WV, int ng, int nstage) { return (int)SmemPlan(pitch, WU, WV, ng, nstage).bytes(); }
+// strips (node pair x rc rows, halo included, padded to whole warps) of ONE ray of a CTA whose tiles are
+// WU x WV; a thread owns one
+int items_for(int WU, int WV, int rc) { return SmemPlan::strips_for(WU, WV, rc); }
 
 // --------------------------------------------------------------------------- planner
 // Groups the rays into sweep units (march axis, direction, one ray per sign pair, band pair), chooses the
@@ -223,12 +233,14 @@ int make_plan(rts_ctx* c)
     //     su = +1 and su = -1 rays as separate units, for planes too large to be resident otherwise) and ring
     //     depth, by least modelled time among the shapes whose CTA fits R times on an SM
     cudaFuncAttributes fa;
-    CUDA_TRY(c, cudaFuncGetAttributes(&fa, rts_sweep_kernel));
-    int bestR = 0;
+    CUDA_TRY(c, cudaFuncGetAttributes(&fa, sweep_fn(56)));
+    int bestR = 0, bestP = 0;
     double bestR_cost = 0.0;
     TypePlan best_tp[3];
     for (int R = (c->user_ctas_per_sm ? c->user_ctas_per_sm : 2); R >= 1; --R) {
-        const int thread_cap = std::min(c->user_threads ? c->user_threads : RTS_SWEEP_THREADS, RTS_SWEEP_THREADS / R) / 64 * 64;
+      for (int pi = 0; pi < NPITCH; ++pi) {
+        const int P = kPitch[pi];
+        const int thread_cap = std::min(c->user_threads ? c->user_threads : RTS_SWEEP_THREADS, RTS_SWEEP_THREADS / R) / 128 * 128;
         const int smem_cap = std::min(c->max_smem_optin, (228 * 1024) / R - 1024 - (int)fa.sharedSizeBytes);
         const int slots = c->sm_count * R;
         bool ok = true;
@@ -239,17 +251,31 @@ int make_plan(rts_ctx* c)
             if (!skel_of[a]) { t.WU = 2; t.WV = 2; t.ntu = (t.n_u + 1) / 2; t.ntv = (t.n_v + 1) / 2; t.items = 0; t.ng = 2; t.nstage = 3; continue; }
             double best_cost = 0.0;
             int bu = 0, bv = 0, bng = 0, bns = 0;
+            // rows per strip: as few row chunks as fit the thread budget (more rows per thread amortise the
+            // per-step overhead), chunks of equal length
+            auto rc_of = [&](int WU, int WV, int ng) {
+                if (c->user_rc) return c->user_rc;
+                const int nrows = WV + c->K - 1, npair = (WU + HALO) / 2;
+                for (int nch = 1; nch <= nrows; ++nch) {
+                    const int rc = (nrows + nch - 1) / nch;
+                    if (rc <= 8 && 2 * ng * items_for(WU, WV, rc) <= thread_cap) return rc;
+                }
+                (void)npair;
+                return 1;
+            };
             const int n_u2 = (t.n_u + 1) & ~1;
+            const int wu_max = std::min(n_u2, P - 2 * HALO);
             for (int ng = 2; ng >= 1; --ng) {
                 if (c->user_ng && ng != c->user_ng) continue;
                 for (int nst = 3; nst >= 2; --nst) {
                     if (c->user_nstage && nst != c->user_nstage) continue;
-                    for (int WU = 2; WU <= std::min(n_u2, 120); WU += 2) {
-                        if (t.userWU && WU != std::min(std::min(n_u2, 120), (t.userWU + 1) & ~1)) continue;
+                    for (int WU = 2; WU <= wu_max; WU += 2) {
+                        if (t.userWU && WU != std::min(wu_max, (t.userWU + 1) & ~1)) continue;
                         for (int WV = 1; WV <= std::min(t.n_v, 120); ++WV) {
                             if (t.userWV && WV != std::min(t.n_v, t.userWV)) continue;
-                            if (smem_for(WU, WV, ng, nst) > smem_cap) break;
-                            if (ng * (((items_for(WU, WV, ng, nst) + MAXIT - 1) / MAXIT + 31) / 32 * 32) > thread_cap) break;
+                            if (smem_for(P, WU, WV, ng, nst) > smem_cap) break;
+                            const int rc_try = rc_of(WU, WV, ng);
+                            if (2 * ng * items_for(WU, WV, rc_try) > thread_cap) break;
                             const int ntu = (t.n_u + WU - 1) / WU, ntv = (t.n_v + WV - 1) / WV;
                             if ((long long)ntu * ntv > slots) continue;          // all tiles of a unit must be resident
                             // all tiles of a unit are resident together, so slots / ntiles units run at a time
@@ -258,9 +284,10 @@ int make_plan(rts_ctx* c)
                             // ragged last tiles run at the pace of the full ones: charge the covered area
                             const double cover = ((double)ntu * WU * ntv * WV) / ((double)t.n_u * t.n_v);
                             // node-rays updated per step, averaged over a block: the u halo is a fixed strip while the
-                            // v halo shrinks from K-1 rows to none; plus the per-step and per-block fixed costs
+                            // v halo shrinks from K-1 rows to none; plus the per-step and per-block fixed costs and the
+                            // box the TMA engine moves per step (the whole pitch, used or not)
                             const double work = 2.0 * ng * (WU + 0.75 * HALO) * (WV + 0.5 * (c->K - 1));
-                            const double fixed = 700.0 + 6.0 * (WU + WV);
+                            const double fixed = 700.0 + 6.0 * (WU + WV) + 0.25 * P * (WV + 2 * HALO);
                             double cost = units / uif * R * cover * (work + fixed);
                             if (nst == 2) cost *= 1.12;                          // the next plane's load is not hidden
                             // within the model's accuracy the tile that is wider along the unit-stride axis is taken
@@ -274,26 +301,28 @@ int make_plan(rts_ctx* c)
             if (!bu) { ok = false; break; }
             t.WU = bu; t.WV = bv; t.ng = bng; t.nstage = bns;
             t.ntu = (t.n_u + bu - 1) / bu; t.ntv = (t.n_v + bv - 1) / bv;
-            t.items = items_for(bu, bv, bng, bns);
+            t.rc = rc_of(bu, bv, bng); t.items = items_for(bu, bv, t.rc);
             costR += best_cost;
         }
-        if (ok && (!bestR || costR < bestR_cost)) { bestR = R; bestR_cost = costR; for (int a = 0; a < 3; ++a) best_tp[a] = tp[a]; }
-        if (c->user_ctas_per_sm) break;
+        if (ok && (!bestR || costR < 0.999 * bestR_cost)) { bestR = R; bestP = P; bestR_cost = costR; for (int a = 0; a < 3; ++a) best_tp[a] = tp[a]; }
+      }
+      if (c->user_ctas_per_sm) break;
     }
     if (bestR) for (int a = 0; a < 3; ++a) c->tp[a] = best_tp[a];
     if (!bestR) return fail(c, RTS_EINVAL, "planner: no tile shape fits (grid too large for one resident unit, or bad override)");
+    c->pitch = bestP;
     c->smem_bytes = 0;
     c->threads = 64;
     for (int a = 0; a < 3; ++a)
         if (skel_of[a]) {
             const TypePlan& t = c->tp[a];
-            c->smem_bytes = std::max(c->smem_bytes, smem_for(t.WU, t.WV, t.ng, t.nstage));
-            c->threads = std::max(c->threads, t.ng * (((t.items + MAXIT - 1) / MAXIT + 31) / 32 * 32));
+            c->smem_bytes = std::max(c->smem_bytes, smem_for(c->pitch, t.WU, t.WV, t.ng, t.nstage));
+            c->threads = std::max(c->threads, 2 * t.ng * t.items);
         }
-    c->threads = (c->threads + 63) / 64 * 64;                  // both group counts split the CTA into whole warps
+    c->threads = (c->threads + 127) / 128 * 128;               // two or four rays split the CTA into whole warps
     {
         int occ = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_sweep_kernel, c->threads, (size_t)c->smem_bytes) != cudaSuccess || occ < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_fn(c->pitch), c->threads, (size_t)c->smem_bytes) != cudaSuccess || occ < 1)
             return fail(c, RTS_ECUDA, "planner: sweep kernel does not fit on an SM");
         c->ctas_per_sm = std::min(bestR, occ);
     }
@@ -342,7 +371,7 @@ int make_plan(rts_ctx* c)
                     d.ntiles = t.ntu * t.ntv;
                     ticket += d.ntiles;
                     d.nz = c->nz;
-                    d.nstage = t.nstage; d.ng = t.ng; d.gsu0 = only_su ? only_su : 1;
+                    d.nstage = t.nstage; d.ng = t.ng; d.gsu0 = only_su ? only_su : 1; d.RC = t.rc;
                     d.nband_ok = (2 * b + 1 < c->nb) ? 2 : 1;
                     const long long nxy = (long long)c->nx * c->ny;
                     d.it_sr = nxy; d.it_sb = (long long)c->n_up * nxy;
@@ -396,24 +425,31 @@ int bind_workspace(rts_ctx* c)
     EncodeFn enc = (EncodeFn)c->encode_fn;
     for (int a = 0; a < 3; ++a) {
         const TypePlan& t = c->tp[a];
-        const cuuint32_t BU = (cuuint32_t)(t.WU + 2 * HALO), BV = (cuuint32_t)(t.WV + 2 * HALO);
-        cuuint64_t dims[4], strides[3];
-        cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
+        const cuuint32_t BW = (cuuint32_t)(2 * c->pitch), BV = (cuuint32_t)(t.WV + 2 * HALO);
+        // dimensions: (unit-stride axis, field, rows, planes, band pair); the box takes both fields of BV rows,
+        // so a stage in shared memory is [BV][kaprho row | S row][pitch]
+        cuuint64_t dims[5], strides[4];
+        cuuint32_t box[5], estr[5] = {1, 1, 1, 1, 1};
         void* base;
+        size_t fieldn;
         if (a == 0) {
             base = ws + c->off_coefB;
-            dims[0] = 2ull * c->PY; dims[1] = (cuuint64_t)c->nx; dims[2] = (cuuint64_t)c->nz; dims[3] = 2ull * c->nbp;
-            box[0] = 2 * BU; box[1] = 1; box[2] = BV; box[3] = 1;
+            fieldn = (size_t)c->nz * c->nx * c->PY;
+            dims[0] = 2ull * c->PY; dims[2] = (cuuint64_t)c->nx; dims[3] = (cuuint64_t)c->nz;
+            box[0] = BW; box[1] = 2; box[2] = 1; box[3] = BV; box[4] = 1;
         } else {
             base = ws + c->off_coefA;
-            dims[0] = 2ull * c->PX; dims[1] = (cuuint64_t)c->PYR; dims[2] = (cuuint64_t)c->nz; dims[3] = 2ull * c->nbp;
-            if (a == 2) { box[0] = 2 * BU; box[1] = BV; box[2] = 1; box[3] = 1; }
-            else        { box[0] = 2 * BU; box[1] = 1; box[2] = BV; box[3] = 1; }
+            fieldn = (size_t)c->nz * c->PYR * c->PX;
+            dims[0] = 2ull * c->PX; dims[2] = (cuuint64_t)c->PYR; dims[3] = (cuuint64_t)c->nz;
+            if (a == 2) { box[0] = BW; box[1] = 2; box[2] = BV; box[3] = 1; box[4] = 1; }
+            else        { box[0] = BW; box[1] = 2; box[2] = 1; box[3] = BV; box[4] = 1; }
         }
-        strides[0] = dims[0] * sizeof(float);
-        strides[1] = strides[0] * dims[1];
-        strides[2] = strides[1] * dims[2];
-        CUresult r = enc(&c->maps.m[a], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
+        dims[1] = 2; dims[4] = (cuuint64_t)c->nbp;
+        strides[0] = fieldn * sizeof(float2);                   // field
+        strides[1] = dims[0] * sizeof(float);                   // rows
+        strides[2] = strides[1] * dims[2];                      // planes
+        strides[3] = 2 * strides[0];                            // band pair
+        CUresult r = enc(&c->maps.m[a], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, base, dims, strides, box, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) {
@@ -481,10 +517,11 @@ int rts_create(rts_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     c->h[0] = dx; c->h[1] = dy; c->h[2] = dz;
     default_rays(c);
     cudaFuncAttributes fa;
-    if ((e = cudaFuncGetAttributes(&fa, rts_sweep_kernel)) != cudaSuccess) return bail(std::string("sweep kernel not loadable: ") + cudaGetErrorString(e));
+    if ((e = cudaFuncGetAttributes(&fa, sweep_fn(56))) != cudaSuccess) return bail(std::string("sweep kernel not loadable: ") + cudaGetErrorString(e));
     c->max_smem_optin = (int)prop.sharedMemPerBlockOptin - (int)fa.sharedSizeBytes;
-    if ((e = cudaFuncSetAttribute(rts_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem_optin)) != cudaSuccess)
-        return bail(std::string("cudaFuncSetAttribute(max dynamic smem): ") + cudaGetErrorString(e));
+    for (int pi = 0; pi < NPITCH; ++pi)
+        if ((e = cudaFuncSetAttribute(sweep_fn(kPitch[pi]), cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem_optin)) != cudaSuccess)
+            return bail(std::string("cudaFuncSetAttribute(max dynamic smem): ") + cudaGetErrorString(e));
     if ((e = cudaEventCreateWithFlags(&c->ev, cudaEventDisableTiming)) != cudaSuccess) return bail(cudaGetErrorString(e));
     {
         cudaDriverEntryPointQueryResult qres;
@@ -593,6 +630,15 @@ int rts_set_exchange_interval(rts_ctx* c, int k)
     return RTS_OK;
 }
 
+int rts_set_ring_depth(rts_ctx* c, int stages)
+{
+    if (!c) return RTS_EINVAL;
+    if (stages != 0 && stages != 2 && stages != 3) return fail(c, RTS_EINVAL, "rts_set_ring_depth: 0, 2 or 3");
+    c->user_nstage = stages;
+    c->planned = false;
+    return RTS_OK;
+}
+
 int rts_set_ctas_per_sm(rts_ctx* c, int n)
 {
     if (!c) return RTS_EINVAL;
@@ -687,7 +733,7 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
         int nunits = (int)c->units.size(), total = c->total_tickets;
         void* args[] = {&c->maps, &dunits, &nunits, &total, &ticket, &Q, &QB, &Itop, &abortf};
         // cooperative launch: every CTA of the grid is resident, which the tile barriers rely on
-        CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_sweep_kernel, dim3(c->grid), dim3(c->threads), args,
+        CUDA_TRY(c, cudaLaunchCooperativeKernel(sweep_fn(c->pitch), dim3(c->grid), dim3(c->threads), args,
                                                 (size_t)c->smem_bytes, st));
     }
     // finalize

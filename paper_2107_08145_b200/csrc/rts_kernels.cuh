@@ -38,9 +38,8 @@ constexpr double PI_D = 3.14159265358979323846;
 // the ray along them.  Slot s of a unit holds a ray with su = (s & 1 ? -1 : +1),
 // sv = (s & 2 ? -1 : +1).
 struct alignas(16) RayC {
-    float w[4];       // bilinear weights, sum == 1 exactly, ordered by stencil row: (lower v row, its
-                      // u-side neighbour, higher v row, its u-side neighbour); the node's own row is
-                      // the higher one for sv > 0 and the lower one for sv < 0
+    float w[4];       // bilinear weights, sum == 1 exactly: (upwind v row, its u-side neighbour, the node's
+                      // own v row, its u-side neighbour) of the previous plane
     float kc;         // 0.5*ds  (opacity sum -> optical path)
     float wq;         // quadrature weight
     int   active;
@@ -62,8 +61,8 @@ struct UnitDesc {
     int WU, WV, ntu, ntv;
     int K, npass, ticket_begin, ntiles;
     int nz, q_in_B, qvec, nstage;          // qvec: heating rows are 16-byte aligned (vector reductions)
-    int ng, gsu0, nband_ok, pad0;          // ray groups (same su) of this unit: 2 (su = +1, -1) or 1 (su = gsu0);
-                                           // nband_ok: bands of the pair that exist (1 or 2)
+    int ng, gsu0, nband_ok, RC;            // ray groups (same su) of this unit: 2 (su = +1, -1) or 1 (su = gsu0);
+                                           // nband_ok: bands of the pair that exist (1 or 2); RC: rows per strip
     RayC ray[NSLOT];
     float* Xex;       // float2 [2][NSLOT][n_v][n_u2]   carried planes at block ends (strips only)
     float* Gu;        // float2 [2][n_m][NSLOT*n_v + NSLOT*n_u2]  per pass parity and plane: far-u column

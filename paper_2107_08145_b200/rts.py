@@ -22,7 +22,7 @@ _ERR = {-1: "RTS_EINVAL", -2: "RTS_ESTATE", -3: "RTS_ECUDA", -4: "RTS_ENOMEM", -
 
 EXPORTS = [
     "rts_create", "rts_destroy", "rts_set_tables", "rts_set_passes", "rts_set_rays", "rts_get_rays",
-    "rts_num_up_rays", "rts_set_tiling", "rts_set_exchange_interval", "rts_set_ctas_per_sm", "rts_workspace_bytes",
+    "rts_num_up_rays", "rts_set_tiling", "rts_set_exchange_interval", "rts_set_ctas_per_sm", "rts_set_ring_depth", "rts_workspace_bytes",
     "rts_set_workspace", "rts_solve", "rts_solve_host", "rts_coefficients", "rts_sync_check",
     "rts_plan_info", "rts_last_error", "rts_enable_timing", "rts_last_timing",
     "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells", "rts_set_thick_skip", "rts_thick_levels",
@@ -62,6 +62,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_set_exchange_interval.argtypes = [c_void_p, c_int]
     lib.rts_set_ctas_per_sm.restype = c_int
     lib.rts_set_ctas_per_sm.argtypes = [c_void_p, c_int]
+    lib.rts_set_ring_depth.restype = c_int
+    lib.rts_set_ring_depth.argtypes = [c_void_p, c_int]
     lib.rts_workspace_bytes.restype = c_size_t
     lib.rts_workspace_bytes.argtypes = [c_void_p]
     lib.rts_set_workspace.restype = c_int
@@ -177,6 +179,9 @@ class RTS:
 
     def set_ctas_per_sm(self, n: int):
         self._check(self._lib.rts_set_ctas_per_sm(self._ctx, n), "rts_set_ctas_per_sm")
+
+    def set_ring_depth(self, n: int):
+        self._check(self._lib.rts_set_ring_depth(self._ctx, n), "rts_set_ring_depth")
 
     def workspace_bytes(self) -> int:
         n = int(self._lib.rts_workspace_bytes(self._ctx))
@@ -311,7 +316,7 @@ class RTS:
 
 
 def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchange_interval: int = 0,
-                cells: bool = False) -> "RTS":
+                cells: bool = False, ring_depth: int = 0) -> "RTS":
     """Create and configure a solver for an `inputs.RTSInputs` problem.  cells=True: the fields of
     `inp` are cell-centred (solve_cells); the RT node grid then has one level more."""
     r = RTS(inp.nx, inp.ny, inp.nz + (1 if cells else 0), inp.dx, inp.dy, inp.dz, inp.nbands)
@@ -325,5 +330,7 @@ def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchan
         r.set_ctas_per_sm(ctas_per_sm)
     if exchange_interval:
         r.set_exchange_interval(exchange_interval)
+    if ring_depth:
+        r.set_ring_depth(ring_depth)
     r.allocate_workspace()
     return r
