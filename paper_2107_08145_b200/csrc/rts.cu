@@ -208,6 +208,7 @@ int make_plan(rts_ctx* c)
     c->PY = (int)align_up((size_t)c->ny, 4) + 2 * HALO;
     c->PYR = c->ny + 2 * HALO;
     c->K = c->user_K ? c->user_K : KMAX;
+    if (const char* e_ = getenv("RTS_TUNE_RC")) c->user_rc = atoi(e_);   // TUNING ONLY
 
     // --- unit skeletons: (march, dir) groups, sub-units with <= 1 ray per slot
     struct Group { int march, dir; std::vector<std::vector<int>> sub; };

@@ -146,7 +146,8 @@ enum : unsigned {
     IT_FARC = 1u << 2,       // core pair holding the far-u column of its ray: writes the seam history
     IT_USTRIP = 1u << 3,     // core pair inside the u exchange strip
     IT_FARV = 1u << 4,       // the last row of the region is the far-v row of a periodic v axis (seam history)
-    IT_DIR = 1u << 5         // row q = 0 is the inflow row of a bounded v axis (set, not updated)
+    IT_DIR = 1u << 5,        // row q = 0 is the inflow row of a bounded v axis (set, not updated)
+    IT_FSEC = 1u << 6        // the far-u column is the second column of the pair
 };
 
 struct GhostEnt { unsigned short xoff, bv; int goff; };   // 8 bytes; slot = goff >> 28; xoff: box row * 2 PITCH + column
@@ -291,43 +292,37 @@ __device__ __forceinline__ f2 node_update(const f2 em1, const f2 wl, const f2 pp
     return fma2(pp, sub2(sp, Stp), v);
 }
 
-// The uncommon tail of one row of a strip (out of line): half pairs, seam histories, exchange strips.
-// s: slot; q: region row; boff: byte offset of the row's pair inside a plane set; bW: its address in the written
-// plane; info: StepCtx::tail; geo = hv | nrows << 8.
-template <int PITCH, int SU>
-__device__ __noinline__ void row_tail(const TaskShared* __restrict__ Sp, const int info, const int s, const unsigned fl,
-                                      const int q, const int geo, const uint32_t boff, const uint32_t bW, const float4 o)
+// what a strip needs for the uncommon stores of a step (seam histories, exchange strips)
+struct TailCtx {
+    f2* GhP;                           // seam history of this plane and pass (far columns, then far rows); null: off
+    f2* XeP;                           // exchange planes of this block's parity; null: no strips this step
+    int gv0, ug;                       // slot * n_v + global v of row q = 0;  global u of the pair
+    int n_u2, far_off;                 // row pitch of the exchange planes; NSLOT*n_v + slot*n_u2 (far-v rows)
+    int hv, nrows, K, gsv;
+};
+
+// Store one finished row of a strip: the carried plane and, where flagged, the seam history (far-u column,
+// far-v row) and the exchange strips.  Inline: a few instructions on the flagged rows only.
+template <int SU>
+__device__ __forceinline__ void row_store(const TailCtx& TC, const unsigned fl, const bool slow, const int q,
+                                          const uint32_t bW, const float4 o)
 {
-    constexpr uint32_t RP = 16u * PITCH;
-    const UnitDesc& U = Sp->U; const TileGeo& G = Sp->G;
-    const int rowN = (int)(boff / RP), c0 = (int)((boff % RP) >> 3);
-    const int hv = geo & 0xff, nrows = geo >> 8;
-    const bool hist = info & 1, strips = info & 2;
+    if (!slow) { sts128<0>(bW, o); return; }
     const bool part = (fl & IT_PART) != 0;
     if (!part) sts128<0>(bW, o); else sts64<0>(bW, make_float2(o.x, o.y));
-    const bool core = (q >= hv) && !(fl & IT_DQ);
-    if (!core) return;
-    const int vN = G.v0 + rowN - HALO, ug = G.u0 + c0 - HALO;
-    if (hist) {
-        f2* const Ghist = reinterpret_cast<f2*>(U.Gu) + (size_t)(info >> 8) * ((size_t)NSLOT * (U.n_v + U.n_u2));
-        if (fl & IT_FARC) {
-            // far-u column of this ray: its values are the next pass's seam ghosts of this plane
-            const bool second = (((SU < 0) ? G.dlo_u : G.dhi_u - 1) - c0) != 0;
-            __stcg(Ghist + s * U.n_v + vN, second ? make_float2(o.z, o.w) : make_float2(o.x, o.y));
-        }
-        if ((fl & IT_FARV) && q == nrows - 1) {
-            // far-v row of this ray (periodic v axis): the next pass's seam ghost row of this plane
-            f2* gv = Ghist + NSLOT * U.n_v + s * U.n_u2 + ug;
-            if (!part) __stcg(reinterpret_cast<float4*>(gv), o);
-            else __stcg(gv, make_float2(o.x, o.y));
+    if (q < TC.hv || (fl & IT_DQ)) return;                       // halo row / halo pair: nothing to publish
+    const int gv = TC.gv0 + q * TC.gsv;
+    if (TC.GhP) {
+        if (fl & IT_FARC)                                        // far-u column: next pass's seam ghosts of this plane
+            __stcg(TC.GhP + gv, (fl & IT_FSEC) ? make_float2(o.z, o.w) : make_float2(o.x, o.y));
+        if ((fl & IT_FARV) && q == TC.nrows - 1) {               // far-v row (periodic v axis)
+            f2* gvp = TC.GhP + TC.far_off + TC.ug;
+            if (!part) __stcg(reinterpret_cast<float4*>(gvp), o);
+            else __stcg(gvp, make_float2(o.x, o.y));
         }
     }
-    if (strips && ((fl & IT_USTRIP) || q >= nrows - U.K)) {
-        // exchange strips at a block end
-        const int par_ex = (info >> 2) & 1;
-        float* xe = U.Xex + 2 * ((((size_t)par_ex * NSLOT + s) * U.n_v + vN) * U.n_u2 + ug);
-        __stcg(reinterpret_cast<float4*>(xe), o);
-    }
+    if (TC.XeP && ((fl & IT_USTRIP) || q >= TC.nrows - TC.K))    // exchange strips at a block end
+        __stcg(reinterpret_cast<float4*>(TC.XeP + (size_t)gv * TC.n_u2 + TC.ug), o);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -337,9 +332,9 @@ __device__ __noinline__ void row_tail(const TaskShared* __restrict__ Sp, const i
 // carried plane of the ray read / written this step.
 template <int PITCH, int SU>
 __device__ __forceinline__ void do_strip(
-    const int s, const unsigned fl, int q, const int qb, const int geo, const int rstep, const RayK& rk,
-    const TaskShared& S, const StepCtx& C, const int qtail, int vrow, const int vstep,
-    uint32_t bP, uint32_t bC, uint32_t bX, uint32_t bW, uint32_t boff)
+    const int s, const unsigned fl, int q, const int qb, const int rstep, const RayK& rk,
+    const TaskShared& S, const StepCtx& C, const TailCtx& TC, const int qtail, int vrow, const int vstep,
+    uint32_t bP, uint32_t bC, uint32_t bX, uint32_t bW)
 {
     constexpr int HP = 8 * PITCH;        // second field (S) of a coefficient row
     const bool zm = S.G.zmarch != 0;
@@ -350,9 +345,8 @@ __device__ __forceinline__ void do_strip(
         const float f = (S.U.ray[s].up ? 1.f : 0.f) - C.a_cur;
         for (; q < qb; ++q) {
             const float4 o = scale4(f, lds128<HP>(bC));
-            if (tail_all || q >= qtail) row_tail<PITCH, SU>(&S, C.tail, s, fl, q, geo, boff, bW, o);
-            else sts128<0>(bW, o);
-            bC += rstep; bW += rstep; boff += rstep;
+            row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);
+            bC += rstep; bW += rstep;
         }
         return;
     }
@@ -360,9 +354,8 @@ __device__ __forceinline__ void do_strip(
         // inflow row of a bounded v axis (v = z): I = S (upward ray, bottom row) or 0 (downward ray, top row)
         const float f = ((s & 2) ? 0.f : 1.f) - ((vrow <= ks) ? 1.f : 0.f);
         const float4 o = scale4(f, lds128<HP>(bC));
-        if (tail_all || q >= qtail) row_tail<PITCH, SU>(&S, C.tail, s, fl, q, geo, boff, bW, o);
-        else sts128<0>(bW, o);
-        bP += rstep; bC += rstep; bX += rstep; bW += rstep; boff += rstep; vrow += vstep; ++q;
+        row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);
+        bP += rstep; bC += rstep; bX += rstep; bW += rstep; vrow += vstep; ++q;
         if (q >= qb) return;
     }
     // upwind rows of the first row
@@ -397,9 +390,8 @@ __device__ __forceinline__ void do_strip(
             v1 = node_update<SU, 1, 2>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, a_u, a_o, a_p);                      \
         }                                                                                                           \
         const float4 o = cat4(v0, v1);                                                                              \
-        if (tail_all || q >= qtail) row_tail<PITCH, SU>(&S, C.tail, s, fl, q, geo, boff, bW, o);                    \
-        else sts128<0>(bW, o);                                                                                      \
-        bP += rstep; bC += rstep; bX += rstep; bW += rstep; boff += rstep; vrow += vstep; ++q;                       \
+        row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);                                                    \
+        bP += rstep; bC += rstep; bX += rstep; bW += rstep; vrow += vstep; ++q;                                     \
     }
 #pragma unroll 1
     while (true) {
@@ -748,7 +740,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
             if (!core_q) ifl |= IT_DQ;
             if (chi - c0 < 2) ifl |= IT_PART;
             const int fc = (gsu > 0) ? G.dhi_u - 1 : G.dlo_u;                  // far-u column of this ray (box)
-            if (core_q && fc >= c0 && fc < c0 + 2) ifl |= IT_FARC;
+            if (core_q && fc >= c0 && fc < c0 + 2) ifl |= IT_FARC | ((fc != c0) ? IT_FSEC : 0u);
             if (core_q && ((gsu > 0) ? (c0 + 2 > HALO + G.wu - K) : (c0 - HALO < K))) ifl |= IT_USTRIP;
             // the last row of the region is the far-v row of a periodic v axis
             if (U.per_v && ((gsv > 0) ? (G.v0 + G.wv == U.n_v) : (G.v0 == 0))) ifl |= IT_FARV;
@@ -769,6 +761,13 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     const int rstep = (gsv > 0) ? RP : -RP;
     const int hv_ = geo & 0xff, nrows_ = geo >> 8;
     const int v_q0 = (gsv > 0) ? G.v0 - hv_ : G.v0 + G.wv - 1 + hv_;  // global v of row q = 0
+    TailCtx TC;
+    TC.gv0 = s * U.n_v + v_q0;
+    TC.ug = G.u0 - HALO + (int)((ioff0 % (uint32_t)RP) >> 3);
+    TC.n_u2 = U.n_u2; TC.far_off = NSLOT * U.n_v + s * U.n_u2;
+    TC.hv = hv_; TC.nrows = nrows_; TC.K = K; TC.gsv = gsv;
+    const size_t g_plane = (size_t)NSLOT * (U.n_v + U.n_u2);
+    const size_t xe_par = (size_t)NSLOT * U.n_v * U.n_u2;
 
     // ================================================================== the march
     int cur = 0, gblk = 0, s_ = 0;
@@ -819,7 +818,9 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                         C.dplane = zmarch && (m == 0);
                         const bool hist = !lastpass;
                         const bool strips = blk_last && more && !(zmarch && m == n_m - 1);
-                        C.tail = (hist ? 1 : 0) | (strips ? 2 : 0) | ((gblk & 1) << 2) | (((pass & 1) * n_m + m) << 8);
+                        C.tail = 0;
+                        TC.GhP = hist ? reinterpret_cast<f2*>(U.Gu) + ((size_t)(pass & 1) * n_m + m) * g_plane : nullptr;
+                        TC.XeP = strips ? reinterpret_cast<f2*>(U.Xex) + (size_t)(gblk & 1) * xe_par : nullptr;
                         C.xmask = IT_PART | (hist ? IT_FARC : 0u) | (strips ? IT_USTRIP : 0u);
                         C.a_prev = (pl - dir <= kstar) ? 1.f : 0.f; C.a_cur = (pl <= kstar) ? 1.f : 0.f;
                         C.zreg = 0;
@@ -827,8 +828,8 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                         const uint32_t o = ioff0 + (uint32_t)(q0 * rstep);
                         const uint32_t bP = aStage0 + (uint32_t)stp * PSB + o, bC = aStage0 + (uint32_t)stc * PSB + o;
                         const uint32_t bX = aXb + (uint32_t)cur * XBB + xslot + o, bW = aXb + (uint32_t)(cur ^ 1) * XBB + xslot + o;
-                        if (gsu < 0) do_strip<PITCH, -1>(s, ifl, q0, qb, geo, rstep, rk, S, C, qtail, v_q0 + gsv * q0, gsv, bP, bC, bX, bW, o);
-                        else         do_strip<PITCH, +1>(s, ifl, q0, qb, geo, rstep, rk, S, C, qtail, v_q0 + gsv * q0, gsv, bP, bC, bX, bW, o);
+                        if (gsu < 0) do_strip<PITCH, -1>(s, ifl, q0, qb, rstep, rk, S, C, TC, qtail, v_q0 + gsv * q0, gsv, bP, bC, bX, bW);
+                        else         do_strip<PITCH, +1>(s, ifl, q0, qb, rstep, rk, S, C, TC, qtail, v_q0 + gsv * q0, gsv, bP, bC, bX, bW);
                     }
                 }
                 // ---- seam ghosts of this plane into the new carried plane
