@@ -220,20 +220,29 @@ __device__ __forceinline__ f2 bil_from(const Row3& up, const Row3& ow, const flo
 // ------------------------------------------------------------------------------------------
 // Attenuation factors of one node (both bands): em1 = 1 - e^-dt, wl = (1 - e^-dt)/dt, pp = psi_p = 1 - wl.
 // EV 0: closed form (exp2 and reciprocal units); accurate for dt >= DTAU_SERIES.
-// EV 1: series of psi_p (11 terms, truncation < 1e-8 relative for dt <= DTAU_SERIES_MAX; no cancellation,
+// EV 1: series of psi_p (8 terms, truncation < 3e-9 relative for dt <= DTAU_SERIES_MAX; no cancellation,
 //       no special-function unit), wl = 1 - psi_p, em1 = dt*wl.
-// EV 2: both, psi_p selected per band (a row whose optical paths span more than DTAU_SERIES .. DTAU_SERIES_MAX).
-constexpr float DTAU_SERIES_MAX = 1.0f;
+// EV 2: both, selected per band (a row whose optical paths span more than DTAU_SERIES .. DTAU_SERIES_MAX).
+// EV 3: the first four terms of the series (every optical path of the row below DTAU_SERIES).
+constexpr float DTAU_SERIES_MAX = 0.5f;
 template <int EV>
 __device__ __forceinline__ void att_factors(const f2 dt, f2& em1, f2& wl, f2& pp)
 {
     f2 pps;
+    if (EV == 3) {
+        // every optical path of the row below DTAU_SERIES: four terms (truncation dt^4/360 < 2e-8)
+        const f2 nd = neg2(dt);
+        f2 q = fma2(nd, bc(1.0f / 120.0f), bc(1.0f / 24.0f));
+        q = fma2(nd, q, bc(1.0f / 6.0f));
+        q = fma2(nd, q, bc(0.5f));
+        pp = mul2(dt, q);
+        wl = sub2(bc(1.f), pp);
+        em1 = mul2(dt, wl);
+        return;
+    }
     if (EV != 0) {
         const f2 nd = neg2(dt);
-        f2 q = fma2(nd, bc(1.0f / 479001600.0f), bc(1.0f / 39916800.0f));
-        q = fma2(nd, q, bc(1.0f / 3628800.0f));
-        q = fma2(nd, q, bc(1.0f / 362880.0f));
-        q = fma2(nd, q, bc(1.0f / 40320.0f));
+        f2 q = fma2(nd, bc(1.0f / 362880.0f), bc(1.0f / 40320.0f));
         q = fma2(nd, q, bc(1.0f / 5040.0f));
         q = fma2(nd, q, bc(1.0f / 720.0f));
         q = fma2(nd, q, bc(1.0f / 120.0f));
@@ -254,11 +263,13 @@ __device__ __forceinline__ void att_factors(const f2 dt, f2& em1, f2& wl, f2& pp
     wl = mul2(em1, make_float2(rcp_approx(dt.x), rcp_approx(dt.y)));
     pp = sub2(bc(1.f), wl);
     if (EV == 2) {
-        // only psi_p is selected; wl and 1 - e^-dt follow from it (closed form: 1 - psi_p = wl exactly,
-        // dt*wl = 1 - e^-dt to an ulp)
-        pp = make_float2(dt.x < DTAU_SERIES ? pps.x : pp.x, dt.y < DTAU_SERIES ? pps.y : pp.y);
-        wl = sub2(bc(1.f), pp);
-        em1 = mul2(dt, wl);
+        // per band: the series values below DTAU_SERIES (wl, em1 derived from psi_p there: no cancellation),
+        // the closed form above (where 1 - psi_p would lose the small wl of a thick path)
+        const f2 wls = sub2(bc(1.f), pps), es = mul2(dt, wls);
+        const bool sx = dt.x < DTAU_SERIES, sy = dt.y < DTAU_SERIES;
+        pp = make_float2(sx ? pps.x : pp.x, sy ? pps.y : pp.y);
+        wl = make_float2(sx ? wls.x : wl.x, sy ? wls.y : wl.y);
+        em1 = make_float2(sx ? es.x : em1.x, sy ? es.y : em1.y);
     }
 }
 
@@ -271,17 +282,25 @@ __device__ __forceinline__ f2 node_update(const f2 em1, const f2 wl, const f2 pp
                                           const float a_u, const float a_o, const float a_p)
 {
     const f2 Xu = bil<SU, J>(xu, xo, w);
+    if (REG == 3) {
+        // uniform regime, f = a_u = 1 - a: one branch-free form of REG 0 (f = 0) and REG 1 (f = 1):
+        //   X = Xu + em1 (f (d + Sp) - Xu) + (wl - f) d,  d = Su - Sp formed first (weights sum to 1);  wl - 1 = -psi_p
+        const f2 d = bil_from<SU, J>(su, so, w, neg2(sp));
+        const f2 t = fma2(bc(a_u), add2(d, sp), neg2(Xu));
+        return fma2(sub2(wl, bc(a_u)), d, fma2(em1, t, Xu));
+    }
     f2 v = fma2(neg2(Xu), em1, Xu);                                // Xu * e^-dt
     if (REG == 0) {
         const f2 d = bil_from<SU, J>(su, so, w, neg2(sp));         // S_u - S_p (weights sum to 1 exactly)
         return fma2(d, wl, v);
     }
-    const f2 pu = sub2(em1, pp);                                   // psi_u = (1 - E) - psi_p
     if (REG == 1) {
-        const f2 Su = bil<SU, J>(su, so, w);
-        v = fma2(pu, Su, v);
-        return fma2(pp, sp, v);
+        // Xu E + psi_u Su + psi_p Sp with psi_u = (1 - E) - psi_p:  Xu + (1 - E)(Su - Xu) - psi_p (Su - Sp)
+        const f2 d = bil_from<SU, J>(su, so, w, neg2(sp));         // Su - Sp
+        const f2 t = sub2(add2(d, sp), Xu);                        // Su - Xu
+        return fma2(neg2(pp), d, fma2(em1, t, Xu));
     }
+    const f2 pu = sub2(em1, pp);                                   // psi_u = (1 - E) - psi_p
     const f2 R0 = fma2(bc(w.y), sid<SU, J>(su), mul2(bc(w.x), cen<J>(su)));
     const f2 R1 = fma2(bc(w.w), sid<SU, J>(so), mul2(bc(w.z), cen<J>(so)));
     const f2 St = fma2(bc(a_o), R1, mul2(bc(a_u), R0));
@@ -374,17 +393,15 @@ __device__ __forceinline__ void do_strip(
         else { a_u = (vrow - vstep <= ks) ? 1.f : 0.f; a_o = (vrow <= ks) ? 1.f : 0.f; a_p = a_o; }                  \
         const f2 sp0 = make_float2(sc.x, sc.y), sp1 = make_float2(sc.z, sc.w);                                      \
         f2 e0, l0, p0, e1, l1, p1;                                                                                  \
-        if (dmin >= DTAU_SERIES) { att_factors<0>(dt0, e0, l0, p0); att_factors<0>(dt1, e1, l1, p1); }              \
-        else if (dmax <= DTAU_SERIES_MAX) { att_factors<1>(dt0, e0, l0, p0); att_factors<1>(dt1, e1, l1, p1); }     \
+        /* one evaluator per warp and row (each is valid for every lane that takes part): no divergence */          \
+        const unsigned am_ = __activemask();                                                                        \
+        if (__all_sync(am_, dmin >= DTAU_SERIES)) { att_factors<0>(dt0, e0, l0, p0); att_factors<0>(dt1, e1, l1, p1); }    \
+        else if (__all_sync(am_, dmax <= DTAU_SERIES_MAX)) { att_factors<1>(dt0, e0, l0, p0); att_factors<1>(dt1, e1, l1, p1); } \
         else { att_factors<2>(dt0, e0, l0, p0); att_factors<2>(dt1, e1, l1, p1); }                                  \
-        const float asum = a_u + a_o + a_p;                                                                         \
         f2 v0, v1;                                                                                                  \
-        if (asum == 3.f) {                                                                                          \
-            v0 = node_update<SU, 0, 0>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, 1.f, 1.f, 1.f);                      \
-            v1 = node_update<SU, 1, 0>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, 1.f, 1.f, 1.f);                      \
-        } else if (asum == 0.f) {                                                                                   \
-            v0 = node_update<SU, 0, 1>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, 0.f, 0.f, 0.f);                      \
-            v1 = node_update<SU, 1, 1>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, 0.f, 0.f, 0.f);                      \
+        if (a_u == a_o && a_o == a_p) {                                                                             \
+            v0 = node_update<SU, 0, 3>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, 1.f - a_p, 0.f, 0.f);                \
+            v1 = node_update<SU, 1, 3>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, 1.f - a_p, 0.f, 0.f);                \
         } else {                                                                                                    \
             v0 = node_update<SU, 0, 2>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, a_u, a_o, a_p);                      \
             v1 = node_update<SU, 1, 2>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, a_u, a_o, a_p);                      \
