@@ -109,6 +109,20 @@ int rts_set_workspace(rts_ctx* ctx, void* workspace_dev, size_t bytes);
 int rts_solve(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const float* P_dev,
               float* Qrad_dev, float* Itop_dev, void* stream);
 
+/* Radiative flux and flux-divergence heating (paper's Flux: "From the specific intensity calculate the average
+ * intensity and radiative fluxes"; reading R21).  rts_enable_flux(1) must precede
+ * rts_workspace_bytes / rts_set_workspace (three more partial fields per sweep unit).  rts_solve_flux is rts_solve plus
+ *   Frad   DEVICE out [3][nz][ny][nx]: F_a = 4 pi sum_b sum_r w_r Omega_{r,a} I_{b,r}, Omega = mu/|mu| (band-integrated)
+ *   Qdiv   DEVICE out [nz][ny][nx] or NULL: -div F, central differences on the node grid, periodic in x and y,
+ *          one-sided on the bottom and top node planes
+ *   Qblend DEVICE out [nz][ny][nx] or NULL: w Qrad + (1 - w) Qdiv, w(k) = exp(-taubar(k)/tau0), taubar(k) = horizontally
+ *          averaged optical depth of band 0 from the top down to level k; tau0 set by rts_set_flux_blend (default 0.1).
+ * Asynchronous on `stream`.  All sums are formed in a fixed order: results are bitwise reproducible. */
+int rts_enable_flux(rts_ctx* ctx, int on);
+int rts_set_flux_blend(rts_ctx* ctx, double tau0);
+int rts_solve_flux(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const float* P_dev,
+                   float* Qrad_dev, float* Itop_dev, float* Frad_dev, float* Qdiv_dev, float* Qblend_dev, void* stream);
+
 /* Same solve with HOST buffers (pinned or pageable): copies rho,T,P to the device, solves,
  * copies Qrad (and Itop if non-NULL) back, synchronises.  The staging buffers live in the
  * workspace (rts_workspace_bytes accounts for them). */

@@ -30,11 +30,12 @@ _PI = ctypes.POINTER(ctypes.c_int)
 
 
 def build(force: bool = False) -> str:
-    """Compile rts_oracle.c -> librts_oracle.so (gcc, -O2, OpenMP, no fast-math)."""
+    """Compile rts_oracle.c -> librts_oracle.so (gcc -O3, OpenMP, no fast-math, no -march: the .so built on the
+    CPU-only box travels to the GPU box)."""
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
         return _LIB
-    cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11",
+    cmd = ["gcc", "-O3", "-fopenmp", "-fPIC", "-shared", "-std=c11",
            "-o", _LIB, _SRC, "-lm"]
     subprocess.run(cmd, check=True)
     return _LIB
@@ -60,7 +61,9 @@ def _load():
         _lib.oracle_solve.restype = _I
         _lib.oracle_solve.argtypes = ([_I, _I, _I, _D, _D, _D, _I, _I, _I, _D, _D, _D, _D,
                                        _PF, _PF, _I, _I, _PD, _PD, _PF, _PF, _PF,
-                                       _PD, _PD, _PD, _I])
+                                       _PD, _PD, _PD, _PD, _I])
+        _lib.oracle_flux_heating.restype = _I
+        _lib.oracle_flux_heating.argtypes = [_I, _I, _I, _D, _D, _D, _PD, _PD, _PD, _D, _PD, _PD]
         _lib.oracle_num_threads.restype = _I
         _lib.oracle_num_threads.argtypes = []
     return _lib
@@ -132,12 +135,13 @@ def sweep_ray(nx, ny, nz, dx, dy, dz, mu, npasses, kaprho, S,
     return I
 
 
-def solve(inp, nthreads: int = 0, want_J: bool = False):
-    """O-7: returns (Q [nz][ny][nx], Itop [nb][n_up][ny][nx]) (+ J [nb][nz][ny][nx])."""
+def solve(inp, nthreads: int = 0, want_J: bool = False, want_F: bool = False):
+    """O-7: returns (Q [nz][ny][nx], Itop [nb][n_up][ny][nx]) (+ J [nb][nz][ny][nx]) (+ O-10 F [3][nz][ny][nx])."""
     lib = _load()
     Q = np.empty(inp.shape, dtype=np.float64)
     Itop = np.empty((inp.nbands, inp.n_up, inp.ny, inp.nx), dtype=np.float64)
     J = np.empty((inp.nbands,) + inp.shape, dtype=np.float64) if want_J else None
+    F = np.empty((3,) + inp.shape, dtype=np.float64) if want_F else None
     mu = np.ascontiguousarray(inp.mu, dtype=np.float64)
     wq = np.ascontiguousarray(inp.wq, dtype=np.float64)
     rc = lib.oracle_solve(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz,
@@ -146,12 +150,32 @@ def solve(inp, nthreads: int = 0, want_J: bool = False):
                           _pf(inp.logkappa), _pf(inp.bandfrac),
                           inp.npasses, inp.nrays, _pd(mu), _pd(wq),
                           _pf(inp.rho), _pf(inp.T), _pf(inp.P),
-                          _pd(Q), _pd(Itop), _pd(J), nthreads)
+                          _pd(Q), _pd(Itop), _pd(J), _pd(F), nthreads)
     if rc != 0:
         raise RuntimeError(f"oracle_solve failed: {rc}")
+    out = (Q, Itop)
     if want_J:
-        return Q, Itop, J
-    return Q, Itop
+        out += (J,)
+    if want_F:
+        out += (F,)
+    return out
+
+
+def flux_heating(inp, F, QJ=None, kaprho0=None, tau0: float = 0.1, want_blend: bool = True):
+    """O-11: (Qdiv, Qblend) from the flux F [3][nz][ny][nx]; Qblend needs QJ and the band-0 kaprho."""
+    lib = _load()
+    F = np.ascontiguousarray(F, dtype=np.float64)
+    Qdiv = np.empty(inp.shape, dtype=np.float64)
+    Qb = np.empty(inp.shape, dtype=np.float64) if want_blend else None
+    if want_blend:
+        QJ = np.ascontiguousarray(QJ, dtype=np.float64)
+        kaprho0 = np.ascontiguousarray(kaprho0, dtype=np.float64)
+    rc = lib.oracle_flux_heating(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, _pd(F),
+                                 _pd(QJ) if want_blend else None, _pd(kaprho0) if want_blend else None,
+                                 float(tau0), _pd(Qdiv), _pd(Qb))
+    if rc != 0:
+        raise RuntimeError(f"oracle_flux_heating failed: {rc}")
+    return Qdiv, Qb
 
 
 def cells_to_nodes(cell: np.ndarray) -> np.ndarray:

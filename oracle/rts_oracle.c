@@ -254,11 +254,17 @@ int oracle_sweep_ray(int nx, int ny, int nz, double dx, double dy, double dz,
 }
 
 /* ---------------------------------------------------------------------------
- * O-7  Full solve: all bands, all rays, J, Q and I_top.
+ * O-7  Full solve: all bands, all rays, J, Q and I_top (+ O-10 radiative flux).
  *   J_b = sum_r w_r I_{b,r}^(P);  Q = 4 pi sum_b kaprho_b (J_b - S_b) at every node;
  *   Itop[b][u][j][i] = I_{b,r}^(P)(i,j,nz-1) for the u-th ray with mu_z > 0 (in ray order).
- *   Optional outputs (may be NULL): Jout [nb][N].
+ *   O-10 (paper's Flux, "From the specific intensity calculate the
+ *   average intensity and radiative fluxes"; reading R21):
+ *     F_a = 4 pi sum_b sum_r w_r Omega_{r,a} I_{b,r}^(P),  Omega_r = mu_r / |mu_r|,  a = x, y, z.
+ *   Optional outputs (may be NULL): Jout [nb][N], Fout [3][N].
  *   nthreads <= 0: all OpenMP threads.
+ *   The (band, ray) sweeps are independent; they run in batches of one sweep per thread and
+ *   each batch is added to J (and F) in (band, ray) order by a loop over the nodes, so the
+ *   sums are formed in the same order for any thread count.
  * ------------------------------------------------------------------------- */
 int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
                  int nb, int nT, int nP,
@@ -266,49 +272,64 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
                  const float* logkappa, const float* bandfrac,
                  int npasses, int nrays, const double* mu, const double* wq,
                  const float* rho, const float* T, const float* P,
-                 double* Q, double* Itop, double* Jout, int nthreads)
+                 double* Q, double* Itop, double* Jout, double* Fout, int nthreads)
 {
     if (nx < 1 || ny < 1 || nz < 2 || nb < 1 || nrays < 1) return -1;
     const size_t N = (size_t)nx * ny * nz;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+    const int nt = omp_get_max_threads();
+#else
+    (void)nthreads;
+    const int nt = 1;
+#endif
+    const int ntask = nb * nrays;
+    const int batch = nt < ntask ? nt : ntask;
     double* kaprho = (double*)malloc(sizeof(double) * N * nb);
     double* S = (double*)malloc(sizeof(double) * N * nb);
     double* J = (double*)calloc(N * nb, sizeof(double));
+    double* Ibuf = (double*)malloc(sizeof(double) * N * (size_t)batch);
     int* upidx = (int*)malloc(sizeof(int) * nrays);
-    if (!kaprho || !S || !J || !upidx) { free(kaprho); free(S); free(J); free(upidx); return -2; }
-#ifdef _OPENMP
-    if (nthreads > 0) omp_set_num_threads(nthreads);
-#else
-    (void)nthreads;
-#endif
+    int* err = (int*)calloc((size_t)batch, sizeof(int));
+    if (!kaprho || !S || !J || !upidx || !Ibuf || !err) { free(kaprho); free(S); free(J); free(upidx); free(Ibuf); free(err); return -2; }
     int rc = oracle_coefficients(nx, ny, nz, nb, nT, nP, logT_min, logT_max, logP_min, logP_max,
                                  logkappa, bandfrac, rho, T, P, kaprho, S);
     int nup = 0;
     for (int r = 0; r < nrays; ++r) upidx[r] = (mu[3 * r + 2] > 0.0) ? nup++ : -1;
+    if (Fout) memset(Fout, 0, sizeof(double) * 3 * N);
 
     int fail = rc;
-    const int ntask = nb * nrays;
-    int task;
-#pragma omp parallel for ordered schedule(dynamic, 1)
-    for (task = 0; task < ntask; ++task) {
-        int b = task / nrays, r = task % nrays;
-        double* I = (double*)malloc(sizeof(double) * N);
-        int e = I ? oracle_sweep_ray(nx, ny, nz, dx, dy, dz, mu + 3 * r, npasses,
-                                     kaprho + (size_t)b * N, S + (size_t)b * N, NULL, 0, I)
-                  : -2;
-        if (e == 0 && Itop && upidx[r] >= 0) {
-            double* dst = Itop + ((size_t)b * nup + upidx[r]) * ny * nx;
-            memcpy(dst, I + (size_t)(nz - 1) * ny * nx, sizeof(double) * ny * nx);
-        }
-        /* J_b = sum_r w_r I_r accumulated in ray order (deterministic for any thread count) */
-#pragma omp ordered
-        {
-            if (e != 0) fail = e;
-            else {
-                double* Jb = J + (size_t)b * N;
-                for (size_t n = 0; n < N; ++n) Jb[n] += wq[r] * I[n];
+    for (int t0 = 0; t0 < ntask && fail == 0; t0 += batch) {
+        const int nb_ = (ntask - t0 < batch) ? ntask - t0 : batch;
+        int q;
+#pragma omp parallel for schedule(static, 1)
+        for (q = 0; q < nb_; ++q) {
+            const int task = t0 + q, b = task / nrays, r = task % nrays;
+            double* I = Ibuf + (size_t)q * N;
+            err[q] = oracle_sweep_ray(nx, ny, nz, dx, dy, dz, mu + 3 * r, npasses,
+                                      kaprho + (size_t)b * N, S + (size_t)b * N, NULL, 0, I);
+            if (err[q] == 0 && Itop && upidx[r] >= 0) {
+                double* dst = Itop + ((size_t)b * nup + upidx[r]) * ny * nx;
+                memcpy(dst, I + (size_t)(nz - 1) * ny * nx, sizeof(double) * ny * nx);
             }
         }
-        free(I);
+        for (q = 0; q < nb_; ++q) if (err[q] != 0) fail = err[q];
+        if (fail != 0) break;
+        /* J_b += w_r I_r and F += 4 pi w_r Omega_r I_r, in (band, ray) order at every node */
+        long n;
+#pragma omp parallel for schedule(static)
+        for (n = 0; n < (long)N; ++n) {
+            for (int qq = 0; qq < nb_; ++qq) {
+                const int task = t0 + qq, b = task / nrays, r = task % nrays;
+                const double Iv = Ibuf[(size_t)qq * N + n];
+                J[(size_t)b * N + n] += wq[r] * Iv;
+                if (Fout) {
+                    const double* m = mu + 3 * r;
+                    const double nrm = sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+                    for (int a = 0; a < 3; ++a) Fout[(size_t)a * N + n] += 4.0 * ORACLE_PI * wq[r] * (m[a] / nrm) * Iv;
+                }
+            }
+        }
     }
     if (fail == 0) {
         long n;
@@ -321,8 +342,56 @@ int oracle_solve(int nx, int ny, int nz, double dx, double dy, double dz,
         }
         if (Jout) memcpy(Jout, J, sizeof(double) * N * nb);
     }
-    free(kaprho); free(S); free(J); free(upidx);
+    free(kaprho); free(S); free(J); free(upidx); free(Ibuf); free(err);
     return fail;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-11  Flux-divergence heating and its blend with the J - S form (
+ *       DESIGN.md reading R21).  On the node grid:
+ *         Qdiv = -(dFx/dx + dFy/dy + dFz/dz),
+ *       central differences, periodic in x and y; on the bottom / top node plane the z
+ *       derivative is the one-sided difference over one spacing.
+ *         Qblend = w Q_J + (1 - w) Qdiv,   w(k) = exp(-taubar(k) / tau0),
+ *       taubar(k) = sum_{k' >= k} <kaprho_0>(k') dz: the horizontally averaged optical depth of
+ *       band 0 from the top down to (and including) level k.  kaprho0: [N] band-0 kaprho.
+ *       Qdiv / Qblend may be NULL.
+ * ------------------------------------------------------------------------- */
+int oracle_flux_heating(int nx, int ny, int nz, double dx, double dy, double dz,
+                        const double* F, const double* QJ, const double* kaprho0, double tau0,
+                        double* Qdiv, double* Qblend)
+{
+    if (nx < 2 || ny < 2 || nz < 2 || !F) return -1;
+    const size_t N = (size_t)nx * ny * nz;
+    const double* Fx = F; const double* Fy = F + N; const double* Fz = F + 2 * N;
+    double* w = (double*)malloc(sizeof(double) * nz);
+    if (!w) return -2;
+    if (Qblend) {
+        if (!QJ || !kaprho0 || !(tau0 > 0.0)) { free(w); return -1; }
+        double tau = 0.0;
+        for (int k = nz - 1; k >= 0; --k) {
+            double s = 0.0;
+            for (size_t n = 0; n < (size_t)nx * ny; ++n) s += kaprho0[(size_t)k * nx * ny + n];
+            tau += s / ((double)nx * ny) * dz;
+            w[k] = exp(-tau / tau0);
+        }
+    }
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const size_t n = ((size_t)k * ny + j) * nx + i;
+                const int ip = (i + 1) % nx, im = (i - 1 + nx) % nx;
+                const int jp = (j + 1) % ny, jm = (j - 1 + ny) % ny;
+                const int kp = (k + 1 < nz) ? k + 1 : k, km = (k > 0) ? k - 1 : k;
+                const double dfx = (Fx[((size_t)k * ny + j) * nx + ip] - Fx[((size_t)k * ny + j) * nx + im]) / (2.0 * dx);
+                const double dfy = (Fy[((size_t)k * ny + jp) * nx + i] - Fy[((size_t)k * ny + jm) * nx + i]) / (2.0 * dy);
+                const double dfz = (Fz[((size_t)kp * ny + j) * nx + i] - Fz[((size_t)km * ny + j) * nx + i]) / (dz * (double)(kp - km));
+                const double qd = -(dfx + dfy + dfz);
+                if (Qdiv) Qdiv[n] = qd;
+                if (Qblend) Qblend[n] = w[k] * QJ[n] + (1.0 - w[k]) * qd;
+            }
+    free(w);
+    return 0;
 }
 
 /* ---------------------------------------------------------------------------

@@ -36,7 +36,7 @@ struct TypePlan {        // per march axis
 
 struct HostUnit {
     UnitDesc d;
-    size_t off_xex, off_g;   // workspace offsets of its exchange planes and seam histories
+    size_t off_xex, off_g, off_part;   // workspace offsets of its exchange planes, seam histories, partial heating
 };
 
 }  // namespace
@@ -46,6 +46,8 @@ struct rts_ctx {
     double h[3] = {0, 0, 0};
     int npass = 3;
     bool thick_skip = true;
+    bool flux = false;           // radiative flux wanted (rts_enable_flux): three more partial fields per unit
+    double tau0 = 0.1;           // blend scale of the flux-divergence heating
     std::vector<HostRay> rays;
     int n_up = 0;
     // tables
@@ -68,7 +70,7 @@ struct rts_ctx {
     int PX = 0, PY = 0, PYR = 0;
     size_t ws_bytes = 0;
     // workspace offsets
-    size_t off_coefA = 0, off_coefB = 0, off_QB = 0, off_ksum = 0, off_kmin = 0, off_lev = 0, off_kstar = 0, off_mthick = 0, off_mthick_b = 0, off_abort = 0,
+    size_t off_coefA = 0, off_coefB = 0, off_partptr = 0, off_parttr = 0, off_ksum = 0, off_kmin = 0, off_lev = 0, off_kstar = 0, off_mthick = 0, off_mthick_b = 0, off_abort = 0,
            off_units = 0, off_bar = 0, off_stage_in = 0, off_stage_out = 0;
     int nblk_a = 0;
     // workspace
@@ -141,6 +143,8 @@ void make_ray_consts(const HostRay& r, RayC& rc)
     const int ord[4] = {2, 3, 0, 1};
     for (int q = 0; q < 4; ++q) rc.w[q] = (float)w[ord[q]];
     rc.kc = (float)(0.5 * r.ds);
+    const double nrm = std::sqrt(r.mu[0] * r.mu[0] + r.mu[1] * r.mu[1] + r.mu[2] * r.mu[2]);
+    for (int a = 0; a < 3; ++a) rc.mu[a] = (float)(r.mu[a] / nrm);
     rc.wq = (float)r.w;
     rc.active = 1;
     rc.up = r.up;
@@ -208,7 +212,6 @@ int make_plan(rts_ctx* c)
     c->PY = (int)align_up((size_t)c->ny, 4) + 2 * HALO;
     c->PYR = c->ny + 2 * HALO;
     c->K = c->user_K ? c->user_K : KMAX;
-    if (const char* e_ = getenv("RTS_TUNE_RC")) c->user_rc = atoi(e_);   // TUNING ONLY
 
     // --- unit skeletons: (march, dir) groups, sub-units with <= 1 ray per slot
     struct Group { int march, dir; std::vector<std::vector<int>> sub; };
@@ -342,7 +345,6 @@ int make_plan(rts_ctx* c)
     const size_t fB = (size_t)c->nz * c->nx * c->PY;
     c->off_coefA = take(sizeof(float2) * fA * 2 * c->nbp);
     c->off_coefB = take(sizeof(float2) * fB * 2 * c->nbp);
-    c->off_QB = take(sizeof(float) * N);
     c->nblk_a = ((c->nx + 31) / 32) * ((c->ny + 31) / 32);
     c->off_ksum = take(sizeof(double) * (size_t)c->nb * c->nz * c->nblk_a);
     c->off_kmin = take(sizeof(float) * (size_t)c->nb * c->nz * c->nblk_a);
@@ -384,12 +386,15 @@ int make_plan(rts_ctx* c)
                         if (only_su == 0 || c->rays[ri].su == only_su) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
                     hu.off_xex = take(sizeof(float2) * 2 * NSLOT * (size_t)d.n_v * d.n_u2);
                     hu.off_g = take(sizeof(float2) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u2));
+                    hu.off_part = take(sizeof(float) * N * (c->flux ? 4 : 1));
                     c->units.push_back(hu);
                 }
             }
     c->total_tickets = ticket;
     c->grid = std::min(slots, c->total_tickets);
     c->off_units = take(sizeof(UnitDesc) * c->units.size());
+    c->off_partptr = take(sizeof(float*) * c->units.size());
+    c->off_parttr = take(sizeof(int) * c->units.size());
     c->off_bar = take(sizeof(int) * c->units.size());
     c->off_stage_in = take(sizeof(float) * N * 3);
     c->off_stage_out = take(sizeof(float) * (N + (size_t)c->nb * c->n_up * c->ny * c->nx));
@@ -408,6 +413,8 @@ int bind_workspace(rts_ctx* c)
         d.Xex = (float*)(ws + hu.off_xex);
         d.Gu = (float*)(ws + hu.off_g);
         d.barrier = (int*)(ws + c->off_bar) + i;
+        d.Qpart = (float*)(ws + hu.off_part);
+        d.Fpart = c->flux ? d.Qpart + (size_t)c->nx * c->ny * c->nz : nullptr;
         d.kstar = (const int*)(ws + c->off_kstar) + d.pair;
         d.mthick = (const int*)(ws + c->off_mthick) + 3 * d.pair;
         // carried strips and seam histories must hold finite numbers from the start: planes that are
@@ -417,6 +424,12 @@ int bind_workspace(rts_ctx* c)
         flat.push_back(d);
     }
     CUDA_TRY(c, cudaMemcpy(ws + c->off_units, flat.data(), sizeof(UnitDesc) * flat.size(), cudaMemcpyHostToDevice));
+    {
+        std::vector<float*> pp; std::vector<int> tr;
+        for (auto& d : flat) { pp.push_back(d.Qpart); tr.push_back(d.q_in_B); }
+        CUDA_TRY(c, cudaMemcpy(ws + c->off_partptr, pp.data(), sizeof(float*) * pp.size(), cudaMemcpyHostToDevice));
+        CUDA_TRY(c, cudaMemcpy(ws + c->off_parttr, tr.data(), sizeof(int) * tr.size(), cudaMemcpyHostToDevice));
+    }
     // coefficient tensors for the TMA engine (fp32 elements, two per node): layout A as (x, y rows, z, field)
     // with the box of the z-march (x, y) or of the y-march (x, z); layout B as (y, x, z, field) with the
     // x-march box (y, z)
@@ -685,13 +698,17 @@ int rts_coefficients(rts_ctx* c, const float* rho, const float* T, const float* 
     return launch_stage_a(c, rho, T, P, kaprho, S, as_stream(stream));
 }
 
-int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, float* Q, float* Itop, void* stream)
+namespace {
+int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, float* Q, float* Itop,
+               float* F, float* Qdiv, float* Qblend, void* stream)
 {
     if (!c) return RTS_EINVAL;
     if (!rho || !T || !P || !Q) return fail(c, RTS_EINVAL, "rts_solve: null pointer");
     if (!c->have_tables) return fail(c, RTS_ESTATE, "rts_solve: tables not set");
     if (!c->ws || !c->planned || !c->maps_ready) return fail(c, RTS_ESTATE, "rts_solve: workspace not set (or configuration changed since)");
     if (((uintptr_t)Q & 15u) != 0) return fail(c, RTS_EINVAL, "rts_solve: Qrad must be 16-byte aligned");
+    if ((F || Qdiv || Qblend) && !c->flux) return fail(c, RTS_ESTATE, "rts_solve_flux: call rts_enable_flux before sizing the workspace");
+    if ((Qdiv || Qblend) && !F) return fail(c, RTS_EINVAL, "rts_solve_flux: Qdiv / Qblend need Frad");
     cudaStream_t st = as_stream(stream);
     const size_t N = (size_t)c->nx * c->ny * c->nz;
     unsigned char* ws = c->ws;
@@ -718,10 +735,6 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     CUDA_TRY(c, cudaGetLastError());
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[1], st));
 
-    // outputs start from zero; x-march sweeps accumulate into the y-fastest QB
-    float* QB = (float*)(ws + c->off_QB);
-    CUDA_TRY(c, cudaMemsetAsync(Q, 0, N * sizeof(float), st));
-    CUDA_TRY(c, cudaMemsetAsync(QB, 0, N * sizeof(float), st));
     CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 8, st));
 
     CUDA_TRY(c, cudaMemsetAsync(ws + c->off_bar, 0, sizeof(int) * c->units.size(), st));
@@ -732,7 +745,7 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
         int* abortf = (int*)(ws + c->off_abort);
         int* ticket = abortf + 1;
         int nunits = (int)c->units.size(), total = c->total_tickets;
-        void* args[] = {&c->maps, &dunits, &nunits, &total, &ticket, &Q, &QB, &Itop, &abortf};
+        void* args[] = {&c->maps, &dunits, &nunits, &total, &ticket, &Itop, &abortf};
         // cooperative launch: every CTA of the grid is resident, which the tile barriers rely on
         CUDA_TRY(c, cudaLaunchCooperativeKernel(sweep_fn(c->pitch), dim3(c->grid), dim3(c->threads), args,
                                                 (size_t)c->smem_bytes, st));
@@ -740,12 +753,56 @@ int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, floa
     // finalize
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[3], st));
     {
+        // the units' partial heating (and flux) summed in unit order: deterministic
+        FinalizeParams fp{};
+        fp.part = (const float* const*)(ws + c->off_partptr); fp.transposed = (const int*)(ws + c->off_parttr);
+        fp.nunits = (int)c->units.size(); fp.nf = F ? 4 : 1;
+        fp.nx = c->nx; fp.ny = c->ny; fp.nz = c->nz;
+        fp.out[0] = Q;
+        for (int a = 0; a < 3; ++a) fp.out[1 + a] = F ? F + (size_t)a * N : nullptr;
         dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, c->nz), block(32, 8);
-        rts_finalize_kernel<<<grid, block, 0, st>>>(Q, QB, c->nx, c->ny, c->nz);
+        rts_finalize_kernel<<<grid, block, 0, st>>>(fp);
         CUDA_TRY(c, cudaGetLastError());
+        if (Qdiv || Qblend) {
+            dim3 g2((c->nx + 255) / 256, c->ny, c->nz);
+            rts_fluxdiv_kernel<<<g2, 256, 0, st>>>(F, Q, Qdiv, Qblend, (const double*)(ws + c->off_lev), c->nx, c->ny, c->nz,
+                                                   (float)c->h[0], (float)c->h[1], (float)c->h[2],
+                                                   1.0 / ((double)c->nx * c->ny), c->h[2], c->tau0);
+            CUDA_TRY(c, cudaGetLastError());
+        }
     }
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[4], st));
     return RTS_OK;
+}
+}  // namespace
+
+int rts_solve(rts_ctx* c, const float* rho, const float* T, const float* P, float* Q, float* Itop, void* stream)
+{
+    return solve_impl(c, rho, T, P, Q, Itop, nullptr, nullptr, nullptr, stream);
+}
+
+int rts_enable_flux(rts_ctx* c, int on)
+{
+    if (!c) return RTS_EINVAL;
+    c->flux = on != 0;
+    c->planned = false;
+    return RTS_OK;
+}
+
+int rts_set_flux_blend(rts_ctx* c, double tau0)
+{
+    if (!c) return RTS_EINVAL;
+    if (!(tau0 > 0.0)) return fail(c, RTS_EINVAL, "rts_set_flux_blend: tau0 must be positive");
+    c->tau0 = tau0;
+    return RTS_OK;
+}
+
+int rts_solve_flux(rts_ctx* c, const float* rho, const float* T, const float* P, float* Q, float* Itop,
+                   float* Frad, float* Qdiv, float* Qblend, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    if (!Frad) return fail(c, RTS_EINVAL, "rts_solve_flux: null Frad");
+    return solve_impl(c, rho, T, P, Q, Itop, Frad, Qdiv, Qblend, stream);
 }
 
 int rts_set_thick_skip(rts_ctx* c, int on)

@@ -45,7 +45,7 @@ struct alignas(16) RayC {
     int   active;
     int   up;         // mu_z > 0
     int   itop;       // index among the upward rays, or -1
-    int   pad0, pad1, pad2;
+    float mu[3];      // unit direction of photon travel (x, y, z): radiative flux
 };
 
 // One sweep unit: the (at most four) rays that march along `march` in direction `dir`, for one
@@ -67,6 +67,9 @@ struct UnitDesc {
     float* Xex;       // float2 [2][NSLOT][n_v][n_u2]   carried planes at block ends (strips only)
     float* Gu;        // float2 [2][n_m][NSLOT*n_v + NSLOT*n_u2]  per pass parity and plane: far-u column
                       //                                of every slot, then (per_v only) far-v row of every slot
+    float* Qpart;     // [N] heating of this unit alone, in the unit's own layout (x- or y-fastest): every node is
+                      // written exactly once per solve, the units are summed in a fixed order by rts_finalize_kernel
+    float* Fpart;     // [3][N] radiative flux of this unit alone (same layout), or null
     int*   barrier;   // arrivals of this unit's tiles (monotonic)
     const int* kstar; // device: switch height of this band pair
     const int* mthick;// device: thick level pairs from the bottom of this band pair (z-march plane skipping)
@@ -341,22 +344,81 @@ __global__ void __launch_bounds__(256) rts_kstar_kernel(const KstarParams p)
 }
 
 // =========================================================================== K_f
-// Q[k][j][i] += QB[k][i][j]  (QB = heating of the x-march sweeps, stored y-fastest)
-__global__ void __launch_bounds__(256) rts_finalize_kernel(float* Q, const float* QB, int nx, int ny, int nz)
+// Q[k][j][i] = sum over the sweep units, in unit order, of the unit's partial heating (deterministic: no
+// atomics anywhere on the heating path).  The partials of the x-march units are stored y-fastest
+// ([nz][nx][ny]) and are transposed through shared memory.  nf fields per unit (1: Q; 4: Q, Fx, Fy, Fz):
+// part[u] points at the unit's first field, the fields are N floats apart; out[f] may be null.
+struct FinalizeParams {
+    const float* const* part;   // device [nunits] partial buffers
+    const int* transposed;      // device [nunits] 1: y-fastest layout
+    int nunits, nf;
+    int nx, ny, nz;
+    float* out[4];
+};
+__global__ void __launch_bounds__(256) rts_finalize_kernel(const FinalizeParams p)
 {
     __shared__ float tile[32][33];
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32, k = blockIdx.z;
+    const size_t N = (size_t)p.nx * p.ny * p.nz;
+    for (int f = 0; f < p.nf; ++f) {
+        if (!p.out[f]) continue;
+        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int u = 0; u < p.nunits; ++u) {
+            const float* src = p.part[u] + (size_t)f * N;
+            if (p.transposed[u]) {
+                __syncthreads();
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const int i = i0 + ty + 8 * r, j = j0 + tx;
-        if (i < nx && j < ny) tile[ty + 8 * r][tx] = QB[((size_t)k * nx + i) * ny + j];
+                for (int r = 0; r < 4; ++r) {
+                    const int i = i0 + ty + 8 * r, j = j0 + tx;
+                    if (i < p.nx && j < p.ny) tile[ty + 8 * r][tx] = __ldcs(src + ((size_t)k * p.nx + i) * p.ny + j);
+                }
+                __syncthreads();
+#pragma unroll
+                for (int r = 0; r < 4; ++r) acc[r] += tile[tx][ty + 8 * r];
+            } else {
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int j = j0 + ty + 8 * r, i = i0 + tx;
+                    if (i < p.nx && j < p.ny) acc[r] += __ldcs(src + ((size_t)k * p.ny + j) * p.nx + i);
+                }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int j = j0 + ty + 8 * r, i = i0 + tx;
+            if (i < p.nx && j < p.ny) p.out[f][((size_t)k * p.ny + j) * p.nx + i] = acc[r];
+        }
     }
-    __syncthreads();
-#pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const int j = j0 + ty + 8 * r, i = i0 + tx;
-        if (i < nx && j < ny) Q[((size_t)k * ny + j) * nx + i] += tile[tx][ty + 8 * r];
+}
+
+// =========================================================================== K_d (NEXT #2)
+// Flux-divergence heating and its blend with the J - S form (paper's Flux; reading R21):
+//   Qdiv = -(dFx/dx + dFy/dy + dFz/dz), central differences on the node grid, periodic in x and y, one-sided
+//   on the bottom and top node planes;  Qblend = w Q_J + (1 - w) Qdiv with w(k) = exp(-taubar(k)/tau0),
+//   taubar(k) = horizontally averaged optical depth of band 0 from the top down to level k (K_k's level sums).
+// Any of Qdiv / Qblend may be null.
+__global__ void __launch_bounds__(256) rts_fluxdiv_kernel(const float* __restrict__ F, const float* __restrict__ QJ,
+                                                          float* __restrict__ Qdiv, float* __restrict__ Qblend,
+                                                          const double* __restrict__ lev0, int nx, int ny, int nz,
+                                                          float hx, float hy, float hz, double inv_nxy, double dz, double tau0)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i >= nx) return;
+    const size_t N = (size_t)nx * ny * nz, row = ((size_t)k * ny + j) * nx;
+    const int ip = (i + 1 == nx) ? 0 : i + 1, im = (i == 0) ? nx - 1 : i - 1;
+    const int jp = (j + 1 == ny) ? 0 : j + 1, jm = (j == 0) ? ny - 1 : j - 1;
+    const float dfx = (F[row + ip] - F[row + im]) * (0.5f / hx);
+    const float dfy = (F[N + ((size_t)k * ny + jp) * nx + i] - F[N + ((size_t)k * ny + jm) * nx + i]) * (0.5f / hy);
+    const int kp = min(k + 1, nz - 1), km = max(k - 1, 0);
+    const float dfz = (F[2 * N + ((size_t)kp * ny + j) * nx + i] - F[2 * N + ((size_t)km * ny + j) * nx + i]) / (hz * (float)(kp - km));
+    const float qd = -(dfx + dfy + dfz);
+    if (Qdiv) Qdiv[row + i] = qd;
+    if (Qblend) {
+        double tau = 0.0;
+        for (int kk = nz - 1; kk >= k; --kk) tau += lev0[kk] * inv_nxy * dz;
+        const float w = (float)exp(-tau / tau0);
+        Qblend[row + i] = w * QJ[row + i] + (1.f - w) * qd;
     }
 }
 

@@ -13,16 +13,15 @@
 //   seams = stencil nodes across a periodic boundary come from the previous pass (Jacobi):
 //           far columns / rows of every plane are kept in G (pass parity) and copied into the
 //           ghost column / row of the carried plane before each step.
-//   group = the rays of a unit with the same su (at most two: sv = +1, -1).  The warps of a CTA are
-//           split between the groups, so su is warp-uniform.
-//   item  = a 2 x 2 node block of one group: the thread-level unit of work.  Every thread owns the
-//           same (at most two) items for the whole task; their descriptors live in registers.
-//           The (kaprho, S) neighbourhood of an item is loaded once and serves both rays and both
-//           bands: every value is a float2 (bands 2p, 2p+1) and all arithmetic is packed (f32x2).
-// Shared-memory layout (PITCH = nodes per box row, a compile-time constant, so that every load of an
-// item is one base register plus an immediate):
-//   coefficient stage   [BV rows][kaprho row | S row][PITCH] float2      one TMA box per plane
-//   carried planes      [2 buffers][group][BV rows][ray sv>0 row | ray sv<0 row][PITCH] float2
+//   strip = the thread-level unit of work: one node pair (two columns) of one ray, the rows of one row chunk,
+//           marched from the upwind end of the v axis.  The upwind rows of kaprho, S and X stay in registers
+//           (sliding window), so a row costs one row load of each; whole warps belong to one ray, so the
+//           ray's signs are warp-uniform.  Every value is a float2 (bands 2p, 2p+1) and all arithmetic is
+//           packed (f32x2).  Every thread owns the same strip for the whole task (descriptors in registers).
+// Shared-memory layout (PITCH = nodes per box row, a compile-time constant, so that every load of a strip
+// is one base register plus an immediate):
+//   coefficient stage   [BV rows][kaprho row | S row][PITCH] float2      one 5-D TMA box per plane
+//   carried planes      [2 buffers][su group][BV rows][ray sv>0 row | ray sv<0 row][PITCH] float2
 // Carried quantity: X = I - a*S with a = 1 at levels k <= kstar (optically thick part, where
 // J - S would cancel) and a = 0 above (thin part, where I << S would cancel).
 #pragma once
@@ -111,10 +110,6 @@ template <int SU, int J> __device__ __forceinline__ f2 sid(const Row3& r)
 {
     return (SU > 0) ? (J == 0 ? r.sd : r.n0) : (J == 0 ? r.n1 : r.sd);
 }
-__device__ __forceinline__ void red_add2(float* p, const float a, const float b)
-{
-    asm volatile("red.relaxed.gpu.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
-}
 
 // watchdog for every wait loop: gives up after ~2^22 unsuccessful probes (seconds) and raises
 // the device-side abort flag so that all CTAs drain instead of hanging the GPU
@@ -171,7 +166,7 @@ struct TaskShared {
     f2* stage0;                        // [nstage] coefficient plane sets
     f2* Xb;                            // [2][ng] carried plane sets
     GhostEnt* gt; HaloEnt* ht;
-    float* Qdst; float* Itop_b;
+    float* Itop_b; float* pad2;
     int* abortf; int* pad1;
 };
 
@@ -471,8 +466,9 @@ __device__ __forceinline__ f2 ghost_fetch(const TaskShared& S, const GhostEnt g,
     return __ldcg(reinterpret_cast<const f2*>(U.Gu) + ((size_t)(psrc & 1) * U.n_m + msrc) * g_plane + (g.goff & 0x0fffffff));
 }
 
-// Heating and emergent intensity of a finished plane (last pass; out of line): reads the new carried
-// plane set Xn (one buffer) and that plane's coefficient stage Kc.
+// Heating, radiative flux and emergent intensity of a finished plane (last pass; out of line): reads the new
+// carried plane set Xn (one buffer) and that plane's coefficient stage Kc.  The unit's contribution goes to its
+// own partial buffers with plain stores: every node is written exactly once, no atomics (deterministic).
 template <int PITCH>
 __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2* __restrict__ Kc, const f2* __restrict__ Xn, const int m_done)
 {
@@ -484,8 +480,10 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
     const int nqc = (G.wu + 1) >> 1;
     const float qb1 = (U.nband_ok == 2) ? FOUR_PI : 0.f;
     const bool zmarch = G.zmarch != 0;
-    float* const Qdst = S.Qdst;
+    float* const Qdst = U.Qpart;
+    float* const Fdst = U.Fpart;
     float* const Itop_b = S.Itop_b;
+    const long long Nn = (long long)U.n_m * U.n_u * U.n_v;
     for (int e = tid; e < nqc * G.wv; e += T) {
         const int row = e / nqc, q = e - row * nqc;
         const int bo = (HALO + row) * RPN + HALO + 2 * q;
@@ -496,7 +494,11 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
         const float a_p = zmarch ? a_of(G, pl) : a_of(G, v);
         const float shs = 1.0f - a_p;
         f2 acc0 = make_float2(0.f, 0.f), acc1 = make_float2(0.f, 0.f);    // node 0 / node 1, per band
+        f2 fl0[3], fl1[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { fl0[a] = make_float2(0.f, 0.f); fl1[a] = make_float2(0.f, 0.f); }
         const f2 s0 = mul2(bc(shs), make_float2(sp.x, sp.y)), s1 = mul2(bc(shs), make_float2(sp.z, sp.w));
+        const f2 as0 = mul2(bc(a_p), make_float2(sp.x, sp.y)), as1 = mul2(bc(a_p), make_float2(sp.z, sp.w));
 #pragma unroll
         for (int s = 0; s < NSLOT; ++s) {
             if (!U.ray[s].active) continue;
@@ -504,6 +506,15 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
             const float wq = U.ray[s].wq;
             acc0 = fma2(bc(wq), sub2(make_float2(x.x, x.y), s0), acc0);       // w_r (I - S)
             acc1 = fma2(bc(wq), sub2(make_float2(x.z, x.w), s1), acc1);
+            if (Fdst) {
+                const f2 i0 = add2(make_float2(x.x, x.y), as0), i1 = add2(make_float2(x.z, x.w), as1);   // I = X + a S
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const float wm = wq * U.ray[s].mu[a];
+                    fl0[a] = fma2(bc(wm), i0, fl0[a]);
+                    fl1[a] = fma2(bc(wm), i1, fl1[a]);
+                }
+            }
             if (Itop_b && U.ray[s].itop >= 0) {
                 const bool top = zmarch ? (m_done == U.n_m - 1 && G.up_z) : (v == U.nz - 1 && !(s & 2));
                 if (top) {
@@ -519,11 +530,20 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
                 }
             }
         }
-        float* qd = Qdst + (long long)pl * U.q_sm + (long long)v * U.q_sv + u;
+        const long long qo = (long long)pl * U.q_sm + (long long)v * U.q_sv + u;
         const float q0 = FOUR_PI * kp.x * acc0.x + qb1 * kp.y * acc0.y;
         const float q1 = FOUR_PI * kp.z * acc1.x + qb1 * kp.w * acc1.y;
-        if (U.qvec && nval == 2) red_add2(qd, q0, q1);
-        else { atomicAdd(qd, q0); if (nval == 2) atomicAdd(qd + 1, q1); }
+        if (U.qvec && nval == 2) *reinterpret_cast<float2*>(Qdst + qo) = make_float2(q0, q1);
+        else { Qdst[qo] = q0; if (nval == 2) Qdst[qo + 1] = q1; }
+        if (Fdst) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const float f0 = FOUR_PI * fl0[a].x + qb1 * fl0[a].y, f1 = FOUR_PI * fl1[a].x + qb1 * fl1[a].y;
+                float* fd = Fdst + (long long)a * Nn + qo;
+                if (U.qvec && nval == 2) *reinterpret_cast<float2*>(fd) = make_float2(f0, f1);
+                else { fd[0] = f0; if (nval == 2) fd[1] = f1; }
+            }
+        }
     }
 }
 
@@ -674,10 +694,9 @@ __device__ __forceinline__ void issue_load(TaskShared& S, const CUtensorMap* cma
 
 template <int PITCH>
 __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f2* __restrict__ smf,
-                         float* __restrict__ Qa, float* __restrict__ Qb, float* __restrict__ Itop_all,
-                         int* abortf)
+                         float* __restrict__ Itop_all, int* abortf)
 {
-    constexpr int RPN = 2 * PITCH;                           // nodes between box rows
+
     const UnitDesc& U = S.U;
     const int tid = threadIdx.x, T = blockDim.x;
     const SmemPlan SP(PITCH, U.WU, U.WV, U.ng, U.nstage);
@@ -699,7 +718,6 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
         S.Xb = S.stage0 + NST * PS;                          // [2][NG] plane sets (ray sv>0 | ray sv<0)
         S.gt = reinterpret_cast<GhostEnt*>(smf + SP.nodes());
         S.ht = reinterpret_cast<HaloEnt*>(S.gt + SP.nghost_max);
-        S.Qdst = U.q_in_B ? Qb : Qa;
         S.Itop_b = Itop_all ? Itop_all + (long long)(2 * U.pair) * U.it_sb : nullptr;
         S.abortf = abortf;
         for (int i = 0; i < NST; ++i) mbar_init(&S.mbar[i], 1);
@@ -898,8 +916,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
 template <int PITCH>
 __global__ void __launch_bounds__(RTS_SWEEP_THREADS, 1)
 rts_sweep_kernel(const __grid_constant__ SweepMaps maps, const UnitDesc* __restrict__ units, int nunits,
-                 int total_tickets, int* ticket_counter,
-                 float* __restrict__ Qa, float* __restrict__ Qb, float* __restrict__ Itop_all, int* abortf)
+                 int total_tickets, int* ticket_counter, float* __restrict__ Itop_all, int* abortf)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(16) TaskShared S;
@@ -924,7 +941,7 @@ rts_sweep_kernel(const __grid_constant__ SweepMaps maps, const UnitDesc* __restr
             for (int w = threadIdx.x; w < (int)(sizeof(UnitDesc) / sizeof(int)); w += blockDim.x) dst[w] = src[w];
         }
         __syncthreads();
-        run_task<PITCH>(S, maps, ticket - S.U.ticket_begin, reinterpret_cast<f2*>(smem_raw), Qa, Qb, Itop_all, abortf);
+        run_task<PITCH>(S, maps, ticket - S.U.ticket_begin, reinterpret_cast<f2*>(smem_raw), Itop_all, abortf);
     }
 }
 

@@ -26,6 +26,7 @@ EXPORTS = [
     "rts_set_workspace", "rts_solve", "rts_solve_host", "rts_coefficients", "rts_sync_check",
     "rts_plan_info", "rts_last_error", "rts_enable_timing", "rts_last_timing",
     "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells", "rts_set_thick_skip", "rts_thick_levels",
+    "rts_enable_flux", "rts_set_flux_blend", "rts_solve_flux",
 ]
 
 
@@ -92,6 +93,12 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_set_thick_skip.argtypes = [c_void_p, c_int]
     lib.rts_thick_levels.restype = c_int
     lib.rts_thick_levels.argtypes = [c_void_p, PI, c_void_p]
+    lib.rts_enable_flux.restype = c_int
+    lib.rts_enable_flux.argtypes = [c_void_p, c_int]
+    lib.rts_set_flux_blend.restype = c_int
+    lib.rts_set_flux_blend.argtypes = [c_void_p, c_double]
+    lib.rts_solve_flux.restype = c_int
+    lib.rts_solve_flux.argtypes = [c_void_p] + [c_void_p] * 8 + [c_void_p]
     lib.rts_last_error.restype = ctypes.c_char_p
     lib.rts_last_error.argtypes = [c_void_p]
     _lib = lib
@@ -227,6 +234,30 @@ class RTS:
                                         self._stream()), "rts_solve")
         return Q, (Itop if want_itop else None)
 
+    def enable_flux(self, on: bool = True):
+        """Must precede allocate_workspace (three more partial fields per sweep unit)."""
+        self._check(self._lib.rts_enable_flux(self._ctx, 1 if on else 0), "rts_enable_flux")
+        self._ws = None
+
+    def set_flux_blend(self, tau0: float):
+        self._check(self._lib.rts_set_flux_blend(self._ctx, float(tau0)), "rts_set_flux_blend")
+
+    def solve_flux(self, rho, T, P, want_div: bool = True, want_blend: bool = True):
+        """rts_solve_flux: returns (Q, Itop, F[3][nz][ny][nx], Qdiv or None, Qblend or None) as CUDA tensors."""
+        torch = self._torch
+        if self._ws is None:
+            self.allocate_workspace()
+        shp = (self.nz, self.ny, self.nx)
+        Q = torch.empty(shp, dtype=torch.float32, device="cuda")
+        Itop = torch.empty((self.nbands, self.num_up_rays(), self.ny, self.nx), dtype=torch.float32, device="cuda")
+        F = torch.empty((3,) + shp, dtype=torch.float32, device="cuda")
+        Qd = torch.empty(shp, dtype=torch.float32, device="cuda") if want_div else None
+        Qb = torch.empty(shp, dtype=torch.float32, device="cuda") if want_blend else None
+        p = lambda t: ctypes.c_void_p(t.data_ptr()) if t is not None else None
+        self._check(self._lib.rts_solve_flux(self._ctx, p(rho), p(T), p(P), p(Q), p(Itop), p(F), p(Qd), p(Qb), self._stream()),
+                    "rts_solve_flux")
+        return Q, Itop, F, Qd, Qb
+
     def solve_host(self, rho, T, P, Q, Itop=None):
         """Host numpy / pinned torch buffers in and out (copies inside the call, synchronous)."""
         if self._ws is None:
@@ -316,7 +347,7 @@ class RTS:
 
 
 def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchange_interval: int = 0,
-                cells: bool = False, ring_depth: int = 0) -> "RTS":
+                cells: bool = False, ring_depth: int = 0, flux: bool = False) -> "RTS":
     """Create and configure a solver for an `inputs.RTSInputs` problem.  cells=True: the fields of
     `inp` are cell-centred (solve_cells); the RT node grid then has one level more."""
     r = RTS(inp.nx, inp.ny, inp.nz + (1 if cells else 0), inp.dx, inp.dy, inp.dz, inp.nbands)
@@ -332,5 +363,7 @@ def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchan
         r.set_exchange_interval(exchange_interval)
     if ring_depth:
         r.set_ring_depth(ring_depth)
+    if flux:
+        r.enable_flux(True)
     r.allocate_workspace()
     return r

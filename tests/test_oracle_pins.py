@@ -543,3 +543,115 @@ def test_O9_solve_cells_of_horizontally_uniform_atmosphere_is_uniform():
     Qc, Itop, node = oracle.solve_cells(inp)
     assert node.nz == inp.nz + 1 and Qc.shape == inp.shape
     assert np.abs(Qc - Qc[:, :1, :1]).max() <= 1e-9 * np.abs(Qc).max()
+
+
+# --------------------------------------------------------------------------- O-10 / O-11 (NEXT #2): flux
+def _flat_table_problem(nx, ny, nz, dx, dy, dz, S3, kaprho, P=8, nb=1):
+    """Inputs whose stage A gives kaprho = const and S = S3 exactly up to the fp32 rounding of T:
+    flat opacity table (log10 kappa = 0), rho = kaprho, band fraction 1, T = (pi S / sigma)^(1/4)."""
+    T = (math.pi * S3 / 5.670374e-5) ** 0.25
+    rho = np.full((nz, ny, nx), kaprho)
+    Pg = np.full((nz, ny, nx), 1.0e4)
+    logk = np.zeros((nb, 4, 4), dtype=np.float32)
+    bf = np.ones((nb, 4), dtype=np.float32)
+    return inputs.make_custom(nx, ny, nz, dx, dy, dz, rho, T, Pg, logk, bf, (3.0, 5.0), (2.0, 6.0), npasses=P)
+
+
+def test_O10_flux_of_tilted_linear_source_in_the_thick_limit():
+    """P3 for all three components: with S linear in space and uniform kaprho every ray carries
+    D_r = -Omega_r . grad S / kaprho (bilinear interpolation is exact on linear fields), so
+    F = 4 pi sum_r w_r Omega_r I_r = -(4 pi / 3) (1 + 7.1e-8) grad S / kaprho  (second moment of the ray set)."""
+    nx, ny, nz = 16, 16, 20
+    dx, dy, dz = 48 * KM, 40 * KM, 32 * KM
+    kr = 8.0 / dz
+    gx, gy, gz = 1.1e3 / dx, -0.7e3 / dy, 2.0e3 / dz
+    z, y, x = np.meshgrid(np.arange(nz) * dz, np.arange(ny) * dy, np.arange(nx) * dx, indexing="ij")
+    S3 = 6.0e5 + gx * x + gy * y + gz * z
+    inp = _flat_table_problem(nx, ny, nz, dx, dy, dz, S3, kr)
+    Q, Itop, F = oracle.solve(inp, want_F=True)
+    c = -(4 * math.pi / 3) * (1 + 7.1e-8) / kr
+    sl = (slice(6, nz - 6), slice(5, ny - 5), slice(5, nx - 5))      # away from the seams (gradient jump) and the inflow planes
+    for a, g in enumerate((gx, gy, gz)):
+        assert np.allclose(F[a][sl], c * g, rtol=1e-4), a              # fp32 rounding of T: 2.4e-7 on S against dS per cell ~ 2e-3 S
+
+
+def test_O10_flux_vanishes_in_an_isothermal_thick_medium_and_flips_under_mirror():
+    nx, ny, nz = 10, 8, 14
+    dx, dy, dz = 48 * KM, 48 * KM, 32 * KM
+    S3 = np.full((nz, ny, nx), 3.0e9)
+    inp = _flat_table_problem(nx, ny, nz, dx, dy, dz, S3, 10.0 / dz, P=3)
+    _, _, F = oracle.solve(inp, want_F=True)
+    assert np.abs(F[:, 2:6]).max() <= 1e-9 * 4 * math.pi * 3.0e9      # I = S for every ray deep inside: sum_r w_r Omega_r = 0
+    # mirror x: F_x flips sign, F_y and F_z do not (the ray set is mirror symmetric)
+    inp = _small_problem(nx=12, ny=10, nz=9, nb=2, P=4)
+    _, _, F = oracle.solve(inp, want_F=True)
+    _, _, Fm = oracle.solve(_transform(inp, lambda a: np.ascontiguousarray(a[:, :, ::-1])), want_F=True)
+    s = np.abs(F).max()
+    assert np.allclose(Fm[0], -F[0][:, :, ::-1], rtol=0, atol=1e-12 * s)
+    assert np.allclose(Fm[1], F[1][:, :, ::-1], rtol=0, atol=1e-12 * s)
+    assert np.allclose(Fm[2], F[2][:, :, ::-1], rtol=0, atol=1e-12 * s)
+
+
+def test_O10_flux_is_the_weighted_vector_sum_of_sweeps():
+    inp = _small_problem(nx=8, ny=6, nz=7, nb=2, P=2)
+    _, _, F = oracle.solve(inp, want_F=True)
+    kap, S = oracle.coefficients(inp)
+    Fm = np.zeros_like(F)
+    for b in range(inp.nbands):
+        for r in range(24):
+            I = oracle.sweep_ray(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.mu[r], inp.npasses, kap[b], S[b])
+            Fm += 4 * math.pi * inp.wq[r] * (inp.mu[r] / np.linalg.norm(inp.mu[r]))[:, None, None, None] * I[None]
+    assert np.allclose(F, Fm, rtol=1e-12, atol=1e-12 * np.abs(Fm).max())
+
+
+def test_O11_flux_divergence_against_numpy_gradient_closed_form_and_telescoping():
+    nx, ny, nz = 12, 10, 9
+    dx, dy, dz = 3.0, 2.0, 1.5
+    rng = np.random.default_rng(11)
+    F = rng.normal(size=(3, nz, ny, nx))
+    inp = _small_problem(nx=nx, ny=ny, nz=nz, nb=1)
+    inp.dx, inp.dy, inp.dz = dx, dy, dz
+    Qdiv, _ = oracle.flux_heating(inp, F, want_blend=False)
+    # library routine: np.gradient (central inside, first-order one-sided at the ends) on periodically padded x, y
+    gx = np.gradient(np.concatenate([F[0][:, :, -1:], F[0], F[0][:, :, :1]], axis=2), dx, axis=2)[:, :, 1:-1]
+    gy = np.gradient(np.concatenate([F[1][:, -1:, :], F[1], F[1][:, :1, :]], axis=1), dy, axis=1)[:, 1:-1, :]
+    gz = np.gradient(F[2], dz, axis=0, edge_order=1)
+    assert np.allclose(Qdiv, -(gx + gy + gz), rtol=1e-13, atol=1e-13)
+    # closed form: central difference of sin is cos * sin(h k)/(h k)
+    x = np.arange(nx) * dx
+    kx = 2 * math.pi / (nx * dx)
+    F2 = np.zeros_like(F)
+    F2[0] = np.sin(kx * x)[None, None, :]
+    Qd2, _ = oracle.flux_heating(inp, F2, want_blend=False)
+    assert np.allclose(Qd2, -(kx * np.cos(kx * x) * np.sin(kx * dx) / (kx * dx))[None, None, :], atol=1e-14)
+    # telescoping: sum_k Qdiv dz = -(1.5 Fz[top] - 0.5 Fz[top-1] + 0.5 Fz[1] - 1.5 Fz[0]) for a purely vertical flux
+    F3 = np.zeros_like(F)
+    F3[2] = F[2]
+    Qd3, _ = oracle.flux_heating(inp, F3, want_blend=False)
+    lhs = Qd3.sum(axis=0) * dz
+    rhs = -(1.5 * F[2][-1] - 0.5 * F[2][-2] + 0.5 * F[2][1] - 1.5 * F[2][0])
+    assert np.allclose(lhs, rhs, atol=1e-12)
+
+
+def test_O11_blend_weights():
+    nx, ny, nz = 6, 5, 8
+    dz = 2.0e6
+    inp = _small_problem(nx=nx, ny=ny, nz=nz, nb=1)
+    inp.dz = dz
+    rng = np.random.default_rng(3)
+    F = rng.normal(size=(3, nz, ny, nx))
+    QJ = rng.normal(size=(nz, ny, nx))
+    kr = 0.05 / dz
+    k0 = np.full((nz, ny, nx), kr)
+    tau0 = 0.1
+    Qdiv, Qb = oracle.flux_heating(inp, F, QJ, k0, tau0=tau0)
+    w = np.exp(-kr * dz * (nz - np.arange(nz)) / tau0)               # uniform medium: taubar(k) = kaprho dz (nz - k)
+    assert np.allclose(Qb, w[:, None, None] * QJ + (1 - w)[:, None, None] * Qdiv, rtol=1e-13, atol=1e-15)
+    # horizontally varying opacity enters through its level mean only
+    k1 = k0 * (1 + 0.5 * np.sin(np.arange(nx)))[None, None, :]
+    k1 *= k0.mean() / k1.mean(axis=(1, 2), keepdims=True)
+    _, Qb1 = oracle.flux_heating(inp, F, QJ, k1, tau0=tau0)
+    assert np.allclose(Qb1, Qb, rtol=1e-12, atol=1e-15)
+    # limits: tau0 -> infinity gives the J - S form, tau0 -> 0 the flux divergence
+    assert np.allclose(oracle.flux_heating(inp, F, QJ, k0, tau0=1e30)[1], QJ, rtol=1e-12)
+    assert np.allclose(oracle.flux_heating(inp, F, QJ, k0, tau0=1e-30)[1], Qdiv, rtol=1e-12)
