@@ -294,3 +294,37 @@ def test_full_size_configs(cfg):
     The oracle finishes each in tens of seconds on the box's cores, so the comparison is
     over every node and every I_top element, not a sample."""
     _check(inputs.make_config(cfg))
+
+
+# ------------------------------------------------------------------ protocol check without compute-sanitizer
+def test_results_barely_depend_on_tiling_and_schedule():
+    """Whatever the tiling, exchange interval, ring depth or CTAs per SM, a node is updated by the same
+    arithmetic except for the per-warp choice between the closed form and the series of the attenuation
+    factors (both accurate to ~1e-7; the warp composition depends on the plan), and the heating is summed in
+    unit order: the results of all plans agree to 2e-6 and each plan is bitwise reproducible.  A race or a
+    stale halo / seam / strip anywhere in the flag protocol breaks this at the 1e-3 level (compute-sanitizer is
+    closed on the GPU pool; this is the stand-in, see profiles/r2_sanitizer.md)."""
+    torch, rts = _gpu()
+    inp = inputs.make_config(3, grid=(60, 52, 44), nbands=3)
+    rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
+    t168 = {0: (16, 8), 1: (16, 8), 2: (16, 8)}
+    plans = [dict(), dict(tiling=t168), dict(tiling=t168, exchange_interval=1), dict(tiling=t168, exchange_interval=2),
+             dict(tiling=t168, exchange_interval=3), dict(tiling=t168, ring_depth=2), dict(tiling=t168, ctas_per_sm=2),
+             dict(tiling=t168, ctas_per_sm=1, ring_depth=2, exchange_interval=2),
+             dict(tiling={0: (12, 5), 1: (20, 7), 2: (8, 11)}), dict(tiling={0: (40, 12), 1: (40, 12), 2: (40, 12)}),
+             dict(tiling={0: (16, 6), 1: (16, 6), 2: (16, 6)}, exchange_interval=2)]
+    ref = None
+    for kw in plans:
+        s = rts.from_inputs(inp, **kw)
+        first = None
+        for rep in range(3):
+            Q, I = s.solve(rho, T, P)
+            s.sync_check()
+            if ref is None:
+                ref = (Q.clone(), I.clone())
+            if first is None:
+                first = (Q.clone(), I.clone())
+            assert torch.equal(Q, first[0]) and torch.equal(I, first[1]), (kw, rep)
+            assert (Q - ref[0]).abs().max().item() <= 2e-6 * ref[0].abs().max().item(), (kw, rep)
+            assert ((I - ref[1]).abs() / ref[1].abs()).max().item() <= 2e-6, (kw, rep)
+        s.close()
