@@ -745,7 +745,9 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     //      tile core + upwind u halo (one HALO of columns) + upwind v halo of depth K-1, clipped to the domain.
     const int nsl = 2 * NG;
     const int TS = T / nsl;
-    const int sidx = tid / TS, e = tid - sidx * TS;
+    // warp w works for ray w % nsl: the warps of one scheduler (w % 4) then run the same ray, i.e. one copy of
+    // the strip code (one sign of su) at a time in its instruction cache
+    const int sidx = (tid >> 5) % nsl, e = ((tid >> 5) / nsl) * 32 + (tid & 31);
     const int s = (NG == 2) ? sidx : (((U.gsu0 < 0) ? 1 : 0) + 2 * sidx);   // slot of this thread's ray
     const int gsu = (s & 1) ? -1 : 1, gsv = (s & 2) ? -1 : 1;
     unsigned ifl = 0;
