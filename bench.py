@@ -14,8 +14,10 @@ configs[2] (4-band RTS on 288^3, the configuration the metric is quoted on).
               compulsory-byte model / its event-timed duration, against MEASURED_PEAKS.json
   cpu_baseline the fp64 oracle, as it stands, on the box's host cores, bounded sample
 
-N > 1 (torchrun): the path is run as N independent replicas (one atmosphere per rank, no
-data-path collective) -> "scaling": "weak".  --impl reference times the oracle (rank 0 only).
+N > 1 (torchrun): by default the path is run as N independent replicas (one atmosphere per rank, no
+data-path collective) -> "scaling": "weak".  --scaling strong shards ONE box by band x octant (rts_set_shard):
+every rank sweeps its units, one NCCL sum all-reduce completes Q_rad and I_top inside the timed region.
+--impl reference times the oracle (rank 0 only).
 """
 from __future__ import annotations
 
@@ -170,6 +172,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--ctas-per-sm", type=int, default=0)
     ap.add_argument("--tile", type=str, default="", help="tuning: 'TU,TV' for all march axes")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one atmosphere per rank; strong = one box sharded by band x octant")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -188,13 +192,15 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    # one independent atmosphere per rank (replicas; no data-path collective)
-    inp = inputs_mod.make_config(args.config, seed_offset=multi.rank_seed_offset(rank))
+    # weak: one independent atmosphere per rank (replicas; no data-path collective)
+    # strong: the same box on every rank, sweep units dealt round robin, one sum all-reduce of Q and I_top
+    strong = (args.scaling == "strong" and world > 1)
+    inp = inputs_mod.make_config(args.config, seed_offset=0 if strong else multi.rank_seed_offset(rank))
     tiling = None
     if args.tile:
         tu, tv = (int(x) for x in args.tile.split(","))
         tiling = {0: (tu, tv), 1: (tu, tv), 2: (tu, tv)}
-    solver = rts.from_inputs(inp, tiling=tiling, ctas_per_sm=args.ctas_per_sm)
+    solver = rts.from_inputs(inp, tiling=tiling, ctas_per_sm=args.ctas_per_sm, shard=(rank, world) if strong else None)
     plan = solver.plan_info()
     solver.enable_timing(True)
     rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
@@ -209,9 +215,14 @@ def main():
     def reduce_max(x):
         return multi.max_over_ranks(x, world, "cuda")
 
+    def step():
+        solver.solve(rho, T, P, Q, Itop)
+        if strong:
+            multi.allreduce_sum(world, Q, Itop)
+
     # ---- device-resident timing
     for _ in range(args.warmup):
-        solver.solve(rho, T, P, Q, Itop)
+        step()
     solver.sync_check()
     sampler = ClockSampler(local_rank)
     if rank == 0:
@@ -221,15 +232,22 @@ def main():
     sweep_ms, stage_a_ms = [], []
     ev0.record()
     for _ in range(args.steps):
-        solver.solve(rho, T, P, Q, Itop)
+        step()
     ev1.record()
     barrier()
-    tm = solver.last_timing()          # per-stage events of the last timed solve (same stream)
-    sweep_ms.append(tm["sweep_ms"]); stage_a_ms.append(tm["stage_a_ms"])
+    solver.sync_check()
+    local_ms = ev0.elapsed_time(ev1) / args.steps
+    # per-stage durations of the kernels (CUDA events recorded on the solve stream inside rts_solve): the same
+    # number of solves again, read back one by one (the events belong to the context, so each read waits)
+    for _ in range(args.steps):
+        solver.solve(rho, T, P, Q, Itop)
+        tm = solver.last_timing()
+        sweep_ms.append(tm["sweep_ms"]); stage_a_ms.append(tm["stage_a_ms"])
     solver.sync_check()
     clocks = sampler.stop() if rank == 0 else None
-    local_ms = ev0.elapsed_time(ev1) / args.steps
     agg = multi.aggregate(local_ms, float(inp.updates), world, "cuda")
+    if strong:                         # one box: the job's units are the box's, not world x
+        agg["value"] = float(inp.updates) / (agg["ms"] * 1e-3)
 
     # ---- end to end through the host-buffer entry point (pinned buffers, copies timed)
     e2e = None
@@ -270,15 +288,20 @@ def main():
         "bound": "hbm", "kernel": "rts_sweep_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
         "algorithmic_bytes_per_launch": s_bytes / rounds, "launches_per_step": rounds,
-        "avg_launch_ms": sweep_launch_ms,
+        "avg_launch_ms": sweep_launch_ms, "min_launch_ms": float(np.min(sweep_ms)) / rounds, "launches_timed": len(sweep_ms),
+        "note": "bound 'hbm' is north_star's reporting convention; the kernel is bound by shared-memory bandwidth "
+                "and issue latency inside a step and by inter-CTA exchange latency between blocks (DESIGN.md 8, profiles/)",
         "solve_frac_of_compulsory_byte_roofline": ((a_bytes + s_bytes) / (local_ms * 1e-3) / 1e9) / peak,
         "stage_a_ms": float(np.mean(stage_a_ms)),
     }
+    # measured DRAM bytes per launch (ncu --set full capture): only when the stored capture is of this workload and plan
     prof = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(prof):
+    if os.path.exists(prof) and world == 1:
         try:
             with open(prof) as fh:
-                roofline["traffic"] = json.load(fh).get("rts_sweep_kernel_dram_bytes_per_launch")
+                tj = json.load(fh)
+            if tj.get("config") == args.config and tj.get("tile_u_z") == plan.get("tile_u_z") and tj.get("tile_v_z") == plan.get("tile_v_z"):
+                roofline["traffic"] = tj.get("rts_sweep_kernel_dram_bytes_per_launch")
         except Exception:
             pass
 
@@ -286,10 +309,7 @@ def main():
     thick = None
     if world == 1:
         levels = solver.thick_levels()
-        h = np.array([inp.dx, inp.dy, inp.dz])
-        with np.errstate(divide="ignore"):
-            tt = h[None, :] / np.abs(np.asarray(inp.mu, dtype=np.float64))
-        n_zrays = int((np.argmin(tt[:, ::-1], axis=1) == 0).sum())          # rays leaving through a z face (ties prefer z)
+        n_zrays = plan["z_march_rays"]                                       # as the library grouped the rays
         skipped = sum(levels) * inp.nx * inp.ny * n_zrays * (inp.npasses - 1)
         thick = {"levels_per_band": levels, "z_march_rays": n_zrays,
                  "skipped_fraction_of_updates": skipped / float(inp.updates)}
@@ -330,11 +350,11 @@ def main():
 
     line = {
         "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": agg["ms"], "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": agg["ms"], "higher_is_better": True, "scaling": "strong" if strong else "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_name(args.config, inp), "grid": [inp.nx, inp.ny, inp.nz],
                    "bands": inp.nbands, "rays": inp.nrays, "passes": inp.npasses,
-                   "updates_per_step": inp.updates, "parallelism": f"replicas x{world}",
+                   "updates_per_step": inp.updates, "parallelism": (f"band x octant shards x{world}, one sum all-reduce of Q and I_top" if strong else f"replicas x{world}"),
                    "cache": "working set (kaprho,S fields, 2 layouts) >> L2: inputs larger than L2, no flush needed",
                    "plan": plan},
         "solve_ms": agg["ms"], "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,

@@ -162,6 +162,17 @@ int rts_sync_check(rts_ctx* ctx, void* stream);
 int rts_set_thick_skip(rts_ctx* ctx, int on);
 int rts_thick_levels(rts_ctx* ctx, int* levels_host, void* stream);
 
+/* Band x octant sharding of ONE box over several GPUs ("for N-bands ... run N
+ * times", PAPER.md:291 strong scaling of one 288^3 box).  The sweep units -- (march axis, direction, band
+ * pair), i.e. the rays of one octant face group for two bands -- are dealt round robin to `nranks` contexts,
+ * one per GPU / process.  After rts_set_shard(rank, nranks) a solve computes stage A for the whole box, sweeps
+ * only this rank's units and returns PARTIAL results: Qrad = the heating of this rank's units, I_top = this
+ * rank's (band, ray) slices, zeros elsewhere.  The caller completes both with one sum all-reduce over the ranks
+ * (NCCL; paper_2107_08145_b200/multi.py).  Call before sizing the workspace (it changes the plan).
+ * rts_shard_info: HOST outputs, units of this rank / of the whole problem.  RTS_EINVAL unless 0 <= rank < nranks. */
+int rts_set_shard(rts_ctx* ctx, int rank, int nranks);
+int rts_shard_info(rts_ctx* ctx, int* units_mine, int* units_all);
+
 /* Per-stage device timing of the last rts_solve (CUDA events recorded on the solve stream
  * inside rts_solve).  rts_last_timing waits for the solve and fills ms4 (HOST) with
  * [0] stage A + switch heights, [1] all sweep launches, [2] finalize, [3] whole solve. */
@@ -172,7 +183,8 @@ int rts_last_timing(rts_ctx* ctx, float* ms4_host);
  * all units), [2] = CTAs per SM of the sweep kernel, [3] = sweep units (march axis x direction
  * x ray group x band), [4] = threads per CTA, [5] = dynamic shared memory per CTA (bytes),
  * [6] = sweep grid (persistent CTAs), [7] = exchange interval, [8..10] = tile_v of march x,y,z,
- * [11..13] = tile_u of march x,y,z.  n = ints in `what` (<= 16). */
+ * [11..13] = tile_u of march x,y,z, [14] = rays that march along z (leave their cell through a z face),
+ * [15] = sweep units of the whole problem (= [3] unless sharded).  n = ints in `what` (<= 16). */
 int rts_plan_info(rts_ctx* ctx, int* what, int n);
 
 const char* rts_last_error(const rts_ctx* ctx);

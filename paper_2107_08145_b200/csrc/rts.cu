@@ -46,6 +46,8 @@ struct rts_ctx {
     double h[3] = {0, 0, 0};
     int npass = 3;
     bool thick_skip = true;
+    int shard_rank = 0, shard_n = 1;   // this context sweeps the units u with u % shard_n == shard_rank (rts_set_shard)
+    int units_all = 0;                 // sweep units of the whole problem
     bool flux = false;           // radiative flux wanted (rts_enable_flux): three more partial fields per unit
     double tau0 = 0.1;           // blend scale of the flux-divergence heating
     std::vector<HostRay> rays;
@@ -337,7 +339,7 @@ int make_plan(rts_ctx* c)
 
     // --- materialise units in ticket order
     c->units.clear();
-    int ticket = 0;
+    int ticket = 0, uidx = 0;
     const size_t N = (size_t)c->nx * c->ny * c->nz;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
@@ -362,6 +364,9 @@ int make_plan(rts_ctx* c)
                     bool any = false;
                     for (int ri : sub) any |= (only_su == 0 || c->rays[ri].su == only_su);
                     if (!any) continue;
+                    // band x octant sharding ("for N-bands ... run N times"): the units are
+                    // dealt round robin to the ranks; a rank sweeps its own and leaves the others' heating at zero
+                    if ((uidx++ % c->shard_n) != c->shard_rank) continue;
                     HostUnit hu{};
                     UnitDesc& d = hu.d;
                     std::memset(&d, 0, sizeof d);
@@ -391,11 +396,13 @@ int make_plan(rts_ctx* c)
                 }
             }
     c->total_tickets = ticket;
+    c->units_all = uidx;
     c->grid = std::min(slots, c->total_tickets);
-    c->off_units = take(sizeof(UnitDesc) * c->units.size());
-    c->off_partptr = take(sizeof(float*) * c->units.size());
-    c->off_parttr = take(sizeof(int) * c->units.size());
-    c->off_bar = take(sizeof(int) * c->units.size());
+    const size_t nu1 = std::max<size_t>(1, c->units.size());
+    c->off_units = take(sizeof(UnitDesc) * nu1);
+    c->off_partptr = take(sizeof(float*) * nu1);
+    c->off_parttr = take(sizeof(int) * nu1);
+    c->off_bar = take(sizeof(int) * nu1);
     c->off_stage_in = take(sizeof(float) * N * 3);
     c->off_stage_out = take(sizeof(float) * (N + (size_t)c->nb * c->n_up * c->ny * c->nx));
     c->ws_bytes = off;
@@ -684,8 +691,11 @@ int rts_plan_info(rts_ctx* c, int* what, int n)
 {
     if (!c || !what) return RTS_EINVAL;
     if (!c->planned) { int rc = make_plan(c); if (rc != RTS_OK) return rc; }
+    int zrays = 0;
+    for (auto& r : c->rays) zrays += (r.march == 2);
     int v[16] = {4, c->total_tickets, c->ctas_per_sm, (int)c->units.size(), c->threads, c->smem_bytes,
-                 c->grid, c->K, c->tp[0].WV, c->tp[1].WV, c->tp[2].WV, c->tp[0].WU, c->tp[1].WU, c->tp[2].WU, 0, 0};
+                 c->grid, c->K, c->tp[0].WV, c->tp[1].WV, c->tp[2].WV, c->tp[0].WU, c->tp[1].WU, c->tp[2].WU,
+                 zrays, c->units_all};
     for (int i = 0; i < n && i < 16; ++i) what[i] = v[i];
     return RTS_OK;
 }
@@ -740,7 +750,9 @@ int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, flo
     CUDA_TRY(c, cudaMemsetAsync(ws + c->off_bar, 0, sizeof(int) * c->units.size(), st));
     // the sweep: one persistent launch, tasks handed out by an in-order ticket counter
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[2], st));
-    {
+    if (c->shard_n > 1 && Itop)    // the emergent intensities of the other ranks' rays stay zero: a sum over ranks completes them
+        CUDA_TRY(c, cudaMemsetAsync(Itop, 0, sizeof(float) * (size_t)c->nb * c->n_up * c->ny * c->nx, st));
+    if (c->total_tickets > 0) {
         const UnitDesc* dunits = (const UnitDesc*)(ws + c->off_units);
         int* abortf = (int*)(ws + c->off_abort);
         int* ticket = abortf + 1;
@@ -803,6 +815,24 @@ int rts_solve_flux(rts_ctx* c, const float* rho, const float* T, const float* P,
     if (!c) return RTS_EINVAL;
     if (!Frad) return fail(c, RTS_EINVAL, "rts_solve_flux: null Frad");
     return solve_impl(c, rho, T, P, Q, Itop, Frad, Qdiv, Qblend, stream);
+}
+
+int rts_set_shard(rts_ctx* c, int rank, int nranks)
+{
+    if (!c) return RTS_EINVAL;
+    if (nranks < 1 || rank < 0 || rank >= nranks) return fail(c, RTS_EINVAL, "rts_set_shard: need 0 <= rank < nranks");
+    c->shard_rank = rank; c->shard_n = nranks;
+    c->planned = false;
+    return RTS_OK;
+}
+
+int rts_shard_info(rts_ctx* c, int* units_mine, int* units_all)
+{
+    if (!c) return RTS_EINVAL;
+    if (!c->planned) { int rc = make_plan(c); if (rc != RTS_OK) return rc; }
+    if (units_mine) *units_mine = (int)c->units.size();
+    if (units_all) *units_all = c->units_all;
+    return RTS_OK;
 }
 
 int rts_set_thick_skip(rts_ctx* c, int on)

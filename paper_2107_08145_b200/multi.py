@@ -1,9 +1,13 @@
-"""N > 1 plumbing of bench.py (host logic only; no kernel and no data-path collective).
+"""N > 1 plumbing of bench.py (host logic only; no kernel).
 
-The path shards by independent problems: as in the paper's weak-scaling runs (one 288^3 block
-per GPU, sec. 6.4) every rank owns one block-local atmosphere and solves it on
-its own GPU; the only communication is the timing reduction (max over ranks).  DESIGN.md,
-"Multi-GPU".  Works with any torch.distributed backend (nccl on GPUs, gloo in the CPU tests).
+Two ways to use several GPUs ("Multi-GPU"):
+  weak    independent problems: as in the paper's weak-scaling runs (one 288^3 block per GPU, PAPER.md:297,
+          sec. 6.4) every rank owns one block-local atmosphere and solves it on its own GPU; the only
+          communication is the timing reduction (max over ranks);
+  strong  ONE box sharded by band x octant: the sweep units are dealt round
+          robin to the ranks (rts_set_shard), every rank sweeps its own units, and ONE sum all-reduce
+          completes Q_rad and I_top (`allreduce_sum`).
+Works with any torch.distributed backend (nccl on GPUs, gloo in the CPU tests).
 """
 from __future__ import annotations
 
@@ -42,3 +46,22 @@ def aggregate(local_ms: float, local_units: float, world: int, device: Optional[
 def reference_arm_runs_here(rank: int) -> bool:
     """`bench.py --impl reference`: rank 0 alone runs and prints; the others exit 0."""
     return rank == 0
+
+
+def shard_units(n_units: int, rank: int, nranks: int) -> list:
+    """The sweep units (in the library's unit order) that rank `rank` of `nranks` sweeps: round robin,
+    the rule of rts_set_shard."""
+    if nranks < 1 or not (0 <= rank < nranks):
+        raise ValueError("need 0 <= rank < nranks")
+    return [u for u in range(n_units) if u % nranks == rank]
+
+
+def allreduce_sum(world: int, *tensors):
+    """The one data-path collective of the strong-scaling mode: sum over ranks of the partial Q_rad / I_top
+    (in place; no-op for one rank)."""
+    if world == 1:
+        return
+    import torch.distributed as dist
+    for t in tensors:
+        if t is not None:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)

@@ -26,7 +26,7 @@ EXPORTS = [
     "rts_set_workspace", "rts_solve", "rts_solve_host", "rts_coefficients", "rts_sync_check",
     "rts_plan_info", "rts_last_error", "rts_enable_timing", "rts_last_timing",
     "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells", "rts_set_thick_skip", "rts_thick_levels",
-    "rts_enable_flux", "rts_set_flux_blend", "rts_solve_flux",
+    "rts_enable_flux", "rts_set_flux_blend", "rts_solve_flux", "rts_set_shard", "rts_shard_info",
 ]
 
 
@@ -99,6 +99,10 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_set_flux_blend.argtypes = [c_void_p, c_double]
     lib.rts_solve_flux.restype = c_int
     lib.rts_solve_flux.argtypes = [c_void_p] + [c_void_p] * 8 + [c_void_p]
+    lib.rts_set_shard.restype = c_int
+    lib.rts_set_shard.argtypes = [c_void_p, c_int, c_int]
+    lib.rts_shard_info.restype = c_int
+    lib.rts_shard_info.argtypes = [c_void_p, PI, PI]
     lib.rts_last_error.restype = ctypes.c_char_p
     lib.rts_last_error.argtypes = [c_void_p]
     _lib = lib
@@ -209,7 +213,7 @@ class RTS:
         self._check(self._lib.rts_plan_info(self._ctx, arr, 16), "rts_plan_info")
         keys = ["launches", "tasks", "ctas_per_sm", "units", "threads", "smem_bytes",
                 "grid", "exchange_interval", "tile_v_x", "tile_v_y", "tile_v_z",
-                "tile_u_x", "tile_u_y", "tile_u_z"]
+                "tile_u_x", "tile_u_y", "tile_u_z", "z_march_rays", "units_all"]
         return dict(zip(keys, [int(v) for v in arr]))
 
     # -- the hot path
@@ -325,6 +329,16 @@ class RTS:
                     "rts_solve_cells")
         return Qc, (Itop if want_itop else None)
 
+    def set_shard(self, rank: int, nranks: int):
+        """Band x octant sharding: this context sweeps the units u with u % nranks == rank; solve() then returns
+        partial Q and I_top that a sum all-reduce over the ranks completes (multi.allreduce_sum)."""
+        self._check(self._lib.rts_set_shard(self._ctx, int(rank), int(nranks)), "rts_set_shard")
+
+    def shard_info(self) -> Tuple[int, int]:
+        a, b = ctypes.c_int(0), ctypes.c_int(0)
+        self._check(self._lib.rts_shard_info(self._ctx, ctypes.byref(a), ctypes.byref(b)), "rts_shard_info")
+        return a.value, b.value
+
     def set_thick_skip(self, on: bool):
         self._check(self._lib.rts_set_thick_skip(self._ctx, 1 if on else 0), "rts_set_thick_skip")
 
@@ -347,7 +361,7 @@ class RTS:
 
 
 def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchange_interval: int = 0,
-                cells: bool = False, ring_depth: int = 0, flux: bool = False) -> "RTS":
+                cells: bool = False, ring_depth: int = 0, flux: bool = False, shard: Optional[Tuple[int, int]] = None) -> "RTS":
     """Create and configure a solver for an `inputs.RTSInputs` problem.  cells=True: the fields of
     `inp` are cell-centred (solve_cells); the RT node grid then has one level more."""
     r = RTS(inp.nx, inp.ny, inp.nz + (1 if cells else 0), inp.dx, inp.dy, inp.dz, inp.nbands)
@@ -365,5 +379,7 @@ def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchan
         r.set_ring_depth(ring_depth)
     if flux:
         r.enable_flux(True)
+    if shard:
+        r.set_shard(*shard)
     r.allocate_workspace()
     return r
