@@ -46,6 +46,7 @@ struct rts_ctx {
     double h[3] = {0, 0, 0};
     int npass = 3;
     bool thick_skip = true;
+    unsigned solve_seq = 0;            // solves launched on this context
     int shard_rank = 0, shard_n = 1;   // this context sweeps the units u with u % shard_n == shard_rank (rts_set_shard)
     int units_all = 0;                 // sweep units of the whole problem
     bool flux = false;           // radiative flux wanted (rts_enable_flux): three more partial fields per unit
@@ -389,7 +390,12 @@ int make_plan(rts_ctx* c)
                     for (int q = 0; q < NSLOT; ++q) d.ray[q].itop = -1;
                     for (int ri : sub)
                         if (only_su == 0 || c->rays[ri].su == only_su) make_ray_consts(c->rays[ri], d.ray[c->rays[ri].slot]);
-                    hu.off_xex = take(sizeof(float2) * 2 * NSLOT * (size_t)d.n_v * d.n_u2);
+                    // tagged exchange: safe when every ray's strips are read by tiles whose own strips (of the opposite
+                    // ray) this tile waits for before it writes the same buffer again (rts_sweep.cuh, block_start)
+                    d.xflag = (t.ng == 2) ? 1 : 0;
+                    for (int q = 0; q < NSLOT; ++q)
+                        if (d.ray[q].active && !d.ray[q ^ 3].active) d.xflag = 0;
+                    hu.off_xex = take(sizeof(float4) * 2 * NSLOT * (size_t)d.n_v * d.n_u2);
                     hu.off_g = take(sizeof(float2) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u2));
                     hu.off_part = take(sizeof(float) * N * (c->flux ? 4 : 1));
                     c->units.push_back(hu);
@@ -426,7 +432,7 @@ int bind_workspace(rts_ctx* c)
         d.mthick = (const int*)(ws + c->off_mthick) + 3 * d.pair;
         // carried strips and seam histories must hold finite numbers from the start: planes that are
         // skipped as optically thick leave their entries untouched, and readers multiply them by exactly 0
-        CUDA_TRY(c, cudaMemset(ws + hu.off_xex, 0, sizeof(float2) * 2 * NSLOT * (size_t)d.n_v * d.n_u2));
+        CUDA_TRY(c, cudaMemset(ws + hu.off_xex, 0, sizeof(float4) * 2 * NSLOT * (size_t)d.n_v * d.n_u2));
         CUDA_TRY(c, cudaMemset(ws + hu.off_g, 0, sizeof(float2) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u2)));
         flat.push_back(d);
     }
@@ -757,7 +763,10 @@ int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, flo
         int* abortf = (int*)(ws + c->off_abort);
         int* ticket = abortf + 1;
         int nunits = (int)c->units.size(), total = c->total_tickets;
-        void* args[] = {&c->maps, &dunits, &nunits, &total, &ticket, &Itop, &abortf};
+        unsigned seq = ++c->solve_seq;                          // tags of this solve's exchange words
+        if ((seq & 0xfffffu) == 0) seq = ++c->solve_seq;
+        seq &= 0xfffffu;
+        void* args[] = {&c->maps, &dunits, &nunits, &total, &ticket, &Itop, &abortf, &seq};
         // cooperative launch: every CTA of the grid is resident, which the tile barriers rely on
         CUDA_TRY(c, cudaLaunchCooperativeKernel(sweep_fn(c->pitch), dim3(c->grid), dim3(c->threads), args,
                                                 (size_t)c->smem_bytes, st));
@@ -883,7 +892,7 @@ int rts_sync_check(rts_ctx* c, void* stream)
         e = cudaMemcpy(&ab, c->ws + c->off_abort, sizeof(int), cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail(c, RTS_ECUDA, std::string("status read: ") + cudaGetErrorString(e));
         if (ab) {
-            char buf[128];
+            char buf[256];
             snprintf(buf, sizeof buf, "sweep kernel watchdog fired (code %d, step %d): a wait did not complete", ab & 15, ab >> 4);
             return fail(c, RTS_ETIMEOUT, buf);
         }

@@ -62,9 +62,11 @@ struct UnitDesc {
     int K, npass, ticket_begin, ntiles;
     int nz, q_in_B, qvec, nstage;          // qvec: heating rows are 16-byte aligned (vector reductions)
     int ng, gsu0, nband_ok, RC;            // ray groups (same su) of this unit: 2 (su = +1, -1) or 1 (su = gsu0);
+    int xflag, pad0_;                      // 1: tagged exchange (every ray of the unit has its opposite ray in the unit)
                                            // nband_ok: bands of the pair that exist (1 or 2); RC: rows per strip
     RayC ray[NSLOT];
-    float* Xex;       // float2 [2][NSLOT][n_v][n_u2]   carried planes at block ends (strips only)
+    float* Xex;       // [2][NSLOT][n_v][n_u2] x 16 bytes: carried planes at block ends (strips only), per node and
+                      // band one 64-bit word (value, tag of the block that wrote it)
     float* Gu;        // float2 [2][n_m][NSLOT*n_v + NSLOT*n_u2]  per pass parity and plane: far-u column
                       //                                of every slot, then (per_v only) far-v row of every slot
     float* Qpart;     // [N] heating of this unit alone, in the unit's own layout (x- or y-fastest): every node is

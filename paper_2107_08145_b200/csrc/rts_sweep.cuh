@@ -122,6 +122,24 @@ __device__ __forceinline__ bool spin_abort(int* abortf, unsigned& spins, int cod
     return false;
 }
 
+// Flagged exchange words: a strip value travels with the tag of the block that wrote it in ONE 64-bit word, so a
+// reader that sees the tag has the value (64-bit scalar accesses are single-copy atomic): no release fence, no
+// flag store and no separate poll between a tile and its neighbours, one L2 round trip instead of four.
+__device__ __forceinline__ void st_tagged2(void* p, const f2 v, const unsigned tag)
+{
+    const unsigned long long a = ((unsigned long long)tag << 32) | __float_as_uint(v.x);
+    const unsigned long long b = ((unsigned long long)tag << 32) | __float_as_uint(v.y);
+    asm volatile("st.global.cg.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
+// (volatile: the same buffer was read two blocks earlier, and a plain or .cg load may be served from the SM's L1)
+__device__ __forceinline__ bool ld_tagged2(const void* p, const unsigned tag, f2& v)
+{
+    unsigned long long a, b;
+    asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+    v = make_float2(__uint_as_float((unsigned)a), __uint_as_float((unsigned)b));
+    return (unsigned)(a >> 32) == tag && (unsigned)(b >> 32) == tag;
+}
+
 __device__ __forceinline__ int wrap(int x, int n) { x %= n; return x < 0 ? x + n : x; }
 
 // TMA engine, tensor form: one 5-D box (u, field, ., ., band pair) of a coefficient layout -> shared memory
@@ -309,10 +327,11 @@ __device__ __forceinline__ f2 node_update(const f2 em1, const f2 wl, const f2 pp
 // what a strip needs for the uncommon stores of a step (seam histories, exchange strips)
 struct TailCtx {
     f2* GhP;                           // seam history of this plane and pass (far columns, then far rows); null: off
-    f2* XeP;                           // exchange planes of this block's parity; null: no strips this step
+    float4* XeP;                       // exchange planes of this block's parity (16 bytes per node); null: no strips this step
     int gv0, ug;                       // slot * n_v + global v of row q = 0;  global u of the pair
     int n_u2, far_off;                 // row pitch of the exchange planes; NSLOT*n_v + slot*n_u2 (far-v rows)
     int hv, nrows, K, gsv;
+    unsigned tag;                      // tag of the block whose strips are published this step (0: plain strips)
 };
 
 // Store one finished row of a strip: the carried plane and, where flagged, the seam history (far-u column,
@@ -335,8 +354,11 @@ __device__ __forceinline__ void row_store(const TailCtx& TC, const unsigned fl, 
             else __stcg(gvp, make_float2(o.x, o.y));
         }
     }
-    if (TC.XeP && ((fl & IT_USTRIP) || q >= TC.nrows - TC.K))    // exchange strips at a block end
-        __stcg(reinterpret_cast<float4*>(TC.XeP + (size_t)gv * TC.n_u2 + TC.ug), o);
+    if (TC.XeP && ((fl & IT_USTRIP) || q >= TC.nrows - TC.K)) {  // exchange strips at a block end
+        float4* xe = TC.XeP + (size_t)gv * TC.n_u2 + TC.ug;          // 16 bytes per node: (value, tag) per band
+        st_tagged2(xe, make_float2(o.x, o.y), TC.tag);
+        st_tagged2(xe + 1, make_float2(o.z, o.w), TC.tag);
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -547,19 +569,25 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
     }
 }
 
-// Block start (out of line): wait until every tile of the unit has published block gblk - 1, then fetch the
-// K-deep halo of the carried plane set Xr from the exchange buffer and the seam ghosts of the previous plane.
+// Block start (out of line): fetch the K-deep halo of the carried plane set Xr from the exchange buffer and the seam
+// ghosts of the previous plane.  Tagged exchange (U.xflag, every ray of the unit has its opposite ray in the unit):
+// the halo words carry the tag of block gblk - 1, a reader spins on the words it needs; the tiles of the unit
+// meet at the arrival counter only at a pass start (seam histories of the whole previous pass).  Otherwise they
+// meet at the counter at every block start.  `skipped`: the publishing step was a thick plane that stored no strips.
 // Returns false if the watchdog fired.
 template <int PITCH>
 __device__ __noinline__ bool block_start(TaskShared* __restrict__ Sp, f2* __restrict__ Xr, const f2* __restrict__ Kp0,
-                                         const int pass, const int blk0, const int gblk, const int s_)
+                                         const int pass, const int blk0, const int gblk, const int s_,
+                                         const unsigned tag, const bool skipped)
 {
     TaskShared& S = *Sp;
     const UnitDesc& U = S.U; const TileGeo& G = S.G;
     const int tid = threadIdx.x, T = blockDim.x;
     const int ngh = S.nghost, nhalo = S.nhalo;
     const bool zmarch = G.zmarch != 0;
+    const bool tagged = U.xflag != 0;
     const bool exch = !(zmarch && blk0 == 0);
+    const bool meet = !tagged || blk0 == 0;
     const int m_prev = (blk0 == 0) ? U.n_m - 1 : blk0 - 1;
     // seam ghosts of the previous plane come from the previous pass: inside a pass (blk0 > 0)
     // they were written more than one block ago, i.e. before the arrival counter this tile
@@ -568,30 +596,43 @@ __device__ __noinline__ bool block_start(TaskShared* __restrict__ Sp, f2* __rest
     const bool pre = exch && pass > 0 && blk0 > 0 && ngh > 0;
     f2 gpre = make_float2(0.f, 0.f);
     if (pre && tid < ngh) gpre = ghost_fetch<PITCH>(S, S.gt[tid], pass - 1, m_prev, nullptr);
-    if (tid == 0) {
-        const int need = gblk * U.ntiles;
-        const int ab = *reinterpret_cast<volatile int*>(S.abortf);
-        unsigned spins = 0, ns = 32;
-        while (ld_acquire(U.barrier) < need) {
-            if (spin_abort(S.abortf, spins, 3 | (s_ << 4))) { S.flag = 1; break; }
-            __nanosleep(ns);
-            if (ns < 256) ns += ns;                  // back off a little: a unit waiting for residency spins long
+    if (meet) {
+        if (tid == 0) {
+            const int need = (tagged ? pass : gblk) * U.ntiles;
+            const int ab = *reinterpret_cast<volatile int*>(S.abortf);
+            unsigned spins = 0, ns = 32;
+            while (ld_acquire(U.barrier) < need) {
+                if (spin_abort(S.abortf, spins, 3 | (s_ << 4))) { S.flag = 1; break; }
+                __nanosleep(ns);
+                if (ns < 256) ns += ns;                  // back off a little: a unit waiting for residency spins long
+            }
+            if (ab != 0) S.flag = 1;
         }
-        if (ab != 0) S.flag = 1;
+        __syncthreads();
+        if (S.flag != 0) return false;                   // uniform: the watchdog fired somewhere
     }
-    __syncthreads();
-    if (S.flag != 0) return false;                   // uniform: the watchdog fired somewhere
     if (exch) {
         // halo pairs lie inside the domain, ghost columns / rows outside it: disjoint stores
-        const f2* xe0 = reinterpret_cast<const f2*>(U.Xex) + (size_t)((gblk - 1) & 1) * NSLOT * (size_t)U.n_v * U.n_u2;
-        for (int e = tid; e < nhalo; e += T) {
-            const HaloEnt h = S.ht[e];
-            const float4 x = __ldcg(reinterpret_cast<const float4*>(xe0 + (size_t)h.slot * U.n_v * U.n_u2 + h.goff));
-            f2* d = Xr + xso<PITCH>(S, h.slot) + h.xoff;
-            const int c0 = h.mask & 15, c1 = h.mask >> 4;
-            if (c0 == 0 && c1 == 2) *reinterpret_cast<float4*>(d) = x;
-            else if (c0 == 0) d[0] = make_float2(x.x, x.y);
-            else if (c1 == 2) d[1] = make_float2(x.z, x.w);
+        if (!skipped) {
+            const float4* xe0 = reinterpret_cast<const float4*>(U.Xex) + (size_t)((gblk - 1) & 1) * NSLOT * (size_t)U.n_v * U.n_u2;
+            for (int e = tid; e < nhalo; e += T) {
+                const HaloEnt h = S.ht[e];
+                const float4* src = xe0 + (size_t)h.slot * U.n_v * U.n_u2 + h.goff;
+                const int c0 = h.mask & 15, c1 = h.mask >> 4;
+                f2 x0 = make_float2(0.f, 0.f), x1 = x0;
+                unsigned spins = 0;
+                while (true) {
+                    bool ok = true;
+                    if (c0 == 0) ok = ld_tagged2(src, tag, x0) || !tagged;
+                    if (c1 == 2) ok = (ld_tagged2(src + 1, tag, x1) || !tagged) && ok;
+                    if (ok) break;
+                    if (spin_abort(S.abortf, spins, 4 | (s_ << 4))) { S.flag = 1; break; }
+                }
+                f2* d = Xr + xso<PITCH>(S, h.slot) + h.xoff;
+                if (c0 == 0 && c1 == 2) *reinterpret_cast<float4*>(d) = cat4(x0, x1);
+                else if (c0 == 0) d[0] = x0;
+                else if (c1 == 2) d[1] = x1;
+            }
         }
         if (ngh > 0) {
             if (pre && tid < ngh) { const GhostEnt g = S.gt[tid]; Xr[xso<PITCH>(S, g.goff >> 28) + g.xoff] = gpre; }
@@ -601,6 +642,7 @@ __device__ __noinline__ bool block_start(TaskShared* __restrict__ Sp, f2* __rest
             }
         }
         __syncthreads();
+        if (S.flag != 0) return false;
     }
     return true;
 }
@@ -648,8 +690,9 @@ __device__ __noinline__ void task_lists(TaskShared* __restrict__ Sp)
         if (!up_u && !up_v) continue;
         const int rlo = max((svp && up_v) ? HALO - K : HALO, G.dlo_v);
         const int rhi = min((!svp && up_v) ? HALO + G.wv + K : HALO + G.wv, G.dhi_v);
-        const int clo = max((su > 0 && up_u) ? 0 : HALO, G.dlo_u);
-        const int chi = min((su < 0 && up_u) ? HALO + G.wu + HALO : HALO + G.wu, G.dhi_u);
+        const int kp = (K + 1) & ~1;                         // the K halo columns, in whole pairs: what the neighbour publishes
+        const int clo = max((su > 0 && up_u) ? HALO - kp : HALO, G.dlo_u);
+        const int chi = min((su < 0 && up_u) ? HALO + G.wu + kp : HALO + G.wu, G.dhi_u);
         const int q_lo = clo >> 1, nq = ((chi + 1) >> 1) - q_lo, nr = rhi - rlo;
         for (int e = tid; e < nr * nq; e += T) {
             const int r = e / nq, row = rlo + r, q = q_lo + (e - r * nq);
@@ -694,7 +737,7 @@ __device__ __forceinline__ void issue_load(TaskShared& S, const CUtensorMap* cma
 
 template <int PITCH>
 __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f2* __restrict__ smf,
-                         float* __restrict__ Itop_all, int* abortf)
+                         float* __restrict__ Itop_all, int* abortf, const unsigned seq)
 {
 
     const UnitDesc& U = S.U;
@@ -731,6 +774,8 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     const int n_m = U.n_m, npass = U.npass, K = U.K;
     const int nsteps = n_m * npass;
     const bool zmarch = (U.march == 2);
+    const bool tagged = U.xflag != 0;
+    const unsigned tag0 = seq << 12;                         // tags of this solve (never 0: the buffers start zeroed)
 
     // ---- coefficient planes through the TMA ring (started first: the tables below hide its latency)
     const CUtensorMap* const cmap = &maps.m[U.march];
@@ -817,7 +862,10 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
             const int blen = min(K, n_m - blk0);
             // ---- block start: wait for the unit, fetch halos and seam ghosts of the previous plane
             if (s_ > 0) {
-                if (!block_start<PITCH>(&S, S.Xb + (size_t)cur * NG * PS, S.stage0 + (size_t)stp * PS, pass, blk0, gblk, s_)) { bail = true; break; }
+                // tag of the strips of block gblk - 1; no strips were stored if their step was a skipped thick plane
+                const bool skipped = zmarch && !lastpass && blk0 > 0 && plane_of(U, blk0 - 1) < G.mthick;
+                if (!block_start<PITCH>(&S, S.Xb + (size_t)cur * NG * PS, S.stage0 + (size_t)stp * PS, pass, blk0, gblk, s_,
+                                        tag0 | ((unsigned)gblk & 0xfffu), skipped)) { bail = true; break; }
             }
             for (int j = 0; j < blen; ++j, ++s_) {
                 const int m = blk0 + j;
@@ -857,7 +905,8 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                         const bool strips = blk_last && more && !(zmarch && m == n_m - 1);
                         C.tail = 0;
                         TC.GhP = hist ? reinterpret_cast<f2*>(U.Gu) + ((size_t)(pass & 1) * n_m + m) * g_plane : nullptr;
-                        TC.XeP = strips ? reinterpret_cast<f2*>(U.Xex) + (size_t)(gblk & 1) * xe_par : nullptr;
+                        TC.XeP = strips ? reinterpret_cast<float4*>(U.Xex) + (size_t)(gblk & 1) * xe_par : nullptr;
+                        TC.tag = tag0 | ((unsigned)(gblk + 1) & 0xfffu);
                         C.xmask = IT_PART | (hist ? IT_FARC : 0u) | (strips ? IT_USTRIP : 0u);
                         C.a_prev = (pl - dir <= kstar) ? 1.f : 0.f; C.a_cur = (pl <= kstar) ? 1.f : 0.f;
                         C.zreg = 0;
@@ -893,7 +942,8 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 // ---- end of step; at a block end publish (release) before anybody waits
                 __syncthreads();
                 if (tid == 0) {
-                    if (blk_last && more) { __threadfence(); atomicAdd(U.barrier, 1); }
+                    // arrival (release): at every block end, or with the tagged exchange at the end of a pass only
+                    if (blk_last && more && (!tagged || m == n_m - 1)) { __threadfence(); atomicAdd(U.barrier, 1); }
                     const int ahead = NST - 1;               // planes in flight beyond the previous one
                     if (s_ + ahead < nsteps) {
                         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -918,7 +968,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
 template <int PITCH>
 __global__ void __launch_bounds__(RTS_SWEEP_THREADS, 1)
 rts_sweep_kernel(const __grid_constant__ SweepMaps maps, const UnitDesc* __restrict__ units, int nunits,
-                 int total_tickets, int* ticket_counter, float* __restrict__ Itop_all, int* abortf)
+                 int total_tickets, int* ticket_counter, float* __restrict__ Itop_all, int* abortf, unsigned seq)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(16) TaskShared S;
@@ -943,7 +993,7 @@ rts_sweep_kernel(const __grid_constant__ SweepMaps maps, const UnitDesc* __restr
             for (int w = threadIdx.x; w < (int)(sizeof(UnitDesc) / sizeof(int)); w += blockDim.x) dst[w] = src[w];
         }
         __syncthreads();
-        run_task<PITCH>(S, maps, ticket - S.U.ticket_begin, reinterpret_cast<f2*>(smem_raw), Itop_all, abortf);
+        run_task<PITCH>(S, maps, ticket - S.U.ticket_begin, reinterpret_cast<f2*>(smem_raw), Itop_all, abortf, seq);
     }
 }
 
