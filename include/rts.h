@@ -53,7 +53,8 @@ extern "C" {
 
 typedef struct rts_ctx rts_ctx;
 
-/* Create a solver for an nx*ny*nz node grid with spacings dx,dy,dz (cm) and nbands bands.
+/* [PAPER.md:78-82, 189: the RTS on a 3-D Cartesian block; 3 rays per octant]
+ * Create a solver for an nx*ny*nz node grid with spacings dx,dy,dz (cm) and nbands bands.
  * nx, ny >= 2 (periodic), nz >= 2, nbands >= 1.  Uses the current CUDA device.
  * Defaults: 24-ray set of BASELINE.json configs[0] (order: r = 3*octant + axis of the large
  * cosine, octant = bx + 2 by + 4 bz, b = 1 for a negative cosine; weights 1/24), 3 passes. */
@@ -61,7 +62,8 @@ int rts_create(rts_ctx** out, int nx, int ny, int nz,
                double dx_cm, double dy_cm, double dz_cm, int nbands);
 int rts_destroy(rts_ctx* ctx);
 
-/* Opacity and band-fraction tables; HOST pointers, copied to the device inside the call.
+/* [PAPER.md:195 "multi-band opacity scheme"; PAPER.md:79 interpol(); readings R8, R9]
+ * Opacity and band-fraction tables; HOST pointers, copied to the device inside the call.
  *   logkappa[b][iT][iP] (iP fastest) = log10 kappa_b on a uniform nT x nP grid in
  *   (log10 T, log10 P) spanning [logT_min, logT_max] x [logP_min, logP_max]; lookups are
  *   bilinear with clamping at the edges.  bandfrac[b][iT] = f_b on the same log10 T grid
@@ -70,10 +72,12 @@ int rts_set_tables(rts_ctx* ctx, int nT, int nP,
                    double logT_min, double logT_max, double logP_min, double logP_max,
                    const float* logkappa_host, const float* bandfrac_host);
 
-/* Number of sweep passes (periodic re-sweeps), >= 1.  Default 3. */
+/* [PAPER.md:72 "iterated 3-4 times", Fig. 8: the while loop around integrate(); R11, R12]
+ * Number of sweep passes (periodic re-sweeps with Jacobi seams), >= 1.  Default 3. */
 int rts_set_passes(rts_ctx* ctx, int npasses);
 
-/* Replace the ray set.  mu_xyz: HOST [nrays][3] directions of photon travel (need not be
+/* [PAPER.md:189 "a set of 3 rays per octant are used to integrate over the unit sphere"; R2, R3]
+ * Replace the ray set.  mu_xyz: HOST [nrays][3] directions of photon travel (need not be
  * normalised; mu_z must be non-zero); weights: HOST [nrays] (J = sum_r w_r I_r).
  * 1 <= nrays <= 256.  Invalidates the workspace size (call rts_workspace_bytes again). */
 int rts_set_rays(rts_ctx* ctx, int nrays, const double* mu_xyz_host, const double* weights_host);
@@ -82,7 +86,8 @@ int rts_get_rays(const rts_ctx* ctx, int* nrays, double* mu_xyz_host, double* we
 /* Number of rays with mu_z > 0 (second extent of I_top). */
 int rts_num_up_rays(const rts_ctx* ctx);
 
-/* Tuning hooks (optional).  march = 0,1,2 selects the sweeps that march along x, y, z.  A sweep
+/* [PAPER.md:221-239: integrate() is the hot spot; its wavefront is re-organised as a plane march, DESIGN.md 7.2]
+ * Tuning hooks (optional).  march = 0,1,2 selects the sweeps that march along x, y, z.  A sweep
  * tile is tile_u nodes of the unit-stride transverse axis (rounded up to a multiple of 4,
  * <= 248) times tile_v nodes of the other transverse axis (<= 120); 0 = the planner's choice.
  * Tiles exchange halos every `steps` planes (1..4; 0 = default 4) and recompute a halo of that
@@ -96,13 +101,15 @@ int rts_set_ctas_per_sm(rts_ctx* ctx, int ctas_per_sm);
  * overlaps the current step), 2 (smaller footprint: larger tiles or two CTAs per SM), 0 = planner's choice. */
 int rts_set_ring_depth(rts_ctx* ctx, int stages);
 
-/* Bytes of device workspace the current configuration needs (0 on error). */
+/* [PAPER.md:249-251: transposed copies of the coefficient arrays -- here two layouts in this workspace, DESIGN.md 6]
+ * Bytes of device workspace the current configuration needs (0 on error). */
 size_t rts_workspace_bytes(rts_ctx* ctx);
 /* Hand over a DEVICE workspace of at least rts_workspace_bytes(), 256-byte aligned.  It must
  * stay valid until the ctx is destroyed or another workspace is set. */
 int rts_set_workspace(rts_ctx* ctx, void* workspace_dev, size_t bytes);
 
-/* The hot path.  DEVICE pointers: rho, T, P in [nz][ny][nx]; Qrad out [nz][ny][nx];
+/* [PAPER.md:197-217 Fig. 8: interpol(); iterate { integrate(); exchange } ; flux() -- stages A-E above]
+ * The hot path.  DEVICE pointers: rho, T, P in [nz][ny][nx]; Qrad out [nz][ny][nx];
  * Itop out [nbands][n_up][ny][nx] or NULL (not wanted).  Qrad must be 16-byte aligned.  stream: a cudaStream_t passed as
  * void* (NULL = default stream).  Asynchronous on that stream; errors of the asynchronous
  * part surface at the next rts_sync_check / synchronising call. */
@@ -123,7 +130,8 @@ int rts_set_flux_blend(rts_ctx* ctx, double tau0);
 int rts_solve_flux(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const float* P_dev,
                    float* Qrad_dev, float* Itop_dev, float* Frad_dev, float* Qdiv_dev, float* Qblend_dev, void* stream);
 
-/* Same solve with HOST buffers (pinned or pageable): copies rho,T,P to the device, solves,
+/* [same operation as rts_solve; the end-to-end entry bench.py's `e2e` times]
+ * Same solve with HOST buffers (pinned or pageable): copies rho,T,P to the device, solves,
  * copies Qrad (and Itop if non-NULL) back, synchronises.  The staging buffers live in the
  * workspace (rts_workspace_bytes accounts for them). */
 int rts_solve_host(rts_ctx* ctx, const float* rho_host, const float* T_host, const float* P_host,
@@ -145,18 +153,21 @@ int rts_nodes_to_cells(rts_ctx* ctx, const float* node_dev, float* cell_dev, voi
 int rts_solve_cells(rts_ctx* ctx, const float* rho_cells_dev, const float* T_cells_dev, const float* P_cells_dev,
                     float* Qrad_cells_dev, float* Itop_dev, void* stream);
 
-/* Stage A alone, for per-stage parity: DEVICE outputs kaprho, S each [nbands][nz][ny][nx]. */
+/* [PAPER.md:79, 204 interpol(); DESIGN.md 1 row A]
+ * Stage A alone, for per-stage parity: DEVICE outputs kaprho, S each [nbands][nz][ny][nx]. */
 int rts_coefficients(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const float* P_dev,
                      float* kaprho_dev, float* S_dev, void* stream);
 
-/* Synchronise `stream` and report the device-side status of the last solve
+/* [no paper passage: error reporting of the persistent kernel of DESIGN.md 7.2]
+ * Synchronise `stream` and report the device-side status of the last solve
  * (RTS_OK, RTS_ETIMEOUT if the sweep watchdog fired, RTS_ECUDA). */
 int rts_sync_check(rts_ctx* ctx, void* stream);
 
-/* Thick-plane shortcut (default on).  Where every optical path of a z-march ray on a level pair
+/* [SURVEY 7, lever 4.ii; only the seam intensities change between the iterations]
+ * Thick-plane shortcut (default on).  Where every optical path of a z-march ray on a level pair
  * exceeds 88.5 the fp32 exp underflows to exactly 0 and the update does not depend on the carried
  * intensity; the sweeps along z skip those planes in the non-final passes.  Results are bit-identical
- * for I_top and identical up to the summation order of the heating atomics.
+ * for I_top and for Q_rad in the final pass (the heating is summed in a fixed order, no atomics).
  * rts_thick_levels: after a solve, HOST out [nbands] = number of level pairs from the bottom that were
  * found thick (synchronises `stream`); skipped updates = levels * nx * ny * (z-march rays) * (passes-1). */
 int rts_set_thick_skip(rts_ctx* ctx, int on);
@@ -173,13 +184,15 @@ int rts_thick_levels(rts_ctx* ctx, int* levels_host, void* stream);
 int rts_set_shard(rts_ctx* ctx, int rank, int nranks);
 int rts_shard_info(rts_ctx* ctx, int* units_mine, int* units_all);
 
-/* Per-stage device timing of the last rts_solve (CUDA events recorded on the solve stream
+/* [measurement only]
+ * Per-stage device timing of the last rts_solve (CUDA events recorded on the solve stream
  * inside rts_solve).  rts_last_timing waits for the solve and fills ms4 (HOST) with
  * [0] stage A + switch heights, [1] all sweep launches, [2] finalize, [3] whole solve. */
 int rts_enable_timing(rts_ctx* ctx, int on);
 int rts_last_timing(rts_ctx* ctx, float* ms4_host);
 
-/* Plan facts for reporting: what[0] = kernels launched per solve, [1] = sweep tasks (tiles of
+/* [measurement only]
+ * Plan facts for reporting: what[0] = kernels launched per solve, [1] = sweep tasks (tiles of
  * all units), [2] = CTAs per SM of the sweep kernel, [3] = sweep units (march axis x direction
  * x ray group x band), [4] = threads per CTA, [5] = dynamic shared memory per CTA (bytes),
  * [6] = sweep grid (persistent CTAs), [7] = exchange interval, [8..10] = tile_v of march x,y,z,
