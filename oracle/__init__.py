@@ -62,6 +62,11 @@ def _load():
         _lib.oracle_solve.argtypes = ([_I, _I, _I, _D, _D, _D, _I, _I, _I, _D, _D, _D, _D,
                                        _PF, _PF, _I, _I, _PD, _PD, _PF, _PF, _PF,
                                        _PD, _PD, _PD, _PD, _I])
+        _lib.oracle_sweep_ray_tol.restype = _I
+        _lib.oracle_sweep_ray_tol.argtypes = [_I, _I, _I, _D, _D, _D, _PD, _D, _I, _PD, _PD, _PD, _PD, _PD, _PD, _PD, _PD, _PI]
+        _lib.oracle_solve_tol.restype = _I
+        _lib.oracle_solve_tol.argtypes = ([_I, _I, _I, _D, _D, _D, _I, _I, _I, _D, _D, _D, _D, _PF, _PF,
+                                           _D, _I, _I, _I, _I, _PD, _PD, _PF, _PF, _PF, _PD, _PD, _PD, _PI, _PD, _I])
         _lib.oracle_flux_heating.restype = _I
         _lib.oracle_flux_heating.argtypes = [_I, _I, _I, _D, _D, _D, _PD, _PD, _PD, _D, _PD, _PD]
         _lib.oracle_num_threads.restype = _I
@@ -133,6 +138,53 @@ def sweep_ray(nx, ny, nz, dx, dy, dz, mu, npasses, kaprho, S,
     if rc != 0:
         raise RuntimeError(f"oracle_sweep_ray failed: {rc}")
     return I
+
+
+def sweep_ray_tol(nx, ny, nz, dx, dy, dz, mu, tol, max_passes, kaprho, S, warm=None):
+    """O-12 for one band and one ray: iterate until the seam faces change by <= tol * max|I| on them.
+    warm = (faceX [nz][ny], faceY [nz][nx]) of I^(0), or None.  Returns (I, (faceX, faceY), relerr per pass, passes)."""
+    lib = _load()
+    kaprho = np.ascontiguousarray(kaprho, dtype=np.float64)
+    S = np.ascontiguousarray(S, dtype=np.float64)
+    mu = np.ascontiguousarray(mu, dtype=np.float64)
+    wx = np.ascontiguousarray(warm[0], dtype=np.float64) if warm is not None else None
+    wy = np.ascontiguousarray(warm[1], dtype=np.float64) if warm is not None else None
+    I = np.empty((nz, ny, nx), dtype=np.float64)
+    fx = np.empty((nz, ny), dtype=np.float64); fy = np.empty((nz, nx), dtype=np.float64)
+    rel = np.zeros(max_passes, dtype=np.float64)
+    used = ctypes.c_int(0)
+    rc = lib.oracle_sweep_ray_tol(nx, ny, nz, dx, dy, dz, _pd(mu), float(tol), int(max_passes), _pd(kaprho), _pd(S),
+                                  _pd(wx), _pd(wy), _pd(I), _pd(fx), _pd(fy), _pd(rel), ctypes.byref(used))
+    if rc != 0:
+        raise RuntimeError(f"oracle_sweep_ray_tol failed: {rc}")
+    return I, (fx, fy), rel[:used.value].copy(), used.value
+
+
+def solve_tol(inp, tol: float, max_passes: int, mode: int = 1, faces: Optional[np.ndarray] = None, nthreads: int = 0):
+    """O-12, all bands and rays.  mode 0: every (band, ray) stops on its own error; mode 1: one pass count for all.
+    faces: None (cold start) or the array returned by an earlier call (warm start).
+    Returns (Q, Itop, faces [nb*nrays][nz*ny + nz*nx], passes_used [nb*nrays], relerr per pass (mode 1))."""
+    lib = _load()
+    Q = np.empty(inp.shape, dtype=np.float64)
+    Itop = np.empty((inp.nbands, inp.n_up, inp.ny, inp.nx), dtype=np.float64)
+    mu = np.ascontiguousarray(inp.mu, dtype=np.float64)
+    wq = np.ascontiguousarray(inp.wq, dtype=np.float64)
+    ntask = inp.nbands * inp.nrays
+    nf = inp.nz * inp.ny + inp.nz * inp.nx
+    warm = faces is not None
+    fc = np.ascontiguousarray(faces, dtype=np.float64).copy() if warm else np.empty((ntask, nf), dtype=np.float64)
+    assert fc.shape == (ntask, nf)
+    used = np.zeros(ntask, dtype=np.int32)
+    rel = np.zeros(max_passes, dtype=np.float64)
+    rc = lib.oracle_solve_tol(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.nbands, inp.nT, inp.nP,
+                              inp.logT_min, inp.logT_max, inp.logP_min, inp.logP_max,
+                              _pf(inp.logkappa), _pf(inp.bandfrac),
+                              float(tol), int(max_passes), int(mode), int(warm),
+                              inp.nrays, _pd(mu), _pd(wq), _pf(inp.rho), _pf(inp.T), _pf(inp.P),
+                              _pd(Q), _pd(Itop), _pd(fc), used.ctypes.data_as(_PI), _pd(rel), nthreads)
+    if rc != 0:
+        raise RuntimeError(f"oracle_solve_tol failed: {rc}")
+    return Q, Itop, fc, used, rel[:int(used.max())].copy()
 
 
 def solve(inp, nthreads: int = 0, want_J: bool = False, want_F: bool = False):

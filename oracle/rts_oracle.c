@@ -32,7 +32,11 @@
  * memoised recursive evaluator on tiny grids, pass fixed point, I-form vs D-form,
  * table stage closed forms, psi check values of SURVEY 8(c) O-6; staggering (O-9):
  * constants, midpoints of linear fields, Fourier-mode attenuation cos(pi m/n),
- * edge levels, sum rule of the back-averaging.  Parity: pinned.
+ * edge levels, sum rule of the back-averaging; flux (O-10 / O-11): thick-limit closed form of all
+ * three components, isothermal zero, mirror flip, numpy gradient, telescoping, blend weights;
+ * error-controlled iteration (O-12): bit-identity with the pinned fixed-pass sweep at equal pass
+ * counts, err_p = face change of consecutive fixed-pass solutions, stop rule, warm start = one
+ * more pass.  Parity: pinned.
  *
  * Layout: all fields [nz][ny][nx], x fastest, idx = (k*ny + j)*nx + i; z is up,
  * k = 0 is the bottom.  cgs units.
@@ -137,6 +141,51 @@ void oracle_psi(double dtau, double* E, double* psi_u, double* psi_p)
     }
 }
 
+/* One pass of O-5 in place: X holds pass p-1 on entry and pass p on exit; faceX / faceY are the
+ * faces i = iface and j = jface of pass p-1 (the only values of pass p-1 that are read). */
+static void sweep_one_pass(int nx, int ny, int nz, int sx, int sy, int sz, int kdir,
+                           int off[4][3], const double* w, double ds,
+                           const double* kaprho, const double* S, int form,
+                           const double* faceX, const double* faceY, double* X)
+{
+    for (int kk = 0; kk < nz; ++kk) {
+        int k = (sz > 0) ? kk : nz - 1 - kk;
+        if (k == kdir) continue;                        /* Dirichlet plane: not updated */
+        for (int jj = 0; jj < ny; ++jj) {
+            int j = (sy > 0) ? jj : ny - 1 - jj;
+            for (int ii = 0; ii < nx; ++ii) {
+                int i = (sx > 0) ? ii : nx - 1 - ii;
+                size_t n = ((size_t)k * ny + j) * nx + i;
+                double Xu = 0.0, ku = 0.0, Su = 0.0;
+                for (int q = 0; q < 4; ++q) {
+                    int iu = i + off[q][0], ju = j + off[q][1], kq = k + off[q][2];
+                    int wrapx = 0, wrapy = 0;
+                    if (iu < 0) { iu += nx; wrapx = 1; } else if (iu >= nx) { iu -= nx; wrapx = 1; }
+                    if (ju < 0) { ju += ny; wrapy = 1; } else if (ju >= ny) { ju -= ny; wrapy = 1; }
+                    /* kq stays inside [0,nz): the Dirichlet plane is never updated */
+                    size_t m = ((size_t)kq * ny + ju) * nx + iu;
+                    double xv;
+                    if (wrapx) xv = faceX[(size_t)kq * ny + ju];       /* iu == iface */
+                    else if (wrapy) xv = faceY[(size_t)kq * nx + iu];  /* ju == jface */
+                    else xv = X[m];
+                    Xu += w[q] * xv;
+                    ku += w[q] * kaprho[m];
+                    Su += w[q] * S[m];
+                }
+                double dtau = 0.5 * (ku + kaprho[n]) * ds;
+                double E, pu, pp;
+                oracle_psi(dtau, &E, &pu, &pp);
+                if (!form) {
+                    X[n] = Xu * E + pu * Su + pp * S[n];
+                } else {
+                    /* D_p = D_u E - (S_p - S_u)(1-E)/dtau ; (1-E)/dtau = E + psi_u */
+                    X[n] = Xu * E - (S[n] - Su) * (E + pu);
+                }
+            }
+        }
+    }
+}
+
 /* ---------------------------------------------------------------------------
  * O-4..O-6  Formal solution for ONE band and ONE ray, all passes.
  *
@@ -211,46 +260,227 @@ int oracle_sweep_ray(int nx, int ny, int nz, double dx, double dy, double dz,
             for (int j = 0; j < ny; ++j) faceX[(size_t)k * ny + j] = X[((size_t)k * ny + j) * nx + iface];
             for (int i = 0; i < nx; ++i) faceY[(size_t)k * nx + i] = X[((size_t)k * ny + jface) * nx + i];
         }
-        for (int kk = 0; kk < nz; ++kk) {
-            int k = (sz > 0) ? kk : nz - 1 - kk;
-            if (k == kdir) continue;                        /* Dirichlet plane: not updated */
-            for (int jj = 0; jj < ny; ++jj) {
-                int j = (sy > 0) ? jj : ny - 1 - jj;
-                for (int ii = 0; ii < nx; ++ii) {
-                    int i = (sx > 0) ? ii : nx - 1 - ii;
-                    size_t n = ((size_t)k * ny + j) * nx + i;
-                    double Xu = 0.0, ku = 0.0, Su = 0.0;
-                    for (int q = 0; q < 4; ++q) {
-                        int iu = i + off[q][0], ju = j + off[q][1], kq = k + off[q][2];
-                        int wrapx = 0, wrapy = 0;
-                        if (iu < 0) { iu += nx; wrapx = 1; } else if (iu >= nx) { iu -= nx; wrapx = 1; }
-                        if (ju < 0) { ju += ny; wrapy = 1; } else if (ju >= ny) { ju -= ny; wrapy = 1; }
-                        /* kq stays inside [0,nz): the Dirichlet plane is never updated */
-                        size_t m = ((size_t)kq * ny + ju) * nx + iu;
-                        double xv;
-                        if (wrapx) xv = faceX[(size_t)kq * ny + ju];       /* iu == iface */
-                        else if (wrapy) xv = faceY[(size_t)kq * nx + iu];  /* ju == jface */
-                        else xv = X[m];
-                        Xu += w[q] * xv;
-                        ku += w[q] * kaprho[m];
-                        Su += w[q] * S[m];
-                    }
-                    double dtau = 0.5 * (ku + kaprho[n]) * ds;
-                    double E, pu, pp;
-                    oracle_psi(dtau, &E, &pu, &pp);
-                    if (!form) {
-                        X[n] = Xu * E + pu * Su + pp * S[n];
-                    } else {
-                        /* D_p = D_u E - (S_p - S_u)(1-E)/dtau ; (1-E)/dtau = E + psi_u */
-                        X[n] = Xu * E - (S[n] - Su) * (E + pu);
-                    }
-                }
-            }
-        }
+        sweep_one_pass(nx, ny, nz, sx, sy, sz, kdir, off, w, ds, kaprho, S, form, faceX, faceY, X);
     }
     if (form) for (size_t n = 0; n < N; ++n) I[n] = X[n] + S[n];
     free(faceX); free(faceY);
     return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-12  Error-controlled iteration and warm start (Fig. 8
+ *       "while(g_maxerr > THRESHOLD) { readbuf(); integrate(); writebuf(); exchange(); err = error();
+ *       MPI_Allreduce(&err, &g_maxerr); }", "iterates the intensities at the boundaries
+ *       ... until the errors are within a prescribed tolerance"; reading R22).
+ *   The boundary intensities of the periodic box are the two faces O-5 keeps: i = iface (all j, k)
+ *   and j = jface (all i, k).  After pass p
+ *       err_p = max over both faces |I^(p) - I^(p-1)|,   scale_p = max over both faces |I^(p)|,
+ *   and the iteration stops at the first p with err_p <= tol * scale_p, or at p = max_passes.
+ *   Warm start: the faces of I^(0) are given (the converged faces of an earlier solve) instead of
+ *   taken from I^(0) = S; no other value of I^(0) is ever read.
+ *
+ *  State of one (band, ray) problem between passes: X (the whole field) and its two faces.
+ * ------------------------------------------------------------------------- */
+typedef struct {
+    int as, sx, sy, sz, kdir, iface, jface;
+    int off[4][3];
+    double w[4], ds;
+} ray_setup;
+
+static int ray_setup_init(int nx, int ny, int nz, double dx, double dy, double dz, const double* mu, ray_setup* r)
+{
+    int sg[3];
+    double f[3];
+    if (oracle_ray_geometry(dx, dy, dz, mu, &r->as, sg, &r->ds, f) != 0) return -1;
+    r->sx = sg[0]; r->sy = sg[1]; r->sz = sg[2];
+    r->kdir = (r->sz > 0) ? 0 : nz - 1;
+    const int as = r->as, c = (as == 0) ? 1 : 0, d = (as == 2) ? 1 : 2;
+    for (int ec = 0; ec < 2; ++ec)
+        for (int ed = 0; ed < 2; ++ed) {
+            int q = ec * 2 + ed;
+            r->off[q][0] = r->off[q][1] = r->off[q][2] = 0;
+            r->off[q][as] = -sg[as];
+            r->off[q][c] = -ec * sg[c];
+            r->off[q][d] = -ed * sg[d];
+            r->w[q] = (ec ? f[c] : 1.0 - f[c]) * (ed ? f[d] : 1.0 - f[d]);
+        }
+    r->iface = (r->sx > 0) ? nx - 1 : 0;
+    r->jface = (r->sy > 0) ? ny - 1 : 0;
+    return 0;
+}
+
+/* I^(0) of O-5 into X; the faces of I^(0) into faceX / faceY (or the warm faces, if given) */
+static void tol_init(int nx, int ny, int nz, const ray_setup* r, const double* S,
+                     const double* warmX, const double* warmY, double* X, double* faceX, double* faceY)
+{
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t n = ((size_t)k * ny + j) * nx + i;
+                X[n] = (k == r->kdir) ? ((r->sz > 0) ? S[n] : 0.0) : S[n];
+            }
+    for (int k = 0; k < nz; ++k) {
+        for (int j = 0; j < ny; ++j)
+            faceX[(size_t)k * ny + j] = warmX ? warmX[(size_t)k * ny + j] : X[((size_t)k * ny + j) * nx + r->iface];
+        for (int i = 0; i < nx; ++i)
+            faceY[(size_t)k * nx + i] = warmY ? warmY[(size_t)k * nx + i] : X[((size_t)k * ny + r->jface) * nx + i];
+    }
+}
+
+/* one pass + error(): faces hold pass p-1 on entry and pass p on exit */
+static void tol_pass(int nx, int ny, int nz, ray_setup* r, const double* kaprho, const double* S,
+                     double* X, double* faceX, double* faceY, double* err, double* scale)
+{
+    sweep_one_pass(nx, ny, nz, r->sx, r->sy, r->sz, r->kdir, r->off, r->w, r->ds, kaprho, S, 0, faceX, faceY, X);
+    double e = 0.0, sc = 0.0;
+    for (int k = 0; k < nz; ++k) {
+        for (int j = 0; j < ny; ++j) {
+            const double v = X[((size_t)k * ny + j) * nx + r->iface], o = faceX[(size_t)k * ny + j];
+            if (fabs(v - o) > e) e = fabs(v - o);
+            if (fabs(v) > sc) sc = fabs(v);
+            faceX[(size_t)k * ny + j] = v;
+        }
+        for (int i = 0; i < nx; ++i) {
+            const double v = X[((size_t)k * ny + r->jface) * nx + i], o = faceY[(size_t)k * nx + i];
+            if (fabs(v - o) > e) e = fabs(v - o);
+            if (fabs(v) > sc) sc = fabs(v);
+            faceY[(size_t)k * nx + i] = v;
+        }
+    }
+    *err = e; *scale = sc;
+}
+
+/* ONE band and ONE ray, iterated to the tolerance.  warmX [nz][ny] / warmY [nz][nx]: faces of I^(0) or NULL.
+ * Outputs: I [nz][ny][nx]; faceX_out / faceY_out (may be NULL): the faces of the final pass; relerr
+ * [max_passes]: err_p / scale_p of every pass run; *passes_used. */
+int oracle_sweep_ray_tol(int nx, int ny, int nz, double dx, double dy, double dz,
+                         const double* mu, double tol, int max_passes,
+                         const double* kaprho, const double* S,
+                         const double* warmX, const double* warmY,
+                         double* I, double* faceX_out, double* faceY_out, double* relerr, int* passes_used)
+{
+    ray_setup r;
+    if (nx < 1 || ny < 1 || nz < 2 || max_passes < 1 || !passes_used) return -1;
+    if (ray_setup_init(nx, ny, nz, dx, dy, dz, mu, &r) != 0) return -1;
+    double* faceX = (double*)malloc(sizeof(double) * (size_t)nz * ny);
+    double* faceY = (double*)malloc(sizeof(double) * (size_t)nz * nx);
+    if (!faceX || !faceY) { free(faceX); free(faceY); return -2; }
+    tol_init(nx, ny, nz, &r, S, warmX, warmY, I, faceX, faceY);
+    int p = 0;
+    while (p < max_passes) {
+        double e, sc;
+        tol_pass(nx, ny, nz, &r, kaprho, S, I, faceX, faceY, &e, &sc);
+        if (relerr) relerr[p] = (sc > 0.0) ? e / sc : 0.0;
+        ++p;
+        if (e <= tol * sc) break;
+    }
+    *passes_used = p;
+    if (faceX_out) memcpy(faceX_out, faceX, sizeof(double) * (size_t)nz * ny);
+    if (faceY_out) memcpy(faceY_out, faceY, sizeof(double) * (size_t)nz * nx);
+    free(faceX); free(faceY);
+    return 0;
+}
+
+/* All bands and rays, iterated to the tolerance; J, Q and I_top as in O-7.
+ *   mode 0: every (band, ray) problem stops on its own error (Fig. 8 read literally: the while loop
+ *           is inside the ray loop);
+ *   mode 1: all problems iterate together until the largest err_p / scale_p of any of them is <= tol
+ *           (one pass count for the whole solve).
+ *   faces: NULL, or in/out [nb*nrays][nz*ny + nz*nx]: on entry (if warm != 0) the faces of I^(0) of
+ *   every problem, on exit the faces of its final pass.  passes_used [nb*nrays];  relerr (may be NULL)
+ *   [max_passes]: mode 1 only, the largest err_p / scale_p of every pass run. */
+int oracle_solve_tol(int nx, int ny, int nz, double dx, double dy, double dz,
+                     int nb, int nT, int nP,
+                     double logT_min, double logT_max, double logP_min, double logP_max,
+                     const float* logkappa, const float* bandfrac,
+                     double tol, int max_passes, int mode, int warm,
+                     int nrays, const double* mu, const double* wq,
+                     const float* rho, const float* T, const float* P,
+                     double* Q, double* Itop, double* faces, int* passes_used, double* relerr, int nthreads)
+{
+    if (nx < 1 || ny < 1 || nz < 2 || nb < 1 || nrays < 1 || max_passes < 1 || !passes_used) return -1;
+    if (warm && !faces) return -1;
+    const size_t N = (size_t)nx * ny * nz, nfx = (size_t)nz * ny, nfy = (size_t)nz * nx, nf = nfx + nfy;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+    const int ntask = nb * nrays;
+    double* kaprho = (double*)malloc(sizeof(double) * N * nb);
+    double* S = (double*)malloc(sizeof(double) * N * nb);
+    double* X = (double*)malloc(sizeof(double) * N * (size_t)ntask);      /* every problem's field */
+    double* fc = (double*)malloc(sizeof(double) * nf * (size_t)ntask);    /* ... and faces */
+    double* te = (double*)malloc(sizeof(double) * 2 * (size_t)ntask);
+    ray_setup* rs = (ray_setup*)malloc(sizeof(ray_setup) * (size_t)nrays);
+    int* done = (int*)calloc((size_t)ntask, sizeof(int));
+    if (!kaprho || !S || !X || !fc || !te || !rs || !done) { free(kaprho); free(S); free(X); free(fc); free(te); free(rs); free(done); return -2; }
+    int rc = oracle_coefficients(nx, ny, nz, nb, nT, nP, logT_min, logT_max, logP_min, logP_max,
+                                 logkappa, bandfrac, rho, T, P, kaprho, S);
+    for (int r = 0; r < nrays && rc == 0; ++r) rc = ray_setup_init(nx, ny, nz, dx, dy, dz, mu + 3 * r, &rs[r]);
+    if (rc == 0) {
+        int t;
+#pragma omp parallel for schedule(static, 1)
+        for (t = 0; t < ntask; ++t) {
+            const int b = t / nrays, r = t % nrays;
+            const double* wf = warm ? faces + (size_t)t * nf : NULL;
+            tol_init(nx, ny, nz, &rs[r], S + (size_t)b * N, wf, wf ? wf + nfx : NULL,
+                     X + (size_t)t * N, fc + (size_t)t * nf, fc + (size_t)t * nf + nfx);
+            passes_used[t] = 0;
+        }
+        for (int p = 0; p < max_passes; ++p) {
+            int active = 0;
+#pragma omp parallel for schedule(static, 1) reduction(+ : active)
+            for (t = 0; t < ntask; ++t) {
+                if (done[t]) continue;
+                const int b = t / nrays, r = t % nrays;
+                ray_setup rr = rs[r];
+                tol_pass(nx, ny, nz, &rr, kaprho + (size_t)b * N, S + (size_t)b * N,
+                         X + (size_t)t * N, fc + (size_t)t * nf, fc + (size_t)t * nf + nfx, &te[2 * t], &te[2 * t + 1]);
+                passes_used[t] = p + 1;
+                ++active;
+            }
+            if (!active) break;
+            double worst = 0.0;
+            for (t = 0; t < ntask; ++t) {
+                if (done[t]) continue;
+                const double rel = (te[2 * t + 1] > 0.0) ? te[2 * t] / te[2 * t + 1] : 0.0;
+                if (rel > worst) worst = rel;
+                if (mode == 0 && te[2 * t] <= tol * te[2 * t + 1]) done[t] = 1;
+            }
+            if (mode == 1) {
+                if (relerr) relerr[p] = worst;
+                if (worst <= tol) break;
+            }
+        }
+        /* J, Q, I_top in (band, ray) order at every node, as in O-7 */
+        int nup = 0;
+        for (int r = 0; r < nrays; ++r) nup += (mu[3 * r + 2] > 0.0);
+        long n;
+#pragma omp parallel for schedule(static)
+        for (n = 0; n < (long)N; ++n) {
+            double q = 0.0;
+            for (int b = 0; b < nb; ++b) {
+                double J = 0.0;
+                for (int r = 0; r < nrays; ++r) J += wq[r] * X[((size_t)b * nrays + r) * N + n];
+                q += 4.0 * ORACLE_PI * kaprho[(size_t)b * N + n] * (J - S[(size_t)b * N + n]);
+            }
+            Q[n] = q;
+        }
+        if (Itop) {
+            int u = 0;
+            for (int r = 0; r < nrays; ++r) {
+                if (!(mu[3 * r + 2] > 0.0)) continue;
+                for (int b = 0; b < nb; ++b)
+                    memcpy(Itop + ((size_t)b * nup + u) * ny * nx,
+                           X + ((size_t)b * nrays + r) * N + (size_t)(nz - 1) * ny * nx, sizeof(double) * ny * nx);
+                ++u;
+            }
+        }
+        if (faces) memcpy(faces, fc, sizeof(double) * nf * (size_t)ntask);
+    }
+    free(kaprho); free(S); free(X); free(fc); free(te); free(rs); free(done);
+    return rc;
 }
 
 /* ---------------------------------------------------------------------------

@@ -655,3 +655,95 @@ def test_O11_blend_weights():
     # limits: tau0 -> infinity gives the J - S form, tau0 -> 0 the flux divergence
     assert np.allclose(oracle.flux_heating(inp, F, QJ, k0, tau0=1e30)[1], QJ, rtol=1e-12)
     assert np.allclose(oracle.flux_heating(inp, F, QJ, k0, tau0=1e-30)[1], Qdiv, rtol=1e-12)
+
+
+# --------------------------------------------------------------------------- O-12 (NEXT #3): error-controlled iteration
+def _faces(I, mu):
+    """The two faces O-5 keeps: i = iface (all j, k) and j = jface (all i, k)."""
+    nz, ny, nx = I.shape
+    iface = nx - 1 if mu[0] > 0 else 0
+    jface = ny - 1 if mu[1] > 0 else 0
+    return I[:, :, iface].copy(), I[:, jface, :].copy()
+
+
+def test_O12_error_is_the_face_change_of_the_fixed_pass_sweeps_and_the_stop_rule():
+    """The error-controlled sweep is tied to the pinned fixed-pass one: after p passes it holds the same field
+    bit for bit, its err_p / scale_p is the change of the two seam faces between the p-pass and the (p-1)-pass
+    solution (pass 0: I^(0) = S, Dirichlet value on the Dirichlet plane) over the largest face intensity, and it
+    stops at the first pass whose error is within the tolerance."""
+    base = inputs.make_config(1, grid=(8, 8, 16), npasses=1)
+    kap, S = oracle.coefficients(base)
+    g = (8, 8, 16, base.dx, base.dy, base.dz)
+    for mu in (base.mu[0], base.mu[7], base.mu[14]):           # an x-, a y- and a z-march ray, different octants
+        fixed = [None] + [oracle.sweep_ray(*g, mu, P, kap[0], S[0]) for P in range(1, 9)]
+        I0 = S[0].copy()
+        kdir = 0 if mu[2] > 0 else 15
+        if mu[2] < 0:
+            I0[kdir] = 0.0
+        fixed[0] = I0
+        want = []
+        for P in range(1, 9):
+            (ax, ay), (bx, by) = _faces(fixed[P], mu), _faces(fixed[P - 1], mu)
+            err = max(np.abs(ax - bx).max(), np.abs(ay - by).max())
+            want.append(err / max(np.abs(ax).max(), np.abs(ay).max()))
+        I, fc, rel, used = oracle.sweep_ray_tol(*g, mu, -1.0, 8, kap[0], S[0])
+        assert used == 8 and np.array_equal(I, fixed[8])       # a negative tolerance never stops early
+        assert np.allclose(rel, want, rtol=1e-12, atol=0)
+        assert np.array_equal(fc[0], _faces(fixed[8], mu)[0]) and np.array_equal(fc[1], _faces(fixed[8], mu)[1])
+        # P8: the change decays from pass to pass and reaches exactly 0 once every characteristic has been traced
+        # back to the inflow plane (the dependence of an upward ray only ever runs downwards)
+        assert all(b <= a for a, b in zip(rel[:-1], rel[1:])) and rel[-1] < 1e-3 * rel[0] and rel[0] > 0
+        nz_ = int((rel > 0).sum())
+        assert nz_ >= 3
+        for k in range(1, nz_):                                # a tolerance between err_k and err_{k+1} stops after k+1 passes
+            tol = math.sqrt(want[k - 1] * want[k])
+            Ik, _, relk, usedk = oracle.sweep_ray_tol(*g, mu, tol, 8, kap[0], S[0])
+            assert usedk == k + 1 and np.array_equal(Ik, fixed[k + 1]) and np.array_equal(relk, rel[:k + 1])
+        assert oracle.sweep_ray_tol(*g, mu, 1e-30, 3, kap[0], S[0])[3] == 3      # the cap
+
+
+def test_O12_warm_start_continues_the_iteration():
+    """Warm start = the faces of an earlier solve as the faces of I^(0): one more pass from the P-pass faces is
+    pass P+1 bit for bit, and from converged faces the first pass already meets the tolerance."""
+    base = inputs.make_config(1, grid=(8, 8, 16), npasses=1)
+    kap, S = oracle.coefficients(base)
+    g = (8, 8, 16, base.dx, base.dy, base.dz)
+    mu = base.mu[3]
+    I3, f3, rel3, _ = oracle.sweep_ray_tol(*g, mu, -1.0, 3, kap[0], S[0])
+    I4w, f4w, rel4w, used = oracle.sweep_ray_tol(*g, mu, -1.0, 1, kap[0], S[0], warm=f3)
+    I4 = oracle.sweep_ray(*g, mu, 4, kap[0], S[0])
+    assert used == 1 and np.array_equal(I4w, I4)
+    I8, f8, rel8, _ = oracle.sweep_ray_tol(*g, mu, -1.0, 8, kap[0], S[0])
+    tol = 2.0 * rel8[-1]
+    cold = oracle.sweep_ray_tol(*g, mu, tol, 20, kap[0], S[0])
+    warm = oracle.sweep_ray_tol(*g, mu, tol, 20, kap[0], S[0], warm=cold[1])
+    assert cold[3] >= 7 and warm[3] == 1 and warm[2][0] <= tol
+    assert np.abs(warm[0] - cold[0]).max() <= tol * np.abs(cold[0]).max()
+
+
+def test_O12_solve_modes_against_the_fixed_pass_solve():
+    """All bands and rays: with a negative tolerance and max_passes = P both modes are the fixed P-pass solve (Q to summation
+    rounding, I_top bit for bit); mode 0 stops every (band, ray) problem on its own error, mode 1 runs all of
+    them as long as the slowest one needs; a warm restart from the returned faces needs one pass."""
+    inp = _small_problem(nx=10, ny=8, nz=9, nb=2, P=3)
+    Q3, I3 = oracle.solve(inp)
+    for mode in (0, 1):
+        Q, It, fc, used, rel = oracle.solve_tol(inp, -1.0, 3, mode=mode)
+        assert (used == 3).all() and np.array_equal(It, I3)
+        assert np.abs(Q - Q3).max() <= 1e-12 * np.abs(Q3).max()
+    kap, S = oracle.coefficients(inp)
+    g = (inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz)
+    tol = 1e-4
+    each = np.array([oracle.sweep_ray_tol(*g, inp.mu[r], tol, 30, kap[b], S[b])[3]
+                     for b in range(inp.nbands) for r in range(inp.nrays)])
+    Q0, I0, f0, used0, _ = oracle.solve_tol(inp, tol, 30, mode=0)
+    assert np.array_equal(used0, each) and each.min() < each.max()
+    Q1, I1, f1, used1, rel1 = oracle.solve_tol(inp, tol, 30, mode=1)
+    assert (used1 == each.max()).all() and len(rel1) == each.max()
+    assert rel1[-1] <= tol < rel1[-2]
+    inp_fixed = _small_problem(nx=10, ny=8, nz=9, nb=2, P=int(each.max()))
+    Qf, If = oracle.solve(inp_fixed)
+    assert np.array_equal(I1, If) and np.abs(Q1 - Qf).max() <= 1e-12 * np.abs(Qf).max()
+    Qw, Iw, fw, usedw, relw = oracle.solve_tol(inp, tol, 30, mode=1, faces=f1)
+    assert (usedw == 1).all() and relw[0] <= tol
+    assert np.abs(Qw - Q1).max() <= 10 * tol * np.abs(Q1).max()
