@@ -173,6 +173,24 @@ int rts_sync_check(rts_ctx* ctx, void* stream);
 int rts_set_thick_skip(rts_ctx* ctx, int on);
 int rts_thick_levels(rts_ctx* ctx, int* levels_host, void* stream);
 
+/* Error-controlled iteration and warm start (Fig. 8 "while(g_maxerr >
+ * THRESHOLD) { ... integrate(); ... exchange(); err = error(); MPI_Allreduce(&err, &g_maxerr); }"
+ * "iterates the intensities at the boundaries ... until the errors are within a prescribed tolerance";
+ * DESIGN.md reading R22).  rts_set_tolerance(tol, max_passes) with max_passes >= 1 replaces the fixed pass
+ * count: a solve sweeps one pass per kernel launch and stops after the first pass p for which, for every
+ * (band, ray),   max over the two periodic seam faces |I(p) - I(p-1)|  <=  tol * max over them |I(p)|
+ * (I(0) = S), or after max_passes passes; tol < 0 never stops early.  Q_rad and I_top are those of the last
+ * pass run.  The solve is then SYNCHRONOUS on `stream` (the host reads the error words after every pass).
+ * max_passes = 0 switches back to rts_set_passes.  Call before sizing the workspace (the mode keeps the last
+ * plane of the x- and y-march sweeps in the workspace).
+ * rts_set_warm_start(1): the next solves do not start from I(0) = S on the seam faces but from the faces the
+ * previous solve on this context ended with (previous time step), as the paper's block-local solve does.
+ * rts_passes_used: HOST outputs (either may be NULL): passes of the last solve, largest relative change of its
+ * last pass.  RTS_ESTATE when the mode is off. */
+int rts_set_tolerance(rts_ctx* ctx, double tol, int max_passes);
+int rts_set_warm_start(rts_ctx* ctx, int on);
+int rts_passes_used(rts_ctx* ctx, int* passes_host, float* relerr_last_host);
+
 /* Band x octant sharding of ONE box over several GPUs ("for N-bands ... run N
  * times", PAPER.md:291 strong scaling of one 288^3 box).  The sweep units -- (march axis, direction, band
  * pair), i.e. the rays of one octant face group for two bands -- are dealt round robin to `nranks` contexts,

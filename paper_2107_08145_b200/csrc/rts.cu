@@ -3,7 +3,17 @@
 // rts_kernels.cuh / rts_sweep.cuh; nothing here (or anywhere in the product) touches oracle/.
 #include "../../include/rts.h"
 #include "rts_kernels.cuh"
+// the sweep kernel twice (see the end of rts_sweep.cuh): fixed pass count, and one pass per launch with error words
+#define RTS_TOLM 0
+#define RTS_MODE_NS fixedp
 #include "rts_sweep.cuh"
+#undef RTS_TOLM
+#undef RTS_MODE_NS
+#define RTS_TOLM 1
+#define RTS_MODE_NS tolp
+#include "rts_sweep.cuh"
+#undef RTS_TOLM
+#undef RTS_MODE_NS
 
 #include <algorithm>
 #include <cmath>
@@ -36,7 +46,7 @@ struct TypePlan {        // per march axis
 
 struct HostUnit {
     UnitDesc d;
-    size_t off_xex, off_g, off_part;   // workspace offsets of its exchange planes, seam histories, partial heating
+    size_t off_xex, off_g, off_part, off_lp;   // workspace offsets of its exchange planes, seam histories, partial heating, last planes
 };
 
 }  // namespace
@@ -46,7 +56,15 @@ struct rts_ctx {
     double h[3] = {0, 0, 0};
     int npass = 3;
     bool thick_skip = true;
-    unsigned solve_seq = 0;            // solves launched on this context
+    unsigned solve_seq = 0;            // sweep launches on this context (tags of the exchange words)
+    // error-controlled iteration (NEXT #3): one pass per launch until the seam faces change by <= tol * max|I|
+    int tol_max_passes = 0;            // 0: off (fixed number of passes in one launch)
+    double tol = 0.0;
+    bool warm = false;                 // keep the seam state between solves
+    int pass_counter = 0;              // passes the seam state has seen (0: cold)
+    int passes_used = 0;
+    float relerr_last = 0.f;
+    size_t off_errw = 0;
     int shard_rank = 0, shard_n = 1;   // this context sweeps the units u with u % shard_n == shard_rank (rts_set_shard)
     int units_all = 0;                 // sweep units of the whole problem
     bool flux = false;           // radiative flux wanted (rts_enable_flux): three more partial fields per unit
@@ -173,13 +191,13 @@ void default_rays(rts_ctx* c)
 // The sweep kernel is compiled for a few shared-memory row pitches (nodes per box row); a plan uses one.
 constexpr int NPITCH = 4;
 const int kPitch[NPITCH] = {24, 56, 72, 128};
-const void* sweep_fn(int pitch)
+const void* sweep_fn(int pitch, bool tolm = false)
 {
     switch (pitch) {
-        case 24: return (const void*)rts_sweep_kernel<24>;
-        case 56: return (const void*)rts_sweep_kernel<56>;
-        case 72: return (const void*)rts_sweep_kernel<72>;
-        default: return (const void*)rts_sweep_kernel<128>;
+        case 24: return tolm ? (const void*)tolp::rts_sweep_kernel<24> : (const void*)fixedp::rts_sweep_kernel<24>;
+        case 56: return tolm ? (const void*)tolp::rts_sweep_kernel<56> : (const void*)fixedp::rts_sweep_kernel<56>;
+        case 72: return tolm ? (const void*)tolp::rts_sweep_kernel<72> : (const void*)fixedp::rts_sweep_kernel<72>;
+        default: return tolm ? (const void*)tolp::rts_sweep_kernel<128> : (const void*)fixedp::rts_sweep_kernel<128>;
     }
 }
 // dynamic shared memory of a CTA whose tiles are WU x WV (SmemPlan: coefficient ring, carried
@@ -398,6 +416,7 @@ int make_plan(rts_ctx* c)
                     hu.off_xex = take(sizeof(float4) * 2 * NSLOT * (size_t)d.n_v * d.n_u2);
                     hu.off_g = take(sizeof(float2) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u2));
                     hu.off_part = take(sizeof(float) * N * (c->flux ? 4 : 1));
+                    hu.off_lp = (c->tol_max_passes > 0 && g.march != 2) ? take(sizeof(float2) * NSLOT * (size_t)d.n_v * d.n_u2) : 0;
                     c->units.push_back(hu);
                 }
             }
@@ -409,6 +428,7 @@ int make_plan(rts_ctx* c)
     c->off_partptr = take(sizeof(float*) * nu1);
     c->off_parttr = take(sizeof(int) * nu1);
     c->off_bar = take(sizeof(int) * nu1);
+    c->off_errw = take(sizeof(unsigned) * nu1 * NSLOT * 4);
     c->off_stage_in = take(sizeof(float) * N * 3);
     c->off_stage_out = take(sizeof(float) * (N + (size_t)c->nb * c->n_up * c->ny * c->nx));
     c->ws_bytes = off;
@@ -428,6 +448,8 @@ int bind_workspace(rts_ctx* c)
         d.barrier = (int*)(ws + c->off_bar) + i;
         d.Qpart = (float*)(ws + hu.off_part);
         d.Fpart = c->flux ? d.Qpart + (size_t)c->nx * c->ny * c->nz : nullptr;
+        d.Lp = (c->tol_max_passes > 0 && d.march != 2) ? (float*)(ws + hu.off_lp) : nullptr;
+        d.errw = (unsigned*)(ws + c->off_errw) + i * NSLOT * 4;
         d.kstar = (const int*)(ws + c->off_kstar) + d.pair;
         d.mthick = (const int*)(ws + c->off_mthick) + 3 * d.pair;
         // carried strips and seam histories must hold finite numbers from the start: planes that are
@@ -486,6 +508,7 @@ int bind_workspace(rts_ctx* c)
         }
     }
     CUDA_TRY(c, cudaMemset(ws + c->off_abort, 0, sizeof(int) * 8));   // status word: a fresh workspace holds garbage
+    c->pass_counter = 0;                                               // a fresh workspace holds no seam state
     c->maps_ready = true;
     return RTS_OK;
 }
@@ -547,8 +570,9 @@ int rts_create(rts_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     if ((e = cudaFuncGetAttributes(&fa, sweep_fn(56))) != cudaSuccess) return bail(std::string("sweep kernel not loadable: ") + cudaGetErrorString(e));
     c->max_smem_optin = (int)prop.sharedMemPerBlockOptin - (int)fa.sharedSizeBytes;
     for (int pi = 0; pi < NPITCH; ++pi)
-        if ((e = cudaFuncSetAttribute(sweep_fn(kPitch[pi]), cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem_optin)) != cudaSuccess)
-            return bail(std::string("cudaFuncSetAttribute(max dynamic smem): ") + cudaGetErrorString(e));
+        for (int tm = 0; tm < 2; ++tm)
+            if ((e = cudaFuncSetAttribute(sweep_fn(kPitch[pi], tm != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem_optin)) != cudaSuccess)
+                return bail(std::string("cudaFuncSetAttribute(max dynamic smem): ") + cudaGetErrorString(e));
     if ((e = cudaEventCreateWithFlags(&c->ev, cudaEventDisableTiming)) != cudaSuccess) return bail(cudaGetErrorString(e));
     {
         cudaDriverEntryPointQueryResult qres;
@@ -751,25 +775,46 @@ int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, flo
     CUDA_TRY(c, cudaGetLastError());
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[1], st));
 
-    CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 8, st));
-
-    CUDA_TRY(c, cudaMemsetAsync(ws + c->off_bar, 0, sizeof(int) * c->units.size(), st));
-    // the sweep: one persistent launch, tasks handed out by an in-order ticket counter
+    // the sweep: one persistent launch, tasks handed out by an in-order ticket counter.  Fixed pass count: one
+    // launch runs all passes.  Error-controlled mode (NEXT #3): one pass per launch; after each the host reads the
+    // units' error words and stops when the seam faces of every (band, ray) changed by <= tol * max|I| on them.
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[2], st));
     if (c->shard_n > 1 && Itop)    // the emergent intensities of the other ranks' rays stay zero: a sum over ranks completes them
         CUDA_TRY(c, cudaMemsetAsync(Itop, 0, sizeof(float) * (size_t)c->nb * c->n_up * c->ny * c->nx, st));
-    if (c->total_tickets > 0) {
+    const bool tolmode = c->tol_max_passes > 0;
+    if (tolmode && !c->warm) c->pass_counter = 0;
+    const int nlaunch = tolmode ? c->tol_max_passes : 1;
+    c->passes_used = 0;
+    for (int it = 0; it < nlaunch && c->total_tickets > 0; ++it) {
+        CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 8, st));
+        CUDA_TRY(c, cudaMemsetAsync(ws + c->off_bar, 0, sizeof(int) * c->units.size(), st));
+        if (tolmode) CUDA_TRY(c, cudaMemsetAsync(ws + c->off_errw, 0, sizeof(unsigned) * c->units.size() * NSLOT * 4, st));
         const UnitDesc* dunits = (const UnitDesc*)(ws + c->off_units);
         int* abortf = (int*)(ws + c->off_abort);
         int* ticket = abortf + 1;
         int nunits = (int)c->units.size(), total = c->total_tickets;
-        unsigned seq = ++c->solve_seq;                          // tags of this solve's exchange words
+        unsigned seq = ++c->solve_seq;                          // tags of this launch's exchange words
         if ((seq & 0xfffffu) == 0) seq = ++c->solve_seq;
         seq &= 0xfffffu;
-        void* args[] = {&c->maps, &dunits, &nunits, &total, &ticket, &Itop, &abortf, &seq};
+        int pbase = tolmode ? c->pass_counter : 0, npl = tolmode ? 1 : 0;
+        void* args[] = {&c->maps, &dunits, &nunits, &total, &ticket, &Itop, &abortf, &seq, &pbase, &npl};
         // cooperative launch: every CTA of the grid is resident, which the tile barriers rely on
-        CUDA_TRY(c, cudaLaunchCooperativeKernel(sweep_fn(c->pitch), dim3(c->grid), dim3(c->threads), args,
+        CUDA_TRY(c, cudaLaunchCooperativeKernel(sweep_fn(c->pitch, tolmode), dim3(c->grid), dim3(c->threads), args,
                                                 (size_t)c->smem_bytes, st));
+        if (!tolmode) break;
+        ++c->pass_counter; ++c->passes_used;
+        std::vector<unsigned> ew(c->units.size() * NSLOT * 4);
+        CUDA_TRY(c, cudaMemcpyAsync(ew.data(), ws + c->off_errw, sizeof(unsigned) * ew.size(), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(c, cudaStreamSynchronize(st));
+        float worst = 0.f;
+        for (size_t q = 0; q < ew.size(); q += 4)
+            for (int b = 0; b < 2; ++b) {
+                float e, sc;
+                std::memcpy(&e, &ew[q + b], 4); std::memcpy(&sc, &ew[q + 2 + b], 4);
+                if (sc > 0.f) worst = std::max(worst, e / sc);
+            }
+        c->relerr_last = worst;
+        if ((double)worst <= c->tol) break;
     }
     // finalize
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[3], st));
@@ -824,6 +869,34 @@ int rts_solve_flux(rts_ctx* c, const float* rho, const float* T, const float* P,
     if (!c) return RTS_EINVAL;
     if (!Frad) return fail(c, RTS_EINVAL, "rts_solve_flux: null Frad");
     return solve_impl(c, rho, T, P, Q, Itop, Frad, Qdiv, Qblend, stream);
+}
+
+int rts_set_tolerance(rts_ctx* c, double tol, int max_passes)
+{
+    if (!c) return RTS_EINVAL;
+    if (max_passes < 0 || max_passes > 4096 || !(tol == tol)) return fail(c, RTS_EINVAL, "rts_set_tolerance: 0 <= max_passes <= 4096, tol not NaN");
+    const bool was = c->tol_max_passes > 0, is = max_passes > 0;
+    c->tol = tol; c->tol_max_passes = max_passes;
+    if (was != is) c->planned = false;             // the last-plane buffers exist in this mode only
+    c->pass_counter = 0;
+    return RTS_OK;
+}
+
+int rts_set_warm_start(rts_ctx* c, int on)
+{
+    if (!c) return RTS_EINVAL;
+    c->warm = on != 0;
+    if (!c->warm) c->pass_counter = 0;
+    return RTS_OK;
+}
+
+int rts_passes_used(rts_ctx* c, int* passes, float* relerr_last)
+{
+    if (!c) return RTS_EINVAL;
+    if (c->tol_max_passes <= 0) return fail(c, RTS_ESTATE, "rts_passes_used: error-controlled mode is off (rts_set_tolerance)");
+    if (passes) *passes = c->passes_used;
+    if (relerr_last) *relerr_last = c->relerr_last;
+    return RTS_OK;
 }
 
 int rts_set_shard(rts_ctx* c, int rank, int nranks)

@@ -73,6 +73,8 @@ struct UnitDesc {
                       // written exactly once per solve, the units are summed in a fixed order by rts_finalize_kernel
     float* Fpart;     // [3][N] radiative flux of this unit alone (same layout), or null
     int*   barrier;   // arrivals of this unit's tiles (monotonic)
+    float* Lp;        // float2 [NSLOT][n_v][n_u2]: x/y-march, error-controlled mode: the last plane of the previous pass
+    unsigned* errw;   // [NSLOT][4] error words of this unit (error-controlled mode), see TaskShared::errs
     const int* kstar; // device: switch height of this band pair
     const int* mthick;// device: thick level pairs from the bottom of this band pair (z-march plane skipping)
     long long q_sm, q_sv;                 // heating strides along (march, v); u stride 1

@@ -24,7 +24,8 @@
 //   carried planes      [2 buffers][su group][BV rows][ray sv>0 row | ray sv<0 row][PITCH] float2
 // Carried quantity: X = I - a*S with a = 1 at levels k <= kstar (optically thick part, where
 // J - S would cancel) and a = 0 above (thin part, where I << S would cancel).
-#pragma once
+#ifndef RTS_SWEEP_SHARED_PART
+#define RTS_SWEEP_SHARED_PART
 #include "rts_kernels.cuh"
 
 #ifndef RTS_SWEEP_THREADS
@@ -180,6 +181,8 @@ struct TaskShared {
     TileGeo G;
     uint64_t mbar[NSTAGE_MAX];
     int ticket, flag, nghost, nhalo;
+    int pbase, tolmode;                // passes done before this launch; error-controlled mode (one pass per launch)
+    unsigned errs[NSLOT][4];           // tolmode: per ray max |I(p) - I(p-1)| on the seam faces (band 0, 1), max |I(p)| (band 0, 1)
     int PS, tu, tv, pad0;              // nodes per plane set; tile coordinates
     f2* stage0;                        // [nstage] coefficient plane sets
     f2* Xb;                            // [2][ng] carried plane sets
@@ -332,109 +335,25 @@ struct TailCtx {
     int n_u2, far_off;                 // row pitch of the exchange planes; NSLOT*n_v + slot*n_u2 (far-v rows)
     int hv, nrows, K, gsv;
     unsigned tag;                      // tag of the block whose strips are published this step (0: plain strips)
+    const f2* GhO;                     // tolmode: seam history of this plane in the previous pass (null: I(0) = S)
+    unsigned* errp;                    // tolmode: this ray's error words in shared memory (else null)
 };
 
 // Store one finished row of a strip: the carried plane and, where flagged, the seam history (far-u column,
 // far-v row) and the exchange strips.  Inline: a few instructions on the flagged rows only.
-template <int SU>
-__device__ __forceinline__ void row_store(const TailCtx& TC, const unsigned fl, const bool slow, const int q,
-                                          const uint32_t bW, const float4 o)
+// Error-controlled iteration (NEXT #3): change of one seam node (both bands) against the previous pass, and the
+// intensity itself, into the ray's error words (non-negative floats order like unsigned integers).
+// xn: new carried value X = I - a S; sn: S; goff: the node's slot in the seam history; dirichlet: the node was set.
+__device__ __noinline__ void seam_error(const f2* GhO, unsigned* errp, const int goff, const f2 xn, const f2 sn, const float a_p, const bool dirichlet)
 {
-    if (!slow) { sts128<0>(bW, o); return; }
-    const bool part = (fl & IT_PART) != 0;
-    if (!part) sts128<0>(bW, o); else sts64<0>(bW, make_float2(o.x, o.y));
-    if (q < TC.hv || (fl & IT_DQ)) return;                       // halo row / halo pair: nothing to publish
-    const int gv = TC.gv0 + q * TC.gsv;
-    if (TC.GhP) {
-        if (fl & IT_FARC)                                        // far-u column: next pass's seam ghosts of this plane
-            __stcg(TC.GhP + gv, (fl & IT_FSEC) ? make_float2(o.z, o.w) : make_float2(o.x, o.y));
-        if ((fl & IT_FARV) && q == TC.nrows - 1) {               // far-v row (periodic v axis)
-            f2* gvp = TC.GhP + TC.far_off + TC.ug;
-            if (!part) __stcg(reinterpret_cast<float4*>(gvp), o);
-            else __stcg(gvp, make_float2(o.x, o.y));
-        }
+    const f2 In = fma2(bc(a_p), sn, xn);                                   // I = X + a S
+    f2 d = make_float2(0.f, 0.f);
+    if (!dirichlet) {
+        if (GhO) { const f2 xo = __ldcg(GhO + goff); d = sub2(xn, xo); }                // same a, S in both passes
+        else d = sub2(In, sn);                                             // I(0) = S
     }
-    if (TC.XeP && ((fl & IT_USTRIP) || q >= TC.nrows - TC.K)) {  // exchange strips at a block end
-        float4* xe = TC.XeP + (size_t)gv * TC.n_u2 + TC.ug;          // 16 bytes per node: (value, tag) per band
-        st_tagged2(xe, make_float2(o.x, o.y), TC.tag);
-        st_tagged2(xe + 1, make_float2(o.z, o.w), TC.tag);
-    }
-}
-
-// ------------------------------------------------------------------------------------------
-// One strip: the rows q0 .. qb-1 of one node pair of one ray, marched from the upwind end of the v axis with the
-// upwind rows of kaprho, S and X kept in registers.  rstep: bytes from a row to the next one downwind (+-RP);
-// oP / oC / oX / oW: byte addresses of row q0's pair in the previous / this plane's coefficient stage and in the
-// carried plane of the ray read / written this step.
-template <int PITCH, int SU>
-__device__ __forceinline__ void do_strip(
-    const int s, const unsigned fl, int q, const int qb, const int rstep, const RayK& rk,
-    const TaskShared& S, const StepCtx& C, const TailCtx& TC, const int qtail, int vrow, const int vstep,
-    uint32_t bP, uint32_t bC, uint32_t bX, uint32_t bW)
-{
-    constexpr int HP = 8 * PITCH;        // second field (S) of a coefficient row
-    const bool zm = S.G.zmarch != 0;
-    const int ks = S.G.kstar;
-    const bool tail_all = (fl & C.xmask) != 0u;
-    if (C.dplane) {
-        // z-march inflow plane: the nodes are set (I = S upward, 0 downward), not updated
-        const float f = (S.U.ray[s].up ? 1.f : 0.f) - C.a_cur;
-        for (; q < qb; ++q) {
-            const float4 o = scale4(f, lds128<HP>(bC));
-            row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);
-            bC += rstep; bW += rstep;
-        }
-        return;
-    }
-    if ((fl & IT_DIR) && q == 0) {
-        // inflow row of a bounded v axis (v = z): I = S (upward ray, bottom row) or 0 (downward ray, top row)
-        const float f = ((s & 2) ? 0.f : 1.f) - ((vrow <= ks) ? 1.f : 0.f);
-        const float4 o = scale4(f, lds128<HP>(bC));
-        row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);
-        bP += rstep; bC += rstep; bX += rstep; bW += rstep; vrow += vstep; ++q;
-        if (q >= qb) return;
-    }
-    // upwind rows of the first row
-    Row3 kA = load_row<SU, 0>(bP - rstep), sA = load_row<SU, HP>(bP - rstep), xA = load_row<SU, 0>(bX - rstep);
-    Row3 kB, sB, xB;
-#define STRIP_ROW(KU, SU_, XU, KO, SO, XO)                                                                          \
-    {                                                                                                               \
-        KO = load_row<SU, 0>(bP); SO = load_row<SU, HP>(bP); XO = load_row<SU, 0>(bX);                              \
-        const float4 kc = lds128<0>(bC), sc = lds128<HP>(bC);                                                       \
-        const f2 dt0 = mul2(add2(make_float2(kc.x, kc.y), bil<SU, 0>(KU, KO, rk.w)), bc(rk.kc));                    \
-        const f2 dt1 = mul2(add2(make_float2(kc.z, kc.w), bil<SU, 1>(KU, KO, rk.w)), bc(rk.kc));                    \
-        const float dmin = fminf(fminf(dt0.x, dt0.y), fminf(dt1.x, dt1.y));                                         \
-        const float dmax = fmaxf(fmaxf(dt0.x, dt0.y), fmaxf(dt1.x, dt1.y));                                         \
-        float a_u, a_o, a_p;                                                                                        \
-        if (zm) { a_u = a_o = C.a_prev; a_p = C.a_cur; }                                                            \
-        else { a_u = (vrow - vstep <= ks) ? 1.f : 0.f; a_o = (vrow <= ks) ? 1.f : 0.f; a_p = a_o; }                  \
-        const f2 sp0 = make_float2(sc.x, sc.y), sp1 = make_float2(sc.z, sc.w);                                      \
-        f2 e0, l0, p0, e1, l1, p1;                                                                                  \
-        /* one evaluator per warp and row (each is valid for every lane that takes part): no divergence */          \
-        const unsigned am_ = __activemask();                                                                        \
-        if (__all_sync(am_, dmin >= DTAU_SERIES)) { att_factors<0>(dt0, e0, l0, p0); att_factors<0>(dt1, e1, l1, p1); }    \
-        else if (__all_sync(am_, dmax <= DTAU_SERIES_MAX)) { att_factors<1>(dt0, e0, l0, p0); att_factors<1>(dt1, e1, l1, p1); } \
-        else { att_factors<2>(dt0, e0, l0, p0); att_factors<2>(dt1, e1, l1, p1); }                                  \
-        f2 v0, v1;                                                                                                  \
-        if (a_u == a_o && a_o == a_p) {                                                                             \
-            v0 = node_update<SU, 0, 3>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, 1.f - a_p, 0.f, 0.f);                \
-            v1 = node_update<SU, 1, 3>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, 1.f - a_p, 0.f, 0.f);                \
-        } else {                                                                                                    \
-            v0 = node_update<SU, 0, 2>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, a_u, a_o, a_p);                      \
-            v1 = node_update<SU, 1, 2>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, a_u, a_o, a_p);                      \
-        }                                                                                                           \
-        const float4 o = cat4(v0, v1);                                                                              \
-        row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);                                                    \
-        bP += rstep; bC += rstep; bX += rstep; bW += rstep; vrow += vstep; ++q;                                     \
-    }
-#pragma unroll 1
-    while (true) {
-        STRIP_ROW(kA, sA, xA, kB, sB, xB)
-        if (q >= qb) break;
-        STRIP_ROW(kB, sB, xB, kA, sA, xA)
-        if (q >= qb) break;
-    }
-#undef STRIP_ROW
+    atomicMax(errp + 0, __float_as_uint(fabsf(d.x))); atomicMax(errp + 1, __float_as_uint(fabsf(d.y)));
+    atomicMax(errp + 2, __float_as_uint(fabsf(In.x))); atomicMax(errp + 3, __float_as_uint(fabsf(In.y)));
 }
 
 // ------------------------------------------------------------------------------------------
@@ -488,6 +407,22 @@ __device__ __forceinline__ f2 ghost_fetch(const TaskShared& S, const GhostEnt g,
     return __ldcg(reinterpret_cast<const f2*>(U.Gu) + ((size_t)(psrc & 1) * U.n_m + msrc) * g_plane + (g.goff & 0x0fffffff));
 }
 
+}  // namespace rts
+#endif  // RTS_SWEEP_SHARED_PART
+
+// ==========================================================================================================
+// The strip code, the task loop and the kernel exist twice: rts.cu includes this file once with RTS_TOLM 0
+// (namespace fixedp: a fixed number of passes in one launch) and once with RTS_TOLM 1 (namespace tolp: the
+// error-controlled mode, one pass per launch).  A macro and not a template parameter: with a bool template
+// parameter the register allocation of the fixed-pass kernel changed (32 -> 120 bytes of spills, +8 % time),
+// although not one instruction of it depends on the mode.
+#ifndef RTS_TOLM
+#error "define RTS_TOLM (0 / 1) and RTS_MODE_NS before including rts_sweep.cuh"
+#endif
+namespace rts { namespace RTS_MODE_NS {
+
+// (the out-of-line parts live in the mode's namespace too: device functions shared by two kernels are
+//  allocated registers for both callers at once, which cost the fixed-pass kernel its allocation)
 // Heating, radiative flux and emergent intensity of a finished plane (last pass; out of line): reads the new
 // carried plane set Xn (one buffer) and that plane's coefficient stage Kc.  The unit's contribution goes to its
 // own partial buffers with plain stores: every node is written exactly once, no atomics (deterministic).
@@ -569,6 +504,46 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
     }
 }
 
+// End of a launch of the error-controlled mode (out of line).  x/y-march: the last plane of the pass is the seam
+// face of the march axis: its change against the previous pass (kept in Lp; pass 0: I(0) = S) goes into the
+// error words and the plane replaces Lp (the next launch starts from it).  All: the error words go to global memory.
+// P: index of the pass that has just ended.
+template <int PITCH>
+__device__ __noinline__ void pass_end(TaskShared* __restrict__ Sp, const f2* __restrict__ Kc, const f2* __restrict__ Xn, const int P)
+{
+    constexpr int RPN = 2 * PITCH;
+    TaskShared& S = *Sp;
+    const UnitDesc& U = S.U; const TileGeo& G = S.G;
+    const int tid = threadIdx.x, T = blockDim.x;
+    __syncthreads();                                          // the seam errors of the last step are in
+    if (!G.zmarch) {
+        f2* Lp = reinterpret_cast<f2*>(U.Lp);
+        for (int i = tid; i < G.wu * G.wv; i += T) {
+            const int row = i / G.wu, col = i - row * G.wu;
+            const int xo = (HALO + row) * RPN + HALO + col;
+            const int v = G.v0 + row, u = G.u0 + col;
+            const f2 Sv = Kc[xo + PITCH];
+            const float a = a_of(G, v);
+#pragma unroll
+            for (int s = 0; s < NSLOT; ++s) {
+                if (!U.ray[s].active) continue;
+                const f2 xn = Xn[xso<PITCH>(S, s) + xo];
+                f2* lp = Lp + ((size_t)s * U.n_v + v) * U.n_u2 + u;
+                const f2 In = fma2(bc(a), Sv, xn);
+                const bool up = !(s & 2);
+                const bool dn = (v == (up ? 0 : U.n_v - 1));      // inflow row: set, never changes
+                f2 d = make_float2(0.f, 0.f);
+                if (!dn) d = (P > 0) ? sub2(xn, __ldcg(lp)) : sub2(In, Sv);
+                __stcg(lp, xn);
+                atomicMax(&S.errs[s][0], __float_as_uint(fabsf(d.x))); atomicMax(&S.errs[s][1], __float_as_uint(fabsf(d.y)));
+                atomicMax(&S.errs[s][2], __float_as_uint(fabsf(In.x))); atomicMax(&S.errs[s][3], __float_as_uint(fabsf(In.y)));
+            }
+        }
+        __syncthreads();
+    }
+    if (tid < NSLOT * 4) atomicMax(U.errw + tid, (&S.errs[0][0])[tid]);
+}
+
 // Block start (out of line): fetch the K-deep halo of the carried plane set Xr from the exchange buffer and the seam
 // ghosts of the previous plane.  Tagged exchange (U.xflag, every ray of the unit has its opposite ray in the unit):
 // the halo words carry the tag of block gblk - 1, a reader spins on the words it needs; the tiles of the unit
@@ -577,13 +552,14 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
 // Returns false if the watchdog fired.
 template <int PITCH>
 __device__ __noinline__ bool block_start(TaskShared* __restrict__ Sp, f2* __restrict__ Xr, const f2* __restrict__ Kp0,
-                                         const int pass, const int blk0, const int gblk, const int s_,
+                                         const int pass2, const int blk0, const int gblk, const int s_,
                                          const unsigned tag, const bool skipped)
 {
     TaskShared& S = *Sp;
     const UnitDesc& U = S.U; const TileGeo& G = S.G;
     const int tid = threadIdx.x, T = blockDim.x;
     const int ngh = S.nghost, nhalo = S.nhalo;
+    const int pass = pass2 & 0xffff, passL = pass2 >> 16;   // global pass index (seam ghosts) / passes of this launch (counter)
     const bool zmarch = G.zmarch != 0;
     const bool tagged = U.xflag != 0;
     const bool exch = !(zmarch && blk0 == 0);
@@ -598,7 +574,7 @@ __device__ __noinline__ bool block_start(TaskShared* __restrict__ Sp, f2* __rest
     if (pre && tid < ngh) gpre = ghost_fetch<PITCH>(S, S.gt[tid], pass - 1, m_prev, nullptr);
     if (meet) {
         if (tid == 0) {
-            const int need = (tagged ? pass : gblk) * U.ntiles;
+            const int need = (tagged ? passL : gblk) * U.ntiles;      // passL: passes of this launch
             const int ab = *reinterpret_cast<volatile int*>(S.abortf);
             unsigned spins = 0, ns = 32;
             while (ld_acquire(U.barrier) < need) {
@@ -712,12 +688,28 @@ __device__ __noinline__ void task_lists(TaskShared* __restrict__ Sp)
     }
     if (!G.zmarch) {
         const f2* Kp0 = S.stage0 + (size_t)(U.nstage - 1) * S.PS;
+        const f2* Lp = reinterpret_cast<const f2*>(U.Lp);
         for (int i = tid; i < BU * BV; i += T) {
             const int bv = i / BU, bu = i - bv * BU;
             const int xo = bv * RPN + bu;
+            const int v = G.v0 - HALO + bv, u = G.u0 - HALO + bu;
+            const bool inside = v >= 0 && v < U.n_v && u >= 0 && u < U.n_u;
 #pragma unroll
             for (int s = 0; s < NSLOT; ++s)
-                if (U.ray[s].active) S.Xb[xso<PITCH>(S, s) + xo] = x_initial<PITCH>(S, Kp0, s, bv, xo, U.n_m - 1);
+                if (U.ray[s].active) {
+                    f2 x;
+                    // a later launch of the error-controlled mode continues from the last plane of the previous pass
+                    if (S.pbase > 0) x = inside ? __ldcg(Lp + ((size_t)s * U.n_v + v) * U.n_u2 + u) : make_float2(0.f, 0.f);
+                    else x = x_initial<PITCH>(S, Kp0, s, bv, xo, U.n_m - 1);
+                    S.Xb[xso<PITCH>(S, s) + xo] = x;
+                }
+        }
+        if (S.pbase > 0) {
+            __syncthreads();
+            for (int e = tid; e < S.nghost; e += T) {         // its seam ghosts: the history of that plane
+                const GhostEnt g = S.gt[e];
+                S.Xb[xso<PITCH>(S, g.goff >> 28) + g.xoff] = ghost_fetch<PITCH>(S, g, S.pbase - 1, U.n_m - 1, nullptr);
+            }
         }
     }
     __syncthreads();
@@ -735,11 +727,127 @@ __device__ __forceinline__ void issue_load(TaskShared& S, const CUtensorMap* cma
     tensor_load5(dst, cmap, 2 * G.u0, 0, c2, c3, U.pair, bar);
 }
 
+template <int SU>
+__device__ __forceinline__ void row_store(const TailCtx& TC, const unsigned fl, const bool slow, const int q,
+                                          const uint32_t bW, const float4 o, const float4 sc = make_float4(0.f, 0.f, 0.f, 0.f),
+                                          const float a_p = 0.f, const bool dirichlet = false)
+{
+    if (!slow) { sts128<0>(bW, o); return; }
+    const bool part = (fl & IT_PART) != 0;
+    if (!part) sts128<0>(bW, o); else sts64<0>(bW, make_float2(o.x, o.y));
+    if (q < TC.hv || (fl & IT_DQ)) return;                       // halo row / halo pair: nothing to publish
+    const int gv = TC.gv0 + q * TC.gsv;
+    if (TC.GhP) {
+        if (fl & IT_FARC) {                                      // far-u column: next pass's seam ghosts of this plane
+            const bool sec = (fl & IT_FSEC) != 0;
+            const f2 xn = sec ? make_float2(o.z, o.w) : make_float2(o.x, o.y);
+            __stcg(TC.GhP + gv, xn);
+            if (RTS_TOLM && TC.errp) seam_error(TC.GhO, TC.errp, gv, xn, sec ? make_float2(sc.z, sc.w) : make_float2(sc.x, sc.y), a_p, dirichlet);
+        }
+        if ((fl & IT_FARV) && q == TC.nrows - 1) {               // far-v row (periodic v axis)
+            f2* gvp = TC.GhP + TC.far_off + TC.ug;
+            if (!part) __stcg(reinterpret_cast<float4*>(gvp), o);
+            else __stcg(gvp, make_float2(o.x, o.y));
+            if (RTS_TOLM && TC.errp) {
+                seam_error(TC.GhO, TC.errp, TC.far_off + TC.ug, make_float2(o.x, o.y), make_float2(sc.x, sc.y), a_p, dirichlet);
+                if (!part) seam_error(TC.GhO, TC.errp, TC.far_off + TC.ug + 1, make_float2(o.z, o.w), make_float2(sc.z, sc.w), a_p, dirichlet);
+            }
+        }
+    }
+    if (TC.XeP && ((fl & IT_USTRIP) || q >= TC.nrows - TC.K)) {  // exchange strips at a block end
+        float4* xe = TC.XeP + (size_t)gv * TC.n_u2 + TC.ug;          // 16 bytes per node: (value, tag) per band
+        st_tagged2(xe, make_float2(o.x, o.y), TC.tag);
+        st_tagged2(xe + 1, make_float2(o.z, o.w), TC.tag);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// One strip: the rows q0 .. qb-1 of one node pair of one ray, marched from the upwind end of the v axis with the
+// upwind rows of kaprho, S and X kept in registers.  rstep: bytes from a row to the next one downwind (+-RP);
+// oP / oC / oX / oW: byte addresses of row q0's pair in the previous / this plane's coefficient stage and in the
+// carried plane of the ray read / written this step.
+template <int PITCH, int SU>
+__device__ __forceinline__ void do_strip(
+    const int s, const unsigned fl, int q, const int qb, const int rstep, const RayK& rk,
+    const TaskShared& S, const StepCtx& C, const TailCtx& TC, const int qtail, int vrow, const int vstep,
+    uint32_t bP, uint32_t bC, uint32_t bX, uint32_t bW)
+{
+    constexpr int HP = 8 * PITCH;        // second field (S) of a coefficient row
+    const bool zm = S.G.zmarch != 0;
+    const int ks = S.G.kstar;
+    const bool tail_all = (fl & C.xmask) != 0u;
+    if (C.dplane) {
+        // z-march inflow plane: the nodes are set (I = S upward, 0 downward), not updated
+        const float f = (S.U.ray[s].up ? 1.f : 0.f) - C.a_cur;
+        for (; q < qb; ++q) {
+            const float4 sc = lds128<HP>(bC);
+            if (RTS_TOLM) row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc), sc, C.a_cur, true);
+            else row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc));
+            bC += rstep; bW += rstep;
+        }
+        return;
+    }
+    if ((fl & IT_DIR) && q == 0) {
+        // inflow row of a bounded v axis (v = z): I = S (upward ray, bottom row) or 0 (downward ray, top row)
+        const float a0 = (vrow <= ks) ? 1.f : 0.f;
+        const float f = ((s & 2) ? 0.f : 1.f) - a0;
+        const float4 sc = lds128<HP>(bC);
+        if (RTS_TOLM) row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc), sc, a0, true);
+        else row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc));
+        bP += rstep; bC += rstep; bX += rstep; bW += rstep; vrow += vstep; ++q;
+        if (q >= qb) return;
+    }
+    // upwind rows of the first row
+    Row3 kA = load_row<SU, 0>(bP - rstep), sA = load_row<SU, HP>(bP - rstep), xA = load_row<SU, 0>(bX - rstep);
+    Row3 kB, sB, xB;
+#define STRIP_ROW(KU, SU_, XU, KO, SO, XO)                                                                          \
+    {                                                                                                               \
+        KO = load_row<SU, 0>(bP); SO = load_row<SU, HP>(bP); XO = load_row<SU, 0>(bX);                              \
+        const float4 kc = lds128<0>(bC), sc = lds128<HP>(bC);                                                       \
+        const f2 dt0 = mul2(add2(make_float2(kc.x, kc.y), bil<SU, 0>(KU, KO, rk.w)), bc(rk.kc));                    \
+        const f2 dt1 = mul2(add2(make_float2(kc.z, kc.w), bil<SU, 1>(KU, KO, rk.w)), bc(rk.kc));                    \
+        const float dmin = fminf(fminf(dt0.x, dt0.y), fminf(dt1.x, dt1.y));                                         \
+        const float dmax = fmaxf(fmaxf(dt0.x, dt0.y), fmaxf(dt1.x, dt1.y));                                         \
+        float a_u, a_o, a_p;                                                                                        \
+        if (zm) { a_u = a_o = C.a_prev; a_p = C.a_cur; }                                                            \
+        else { a_u = (vrow - vstep <= ks) ? 1.f : 0.f; a_o = (vrow <= ks) ? 1.f : 0.f; a_p = a_o; }                  \
+        const f2 sp0 = make_float2(sc.x, sc.y), sp1 = make_float2(sc.z, sc.w);                                      \
+        f2 e0, l0, p0, e1, l1, p1;                                                                                  \
+        /* one evaluator per warp and row (each is valid for every lane that takes part): no divergence */          \
+        const unsigned am_ = __activemask();                                                                        \
+        if (__all_sync(am_, dmin >= DTAU_SERIES)) { att_factors<0>(dt0, e0, l0, p0); att_factors<0>(dt1, e1, l1, p1); }    \
+        else if (__all_sync(am_, dmax <= DTAU_SERIES_MAX)) { att_factors<1>(dt0, e0, l0, p0); att_factors<1>(dt1, e1, l1, p1); } \
+        else { att_factors<2>(dt0, e0, l0, p0); att_factors<2>(dt1, e1, l1, p1); }                                  \
+        f2 v0, v1;                                                                                                  \
+        if (a_u == a_o && a_o == a_p) {                                                                             \
+            v0 = node_update<SU, 0, 3>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, 1.f - a_p, 0.f, 0.f);                \
+            v1 = node_update<SU, 1, 3>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, 1.f - a_p, 0.f, 0.f);                \
+        } else {                                                                                                    \
+            v0 = node_update<SU, 0, 2>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, a_u, a_o, a_p);                      \
+            v1 = node_update<SU, 1, 2>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, a_u, a_o, a_p);                      \
+        }                                                                                                           \
+        const float4 o = cat4(v0, v1);                                                                              \
+        if (RTS_TOLM) row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o, sc, a_p, false);                          \
+        else row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);                                         \
+        bP += rstep; bC += rstep; bX += rstep; bW += rstep; vrow += vstep; ++q;                                     \
+    }
+#pragma unroll 1
+    while (true) {
+        STRIP_ROW(kA, sA, xA, kB, sB, xB)
+        if (q >= qb) break;
+        STRIP_ROW(kB, sB, xB, kA, sA, xA)
+        if (q >= qb) break;
+    }
+#undef STRIP_ROW
+}
+
 template <int PITCH>
 __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f2* __restrict__ smf,
-                         float* __restrict__ Itop_all, int* abortf, const unsigned seq)
+                         float* __restrict__ Itop_all, int* abortf, const unsigned seq, const int pbase_arg, const int npass_launch)
 {
+    const int pbase = RTS_TOLM ? pbase_arg : 0;                  // the fixed-pass kernel knows neither: nothing of this mode costs it a register
 
+    constexpr int tolmode = RTS_TOLM ? 1 : 0;
     const UnitDesc& U = S.U;
     const int tid = threadIdx.x, T = blockDim.x;
     const SmemPlan SP(PITCH, U.WU, U.WV, U.ng, U.nstage);
@@ -766,12 +874,14 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
         for (int i = 0; i < NST; ++i) mbar_init(&S.mbar[i], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         S.flag = 0; S.nghost = 0; S.nhalo = 0;
+        S.pbase = pbase; S.tolmode = tolmode;
+        for (int i = 0; i < NSLOT * 4; ++i) (&S.errs[0][0])[i] = 0u;
     }
     for (int i = tid; i < SP.nodes(); i += T) smf[i] = make_float2(0.f, 0.f);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
     const TileGeo& G = S.G;
-    const int n_m = U.n_m, npass = U.npass, K = U.K;
+    const int n_m = U.n_m, npass = RTS_TOLM ? npass_launch : U.npass, K = U.K;
     const int nsteps = n_m * npass;
     const bool zmarch = (U.march == 2);
     const bool tagged = U.xflag != 0;
@@ -789,7 +899,6 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     //      so the ray's signs are warp-uniform); strip index e enumerates (row chunk, node pair) of the ray's region:
     //      tile core + upwind u halo (one HALO of columns) + upwind v halo of depth K-1, clipped to the domain.
     const int nsl = 2 * NG;
-    const int TS = T / nsl;
     // warp w works for ray w % nsl: the warps of one scheduler (w % 4) then run the same ray, i.e. one copy of
     // the strip code (one sign of su) at a time in its instruction cache
     const int sidx = (tid >> 5) % nsl, e = ((tid >> 5) / nsl) * 32 + (tid & 31);
@@ -858,13 +967,17 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     bool bail = false;
     for (int pass = 0; pass < npass && !bail; ++pass) {
         const bool lastpass = (pass == npass - 1);
+        const int P = RTS_TOLM ? pbase + pass : pass;            // passes done before this one (earlier launches included)
+        // error-controlled mode: every pass may be the last one: it writes the heating and I_top, keeps its seam
+        // history and skips nothing
+        const bool qon = lastpass || tolmode, hist_on = !lastpass || tolmode, may_skip = !lastpass && !tolmode;
         for (int blk0 = 0; blk0 < n_m && !bail; blk0 += K) {
             const int blen = min(K, n_m - blk0);
             // ---- block start: wait for the unit, fetch halos and seam ghosts of the previous plane
             if (s_ > 0) {
                 // tag of the strips of block gblk - 1; no strips were stored if their step was a skipped thick plane
-                const bool skipped = zmarch && !lastpass && blk0 > 0 && plane_of(U, blk0 - 1) < G.mthick;
-                if (!block_start<PITCH>(&S, S.Xb + (size_t)cur * NG * PS, S.stage0 + (size_t)stp * PS, pass, blk0, gblk, s_,
+                const bool skipped = zmarch && may_skip && blk0 > 0 && plane_of(U, blk0 - 1) < G.mthick;
+                if (!block_start<PITCH>(&S, S.Xb + (size_t)cur * NG * PS, S.stage0 + (size_t)stp * PS, P | (pass << 16), blk0, gblk, s_,
                                         tag0 | ((unsigned)gblk & 0xfffu), skipped)) { bail = true; break; }
             }
             for (int j = 0; j < blen; ++j, ++s_) {
@@ -880,13 +993,13 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 }
                 par_bits ^= 1u << stc;
                 // ---- heating / emergent intensity of the previous step's plane
-                if (lastpass && m > 0) q_pass<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, m - 1);
+                if (qon && m > 0) q_pass<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, m - 1);
                 // ---- seam ghosts for the next step (previous pass, this plane): fetch now, store after the update
                 const bool ghost_next = !blk_last && more && ngh > 0;
                 f2 gval[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
-                if (ghost_next && pass > 0) {
+                if (ghost_next && P > 0) {
 #pragma unroll
-                    for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) gval[i] = ghost_fetch<PITCH>(S, S.gt[e], pass - 1, m, nullptr); }
+                    for (int i = 0; i < 2; ++i) { const int e = tid + i * T; if (e < ngh) gval[i] = ghost_fetch<PITCH>(S, S.gt[e], P - 1, m, nullptr); }
                 }
 
                 // ---- the update
@@ -894,17 +1007,19 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 // exceeds DTAU_SKIP, e^-dtau is exactly 0 and the new plane does not depend on the carried one.
                 // The planes pl < mthick only feed such planes (and seam ghosts that are multiplied by 0), so
                 // their updates are skipped; plane mthick restarts from whatever finite values the buffers hold.
-                if (!(zmarch && !lastpass && pl < mthick)) {
+                if (!(zmarch && may_skip && pl < mthick)) {
                     // first row of this step: halo rows deeper than the remaining halo depth are not updated any more
                     const int q0 = max(qa, hv_ - hj);
                     if (q0 < qb && !((ifl & IT_DQ) && hj == 0)) {
                         StepCtx C;
                         C.hj = hj;
                         C.dplane = zmarch && (m == 0);
-                        const bool hist = !lastpass;
+                        const bool hist = hist_on;
                         const bool strips = blk_last && more && !(zmarch && m == n_m - 1);
                         C.tail = 0;
-                        TC.GhP = hist ? reinterpret_cast<f2*>(U.Gu) + ((size_t)(pass & 1) * n_m + m) * g_plane : nullptr;
+                        TC.GhP = hist ? reinterpret_cast<f2*>(U.Gu) + ((size_t)(P & 1) * n_m + m) * g_plane : nullptr;
+                        if (RTS_TOLM) TC.GhO = (tolmode && P > 0) ? reinterpret_cast<const f2*>(U.Gu) + ((size_t)((P - 1) & 1) * n_m + m) * g_plane : nullptr;
+                        if (RTS_TOLM) TC.errp = tolmode ? &S.errs[s][0] : nullptr;
                         TC.XeP = strips ? reinterpret_cast<float4*>(U.Xex) + (size_t)(gblk & 1) * xe_par : nullptr;
                         TC.tag = tag0 | ((unsigned)(gblk + 1) & 0xfffu);
                         C.xmask = IT_PART | (hist ? IT_FARC : 0u) | (strips ? IT_USTRIP : 0u);
@@ -921,7 +1036,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 // ---- seam ghosts of this plane into the new carried plane
                 if (ghost_next) {
                     f2* const Xw = S.Xb + (size_t)(cur ^ 1) * NG * PS;
-                    if (pass > 0) {
+                    if (P > 0) {
 #pragma unroll
                         for (int i = 0; i < 2; ++i) {
                             const int e = tid + i * T;
@@ -929,7 +1044,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                         }
                         for (int e = tid + 2 * T; e < ngh; e += T) {
                             const GhostEnt g = S.gt[e];
-                            Xw[xso<PITCH>(S, g.goff >> 28) + g.xoff] = ghost_fetch<PITCH>(S, g, pass - 1, m, nullptr);
+                            Xw[xso<PITCH>(S, g.goff >> 28) + g.xoff] = ghost_fetch<PITCH>(S, g, P - 1, m, nullptr);
                         }
                     } else {
                         const f2* Kc = S.stage0 + (size_t)stc * PS;
@@ -959,6 +1074,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     }
     // heating / emergent intensity of the last plane
     if (!bail) q_pass<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, n_m - 1);
+    if (tolmode && !bail) pass_end<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, pbase + npass - 1);
     __syncthreads();
     if (tid == 0)
         for (int i = 0; i < NST; ++i)
@@ -968,7 +1084,8 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
 template <int PITCH>
 __global__ void __launch_bounds__(RTS_SWEEP_THREADS, 1)
 rts_sweep_kernel(const __grid_constant__ SweepMaps maps, const UnitDesc* __restrict__ units, int nunits,
-                 int total_tickets, int* ticket_counter, float* __restrict__ Itop_all, int* abortf, unsigned seq)
+                 int total_tickets, int* ticket_counter, float* __restrict__ Itop_all, int* abortf, unsigned seq,
+                 int pbase, int npass_launch)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(16) TaskShared S;
@@ -993,8 +1110,8 @@ rts_sweep_kernel(const __grid_constant__ SweepMaps maps, const UnitDesc* __restr
             for (int w = threadIdx.x; w < (int)(sizeof(UnitDesc) / sizeof(int)); w += blockDim.x) dst[w] = src[w];
         }
         __syncthreads();
-        run_task<PITCH>(S, maps, ticket - S.U.ticket_begin, reinterpret_cast<f2*>(smem_raw), Itop_all, abortf, seq);
+        run_task<PITCH>(S, maps, ticket - S.U.ticket_begin, reinterpret_cast<f2*>(smem_raw), Itop_all, abortf, seq, pbase, npass_launch);
     }
 }
 
-}  // namespace rts
+} }  // namespace rts::RTS_MODE_NS

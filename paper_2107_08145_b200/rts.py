@@ -27,6 +27,7 @@ EXPORTS = [
     "rts_plan_info", "rts_last_error", "rts_enable_timing", "rts_last_timing",
     "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells", "rts_set_thick_skip", "rts_thick_levels",
     "rts_enable_flux", "rts_set_flux_blend", "rts_solve_flux", "rts_set_shard", "rts_shard_info",
+    "rts_set_tolerance", "rts_set_warm_start", "rts_passes_used",
 ]
 
 
@@ -99,6 +100,12 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_set_flux_blend.argtypes = [c_void_p, c_double]
     lib.rts_solve_flux.restype = c_int
     lib.rts_solve_flux.argtypes = [c_void_p] + [c_void_p] * 8 + [c_void_p]
+    lib.rts_set_tolerance.restype = c_int
+    lib.rts_set_tolerance.argtypes = [c_void_p, c_double, c_int]
+    lib.rts_set_warm_start.restype = c_int
+    lib.rts_set_warm_start.argtypes = [c_void_p, c_int]
+    lib.rts_passes_used.restype = c_int
+    lib.rts_passes_used.argtypes = [c_void_p, PI, PF]
     lib.rts_set_shard.restype = c_int
     lib.rts_set_shard.argtypes = [c_void_p, c_int, c_int]
     lib.rts_shard_info.restype = c_int
@@ -329,6 +336,20 @@ class RTS:
                     "rts_solve_cells")
         return Qc, (Itop if want_itop else None)
 
+    def set_tolerance(self, tol: float, max_passes: int):
+        """Error-controlled iteration (NEXT #3): sweep until the seam faces of every (band, ray) change by at most
+        tol * max|I| on them, at most max_passes passes (0: back to the fixed pass count).  Call before
+        allocate_workspace."""
+        self._check(self._lib.rts_set_tolerance(self._ctx, float(tol), int(max_passes)), "rts_set_tolerance")
+
+    def set_warm_start(self, on: bool = True):
+        self._check(self._lib.rts_set_warm_start(self._ctx, 1 if on else 0), "rts_set_warm_start")
+
+    def passes_used(self) -> Tuple[int, float]:
+        n, e = ctypes.c_int(0), ctypes.c_float(0.0)
+        self._check(self._lib.rts_passes_used(self._ctx, ctypes.byref(n), ctypes.byref(e)), "rts_passes_used")
+        return n.value, e.value
+
     def set_shard(self, rank: int, nranks: int):
         """Band x octant sharding: this context sweeps the units u with u % nranks == rank; solve() then returns
         partial Q and I_top that a sum all-reduce over the ranks completes (multi.allreduce_sum)."""
@@ -361,7 +382,8 @@ class RTS:
 
 
 def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchange_interval: int = 0,
-                cells: bool = False, ring_depth: int = 0, flux: bool = False, shard: Optional[Tuple[int, int]] = None) -> "RTS":
+                cells: bool = False, ring_depth: int = 0, flux: bool = False, shard: Optional[Tuple[int, int]] = None,
+                tolerance: Optional[Tuple[float, int]] = None) -> "RTS":
     """Create and configure a solver for an `inputs.RTSInputs` problem.  cells=True: the fields of
     `inp` are cell-centred (solve_cells); the RT node grid then has one level more."""
     r = RTS(inp.nx, inp.ny, inp.nz + (1 if cells else 0), inp.dx, inp.dy, inp.dz, inp.nbands)
@@ -381,5 +403,7 @@ def from_inputs(inp, tiling: Optional[dict] = None, ctas_per_sm: int = 0, exchan
         r.enable_flux(True)
     if shard:
         r.set_shard(*shard)
+    if tolerance:
+        r.set_tolerance(*tolerance)
     r.allocate_workspace()
     return r
