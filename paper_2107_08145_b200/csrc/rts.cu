@@ -770,7 +770,7 @@ int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, flo
             }
         kp.kstar_pair = (int*)(ws + c->off_kstar); kp.mthick_pair = (int*)(ws + c->off_mthick);
         kp.mthick_band = (int*)(ws + c->off_mthick_b); kp.lev = (double*)(ws + c->off_lev);
-        rts_kstar_kernel<<<c->nbp, 256, 0, st>>>(kp);
+        rts_kstar_kernel<<<c->nbp, 1024, 0, st>>>(kp);             // 32 warps: the level sums are latency-bound loads
     }
     CUDA_TRY(c, cudaGetLastError());
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[1], st));

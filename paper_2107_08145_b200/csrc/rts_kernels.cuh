@@ -289,7 +289,7 @@ struct KstarParams {
     int* mthick_band;        // [nb][3]    (reporting)
     double* lev;             // scratch [nb][2][nz]
 };
-__global__ void __launch_bounds__(256) rts_kstar_kernel(const KstarParams p)
+__global__ void __launch_bounds__(1024) rts_kstar_kernel(const KstarParams p)
 {
     __shared__ int sh_ks[2], sh_mt[2][3];
     const int pr = blockIdx.x;
