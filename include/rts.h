@@ -133,7 +133,8 @@ int rts_solve_flux(rts_ctx* ctx, const float* rho_dev, const float* T_dev, const
 /* [same operation as rts_solve; the end-to-end entry bench.py's `e2e` times]
  * Same solve with HOST buffers (pinned or pageable): copies rho,T,P to the device, solves,
  * copies Qrad (and Itop if non-NULL) back, synchronises.  The staging buffers live in the
- * workspace (rts_workspace_bytes accounts for them). */
+ * workspace (rts_workspace_bytes accounts for them).  The inputs travel in 8 slabs of levels on an internal
+ * second stream while stage A follows slab by slab on `stream`; I_top goes back while the finalize kernel runs. */
 int rts_solve_host(rts_ctx* ctx, const float* rho_host, const float* T_host, const float* P_host,
                    float* Qrad_host, float* Itop_host, void* stream);
 

@@ -101,6 +101,8 @@ struct rts_ctx {
     cudaEvent_t ev = nullptr;
     bool timing = false;
     cudaEvent_t tev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    cudaStream_t copy_stream = nullptr;        // rts_solve_host: copies overlap the kernels
+    cudaEvent_t hev[10] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     std::string err;
 };
 
@@ -516,8 +518,9 @@ int bind_workspace(rts_ctx* c)
 cudaStream_t as_stream(void* s) { return (cudaStream_t)s; }
 
 int launch_stage_a(rts_ctx* c, const float* rho, const float* T, const float* P, float* plain_k, float* plain_s,
-                   cudaStream_t st)
+                   cudaStream_t st, int k0 = 0, int nk = -1)
 {
+    if (nk < 0) nk = c->nz;
     CoefParams p{};
     p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nb = c->nb; p.nT = c->nT; p.nP = c->nP;
     p.logT_min = c->logT_min; p.inv_dT = (c->nT - 1) / (c->logT_max - c->logT_min);
@@ -530,8 +533,8 @@ int launch_stage_a(rts_ctx* c, const float* rho, const float* T, const float* P,
     p.strideB_n = (long long)c->nz * c->nx * c->PY;
     p.ksum = (double*)(c->ws + c->off_ksum);
     p.kmin = (float*)(c->ws + c->off_kmin);
-    p.plain_k = plain_k; p.plain_s = plain_s;
-    dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, c->nz), block(32, 8);
+    p.plain_k = plain_k; p.plain_s = plain_s; p.k0 = k0;
+    dim3 grid((c->nx + 31) / 32, (c->ny + 31) / 32, nk), block(32, 8);
     rts_coef_kernel<<<grid, block, 0, st>>>(p);
     CUDA_TRY(c, cudaGetLastError());
     return RTS_OK;
@@ -591,6 +594,8 @@ int rts_destroy(rts_ctx* c)
     if (c->d_bandfrac) cudaFree(c->d_bandfrac);
     if (c->ev) cudaEventDestroy(c->ev);
     for (auto& e : c->tev) if (e) cudaEventDestroy(e);
+    for (auto& e : c->hev) if (e) cudaEventDestroy(e);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
     return RTS_OK;
 }
@@ -740,7 +745,7 @@ int rts_coefficients(rts_ctx* c, const float* rho, const float* T, const float* 
 
 namespace {
 int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, float* Q, float* Itop,
-               float* F, float* Qdiv, float* Qblend, void* stream)
+               float* F, float* Qdiv, float* Qblend, void* stream, bool stage_a_done = false, cudaEvent_t after_sweep = nullptr)
 {
     if (!c) return RTS_EINVAL;
     if (!rho || !T || !P || !Q) return fail(c, RTS_EINVAL, "rts_solve: null pointer");
@@ -755,7 +760,7 @@ int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, flo
 
     // stage A + switch heights
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[0], st));
-    int rc = launch_stage_a(c, rho, T, P, nullptr, nullptr, st);
+    int rc = stage_a_done ? RTS_OK : launch_stage_a(c, rho, T, P, nullptr, nullptr, st);   // (rts_solve_host ran it slab by slab)
     if (rc != RTS_OK) return rc;
     {
         KstarParams kp{};
@@ -818,6 +823,7 @@ int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, flo
     }
     // finalize
     if (c->timing) CUDA_TRY(c, cudaEventRecord(c->tev[3], st));
+    if (after_sweep) CUDA_TRY(c, cudaEventRecord(after_sweep, st));
     {
         // the units' partial heating (and flux) summed in unit order: deterministic
         FinalizeParams fp{};
@@ -983,13 +989,40 @@ int rts_solve_host(rts_ctx* c, const float* rho, const float* T, const float* P,
     const size_t nI = (size_t)c->nb * c->n_up * c->ny * c->nx;
     float* din = (float*)(c->ws + c->off_stage_in);
     float* dout = (float*)(c->ws + c->off_stage_out);
-    CUDA_TRY(c, cudaMemcpyAsync(din, rho, N * sizeof(float), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(c, cudaMemcpyAsync(din + N, T, N * sizeof(float), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(c, cudaMemcpyAsync(din + 2 * N, P, N * sizeof(float), cudaMemcpyHostToDevice, st));
-    int rc = rts_solve(c, din, din + N, din + 2 * N, dout, Itop ? dout + N : nullptr, stream);
+    // Copies and kernels overlap: rho, T, P arrive in slabs of levels on a second stream, stage A follows slab by
+    // slab on the caller's stream; I_top goes back while the finalize kernel runs.
+    if (!c->copy_stream) {
+        CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (auto& e : c->hev) CUDA_TRY(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    constexpr int NSLAB = 8;
+    CUDA_TRY(c, cudaEventRecord(c->hev[NSLAB], st));                      // earlier work on the caller's stream still reads din
+    CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->hev[NSLAB], 0));
+    const size_t plane = (size_t)c->nx * c->ny;
+    for (int sl = 0; sl < NSLAB; ++sl) {
+        const int k0 = (int)((long long)c->nz * sl / NSLAB), k1 = (int)((long long)c->nz * (sl + 1) / NSLAB);
+        if (k1 <= k0) continue;
+        const size_t o = plane * k0, n = plane * (k1 - k0) * sizeof(float);
+        CUDA_TRY(c, cudaMemcpyAsync(din + o, rho + o, n, cudaMemcpyHostToDevice, c->copy_stream));
+        CUDA_TRY(c, cudaMemcpyAsync(din + N + o, T + o, n, cudaMemcpyHostToDevice, c->copy_stream));
+        CUDA_TRY(c, cudaMemcpyAsync(din + 2 * N + o, P + o, n, cudaMemcpyHostToDevice, c->copy_stream));
+        CUDA_TRY(c, cudaEventRecord(c->hev[sl], c->copy_stream));
+        CUDA_TRY(c, cudaStreamWaitEvent(st, c->hev[sl], 0));
+        if (!c->have_tables) return fail(c, RTS_ESTATE, "rts_solve_host: tables not set");
+        int rcA = launch_stage_a(c, din, din + N, din + 2 * N, nullptr, nullptr, st, k0, k1 - k0);
+        if (rcA != RTS_OK) return rcA;
+    }
+    int rc = solve_impl(c, din, din + N, din + 2 * N, dout, Itop ? dout + N : nullptr, nullptr, nullptr, nullptr, stream,
+                        true, c->hev[NSLAB + 1]);
     if (rc != RTS_OK) return rc;
+    if (Itop && c->tol_max_passes <= 0) {
+        CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->hev[NSLAB + 1], 0));
+        CUDA_TRY(c, cudaMemcpyAsync(Itop, dout + N, nI * sizeof(float), cudaMemcpyDeviceToHost, c->copy_stream));
+    } else if (Itop) {
+        CUDA_TRY(c, cudaMemcpyAsync(Itop, dout + N, nI * sizeof(float), cudaMemcpyDeviceToHost, st));
+    }
     CUDA_TRY(c, cudaMemcpyAsync(Q, dout, N * sizeof(float), cudaMemcpyDeviceToHost, st));
-    if (Itop) CUDA_TRY(c, cudaMemcpyAsync(Itop, dout + N, nI * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(c->copy_stream));
     return rts_sync_check(c, stream);
 }
 

@@ -146,6 +146,7 @@ struct CoefParams {
     double* ksum;            // [nb][nz][nblk] partial sums (nblk = gridDim.x*gridDim.y), or null
     float* kmin;             // [nb][nz][nblk] partial minima of kaprho (with ksum)
     float* plain_k; float* plain_s;              // optional [nb][N] outputs (rts_coefficients)
+    int k0;                                      // first level of this launch (gridDim.z levels: rts_solve_host feeds slabs)
 };
 
 __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
@@ -154,7 +155,7 @@ __global__ void __launch_bounds__(256) rts_coef_kernel(const CoefParams p)
     __shared__ double red[2][8];
     __shared__ float redm[2][8];
     const int tx = threadIdx.x, ty = threadIdx.y;
-    const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32, k = blockIdx.z;
+    const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32, k = p.k0 + blockIdx.z;
     const int i = i0 + tx;
     const long long N = (long long)p.nx * p.ny * p.nz;
 
