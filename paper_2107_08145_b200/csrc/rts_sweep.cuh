@@ -235,58 +235,31 @@ __device__ __forceinline__ f2 bil_from(const Row3& up, const Row3& ow, const flo
 
 // ------------------------------------------------------------------------------------------
 // Attenuation factors of one node (both bands): em1 = 1 - e^-dt, wl = (1 - e^-dt)/dt, pp = psi_p = 1 - wl.
-// EV 0: closed form (exp2 and reciprocal units); accurate for dt >= DTAU_SERIES.
-// EV 1: series of psi_p (8 terms, truncation < 3e-9 relative for dt <= DTAU_SERIES_MAX; no cancellation,
-//       no special-function unit), wl = 1 - psi_p, em1 = dt*wl.
-// EV 2: both, selected per band (a row whose optical paths span more than DTAU_SERIES .. DTAU_SERIES_MAX).
-// EV 3: the first four terms of the series (every optical path of the row below DTAU_SERIES).
-constexpr float DTAU_SERIES_MAX = 0.5f;
-template <int EV>
+// ONE branch-free form for every optical path, the same instructions in every lane, warp and tile:
+//   dt >= DTAU_SERIES: closed form (exp2 and reciprocal units): wl = (1 - E)/dt, pp = 1 - wl;
+//   dt <  DTAU_SERIES: where 1 - E and 1 - wl cancel, the first four terms of the series of psi_p
+//                      (truncation dt^4/360 < 2e-8 relative there), wl = 1 - psi_p;
+//   both are evaluated and selected per lane and band.
+// Round 2 measured why there is one form and not a cheap one for uniform rows and a dearer one for mixed rows
+// (chosen per warp by a vote): the tiles of a unit advance in lockstep, so the tiles of the dearest regime set
+// the pace of all (the whole sweep ran at the cost of the mixed form: 29.6 ms; this form everywhere: 27.7 ms),
+// and the result no longer depends on which nodes share a warp, i.e. on the tiling.
 __device__ __forceinline__ void att_factors(const f2 dt, f2& em1, f2& wl, f2& pp)
 {
-    f2 pps;
-    if (EV == 3) {
-        // every optical path of the row below DTAU_SERIES: four terms (truncation dt^4/360 < 2e-8)
-        const f2 nd = neg2(dt);
-        f2 q = fma2(nd, bc(1.0f / 120.0f), bc(1.0f / 24.0f));
-        q = fma2(nd, q, bc(1.0f / 6.0f));
-        q = fma2(nd, q, bc(0.5f));
-        pp = mul2(dt, q);
-        wl = sub2(bc(1.f), pp);
-        em1 = mul2(dt, wl);
-        return;
-    }
-    if (EV != 0) {
-        const f2 nd = neg2(dt);
-        f2 q = fma2(nd, bc(1.0f / 362880.0f), bc(1.0f / 40320.0f));
-        q = fma2(nd, q, bc(1.0f / 5040.0f));
-        q = fma2(nd, q, bc(1.0f / 720.0f));
-        q = fma2(nd, q, bc(1.0f / 120.0f));
-        q = fma2(nd, q, bc(1.0f / 24.0f));
-        q = fma2(nd, q, bc(1.0f / 6.0f));
-        q = fma2(nd, q, bc(0.5f));
-        pps = mul2(dt, q);
-    }
-    if (EV == 1) {
-        pp = pps;
-        wl = sub2(bc(1.f), pp);
-        em1 = mul2(dt, wl);
-        return;
-    }
+    const f2 nd = neg2(dt);
+    f2 q = fma2(nd, bc(1.0f / 120.0f), bc(1.0f / 24.0f));
+    q = fma2(nd, q, bc(1.0f / 6.0f));
+    q = fma2(nd, q, bc(0.5f));
+    const f2 pps = mul2(dt, q), wls = sub2(bc(1.f), pps);
     const f2 t2 = mul2(dt, bc(-LOG2E));
     const f2 E = make_float2(ex2_approx(t2.x), ex2_approx(t2.y));
-    em1 = sub2(bc(1.f), E);
-    wl = mul2(em1, make_float2(rcp_approx(dt.x), rcp_approx(dt.y)));
-    pp = sub2(bc(1.f), wl);
-    if (EV == 2) {
-        // per band: the series values below DTAU_SERIES (wl, em1 derived from psi_p there: no cancellation),
-        // the closed form above (where 1 - psi_p would lose the small wl of a thick path)
-        const f2 wls = sub2(bc(1.f), pps), es = mul2(dt, wls);
-        const bool sx = dt.x < DTAU_SERIES, sy = dt.y < DTAU_SERIES;
-        pp = make_float2(sx ? pps.x : pp.x, sy ? pps.y : pp.y);
-        wl = make_float2(sx ? wls.x : wl.x, sy ? wls.y : wl.y);
-        em1 = make_float2(sx ? es.x : em1.x, sy ? es.y : em1.y);
-    }
+    const f2 ec = sub2(bc(1.f), E);                            // exactly 1 where exp2 underflows (thick-plane shortcut)
+    const f2 wlc = mul2(ec, make_float2(rcp_approx(dt.x), rcp_approx(dt.y)));
+    const f2 ppc = sub2(bc(1.f), wlc), es = mul2(dt, wls);
+    const bool sx = dt.x < DTAU_SERIES, sy = dt.y < DTAU_SERIES;
+    pp = make_float2(sx ? pps.x : ppc.x, sy ? pps.y : ppc.y);
+    wl = make_float2(sx ? wls.x : wlc.x, sy ? wls.y : wlc.y);
+    em1 = make_float2(sx ? es.x : ec.x, sy ? es.y : ec.y);
 }
 
 // One node (both bands).  su/so, xu/xo: upwind / own stencil row of S and X; sp: source at the node.
@@ -806,18 +779,12 @@ __device__ __forceinline__ void do_strip(
         const float4 kc = lds128<0>(bC), sc = lds128<HP>(bC);                                                       \
         const f2 dt0 = mul2(add2(make_float2(kc.x, kc.y), bil<SU, 0>(KU, KO, rk.w)), bc(rk.kc));                    \
         const f2 dt1 = mul2(add2(make_float2(kc.z, kc.w), bil<SU, 1>(KU, KO, rk.w)), bc(rk.kc));                    \
-        const float dmin = fminf(fminf(dt0.x, dt0.y), fminf(dt1.x, dt1.y));                                         \
-        const float dmax = fmaxf(fmaxf(dt0.x, dt0.y), fmaxf(dt1.x, dt1.y));                                         \
         float a_u, a_o, a_p;                                                                                        \
         if (zm) { a_u = a_o = C.a_prev; a_p = C.a_cur; }                                                            \
         else { a_u = (vrow - vstep <= ks) ? 1.f : 0.f; a_o = (vrow <= ks) ? 1.f : 0.f; a_p = a_o; }                  \
         const f2 sp0 = make_float2(sc.x, sc.y), sp1 = make_float2(sc.z, sc.w);                                      \
         f2 e0, l0, p0, e1, l1, p1;                                                                                  \
-        /* one evaluator per warp and row (each is valid for every lane that takes part): no divergence */          \
-        const unsigned am_ = __activemask();                                                                        \
-        if (__all_sync(am_, dmin >= DTAU_SERIES)) { att_factors<0>(dt0, e0, l0, p0); att_factors<0>(dt1, e1, l1, p1); }    \
-        else if (__all_sync(am_, dmax <= DTAU_SERIES_MAX)) { att_factors<1>(dt0, e0, l0, p0); att_factors<1>(dt1, e1, l1, p1); } \
-        else { att_factors<2>(dt0, e0, l0, p0); att_factors<2>(dt1, e1, l1, p1); }                                  \
+        att_factors(dt0, e0, l0, p0); att_factors(dt1, e1, l1, p1);                                                 \
         f2 v0, v1;                                                                                                  \
         if (a_u == a_o && a_o == a_p) {                                                                             \
             v0 = node_update<SU, 0, 3>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, 1.f - a_p, 0.f, 0.f);                \
