@@ -262,6 +262,26 @@ __device__ __forceinline__ void att_factors(const f2 dt, f2& em1, f2& wl, f2& pp
     em1 = make_float2(sx ? es.x : ec.x, sy ? es.y : ec.y);
 }
 
+// The same for the uniform regimes (a the same on both stencil rows and at the node, f = 1 - a): they need
+// em1 and c = wl - f only.  For f = 1 (the direct part) c = -psi_p comes straight from the series where it is
+// small, and psi_p itself is not formed.
+__device__ __forceinline__ void att_uniform(const f2 dt, const float f, f2& em1, f2& c)
+{
+    const f2 nd = neg2(dt);
+    f2 q = fma2(nd, bc(1.0f / 120.0f), bc(1.0f / 24.0f));
+    q = fma2(nd, q, bc(1.0f / 6.0f));
+    q = fma2(nd, q, bc(0.5f));
+    const f2 pps = mul2(dt, q);
+    const f2 cs = sub2(bc(1.f - f), pps), es = fma2(nd, pps, dt);          // (1 - psi_p) - f;  dt (1 - psi_p)
+    const f2 t2 = mul2(dt, bc(-LOG2E));
+    const f2 E = make_float2(ex2_approx(t2.x), ex2_approx(t2.y));
+    const f2 ec = sub2(bc(1.f), E);                            // exactly 1 where exp2 underflows (thick-plane shortcut)
+    const f2 cc = fma2(ec, make_float2(rcp_approx(dt.x), rcp_approx(dt.y)), bc(-f));
+    const bool sx = dt.x < DTAU_SERIES, sy = dt.y < DTAU_SERIES;
+    c = make_float2(sx ? cs.x : cc.x, sy ? cs.y : cc.y);
+    em1 = make_float2(sx ? es.x : ec.x, sy ? es.y : ec.y);
+}
+
 // One node (both bands).  su/so, xu/xo: upwind / own stencil row of S and X; sp: source at the node.
 // REG 0: departure-carried part (a = 1 on both stencil rows and at the node); 1: direct part (a = 0);
 // 2: general (a per row).
@@ -274,9 +294,10 @@ __device__ __forceinline__ f2 node_update(const f2 em1, const f2 wl, const f2 pp
     if (REG == 3) {
         // uniform regime, f = a_u = 1 - a: one branch-free form of REG 0 (f = 0) and REG 1 (f = 1):
         //   X = Xu + em1 (f (d + Sp) - Xu) + (wl - f) d,  d = Su - Sp formed first (weights sum to 1);  wl - 1 = -psi_p
+        //   (here `wl` carries c = wl - f of att_uniform)
         const f2 d = bil_from<SU, J>(su, so, w, neg2(sp));
         const f2 t = fma2(bc(a_u), add2(d, sp), neg2(Xu));
-        return fma2(sub2(wl, bc(a_u)), d, fma2(em1, t, Xu));
+        return fma2(wl, d, fma2(em1, t, Xu));
     }
     f2 v = fma2(neg2(Xu), em1, Xu);                                // Xu * e^-dt
     if (REG == 0) {
@@ -784,12 +805,13 @@ __device__ __forceinline__ void do_strip(
         else { a_u = (vrow - vstep <= ks) ? 1.f : 0.f; a_o = (vrow <= ks) ? 1.f : 0.f; a_p = a_o; }                  \
         const f2 sp0 = make_float2(sc.x, sc.y), sp1 = make_float2(sc.z, sc.w);                                      \
         f2 e0, l0, p0, e1, l1, p1;                                                                                  \
-        att_factors(dt0, e0, l0, p0); att_factors(dt1, e1, l1, p1);                                                 \
         f2 v0, v1;                                                                                                  \
         if (a_u == a_o && a_o == a_p) {                                                                             \
-            v0 = node_update<SU, 0, 3>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, 1.f - a_p, 0.f, 0.f);                \
-            v1 = node_update<SU, 1, 3>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, 1.f - a_p, 0.f, 0.f);                \
+            att_uniform(dt0, 1.f - a_p, e0, l0); att_uniform(dt1, 1.f - a_p, e1, l1);                               \
+            v0 = node_update<SU, 0, 3>(e0, l0, l0, SU_, SO, XU, XO, sp0, rk.w, 1.f - a_p, 0.f, 0.f);                \
+            v1 = node_update<SU, 1, 3>(e1, l1, l1, SU_, SO, XU, XO, sp1, rk.w, 1.f - a_p, 0.f, 0.f);                \
         } else {                                                                                                    \
+            att_factors(dt0, e0, l0, p0); att_factors(dt1, e1, l1, p1);                                             \
             v0 = node_update<SU, 0, 2>(e0, l0, p0, SU_, SO, XU, XO, sp0, rk.w, a_u, a_o, a_p);                      \
             v1 = node_update<SU, 1, 2>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, a_u, a_o, a_p);                      \
         }                                                                                                           \
