@@ -157,11 +157,8 @@ __device__ __forceinline__ void tensor_load5(void* dst, const CUtensorMap* map, 
 enum : unsigned {
     IT_DQ = 1u << 0,         // halo pair in u: only active while the remaining halo depth is > 0
     IT_PART = 1u << 1,       // only the first column of the pair exists (odd n_u)
-    IT_FARC = 1u << 2,       // core pair holding the far-u column of its ray: writes the seam history
     IT_USTRIP = 1u << 3,     // core pair inside the u exchange strip
-    IT_FARV = 1u << 4,       // the last row of the region is the far-v row of a periodic v axis (seam history)
-    IT_DIR = 1u << 5,        // row q = 0 is the inflow row of a bounded v axis (set, not updated)
-    IT_FSEC = 1u << 6        // the far-u column is the second column of the pair
+    IT_DIR = 1u << 5         // row q = 0 is the inflow row of a bounded v axis (set, not updated)
 };
 
 struct GhostEnt { unsigned short xoff, bv; int goff; };   // 8 bytes; slot = goff >> 28; xoff: box row * 2 PITCH + column
@@ -321,34 +318,14 @@ __device__ __forceinline__ f2 node_update(const f2 em1, const f2 wl, const f2 pp
     return fma2(pp, sub2(sp, Stp), v);
 }
 
-// what a strip needs for the uncommon stores of a step (seam histories, exchange strips)
+// what a strip needs for the uncommon stores of a step (exchange strips)
 struct TailCtx {
-    f2* GhP;                           // seam history of this plane and pass (far columns, then far rows); null: off
     float4* XeP;                       // exchange planes of this block's parity (16 bytes per node); null: no strips this step
     int gv0, ug;                       // slot * n_v + global v of row q = 0;  global u of the pair
-    int n_u2, far_off;                 // row pitch of the exchange planes; NSLOT*n_v + slot*n_u2 (far-v rows)
+    int n_u2;                          // row pitch of the exchange planes
     int hv, nrows, K, gsv;
     unsigned tag;                      // tag of the block whose strips are published this step (0: plain strips)
-    const f2* GhO;                     // tolmode: seam history of this plane in the previous pass (null: I(0) = S)
-    unsigned* errp;                    // tolmode: this ray's error words in shared memory (else null)
 };
-
-// Store one finished row of a strip: the carried plane and, where flagged, the seam history (far-u column,
-// far-v row) and the exchange strips.  Inline: a few instructions on the flagged rows only.
-// Error-controlled iteration (NEXT #3): change of one seam node (both bands) against the previous pass, and the
-// intensity itself, into the ray's error words (non-negative floats order like unsigned integers).
-// xn: new carried value X = I - a S; sn: S; goff: the node's slot in the seam history; dirichlet: the node was set.
-__device__ __noinline__ void seam_error(const f2* GhO, unsigned* errp, const int goff, const f2 xn, const f2 sn, const float a_p, const bool dirichlet)
-{
-    const f2 In = fma2(bc(a_p), sn, xn);                                   // I = X + a S
-    f2 d = make_float2(0.f, 0.f);
-    if (!dirichlet) {
-        if (GhO) { const f2 xo = __ldcg(GhO + goff); d = sub2(xn, xo); }                // same a, S in both passes
-        else d = sub2(In, sn);                                             // I(0) = S
-    }
-    atomicMax(errp + 0, __float_as_uint(fabsf(d.x))); atomicMax(errp + 1, __float_as_uint(fabsf(d.y)));
-    atomicMax(errp + 2, __float_as_uint(fabsf(In.x))); atomicMax(errp + 3, __float_as_uint(fabsf(In.y)));
-}
 
 // ------------------------------------------------------------------------------------------
 // shared-memory carve-up of a CTA (float2 nodes), every part 128-byte aligned.  A plane set is BV rows of
@@ -494,6 +471,54 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
                 if (U.qvec && nval == 2) *reinterpret_cast<float2*>(fd) = make_float2(f0, f1);
                 else { fd[0] = f0; if (nval == 2) fd[1] = f1; }
             }
+        }
+    }
+}
+
+// Seam histories of a finished plane (out of line): the far-u column and, on a periodic v axis, the far-v row of
+// every ray are copied from the carried plane set Xn (one buffer) to Gu[parity of pass P][m_done]: the next pass's
+// Jacobi ghosts of that plane.  Error-controlled mode: their change against the previous pass and the intensity
+// itself go into the ray's error words (Kc: the plane's coefficient stage, for S).
+template <int PITCH>
+__device__ __noinline__ void hist_pass(TaskShared* __restrict__ Sp, const f2* __restrict__ Kc, const f2* __restrict__ Xn, const int m_done, const int P)
+{
+    constexpr int RPN = 2 * PITCH;
+    TaskShared& S = *Sp;
+    const UnitDesc& U = S.U; const TileGeo& G = S.G;
+    const int tid = threadIdx.x, T = blockDim.x;
+    const size_t g_plane = (size_t)NSLOT * (U.n_v + U.n_u2);
+    f2* const GhP = reinterpret_cast<f2*>(U.Gu) + ((size_t)(P & 1) * U.n_m + m_done) * g_plane;
+    const f2* const GhO = (RTS_TOLM && P > 0) ? reinterpret_cast<const f2*>(U.Gu) + ((size_t)((P - 1) & 1) * U.n_m + m_done) * g_plane : nullptr;
+    const bool zmarch = G.zmarch != 0;
+    const int per = G.wv + (U.per_v ? G.wu : 0);                 // far-column nodes, then far-row nodes of one ray
+    for (int i = tid; i < NSLOT * per; i += T) {
+        const int s = i / per, j = i - s * per;
+        if (!U.ray[s].active) continue;
+        const int su = (s & 1) ? -1 : 1, sv = (s & 2) ? -1 : 1;
+        int bu, bv, goff;
+        if (j < G.wv) {                                          // far-u column of this ray, if this tile holds it
+            bu = (su > 0) ? G.dhi_u - 1 : G.dlo_u; bv = HALO + j;
+            if (bu < HALO || bu >= HALO + G.wu) continue;
+            goff = s * U.n_v + G.v0 + j;
+        } else {                                                 // far-v row
+            bv = (sv > 0) ? G.dhi_v - 1 : G.dlo_v; bu = HALO + (j - G.wv);
+            if (bv < HALO || bv >= HALO + G.wv) continue;
+            goff = NSLOT * U.n_v + s * U.n_u2 + G.u0 + (j - G.wv);
+        }
+        const int xo = bv * RPN + bu;
+        const f2 xn = Xn[xso<PITCH>(S, s) + xo];
+        __stcg(GhP + goff, xn);
+        if (RTS_TOLM) {
+            const int v = G.v0 - HALO + bv;
+            const f2 Sv = Kc[xo + PITCH];
+            const float a = zmarch ? a_of(G, plane_of(U, m_done)) : a_of(G, v);
+            const bool up = zmarch ? (G.up_z != 0) : !(s & 2);
+            const bool dn = zmarch ? (m_done == 0) : (v == (up ? 0 : U.n_v - 1));   // inflow node: set, never changes
+            const f2 In = fma2(bc(a), Sv, xn);                   // I = X + a S
+            f2 d = make_float2(0.f, 0.f);
+            if (!dn) d = GhO ? sub2(xn, __ldcg(GhO + goff)) : sub2(In, Sv);     // same a, S in both passes; I(0) = S
+            atomicMax(&S.errs[s][0], __float_as_uint(fabsf(d.x))); atomicMax(&S.errs[s][1], __float_as_uint(fabsf(d.y)));
+            atomicMax(&S.errs[s][2], __float_as_uint(fabsf(In.x))); atomicMax(&S.errs[s][3], __float_as_uint(fabsf(In.y)));
         }
     }
 }
@@ -721,33 +746,19 @@ __device__ __forceinline__ void issue_load(TaskShared& S, const CUtensorMap* cma
     tensor_load5(dst, cmap, 2 * G.u0, 0, c2, c3, U.pair, bar);
 }
 
+// Store one finished row of a strip: the carried plane and, at a block end, the exchange strips.  Inline: a few
+// instructions on the flagged rows only.  (The seam histories are copied from the finished plane by hist_pass: a
+// strip that stored them row by row dragged its whole warp through this slow path, and the edge tiles, which
+// alone have such strips, set the pace of their unit.)
 template <int SU>
 __device__ __forceinline__ void row_store(const TailCtx& TC, const unsigned fl, const bool slow, const int q,
-                                          const uint32_t bW, const float4 o, const float4 sc = make_float4(0.f, 0.f, 0.f, 0.f),
-                                          const float a_p = 0.f, const bool dirichlet = false)
+                                          const uint32_t bW, const float4 o)
 {
     if (!slow) { sts128<0>(bW, o); return; }
     const bool part = (fl & IT_PART) != 0;
     if (!part) sts128<0>(bW, o); else sts64<0>(bW, make_float2(o.x, o.y));
     if (q < TC.hv || (fl & IT_DQ)) return;                       // halo row / halo pair: nothing to publish
     const int gv = TC.gv0 + q * TC.gsv;
-    if (TC.GhP) {
-        if (fl & IT_FARC) {                                      // far-u column: next pass's seam ghosts of this plane
-            const bool sec = (fl & IT_FSEC) != 0;
-            const f2 xn = sec ? make_float2(o.z, o.w) : make_float2(o.x, o.y);
-            __stcg(TC.GhP + gv, xn);
-            if (RTS_TOLM && TC.errp) seam_error(TC.GhO, TC.errp, gv, xn, sec ? make_float2(sc.z, sc.w) : make_float2(sc.x, sc.y), a_p, dirichlet);
-        }
-        if ((fl & IT_FARV) && q == TC.nrows - 1) {               // far-v row (periodic v axis)
-            f2* gvp = TC.GhP + TC.far_off + TC.ug;
-            if (!part) __stcg(reinterpret_cast<float4*>(gvp), o);
-            else __stcg(gvp, make_float2(o.x, o.y));
-            if (RTS_TOLM && TC.errp) {
-                seam_error(TC.GhO, TC.errp, TC.far_off + TC.ug, make_float2(o.x, o.y), make_float2(sc.x, sc.y), a_p, dirichlet);
-                if (!part) seam_error(TC.GhO, TC.errp, TC.far_off + TC.ug + 1, make_float2(o.z, o.w), make_float2(sc.z, sc.w), a_p, dirichlet);
-            }
-        }
-    }
     if (TC.XeP && ((fl & IT_USTRIP) || q >= TC.nrows - TC.K)) {  // exchange strips at a block end
         float4* xe = TC.XeP + (size_t)gv * TC.n_u2 + TC.ug;          // 16 bytes per node: (value, tag) per band
         st_tagged2(xe, make_float2(o.x, o.y), TC.tag);
@@ -775,8 +786,7 @@ __device__ __forceinline__ void do_strip(
         const float f = (S.U.ray[s].up ? 1.f : 0.f) - C.a_cur;
         for (; q < qb; ++q) {
             const float4 sc = lds128<HP>(bC);
-            if (RTS_TOLM) row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc), sc, C.a_cur, true);
-            else row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc));
+            row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc));
             bC += rstep; bW += rstep;
         }
         return;
@@ -786,8 +796,7 @@ __device__ __forceinline__ void do_strip(
         const float a0 = (vrow <= ks) ? 1.f : 0.f;
         const float f = ((s & 2) ? 0.f : 1.f) - a0;
         const float4 sc = lds128<HP>(bC);
-        if (RTS_TOLM) row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc), sc, a0, true);
-        else row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc));
+        row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, scale4(f, sc));
         bP += rstep; bC += rstep; bX += rstep; bW += rstep; vrow += vstep; ++q;
         if (q >= qb) return;
     }
@@ -816,8 +825,7 @@ __device__ __forceinline__ void do_strip(
             v1 = node_update<SU, 1, 2>(e1, l1, p1, SU_, SO, XU, XO, sp1, rk.w, a_u, a_o, a_p);                      \
         }                                                                                                           \
         const float4 o = cat4(v0, v1);                                                                              \
-        if (RTS_TOLM) row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o, sc, a_p, false);                          \
-        else row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);                                         \
+        row_store<SU>(TC, fl, tail_all || q >= qtail, q, bW, o);                                                    \
         bP += rstep; bC += rstep; bX += rstep; bW += rstep; vrow += vstep; ++q;                                     \
     }
 #pragma unroll 1
@@ -919,11 +927,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
             const bool core_q = (c0 >= HALO) && (c0 < HALO + G.wu);
             if (!core_q) ifl |= IT_DQ;
             if (chi - c0 < 2) ifl |= IT_PART;
-            const int fc = (gsu > 0) ? G.dhi_u - 1 : G.dlo_u;                  // far-u column of this ray (box)
-            if (core_q && fc >= c0 && fc < c0 + 2) ifl |= IT_FARC | ((fc != c0) ? IT_FSEC : 0u);
             if (core_q && ((gsu > 0) ? (c0 + 2 > HALO + G.wu - K) : (c0 - HALO < K))) ifl |= IT_USTRIP;
-            // the last row of the region is the far-v row of a periodic v axis
-            if (U.per_v && ((gsv > 0) ? (G.v0 + G.wv == U.n_v) : (G.v0 == 0))) ifl |= IT_FARV;
             // row q = 0 is the inflow row of a bounded v axis (x/y-march: v = z)
             if (!zmarch && ((gsv > 0) ? (G.v0 - hv == 0) : (G.v0 + G.wv + hv == U.n_v))) ifl |= IT_DIR;
         }
@@ -944,9 +948,8 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     TailCtx TC;
     TC.gv0 = s * U.n_v + v_q0;
     TC.ug = G.u0 - HALO + (int)((ioff0 % (uint32_t)RP) >> 3);
-    TC.n_u2 = U.n_u2; TC.far_off = NSLOT * U.n_v + s * U.n_u2;
+    TC.n_u2 = U.n_u2;
     TC.hv = hv_; TC.nrows = nrows_; TC.K = K; TC.gsv = gsv;
-    const size_t g_plane = (size_t)NSLOT * (U.n_v + U.n_u2);
     const size_t xe_par = (size_t)NSLOT * U.n_v * U.n_u2;
 
     // ================================================================== the march
@@ -983,6 +986,8 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 par_bits ^= 1u << stc;
                 // ---- heating / emergent intensity of the previous step's plane
                 if (qon && m > 0) q_pass<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, m - 1);
+                // ---- seam histories of the previous step's plane (the last plane of a pass: below, before the arrival)
+                if (hist_on && m > 0) hist_pass<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, m - 1, P);
                 // ---- seam ghosts for the next step (previous pass, this plane): fetch now, store after the update
                 const bool ghost_next = !blk_last && more && ngh > 0;
                 f2 gval[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
@@ -1003,18 +1008,14 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                         StepCtx C;
                         C.hj = hj;
                         C.dplane = zmarch && (m == 0);
-                        const bool hist = hist_on;
                         const bool strips = blk_last && more && !(zmarch && m == n_m - 1);
                         C.tail = 0;
-                        TC.GhP = hist ? reinterpret_cast<f2*>(U.Gu) + ((size_t)(P & 1) * n_m + m) * g_plane : nullptr;
-                        if (RTS_TOLM) TC.GhO = (tolmode && P > 0) ? reinterpret_cast<const f2*>(U.Gu) + ((size_t)((P - 1) & 1) * n_m + m) * g_plane : nullptr;
-                        if (RTS_TOLM) TC.errp = tolmode ? &S.errs[s][0] : nullptr;
                         TC.XeP = strips ? reinterpret_cast<float4*>(U.Xex) + (size_t)(gblk & 1) * xe_par : nullptr;
                         TC.tag = tag0 | ((unsigned)(gblk + 1) & 0xfffu);
-                        C.xmask = IT_PART | (hist ? IT_FARC : 0u) | (strips ? IT_USTRIP : 0u);
+                        C.xmask = IT_PART | (strips ? IT_USTRIP : 0u);
                         C.a_prev = (pl - dir <= kstar) ? 1.f : 0.f; C.a_cur = (pl <= kstar) ? 1.f : 0.f;
                         C.zreg = 0;
-                        const int qtail = min(strips ? nrows_ - K : (1 << 20), (hist && (ifl & IT_FARV)) ? nrows_ - 1 : (1 << 20));
+                        const int qtail = strips ? nrows_ - K : (1 << 20);
                         const uint32_t o = ioff0 + (uint32_t)(q0 * rstep);
                         const uint32_t bP = aStage0 + (uint32_t)stp * PSB + o, bC = aStage0 + (uint32_t)stc * PSB + o;
                         const uint32_t bX = aXb + (uint32_t)cur * XBB + xslot + o, bW = aXb + (uint32_t)(cur ^ 1) * XBB + xslot + o;
@@ -1045,6 +1046,10 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 }
                 // ---- end of step; at a block end publish (release) before anybody waits
                 __syncthreads();
+                if (hist_on && m == n_m - 1) {               // the pass ends: its last plane's histories precede the arrival
+                    hist_pass<PITCH>(&S, S.stage0 + (size_t)stc * PS, S.Xb + (size_t)(cur ^ 1) * NG * PS, m, P);
+                    __syncthreads();
+                }
                 if (tid == 0) {
                     // arrival (release): at every block end, or with the tagged exchange at the end of a pass only
                     if (blk_last && more && (!tagged || m == n_m - 1)) { __threadfence(); atomicAdd(U.barrier, 1); }
