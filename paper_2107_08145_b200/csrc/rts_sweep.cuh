@@ -179,6 +179,7 @@ struct TaskShared {
     uint64_t mbar[NSTAGE_MAX];
     int ticket, flag, nghost, nhalo;
     int pbase, tolmode;                // passes done before this launch; error-controlled mode (one pass per launch)
+    int has_hist, pad3;                // this tile holds the far-u column or far-v row of some ray (seam histories)
     unsigned errs[NSLOT][4];           // tolmode: per ray max |I(p) - I(p-1)| on the seam faces (band 0, 1), max |I(p)| (band 0, 1)
     int PS, tu, tv, pad0;              // nodes per plane set; tile coordinates
     f2* stage0;                        // [nstage] coefficient plane sets
@@ -872,6 +873,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         S.flag = 0; S.nghost = 0; S.nhalo = 0;
         S.pbase = pbase; S.tolmode = tolmode;
+        S.has_hist = (G.u0 == 0) || (G.u0 + G.wu == U.n_u) || (U.per_v && ((G.v0 == 0) || (G.v0 + G.wv == U.n_v)));
         for (int i = 0; i < NSLOT * 4; ++i) (&S.errs[0][0])[i] = 0u;
     }
     for (int i = tid; i < SP.nodes(); i += T) smf[i] = make_float2(0.f, 0.f);
@@ -881,6 +883,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
     const int n_m = U.n_m, npass = RTS_TOLM ? npass_launch : U.npass, K = U.K;
     const int nsteps = n_m * npass;
     const bool zmarch = (U.march == 2);
+    const bool has_hist = S.has_hist != 0;
     const bool tagged = U.xflag != 0;
     const unsigned tag0 = seq << 12;                         // tags of this solve (never 0: the buffers start zeroed)
 
@@ -987,7 +990,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 // ---- heating / emergent intensity of the previous step's plane
                 if (qon && m > 0) q_pass<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, m - 1);
                 // ---- seam histories of the previous step's plane (the last plane of a pass: below, before the arrival)
-                if (hist_on && m > 0) hist_pass<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, m - 1, P);
+                if (hist_on && m > 0 && has_hist) hist_pass<PITCH>(&S, S.stage0 + (size_t)stp * PS, S.Xb + (size_t)cur * NG * PS, m - 1, P);
                 // ---- seam ghosts for the next step (previous pass, this plane): fetch now, store after the update
                 const bool ghost_next = !blk_last && more && ngh > 0;
                 f2 gval[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
@@ -1046,7 +1049,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                 }
                 // ---- end of step; at a block end publish (release) before anybody waits
                 __syncthreads();
-                if (hist_on && m == n_m - 1) {               // the pass ends: its last plane's histories precede the arrival
+                if (hist_on && m == n_m - 1 && has_hist) {   // the pass ends: its last plane's histories precede the arrival
                     hist_pass<PITCH>(&S, S.stage0 + (size_t)stc * PS, S.Xb + (size_t)(cur ^ 1) * NG * PS, m, P);
                     __syncthreads();
                 }
