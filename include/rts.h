@@ -160,8 +160,8 @@ int rts_coefficients(rts_ctx* ctx, const float* rho_dev, const float* T_dev, con
                      float* kaprho_dev, float* S_dev, void* stream);
 
 /* [no paper passage: error reporting of the persistent kernel of DESIGN.md 7.2]
- * Synchronise `stream` and report the device-side status of the last solve
- * (RTS_OK, RTS_ETIMEOUT if the sweep watchdog fired, RTS_ECUDA). */
+ * Synchronise `stream` and report the device-side status of the solves since the last check
+ * (RTS_OK, RTS_ETIMEOUT if the sweep watchdog fired in any of them -- the status is sticky until read --, RTS_ECUDA). */
 int rts_sync_check(rts_ctx* ctx, void* stream);
 
 /* [SURVEY 7, lever 4.ii; only the seam intensities change between the iterations]

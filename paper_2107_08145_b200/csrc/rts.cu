@@ -375,7 +375,8 @@ int make_plan(rts_ctx* c)
     c->off_kstar = take(sizeof(int) * c->nbp);
     c->off_mthick = take(sizeof(int) * c->nbp * 3);
     c->off_mthick_b = take(sizeof(int) * c->nb * 3);
-    c->off_abort = take(sizeof(int) * 8);                    // [0] watchdog, [1] ticket counter
+    c->off_abort = take(sizeof(int) * 8);                    // [0] watchdog of the running launch, [1] ticket counter,
+                                                             // [2] first watchdog code since the last rts_sync_check (sticky)
     for (auto& g : groups)
         for (auto& sub : g.sub)
             for (int b = 0; b < c->nbp; ++b) {
@@ -791,7 +792,7 @@ int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, flo
     const int nlaunch = tolmode ? c->tol_max_passes : 1;
     c->passes_used = 0;
     for (int it = 0; it < nlaunch && c->total_tickets > 0; ++it) {
-        CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 8, st));
+        CUDA_TRY(c, cudaMemsetAsync(ws + c->off_abort, 0, sizeof(int) * 2, st));   // not the sticky word
         CUDA_TRY(c, cudaMemsetAsync(ws + c->off_bar, 0, sizeof(int) * c->units.size(), st));
         if (tolmode) CUDA_TRY(c, cudaMemsetAsync(ws + c->off_errw, 0, sizeof(unsigned) * c->units.size() * NSLOT * 4, st));
         const UnitDesc* dunits = (const UnitDesc*)(ws + c->off_units);
@@ -967,10 +968,13 @@ int rts_sync_check(rts_ctx* c, void* stream)
     cudaError_t e = cudaStreamSynchronize(as_stream(stream));
     if (e != cudaSuccess) return fail(c, RTS_ECUDA, std::string("stream sync: ") + cudaGetErrorString(e));
     if (c->ws) {
+        // the sticky word: a watchdog that fired in any solve queued since the last check is reported, not only the
+        // last solve's (every solve clears the word its own launches test)
         int ab = 0;
-        e = cudaMemcpy(&ab, c->ws + c->off_abort, sizeof(int), cudaMemcpyDeviceToHost);
+        e = cudaMemcpy(&ab, c->ws + c->off_abort + 2 * sizeof(int), sizeof(int), cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail(c, RTS_ECUDA, std::string("status read: ") + cudaGetErrorString(e));
         if (ab) {
+            cudaMemset(c->ws + c->off_abort + 2 * sizeof(int), 0, sizeof(int));
             char buf[256];
             snprintf(buf, sizeof buf, "sweep kernel watchdog fired (code %d, step %d): a wait did not complete", ab & 15, ab >> 4);
             return fail(c, RTS_ETIMEOUT, buf);

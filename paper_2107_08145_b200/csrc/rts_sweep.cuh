@@ -118,7 +118,7 @@ __device__ __forceinline__ bool spin_abort(int* abortf, unsigned& spins, int cod
 {
     if ((++spins & 255u) == 0u) {
         if (*reinterpret_cast<volatile int*>(abortf) != 0) return true;
-        if (spins > (1u << 22)) { atomicCAS(abortf, 0, code); return true; }
+        if (spins > (1u << 22)) { atomicCAS(abortf, 0, code); atomicCAS(abortf + 2, 0, code); return true; }   // [2]: sticky copy
     }
     return false;
 }
