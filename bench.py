@@ -170,8 +170,6 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--ctas-per-sm", type=int, default=0)
-    ap.add_argument("--tile", type=str, default="", help="tuning: 'TU,TV' for all march axes")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one atmosphere per rank; strong = one box sharded by band x octant")
     args = ap.parse_args()
@@ -196,11 +194,7 @@ def main():
     # strong: the same box on every rank, sweep units dealt round robin, one sum all-reduce of Q and I_top
     strong = (args.scaling == "strong" and world > 1)
     inp = inputs_mod.make_config(args.config, seed_offset=0 if strong else multi.rank_seed_offset(rank))
-    tiling = None
-    if args.tile:
-        tu, tv = (int(x) for x in args.tile.split(","))
-        tiling = {0: (tu, tv), 1: (tu, tv), 2: (tu, tv)}
-    solver = rts.from_inputs(inp, tiling=tiling, ctas_per_sm=args.ctas_per_sm, shard=(rank, world) if strong else None)
+    solver = rts.from_inputs(inp, shard=(rank, world) if strong else None)
     plan = solver.plan_info()
     solver.enable_timing(True)
     rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
