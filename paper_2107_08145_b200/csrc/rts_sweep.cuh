@@ -413,7 +413,9 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
     float* const Fdst = U.Fpart;
     float* const Itop_b = S.Itop_b;
     const long long Nn = (long long)U.n_m * U.n_u * U.n_v;
-    for (int e = tid; e < nqc * G.wv; e += T) {
+    // element tid, then 2T-1-tid, ...: the leftover elements of a second turn (576 node pairs on 512 threads at 48 x 24)
+    // go to the last warps, whose strips are the short ones (8 of 32 lanes, one row less), not to warps 0 and 1
+    for (int it = 0, e = tid; e < nqc * G.wv; ++it, e = (it + 1) * T - 1 - ((it & 1) ? tid : (T - 1 - tid))) {
         const int row = e / nqc, q = e - row * nqc;
         const int bo = (HALO + row) * RPN + HALO + 2 * q;
         const int v = G.v0 + row, u = G.u0 + 2 * q;
