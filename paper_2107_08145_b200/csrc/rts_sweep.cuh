@@ -413,6 +413,8 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
     float* const Fdst = U.Fpart;
     float* const Itop_b = S.Itop_b;
     const long long Nn = (long long)U.n_m * U.n_u * U.n_v;
+    // does this plane (z-march) or this tile (x/y-march: its top row) hold emergent intensities at all?
+    const bool topstep = Itop_b && (zmarch ? (m_done == U.n_m - 1 && G.up_z) : (G.v0 + G.wv == U.nz));
     // element tid, then 2T-1-tid, ...: the leftover elements of a second turn (576 node pairs on 512 threads at 48 x 24)
     // go to the last warps, whose strips are the short ones (8 of 32 lanes, one row less), not to warps 0 and 1
     for (int it = 0, e = tid; e < nqc * G.wv; ++it, e = (it + 1) * T - 1 - ((it & 1) ? tid : (T - 1 - tid))) {
@@ -446,8 +448,8 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
                     fl1[a] = fma2(bc(wm), i1, fl1[a]);
                 }
             }
-            if (Itop_b && U.ray[s].itop >= 0) {
-                const bool top = zmarch ? (m_done == U.n_m - 1 && G.up_z) : (v == U.nz - 1 && !(s & 2));
+            if (topstep && U.ray[s].itop >= 0) {
+                const bool top = zmarch || (v == U.nz - 1 && !(s & 2));
                 if (top) {
                     float* dst = Itop_b + (long long)U.ray[s].itop * U.it_sr + (zmarch ? (long long)v : (long long)pl) * U.it_so;
                     const float xa[4] = {x.x, x.y, x.z, x.w}, sa[4] = {sp.x, sp.y, sp.z, sp.w};
