@@ -179,7 +179,8 @@ struct TaskShared {
     uint64_t mbar[NSTAGE_MAX];
     int ticket, flag, nghost, nhalo;
     int pbase, tolmode;                // passes done before this launch; error-controlled mode (one pass per launch)
-    int has_hist, pad3;                // this tile holds the far-u column or far-v row of some ray (seam histories)
+    int has_hist, qrev;                // this tile holds the far-u column or far-v row of some ray (seam histories);
+                                       // the last warp of every ray has at most half its lanes busy (heating pass)
     unsigned errs[NSLOT][4];           // tolmode: per ray max |I(p) - I(p-1)| on the seam faces (band 0, 1), max |I(p)| (band 0, 1)
     int PS, tu, tv, pad0;              // nodes per plane set; tile coordinates
     f2* stage0;                        // [nstage] coefficient plane sets
@@ -415,9 +416,11 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
     const long long Nn = (long long)U.n_m * U.n_u * U.n_v;
     // does this plane (z-march) or this tile (x/y-march: its top row) hold emergent intensities at all?
     const bool topstep = Itop_b && (zmarch ? (m_done == U.n_m - 1 && G.up_z) : (G.v0 + G.wv == U.nz));
-    // element tid, then 2T-1-tid, ...: the leftover elements of a second turn (576 node pairs on 512 threads at 48 x 24)
-    // go to the last warps, whose strips are the short ones (8 of 32 lanes, one row less), not to warps 0 and 1
-    for (int it = 0, e = tid; e < nqc * G.wv; ++it, e = (it + 1) * T - 1 - ((it & 1) ? tid : (T - 1 - tid))) {
+    // element tid, then 2T-1-tid, ...: where the last warp of a ray is mostly idle in the strips (8 of 32 lanes at
+    // 48 x 24), the leftover elements of a second turn (576 node pairs on 512 threads) go to the last warps, not
+    // to warps 0 and 1
+    const bool qrev = S.qrev != 0;
+    for (int it = 0, e = tid; e < nqc * G.wv; ++it, e = qrev ? (it + 1) * T - 1 - ((it & 1) ? tid : (T - 1 - tid)) : e + T) {
         const int row = e / nqc, q = e - row * nqc;
         const int bo = (HALO + row) * RPN + HALO + 2 * q;
         const int v = G.v0 + row, u = G.u0 + 2 * q;
@@ -877,6 +880,7 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         S.flag = 0; S.nghost = 0; S.nhalo = 0;
         S.pbase = pbase; S.tolmode = tolmode;
+        { const int ns_ = ((U.WU + HALO) / 2) * ((U.WV + U.K - 1 + U.RC - 1) / U.RC); S.qrev = ((ns_ & 31) != 0) && ((ns_ & 31) <= 16); }
         S.has_hist = (G.u0 == 0) || (G.u0 + G.wu == U.n_u) || (U.per_v && ((G.v0 == 0) || (G.v0 + G.wv == U.n_v)));
         for (int i = 0; i < NSLOT * 4; ++i) (&S.errs[0][0])[i] = 0u;
     }
