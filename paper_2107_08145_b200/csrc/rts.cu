@@ -455,8 +455,9 @@ int bind_workspace(rts_ctx* c)
         d.errw = (unsigned*)(ws + c->off_errw) + i * NSLOT * 4;
         d.kstar = (const int*)(ws + c->off_kstar) + d.pair;
         d.mthick = (const int*)(ws + c->off_mthick) + 3 * d.pair;
-        // carried strips and seam histories must hold finite numbers from the start: planes that are
-        // skipped as optically thick leave their entries untouched, and readers multiply them by exactly 0
+        // exchange strips must not carry a stale tag and seam histories must be finite from the start (a skipped
+        // thick plane copies its history from a carried plane that every task starts from zeros, and the exchange
+        // strips of a skipped block are not read: nothing of an earlier solve reaches a later one)
         CUDA_TRY(c, cudaMemset(ws + hu.off_xex, 0, sizeof(float4) * 2 * NSLOT * (size_t)d.n_v * d.n_u2));
         CUDA_TRY(c, cudaMemset(ws + hu.off_g, 0, sizeof(float2) * 2 * (size_t)d.n_m * NSLOT * (size_t)(d.n_v + d.n_u2)));
         flat.push_back(d);

@@ -246,6 +246,33 @@ def test_repeated_solves_on_one_context_agree():
     s.close()
 
 
+def test_bad_input_does_not_reach_the_next_solve():
+    """A solve fed NaN must not poison the next, valid solve on the same context.  The only state a solve inherits
+    is the workspace; on planes skipped as optically thick the seam histories are still rewritten in every pass
+    (hist_pass copies the carried plane, which each task starts from zeros) and no exchange strip of a skipped block
+    is read, so nothing of an earlier solve is ever multiplied by the exact 0 of a thick plane."""
+    torch, rts = _gpu()
+    inp = inputs.make_config(4, grid=(44, 40, 60), nbands=6)
+    rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
+    s = rts.from_inputs(inp, tiling={0: (16, 12), 1: (16, 12), 2: (16, 12)})
+    Q1, I1 = s.solve(rho, T, P); s.sync_check()
+    assert max(s.thick_levels()) >= 4
+    Q1 = Q1.clone(); I1 = I1.clone()
+    # the bad solve: thin everywhere (no plane skipped, every seam history written) and NaN on the top plane, which
+    # the downward rays carry through the whole box
+    T_bad = T.clone(); T_bad[-1] = float("nan")
+    Qb, _ = s.solve(rho * 1e-8, T_bad, P)
+    assert not torch.isfinite(Qb).all()
+    try:
+        s.sync_check()
+    except Exception:
+        pass                                       # whatever the bad solve reports, the context stays usable
+    Q2, I2 = s.solve(rho, T, P); s.sync_check()
+    s.close()
+    assert torch.isfinite(Q2).all() and torch.isfinite(I2).all()
+    assert torch.equal(I1, I2) and torch.equal(Q1, Q2)
+
+
 def test_error_codes():
     torch, rts = _gpu()
     lib = rts.load_library()
