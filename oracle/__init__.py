@@ -67,6 +67,8 @@ def _load():
         _lib.oracle_solve_tol.restype = _I
         _lib.oracle_solve_tol.argtypes = ([_I, _I, _I, _D, _D, _D, _I, _I, _I, _D, _D, _D, _D, _PF, _PF,
                                            _D, _I, _I, _I, _I, _PD, _PD, _PF, _PF, _PF, _PD, _PD, _PD, _PI, _PD, _I])
+        _lib.oracle_scatter_solve.restype = _I
+        _lib.oracle_scatter_solve.argtypes = [_I, _I, _I, _D, _D, _D, _I, _PD, _PD, _PD, _PD, _PD, _I, _I, _PD, _PD, _PD, _PD]
         _lib.oracle_flux_heating.restype = _I
         _lib.oracle_flux_heating.argtypes = [_I, _I, _I, _D, _D, _D, _PD, _PD, _PD, _D, _PD, _PD]
         _lib.oracle_num_threads.restype = _I
@@ -185,6 +187,28 @@ def solve_tol(inp, tol: float, max_passes: int, mode: int = 1, faces: Optional[n
     if rc != 0:
         raise RuntimeError(f"oracle_solve_tol failed: {rc}")
     return Q, Itop, fc, used, rel[:int(used.max())].copy()
+
+
+def scatter_solve(nx, ny, nz, dx, dy, dz, mu, wq, kaprho, B, eps, niter: int, gs: bool = True, want_I: bool = False):
+    """O-13, one band: S = (1 - eps) J + eps B iterated niter times with the source update along the ray (gs) or
+    as a Jacobi / Lambda iteration.  Returns (S, J [nz][ny][nx], change [niter]) (+ I [nrays][nz][ny][nx])."""
+    lib = _load()
+    mu = np.ascontiguousarray(mu, dtype=np.float64)
+    wq = np.ascontiguousarray(wq, dtype=np.float64)
+    kaprho = np.ascontiguousarray(kaprho, dtype=np.float64)
+    B = np.ascontiguousarray(B, dtype=np.float64)
+    eps = np.ascontiguousarray(np.broadcast_to(eps, (nz, ny, nx)), dtype=np.float64)
+    assert kaprho.shape == (nz, ny, nx) and B.shape == (nz, ny, nx)
+    S = np.empty((nz, ny, nx), dtype=np.float64)
+    J = np.empty((nz, ny, nx), dtype=np.float64)
+    Iall = np.empty((len(wq), nz, ny, nx), dtype=np.float64) if want_I else None
+    change = np.zeros(max(niter, 1), dtype=np.float64)
+    rc = lib.oracle_scatter_solve(nx, ny, nz, dx, dy, dz, len(wq), _pd(mu), _pd(wq), _pd(kaprho), _pd(B), _pd(eps),
+                                  int(niter), 1 if gs else 0, _pd(S), _pd(J), _pd(Iall), _pd(change))
+    if rc != 0:
+        raise RuntimeError(f"oracle_scatter_solve failed: {rc}")
+    out = (S, J, change[:niter].copy())
+    return out + (Iall,) if want_I else out
 
 
 def solve(inp, nthreads: int = 0, want_J: bool = False, want_F: bool = False):

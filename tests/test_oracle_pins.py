@@ -747,3 +747,81 @@ def test_O12_solve_modes_against_the_fixed_pass_solve():
     Qw, Iw, fw, usedw, relw = oracle.solve_tol(inp, tol, 30, mode=1, faces=f1)
     assert (usedw == 1).all() and relw[0] <= tol
     assert np.abs(Qw - Q1).max() <= 10 * tol * np.abs(Q1).max()
+
+
+# --------------------------------------------------------------------------- O-13 (NEXT #4: scattering, source update along the ray)
+def _scatter_case(nx=4, ny=3, nz=6, seed=5):
+    rng = np.random.default_rng(seed)
+    mu, w = inputs.carlson24()
+    dx = dy = dz = 30 * KM
+    z = np.arange(nz)[:, None, None]
+    kap = 3e-7 * np.exp(-0.5 * z) * (1.0 + 0.3 * rng.random((nz, ny, nx)))       # ~0.9 per cell at the bottom
+    Bt = 2.0 * np.exp(-0.3 * z) * (1.0 + 0.2 * rng.random((nz, ny, nx)))
+    eps = 0.05 + 0.5 * rng.random((nz, ny, nx))
+    return nx, ny, nz, dx, dy, dz, mu, w, kap, Bt, eps
+
+
+def test_O13_with_eps_one_is_the_fixed_pass_formal_solution():
+    """eps = 1: S stays B, and n iterations are n Jacobi-seam passes of O-5 for every ray (the plane-by-plane
+    visiting order of O-13 against the k, j, i order of the pinned O-5) and J their weighted sum."""
+    nx, ny, nz, dx, dy, dz, mu, w, kap, Bt, _ = _scatter_case()
+    S, J, ch, I = oracle.scatter_solve(nx, ny, nz, dx, dy, dz, mu, w, kap, Bt, 1.0, 3, gs=True, want_I=True)
+    assert np.array_equal(S, Bt) and np.all(ch == 0.0)
+    Jref = np.zeros_like(J)
+    for r in range(24):
+        Ir = oracle.sweep_ray(nx, ny, nz, dx, dy, dz, mu[r], 3, kap, Bt)
+        assert np.abs(I[r] - Ir).max() <= 1e-13 * np.abs(Ir).max()
+        Jref += w[r] * Ir
+    assert np.abs(J - Jref).max() <= 1e-12 * np.abs(Jref).max()
+
+
+def test_O13_fixed_point_is_the_solution_of_the_linear_system():
+    """J is linear in S (the bottom inflow I = S included), so the converged source function solves
+    (1 - (1 - eps) L) S = eps B with L built column by column from the pinned periodic formal solution (O-5 with
+    enough passes for the seams to converge).  Both iterations must end there; the incremental J of the
+    Gauss-Seidel form must equal the weighted sum of its intensities."""
+    nx, ny, nz, dx, dy, dz, mu, w, kap, Bt, eps = _scatter_case()
+    N = nx * ny * nz
+    L = np.zeros((N, N))
+    for c in range(N):
+        e = np.zeros(N); e[c] = 1.0
+        e = e.reshape(nz, ny, nx)
+        col = np.zeros((nz, ny, nx))
+        for r in range(24):
+            col += w[r] * oracle.sweep_ray(nx, ny, nz, dx, dy, dz, mu[r], 60, kap, e)
+        L[:, c] = col.ravel()
+    Sstar = np.linalg.solve(np.eye(N) - (1.0 - eps.ravel())[:, None] * L, (eps * Bt).ravel()).reshape(nz, ny, nx)
+    Sg, Jg, chg, Ig = oracle.scatter_solve(nx, ny, nz, dx, dy, dz, mu, w, kap, Bt, eps, 300, gs=True, want_I=True)
+    Sj, Jj, chj = oracle.scatter_solve(nx, ny, nz, dx, dy, dz, mu, w, kap, Bt, eps, 300, gs=False)
+    assert np.abs(Sg - Sstar).max() <= 1e-10 * Sstar.max()
+    assert np.abs(Sj - Sstar).max() <= 1e-10 * Sstar.max()
+    assert np.abs(Jg - np.tensordot(w, Ig, axes=1)).max() <= 1e-12 * Jg.max()
+    assert np.abs(Sg - ((1.0 - eps) * Jg + eps * Bt)).max() <= 1e-13 * Sg.max()
+    # the reason for the scheme (PAPER.md:261): fewer iterations than the Jacobi form
+    e_g = [np.abs(oracle.scatter_solve(nx, ny, nz, dx, dy, dz, mu, w, kap, Bt, eps, n, gs=True)[0] - Sstar).max() for n in (5, 10)]
+    e_j = [np.abs(oracle.scatter_solve(nx, ny, nz, dx, dy, dz, mu, w, kap, Bt, eps, n, gs=False)[0] - Sstar).max() for n in (5, 10)]
+    assert e_g[0] < e_j[0] and e_g[1] < e_j[1]
+
+
+def test_O13_sqrt_eps_law_of_the_isothermal_semi_infinite_atmosphere():
+    """Isothermal, constant eps, semi-infinite: S(tau = 0) = sqrt(eps) B, exact in every discrete-ordinate
+    approximation (Chandrasekhar, Radiative Transfer, ch. XI).  Horizontally uniform column of vertical optical depth
+    100 whose cells thin out by 1e5 towards the top; what is left is the linear-source discretisation of tau, which
+    halves when the number of levels doubles."""
+    mu, w = inputs.carlson24()
+    nx = ny = 2
+    dz = 10 * KM
+    err = {}
+    for nz in (90, 180):
+        prof = np.exp(-(np.arange(nz) / (nz - 1.0)) * math.log(1e5))
+        kap = np.broadcast_to((prof / prof.sum() * 100.0 / dz)[:, None, None], (nz, ny, nx)).copy()
+        Bt = np.ones((nz, ny, nx))
+        for eps in (0.1, 0.3):
+            S, J, ch = oracle.scatter_solve(nx, ny, nz, dz, dz, dz, mu, w, kap, Bt, eps, 1000, gs=True)
+            assert ch[-1] < 1e-8
+            err[nz, eps] = S[nz - 1, 0, 0] / math.sqrt(eps) - 1.0
+            assert abs(err[nz, eps]) <= 0.01
+            assert S[0, 0, 0] == pytest.approx(1.0, rel=1e-6)             # thermalised at depth
+            assert np.all(np.diff(S[:, 0, 0]) <= 1e-12)                   # monotonic outward
+    for eps in (0.1, 0.3):
+        assert abs(err[180, eps]) < 0.6 * abs(err[90, eps])
