@@ -14,6 +14,7 @@
 #include "rts_sweep.cuh"
 #undef RTS_TOLM
 #undef RTS_MODE_NS
+#include "rts_scatter.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -61,6 +62,7 @@ struct rts_ctx {
     int tol_max_passes = 0;            // 0: off (fixed number of passes in one launch)
     double tol = 0.0;
     bool warm = false;                 // keep the seam state between solves
+    std::vector<ScatRay> scat_rays;    // ray constants of the last rts_scatter_solve (kept until its copy has run)
     int pass_counter = 0;              // passes the seam state has seen (0: cold)
     int passes_used = 0;
     float relerr_last = 0.f;
@@ -1083,6 +1085,91 @@ int rts_solve_cells(rts_ctx* c, const float* rho_c, const float* T_c, const floa
     return launch_n2c(c, qn, Qc, as_stream(stream));
 }
 
+// ---- scattering source function, source update along the ray (NEXT #4; rts_scatter.cuh)
+static size_t scatter_layout(const rts_ctx* c, int niter, size_t off[8])
+{
+    const size_t N = (size_t)c->nx * c->ny * c->nz, nr = c->rays.size();
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
+    off[0] = take(sizeof(double) * N * nr);                      // I_r
+    off[1] = take(sizeof(double) * (size_t)c->nz * c->ny);       // faceX
+    off[2] = take(sizeof(double) * (size_t)c->nz * c->nx);       // faceY
+    off[3] = take(sizeof(double) * N);                           // S of the previous iteration
+    off[4] = take(sizeof(ScatRay) * nr);
+    off[5] = take(sizeof(unsigned long long) * 2 * (size_t)std::max(niter, 1));
+    off[6] = take(sizeof(unsigned) * 4);
+    return o;
+}
+
+size_t rts_scatter_workspace_bytes(rts_ctx* c, int niter)
+{
+    if (!c || niter < 0 || niter > 65536) return 0;
+    size_t off[8];
+    return scatter_layout(c, niter, off);
+}
+
+int rts_scatter_solve(rts_ctx* c, const float* kaprho, const float* B, const float* eps, int niter, int gauss_seidel,
+                      void* workspace, size_t ws_bytes, double* S, double* J, double* change_host, void* stream)
+{
+    if (!c) return RTS_EINVAL;
+    if (!kaprho || !B || !eps || !S || !J || !workspace) return fail(c, RTS_EINVAL, "rts_scatter_solve: null pointer");
+    if (niter < 0 || niter > 65536) return fail(c, RTS_EINVAL, "rts_scatter_solve: 0 <= niter <= 65536");
+    size_t off[8];
+    const size_t need = scatter_layout(c, niter, off);
+    if (((uintptr_t)workspace & 255u) != 0 || ws_bytes < need) return fail(c, RTS_EINVAL, "rts_scatter_solve: workspace misaligned or too small");
+    cudaStream_t st = as_stream(stream);
+    unsigned char* ws = (unsigned char*)workspace;
+    // ray geometry (reading R3) in node offsets
+    c->scat_rays.clear();
+    for (HostRay r : c->rays) {
+        if (ray_geometry(c->h, r) != 0) return fail(c, RTS_EINVAL, "ray with mu_z == 0");
+        ScatRay q{};
+        const int as = r.march, ua = (as == 0) ? 1 : 0, va = (as == 2) ? 1 : 2;
+        q.as = as; q.dir = r.dir; q.up = r.up; q.kdir = r.up ? 0 : c->nz - 1;
+        int sg[3]; sg[as] = r.dir; sg[ua] = r.su; sg[va] = r.sv;
+        q.iface = (sg[0] > 0) ? c->nx - 1 : 0; q.jface = (sg[1] > 0) ? c->ny - 1 : 0;
+        for (int eu = 0; eu < 2; ++eu)
+            for (int ev = 0; ev < 2; ++ev) {
+                const int t = eu * 2 + ev;
+                q.off[t][0] = q.off[t][1] = q.off[t][2] = 0;
+                q.off[t][as] = -sg[as]; q.off[t][ua] = -eu * sg[ua]; q.off[t][va] = -ev * sg[va];
+                q.w[t] = (eu ? r.fu : 1.0 - r.fu) * (ev ? r.fv : 1.0 - r.fv);
+            }
+        q.ds = r.ds; q.wq = r.w;
+        c->scat_rays.push_back(q);
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(ws + off[4], c->scat_rays.data(), sizeof(ScatRay) * c->scat_rays.size(), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(c, cudaMemsetAsync(ws + off[5], 0, sizeof(unsigned long long) * 2 * (size_t)std::max(niter, 1), st));
+    CUDA_TRY(c, cudaMemsetAsync(ws + off[6], 0, sizeof(unsigned) * 4, st));
+    ScatParams p{};
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nrays = (int)c->rays.size(); p.niter = niter; p.gs = gauss_seidel != 0;
+    p.kaprho = kaprho; p.B = B; p.eps = eps;
+    p.rays = (const ScatRay*)(ws + off[4]);
+    p.I = (double*)(ws + off[0]); p.faceX = (double*)(ws + off[1]); p.faceY = (double*)(ws + off[2]); p.Sold = (double*)(ws + off[3]);
+    p.S = S; p.J = J;
+    p.chg = (unsigned long long*)(ws + off[5]); p.bar = (unsigned*)(ws + off[6]);
+    int occ = 0;
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_scatter_kernel, 256, 0));
+    if (occ < 1) return fail(c, RTS_ECUDA, "rts_scatter_solve: kernel does not fit on an SM");
+    const size_t plane_max = (size_t)std::max(c->nx, c->ny) * std::max(std::max(c->nx, c->ny), c->nz);
+    const int grid = (int)std::max<size_t>(1, std::min<size_t>((size_t)c->sm_count * std::min(occ, 4), (plane_max + 255) / 256));
+    void* args[] = {&p};
+    // cooperative launch: every CTA is resident, which the grid-wide barrier between planes relies on
+    CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_scatter_kernel, dim3(grid), dim3(256), args, 0, st));
+    std::vector<unsigned long long> chg(2 * (size_t)std::max(niter, 1));
+    unsigned flags[4] = {0, 0, 0, 0};
+    CUDA_TRY(c, cudaMemcpyAsync(chg.data(), ws + off[5], sizeof(unsigned long long) * chg.size(), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaMemcpyAsync(flags, ws + off[6], sizeof(flags), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    if (flags[1] != 0) return fail(c, RTS_ETIMEOUT, "rts_scatter_solve: the grid barrier timed out");
+    if (change_host)
+        for (int it = 0; it < niter; ++it) {
+            double e, sc;
+            std::memcpy(&e, &chg[2 * it], 8); std::memcpy(&sc, &chg[2 * it + 1], 8);
+            change_host[it] = (sc > 0.0) ? e / sc : 0.0;
+        }
+    return RTS_OK;
+}
 
 const char* rts_last_error(const rts_ctx* c)
 {

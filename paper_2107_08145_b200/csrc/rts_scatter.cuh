@@ -1,0 +1,176 @@
+// Scattering source function with the source update along the ray ("a
+// Gauss-Seidel convergence scheme ... updating the source function for each point along the ray, and then using
+// the 'new' source function to integrate the intensity at the next point along the ray.  This algorithm requires a
+// combined treatment of interpolation and integration"; reading R23).  One band per call:
+//     S = (1 - eps) J + eps B,   J = sum_r w_r I_r,
+// the rays visited in index order, the planes of a ray along its exit-face axis in upwind order, all nodes of a plane
+// at once (they read the previous plane only), one Jacobi-seam pass of the periodic faces per iteration.
+//
+// A first, plain kernel: fp64 throughout, one persistent cooperative grid, a grid-wide barrier after every plane
+// (the update of S couples every ray to the one before it, so the 24 rays cannot run side by side as they do in
+// rts_sweep_kernel).  It is launch- and barrier-bound at the sizes tested; DESIGN.md 7.5 has the numbers.
+#pragma once
+#include <cstdint>
+
+namespace rts {
+
+struct ScatRay {
+    int as, dir, kdir, up;             // exit-face axis, direction along it, Dirichlet level, mu_z > 0
+    int iface, jface;                  // periodic faces kept from the previous iteration
+    int off[4][3];                     // the 4 stencil nodes of the upwind face (i, j, k offsets)
+    double w[4];                       // their bilinear weights
+    double ds, wq;                     // path length to the upwind face; quadrature weight
+};
+
+struct ScatParams {
+    int nx, ny, nz, nrays, niter, gs;
+    const float* kaprho; const float* B; const float* eps;    // [N] each
+    const ScatRay* rays;
+    double* I;                         // [nrays][N]
+    double* faceX; double* faceY;      // [nz][ny], [nz][nx]
+    double* Sold;                      // [N]
+    double* S; double* J;              // [N] outputs
+    unsigned long long* chg;           // [niter][2]: bit patterns of max |S - Sold|, max |S|
+    unsigned* bar;                     // [0] arrivals (monotonic), [1] abort flag
+};
+
+// grid-wide barrier on a monotonic counter (the grid is launched cooperatively: every CTA is resident).
+// Returns false if the watchdog fired (a CTA waited ~4 s): everybody leaves.
+__device__ __forceinline__ bool scat_grid_sync(unsigned* bar, unsigned& gen)
+{
+    __syncthreads();
+    __shared__ int ok;
+    if (threadIdx.x == 0) {
+        ++gen;
+        __threadfence();
+        atomicAdd(bar, 1u);
+        const unsigned need = gen * gridDim.x;
+        unsigned spins = 0;
+        int good = 1;
+        while (true) {
+            unsigned v;
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+            if (v >= need) break;
+            if (*reinterpret_cast<volatile unsigned*>(bar + 1) != 0u) { good = 0; break; }
+            if (++spins > (1u << 24)) { atomicExch(bar + 1, 1u); good = 0; break; }
+            __nanosleep(200);
+        }
+        ok = good;
+    }
+    __syncthreads();
+    return ok != 0;
+}
+
+// E = e^-dtau, psi_u, psi_p of the linear-source integration (series below 1e-3 where the closed forms cancel)
+__device__ __forceinline__ void scat_psi(const double d, double& E, double& pu, double& pp)
+{
+    E = exp(-d);
+    if (d < 1e-3) {
+        pp = d * (0.5 - d * (1.0 / 6.0 - d * (1.0 / 24.0 - d * (1.0 / 120.0))));
+        pu = d * (0.5 - d * (1.0 / 3.0 - d * (1.0 / 8.0 - d * (1.0 / 30.0))));
+    } else {
+        const double w1 = (1.0 - E) / d;
+        pu = w1 - E; pp = 1.0 - w1;
+    }
+}
+
+__global__ void __launch_bounds__(256) rts_scatter_kernel(const ScatParams p)
+{
+    const int nx = p.nx, ny = p.ny, nz = p.nz;
+    const size_t N = (size_t)nx * ny * nz;
+    const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, gsz = (size_t)gridDim.x * blockDim.x;
+    unsigned gen = 0;
+    const int dim[3] = {nx, ny, nz};
+
+    // start: S = B, I_r = I(0) (S everywhere, 0 on the top plane of a downward ray), J = sum_r w_r I_r
+    for (size_t n = gtid; n < N; n += gsz) {
+        const double b = (double)p.B[n];
+        const int k = (int)(n / ((size_t)nx * ny));
+        double j = 0.0;
+        for (int r = 0; r < p.nrays; ++r) {
+            const ScatRay& q = p.rays[r];
+            const double i0 = (k == q.kdir && !q.up) ? 0.0 : b;
+            p.I[(size_t)r * N + n] = i0;
+            j += q.wq * i0;
+        }
+        p.S[n] = b; p.J[n] = j;
+    }
+    if (!scat_grid_sync(p.bar, gen)) return;
+
+    for (int it = 0; it < p.niter; ++it) {
+        for (size_t n = gtid; n < N; n += gsz) p.Sold[n] = p.S[n];
+        for (int r = 0; r < p.nrays; ++r) {
+            const ScatRay q = p.rays[r];
+            double* const X = p.I + (size_t)r * N;
+            // the periodic faces of the previous iteration (Jacobi seam ghosts)
+            for (size_t e = gtid; e < (size_t)nz * (ny + nx); e += gsz) {
+                const int k = (int)(e / (size_t)(ny + nx)), t = (int)(e - (size_t)k * (ny + nx));
+                if (t < ny) p.faceX[(size_t)k * ny + t] = X[((size_t)k * ny + t) * nx + q.iface];
+                else p.faceY[(size_t)k * nx + (t - ny)] = X[((size_t)k * ny + q.jface) * nx + (t - ny)];
+            }
+            if (!scat_grid_sync(p.bar, gen)) return;
+            const int as = q.as, ua = (as == 0) ? 1 : 0, va = (as == 2) ? 1 : 2;
+            const int n_u = dim[ua], n_v = dim[va], n_m = dim[as];
+            for (int mm = 0; mm < n_m; ++mm) {
+                const int pl = (q.dir > 0) ? mm : n_m - 1 - mm;
+                for (size_t e = gtid; e < (size_t)n_u * n_v; e += gsz) {
+                    int idx[3];
+                    idx[as] = pl; idx[va] = (int)(e / n_u); idx[ua] = (int)(e - (size_t)idx[va] * n_u);
+                    const int i = idx[0], j = idx[1], k = idx[2];
+                    const size_t n = ((size_t)k * ny + j) * nx + i;
+                    const double Sn = p.S[n];
+                    double Inew;
+                    if (k == q.kdir) Inew = q.up ? Sn : 0.0;
+                    else {
+                        double Xu = 0.0, ku = 0.0, Su = 0.0;
+#pragma unroll
+                        for (int t = 0; t < 4; ++t) {
+                            int iu = i + q.off[t][0], ju = j + q.off[t][1];
+                            const int kq = k + q.off[t][2];
+                            bool wx = false, wy = false;
+                            if (iu < 0) { iu += nx; wx = true; } else if (iu >= nx) { iu -= nx; wx = true; }
+                            if (ju < 0) { ju += ny; wy = true; } else if (ju >= ny) { ju -= ny; wy = true; }
+                            const size_t m = ((size_t)kq * ny + ju) * nx + iu;
+                            const double xv = wx ? p.faceX[(size_t)kq * ny + ju] : (wy ? p.faceY[(size_t)kq * nx + iu] : X[m]);
+                            Xu += q.w[t] * xv;
+                            ku += q.w[t] * (double)p.kaprho[m];
+                            Su += q.w[t] * p.S[m];
+                        }
+                        const double dtau = 0.5 * (ku + (double)p.kaprho[n]) * q.ds;
+                        double E, pu, pp;
+                        scat_psi(dtau, E, pu, pp);
+                        Inew = Xu * E + pu * Su + pp * Sn;
+                    }
+                    if (p.gs) {
+                        const double jn = p.J[n] + q.wq * (Inew - X[n]);
+                        const double ep = (double)p.eps[n];
+                        p.J[n] = jn;
+                        p.S[n] = (1.0 - ep) * jn + ep * (double)p.B[n];
+                    }
+                    X[n] = Inew;
+                }
+                if (!scat_grid_sync(p.bar, gen)) return;
+            }
+        }
+        if (!p.gs) {
+            for (size_t n = gtid; n < N; n += gsz) {
+                double a = 0.0;
+                for (int r = 0; r < p.nrays; ++r) a += p.rays[r].wq * p.I[(size_t)r * N + n];
+                const double ep = (double)p.eps[n];
+                p.J[n] = a;
+                p.S[n] = (1.0 - ep) * a + ep * (double)p.B[n];
+            }
+        }
+        // change of this iteration (positive doubles order like their bit patterns)
+        double e = 0.0, sc = 0.0;
+        for (size_t n = gtid; n < N; n += gsz) { const double s = p.S[n]; e = fmax(e, fabs(s - p.Sold[n])); sc = fmax(sc, fabs(s)); }
+        for (int o = 16; o > 0; o >>= 1) { e = fmax(e, __shfl_xor_sync(0xffffffffu, e, o)); sc = fmax(sc, __shfl_xor_sync(0xffffffffu, sc, o)); }
+        if ((threadIdx.x & 31) == 0) {
+            atomicMax(p.chg + 2 * it, (unsigned long long)__double_as_longlong(e));
+            atomicMax(p.chg + 2 * it + 1, (unsigned long long)__double_as_longlong(sc));
+        }
+        if (!scat_grid_sync(p.bar, gen)) return;
+    }
+}
+
+}  // namespace rts

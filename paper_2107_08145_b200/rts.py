@@ -28,6 +28,7 @@ EXPORTS = [
     "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells", "rts_set_thick_skip", "rts_thick_levels",
     "rts_enable_flux", "rts_set_flux_blend", "rts_solve_flux", "rts_set_shard", "rts_shard_info",
     "rts_set_tolerance", "rts_set_warm_start", "rts_passes_used",
+    "rts_scatter_workspace_bytes", "rts_scatter_solve",
 ]
 
 
@@ -100,6 +101,11 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_set_flux_blend.argtypes = [c_void_p, c_double]
     lib.rts_solve_flux.restype = c_int
     lib.rts_solve_flux.argtypes = [c_void_p] + [c_void_p] * 8 + [c_void_p]
+    lib.rts_scatter_workspace_bytes.restype = ctypes.c_size_t
+    lib.rts_scatter_workspace_bytes.argtypes = [c_void_p, c_int]
+    lib.rts_scatter_solve.restype = c_int
+    lib.rts_scatter_solve.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, ctypes.c_size_t,
+                                      c_void_p, c_void_p, ctypes.POINTER(ctypes.c_double), c_void_p]
     lib.rts_set_tolerance.restype = c_int
     lib.rts_set_tolerance.argtypes = [c_void_p, c_double, c_int]
     lib.rts_set_warm_start.restype = c_int
@@ -341,6 +347,25 @@ class RTS:
         tol * max|I| on them, at most max_passes passes (0: back to the fixed pass count).  Call before
         allocate_workspace."""
         self._check(self._lib.rts_set_tolerance(self._ctx, float(tol), int(max_passes)), "rts_set_tolerance")
+
+    def scatter_solve(self, kaprho, B, eps, niter: int, gauss_seidel: bool = True):
+        """NEXT #4, one band: S = (1 - eps) J + eps B with the source update along the ray (or as a Jacobi iteration).
+        kaprho, B, eps: CUDA float32 [nz][ny][nx].  Returns (S, J CUDA float64 [nz][ny][nx], change per iteration)."""
+        torch = self._torch
+        shp = (self.nz, self.ny, self.nx)
+        for t in (kaprho, B, eps):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == shp
+        nbytes = int(self._lib.rts_scatter_workspace_bytes(self._ctx, int(niter)))
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+        base = (ws.data_ptr() + 255) & ~255
+        S = torch.empty(shp, dtype=torch.float64, device="cuda")
+        J = torch.empty(shp, dtype=torch.float64, device="cuda")
+        change = (ctypes.c_double * max(int(niter), 1))()
+        self._check(self._lib.rts_scatter_solve(self._ctx, ctypes.c_void_p(kaprho.data_ptr()), ctypes.c_void_p(B.data_ptr()),
+                                                ctypes.c_void_p(eps.data_ptr()), int(niter), 1 if gauss_seidel else 0,
+                                                ctypes.c_void_p(base), nbytes, ctypes.c_void_p(S.data_ptr()),
+                                                ctypes.c_void_p(J.data_ptr()), change, self._stream()), "rts_scatter_solve")
+        return S, J, [float(change[i]) for i in range(int(niter))]
 
     def set_warm_start(self, on: bool = True):
         self._check(self._lib.rts_set_warm_start(self._ctx, 1 if on else 0), "rts_set_warm_start")

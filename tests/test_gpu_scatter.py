@@ -1,0 +1,75 @@
+"""NEXT #4 on the GPU: scattering source function with the source update along the ray against
+the fp64 oracle O-13, element by element, through the C-ABI.  Both sides get the same fp32 kaprho, B and eps (the
+CUDA path's stage-A output); the kernel computes in fp64, so the tolerance is that of a different summation order."""
+import numpy as np
+import pytest
+
+from paper_2107_08145_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def _case(cfg, grid, band, eps_lo):
+    import torch
+    from paper_2107_08145_b200 import rts
+    inp = inputs.make_config(cfg, grid=grid)
+    s = rts.from_inputs(inp)
+    rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
+    k, B = s.coefficients(rho, T, P)
+    s.sync_check()
+    rng = np.random.default_rng(17)
+    eps = (eps_lo + (1.0 - eps_lo) * rng.random(inp.shape)).astype(np.float32)
+    return inp, s, k[band].contiguous(), B[band].contiguous(), torch.from_numpy(eps).cuda()
+
+
+@pytest.mark.parametrize("cfg,grid,band,niter,gs", [
+    (1, (24, 20, 18), 0, 6, True),
+    (1, (24, 20, 18), 0, 6, False),
+    (3, (37, 41, 30), 2, 4, True),      # ragged widths, a thick band
+    (5, (30, 34, 61), 1, 3, True),
+    (2, (5, 3, 2), 0, 5, True),         # two levels: every node is a Dirichlet node for half of the rays
+])
+def test_scatter_against_oracle(cfg, grid, band, niter, gs):
+    import oracle
+    inp, s, k, B, eps = _case(cfg, grid, band, 0.05)
+    S, J, change = s.scatter_solve(k, B, eps, niter, gauss_seidel=gs)
+    s.sync_check()
+    So, Jo, cho = oracle.scatter_solve(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.mu, inp.wq,
+                                       k.cpu().numpy().astype(np.float64), B.cpu().numpy().astype(np.float64),
+                                       eps.cpu().numpy().astype(np.float64), niter, gs=gs)
+    s.close()
+    S = S.cpu().numpy(); J = J.cpu().numpy()
+    assert np.isfinite(S).all() and np.isfinite(J).all()
+    assert np.abs(S - So).max() <= TOL * np.abs(So).max()
+    assert np.abs(J - Jo).max() <= TOL * np.abs(Jo).max()
+    assert np.allclose(change, cho, rtol=1e-6, atol=1e-14)
+
+
+def test_eps_one_is_the_lte_source_and_zero_iterations_return_the_start():
+    import torch
+    inp, s, k, B, eps = _case(1, (16, 12, 10), 0, 0.05)
+    one = torch.ones_like(eps)
+    S, J, change = s.scatter_solve(k, B, one, 3)
+    assert torch.equal(S, B.double()) and change == [0.0, 0.0, 0.0]
+    S0, J0, ch0 = s.scatter_solve(k, B, eps, 0)
+    assert torch.equal(S0, B.double()) and ch0 == []
+    # J of the start: sum_r w_r I(0), I(0) = S except 0 on the top plane of the downward rays
+    wdown = float(sum(w for m, w in zip(inp.mu, inp.wq) if m[2] < 0))
+    Jref = B.double().clone(); Jref[-1] *= (1.0 - wdown)
+    assert torch.allclose(J0, Jref, rtol=1e-13, atol=0.0)
+    s.close()
+
+
+def test_gauss_seidel_needs_fewer_iterations_than_jacobi_on_the_gpu():
+    """The point of the scheme: after the same number of iterations the Gauss-Seidel form is closer
+    to the converged source function."""
+    inp, s, k, B, eps = _case(3, (20, 16, 24), 1, 0.02)
+    Sref, _, ch = s.scatter_solve(k, B, eps, 400)
+    assert ch[-1] < 1e-9
+    Sg, _, _ = s.scatter_solve(k, B, eps, 8, gauss_seidel=True)
+    Sj, _, _ = s.scatter_solve(k, B, eps, 8, gauss_seidel=False)
+    s.close()
+    eg = float((Sg - Sref).abs().max()); ej = float((Sj - Sref).abs().max())
+    assert eg < ej
