@@ -35,7 +35,8 @@ struct ScatParams {
 };
 
 // grid-wide barrier on a monotonic counter (the grid is launched cooperatively: every CTA is resident).
-// Returns false if the watchdog fired (a CTA waited ~4 s): everybody leaves.
+// Returns false if the watchdog fired: everybody leaves.  No back-off in the spin: at most a few hundred CTAs poll one
+// word, and a plane step is a few microseconds.
 __device__ __forceinline__ bool scat_grid_sync(unsigned* bar, unsigned& gen)
 {
     __syncthreads();
@@ -52,8 +53,7 @@ __device__ __forceinline__ bool scat_grid_sync(unsigned* bar, unsigned& gen)
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
             if (v >= need) break;
             if (*reinterpret_cast<volatile unsigned*>(bar + 1) != 0u) { good = 0; break; }
-            if (++spins > (1u << 24)) { atomicExch(bar + 1, 1u); good = 0; break; }
-            __nanosleep(200);
+            if (++spins > (1u << 28)) { atomicExch(bar + 1, 1u); good = 0; break; }      // ~10 s: the watchdog
         }
         ok = good;
     }
