@@ -62,6 +62,7 @@ struct rts_ctx {
     int tol_max_passes = 0;            // 0: off (fixed number of passes in one launch)
     double tol = 0.0;
     bool warm = false;                 // keep the seam state between solves
+    int nplain = 0;                    // partial-heating buffers in the x-fastest layout (summed first by the finalize kernel)
     std::vector<ScatRay> scat_rays;    // ray constants of the last rts_scatter_solve (kept until its copy has run)
     int pass_counter = 0;              // passes the seam state has seen (0: cold)
     int passes_used = 0;
@@ -93,7 +94,7 @@ struct rts_ctx {
     int PX = 0, PY = 0, PYR = 0;
     size_t ws_bytes = 0;
     // workspace offsets
-    size_t off_coefA = 0, off_coefB = 0, off_partptr = 0, off_parttr = 0, off_ksum = 0, off_kmin = 0, off_lev = 0, off_kstar = 0, off_mthick = 0, off_mthick_b = 0, off_abort = 0,
+    size_t off_coefA = 0, off_coefB = 0, off_partptr = 0, off_ksum = 0, off_kmin = 0, off_lev = 0, off_kstar = 0, off_mthick = 0, off_mthick_b = 0, off_abort = 0,
            off_units = 0, off_bar = 0, off_stage_in = 0, off_stage_out = 0;
     int nblk_a = 0;
     // workspace
@@ -431,7 +432,6 @@ int make_plan(rts_ctx* c)
     const size_t nu1 = std::max<size_t>(1, c->units.size());
     c->off_units = take(sizeof(UnitDesc) * nu1);
     c->off_partptr = take(sizeof(float*) * nu1);
-    c->off_parttr = take(sizeof(int) * nu1);
     c->off_bar = take(sizeof(int) * nu1);
     c->off_errw = take(sizeof(unsigned) * nu1 * NSLOT * 4);
     c->off_stage_in = take(sizeof(float) * N * 3);
@@ -466,10 +466,12 @@ int bind_workspace(rts_ctx* c)
     }
     CUDA_TRY(c, cudaMemcpy(ws + c->off_units, flat.data(), sizeof(UnitDesc) * flat.size(), cudaMemcpyHostToDevice));
     {
-        std::vector<float*> pp; std::vector<int> tr;
-        for (auto& d : flat) { pp.push_back(d.Qpart); tr.push_back(d.q_in_B); }
+        // the finalize kernel sums the x-fastest partials first (unit order), then the y-fastest ones (unit order)
+        std::vector<float*> pp;
+        for (auto& d : flat) if (!d.q_in_B) pp.push_back(d.Qpart);
+        c->nplain = (int)pp.size();
+        for (auto& d : flat) if (d.q_in_B) pp.push_back(d.Qpart);
         CUDA_TRY(c, cudaMemcpy(ws + c->off_partptr, pp.data(), sizeof(float*) * pp.size(), cudaMemcpyHostToDevice));
-        CUDA_TRY(c, cudaMemcpy(ws + c->off_parttr, tr.data(), sizeof(int) * tr.size(), cudaMemcpyHostToDevice));
     }
     // coefficient tensors for the TMA engine (fp32 elements, two per node): layout A as (x, y rows, z, field)
     // with the box of the z-march (x, y) or of the y-march (x, z); layout B as (y, x, z, field) with the
@@ -831,7 +833,7 @@ int solve_impl(rts_ctx* c, const float* rho, const float* T, const float* P, flo
     {
         // the units' partial heating (and flux) summed in unit order: deterministic
         FinalizeParams fp{};
-        fp.part = (const float* const*)(ws + c->off_partptr); fp.transposed = (const int*)(ws + c->off_parttr);
+        fp.part = (const float* const*)(ws + c->off_partptr); fp.nplain = c->nplain;
         fp.nunits = (int)c->units.size(); fp.nf = F ? 4 : 1;
         fp.nx = c->nx; fp.ny = c->ny; fp.nz = c->nz;
         fp.out[0] = Q;

@@ -356,8 +356,8 @@ __global__ void __launch_bounds__(1024) rts_kstar_kernel(const KstarParams p)
 // ([nz][nx][ny]) and are transposed through shared memory.  nf fields per unit (1: Q; 4: Q, Fx, Fy, Fz):
 // part[u] points at the unit's first field, the fields are N floats apart; out[f] may be null.
 struct FinalizeParams {
-    const float* const* part;   // device [nunits] partial buffers
-    const int* transposed;      // device [nunits] 1: y-fastest layout
+    const float* const* part;   // device [nunits] partial buffers: the x-fastest ones first, then the y-fastest ones
+    int nplain;                 // number of x-fastest buffers
     int nunits, nf;
     int nx, ny, nz;
     float* out[4];
@@ -368,33 +368,69 @@ __global__ void __launch_bounds__(256) rts_finalize_kernel(const FinalizeParams 
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32, k = blockIdx.z;
     const size_t N = (size_t)p.nx * p.ny * p.nz;
+    const int ii = i0 + tx;
     for (int f = 0; f < p.nf; ++f) {
         if (!p.out[f]) continue;
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
-        for (int u = 0; u < p.nunits; ++u) {
-            const float* src = p.part[u] + (size_t)f * N;
-            if (p.transposed[u]) {
-                __syncthreads();
+        // x-fastest partials, four buffers' loads in flight together (the sum stays in buffer order)
+        int u = 0;
+        for (; u + 4 <= p.nplain; u += 4) {
+            float v[4][4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float* src = p.part[u + q] + (size_t)f * N;
 #pragma unroll
                 for (int r = 0; r < 4; ++r) {
-                    const int i = i0 + ty + 8 * r, j = j0 + tx;
-                    if (i < p.nx && j < p.ny) tile[ty + 8 * r][tx] = __ldcs(src + ((size_t)k * p.nx + i) * p.ny + j);
+                    const int j = j0 + ty + 8 * r;
+                    v[q][r] = (ii < p.nx && j < p.ny) ? __ldcs(src + ((size_t)k * p.ny + j) * p.nx + ii) : 0.f;
                 }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int r = 0; r < 4; ++r) acc[r] += v[q][r];
+        }
+        for (; u < p.nplain; ++u) {
+            const float* src = p.part[u] + (size_t)f * N;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int j = j0 + ty + 8 * r;
+                if (ii < p.nx && j < p.ny) acc[r] += __ldcs(src + ((size_t)k * p.ny + j) * p.nx + ii);
+            }
+        }
+        // y-fastest partials (x-march units), transposed through shared memory; two buffers' loads in flight
+        for (; u < p.nunits; u += 2) {
+            const bool two = (u + 1 < p.nunits);
+            const float* s0 = p.part[u] + (size_t)f * N;
+            const float* s1 = two ? p.part[u + 1] + (size_t)f * N : s0;
+            float a[4], b[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int i = i0 + ty + 8 * r, j = j0 + tx;
+                const bool in = (i < p.nx && j < p.ny);
+                const size_t o = ((size_t)k * p.nx + i) * p.ny + j;
+                a[r] = in ? __ldcs(s0 + o) : 0.f;
+                b[r] = (in && two) ? __ldcs(s1 + o) : 0.f;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 4; ++r) tile[ty + 8 * r][tx] = a[r];
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 4; ++r) acc[r] += tile[tx][ty + 8 * r];
+            if (two) {
+                __syncthreads();
+#pragma unroll
+                for (int r = 0; r < 4; ++r) tile[ty + 8 * r][tx] = b[r];
                 __syncthreads();
 #pragma unroll
                 for (int r = 0; r < 4; ++r) acc[r] += tile[tx][ty + 8 * r];
-            } else {
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const int j = j0 + ty + 8 * r, i = i0 + tx;
-                    if (i < p.nx && j < p.ny) acc[r] += __ldcs(src + ((size_t)k * p.ny + j) * p.nx + i);
-                }
             }
         }
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
-            const int j = j0 + ty + 8 * r, i = i0 + tx;
-            if (i < p.nx && j < p.ny) p.out[f][((size_t)k * p.ny + j) * p.nx + i] = acc[r];
+            const int j = j0 + ty + 8 * r;
+            if (ii < p.nx && j < p.ny) p.out[f][((size_t)k * p.ny + j) * p.nx + ii] = acc[r];
         }
     }
 }
