@@ -335,26 +335,24 @@ def main():
                 "note": "one field per launch; source + destination exceed the L2 at the 288^3 and 512x512x192 sizes"}
         del cell, node
 
-    # ---- scattering source function: band 0 of the same atmosphere, eps = 0.1, two iterations
-    #      of the source update along the ray (fp64 kernel, one grid barrier per plane: DESIGN.md 7.5)
+    # ---- scattering source function: all bands of the same atmosphere, eps = 0.1, two
+    #      iterations of the source update along the ray (fp64 kernel, one grid barrier per plane: DESIGN.md 7.5)
     scat = None
     if world == 1:
         kap, Bsrc = solver.coefficients(rho, T, P)
-        k0, B0 = kap[0].contiguous(), Bsrc[0].contiguous()
-        del kap, Bsrc
-        eps = torch.full_like(k0, 0.1)
-        solver.scatter_solve(k0, B0, eps, 1)
+        eps = torch.full_like(kap, 0.1)
+        solver.scatter_solve(kap, Bsrc, eps, 1)
         n_it = 2
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize(); a.record()
-        _, _, change = solver.scatter_solve(k0, B0, eps, n_it)
+        _, _, change = solver.scatter_solve(kap, Bsrc, eps, n_it)
         b.record(); torch.cuda.synchronize()
         t_it = a.elapsed_time(b) / n_it
-        scat = {"ms_per_iteration": t_it, "node_ray_updates_per_s": inp.ncells * inp.nrays / (t_it * 1e-3), "dtype": "f64",
-                "bands": 1, "rays": inp.nrays, "eps": 0.1, "scheme": "source update along the ray (Gauss-Seidel)",
-                "last_change": change[-1],
-                "note": "barrier- and latency-bound: one grid-wide barrier per plane of every ray"}
-        del k0, B0, eps
+        scat = {"ms_per_iteration": t_it, "node_band_ray_updates_per_s": inp.ncells * inp.nbands * inp.nrays / (t_it * 1e-3),
+                "dtype": "f64", "bands": inp.nbands, "rays": inp.nrays, "eps": 0.1,
+                "scheme": "source update along the ray (Gauss-Seidel)", "last_change_per_band": change[-1],
+                "note": "one grid-wide barrier per plane of every ray; small grids are bound by it, 288^3 by the L2 sector traffic of the strided x-march planes"}
+        del kap, Bsrc, eps
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:

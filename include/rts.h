@@ -206,22 +206,25 @@ int rts_shard_info(rts_ctx* ctx, int* units_mine, int* units_all);
 /* Scattering source function with the source update along the ray ("it is
  * preferable to use a Gauss-Seidel convergence scheme.  As the intensity is integrated along the ray, this scheme
  * will require updating the source function for each point along the ray, and then using the 'new' source function
- * to integrate the intensity at the next point along the ray"; reading R23).  ONE band per call:
+ * to integrate the intensity at the next point along the ray"; reading R23).  For each of `nbands`
+ * independent bands:
  *     S = (1 - eps) J + eps B,   J = sum_r w_r I_r,
- * kaprho, B (the thermal source), eps (photon destruction probability, 0 < eps <= 1): DEVICE float [nz][ny][nx],
- * e.g. one band of rts_coefficients.  Start S = B; every iteration visits the context's rays in index order, the
- * planes of a ray along its exit-face axis in upwind order, and at every node forms the short-characteristic
- * intensity from the CURRENT S, then (gauss_seidel != 0) J += w_r (I_new - I_old), S = (1 - eps) J + eps B at once,
- * or (gauss_seidel == 0, the Jacobi / Lambda iteration) S from all rays after the last one.  The periodic seams
- * take one Jacobi pass per iteration.  niter iterations, 0 <= niter <= 65536.
- * Outputs: S, J DEVICE double [nz][ny][nx] (this kernel computes in fp64); change_host (HOST [niter], may be NULL):
- * max|S - S_previous| / max|S| of every iteration.  workspace: DEVICE, 256-byte aligned, at least
- * rts_scatter_workspace_bytes(ctx, niter) bytes (24 doubles per node for 24 rays), borrowed for the call.
- * Synchronous on `stream` (the host reads the change words).  RTS_ETIMEOUT if the grid barrier's watchdog fired. */
-size_t rts_scatter_workspace_bytes(rts_ctx* ctx, int niter);
-int rts_scatter_solve(rts_ctx* ctx, const float* kaprho_dev, const float* B_dev, const float* eps_dev, int niter,
-                      int gauss_seidel, void* workspace_dev, size_t workspace_bytes, double* S_dev, double* J_dev,
-                      double* change_host, void* stream);
+ * kaprho, B (the thermal source), eps (photon destruction probability, 0 < eps <= 1): DEVICE float
+ * [nbands][nz][ny][nx], e.g. the output of rts_coefficients (nbands need not be the context's band count).
+ * Start S = B; every iteration visits the context's rays in index order, the planes of a ray along its exit-face
+ * axis in upwind order, and at every node forms the short-characteristic intensity from the CURRENT S, then
+ * (gauss_seidel != 0) J += w_r (I_new - I_old), S = (1 - eps) J + eps B at once, or (gauss_seidel == 0, the
+ * Jacobi / Lambda iteration) S from all rays after the last one.  The periodic seams take one Jacobi pass per
+ * iteration.  The bands share every plane step (and its grid barrier).  niter iterations, 0 <= niter <= 65536.
+ * Outputs: S, J DEVICE double [nbands][nz][ny][nx] (this kernel computes in fp64); change_host (HOST
+ * [niter][nbands], may be NULL): max|S - S_previous| / max|S| of every iteration and band.  workspace: DEVICE,
+ * 256-byte aligned, at least rts_scatter_workspace_bytes(ctx, nbands, niter) bytes (one double per ray, node and
+ * band: 4.6 GB per band at 288^3 with 24 rays), borrowed for the call.  Synchronous on `stream` (the host reads
+ * the change words).  RTS_ETIMEOUT if the grid barrier's watchdog fired; RTS_EINVAL for bad arguments. */
+size_t rts_scatter_workspace_bytes(rts_ctx* ctx, int nbands, int niter);
+int rts_scatter_solve(rts_ctx* ctx, int nbands, const float* kaprho_dev, const float* B_dev, const float* eps_dev,
+                      int niter, int gauss_seidel, void* workspace_dev, size_t workspace_bytes, double* S_dev,
+                      double* J_dev, double* change_host, void* stream);
 
 /* [measurement only]
  * Per-stage device timing of the last rts_solve (CUDA events recorded on the solve stream

@@ -1088,36 +1088,36 @@ int rts_solve_cells(rts_ctx* c, const float* rho_c, const float* T_c, const floa
 }
 
 // ---- scattering source function, source update along the ray (NEXT #4; rts_scatter.cuh)
-static size_t scatter_layout(const rts_ctx* c, int niter, size_t off[8])
+static size_t scatter_layout(const rts_ctx* c, int nbands, int niter, size_t off[8])
 {
-    const size_t N = (size_t)c->nx * c->ny * c->nz, nr = c->rays.size();
+    const size_t N = (size_t)c->nx * c->ny * c->nz, nr = c->rays.size(), nb = (size_t)nbands;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
-    off[0] = take(sizeof(double) * N * nr);                      // I_r
-    off[1] = take(sizeof(double) * (size_t)c->nz * c->ny);       // faceX
-    off[2] = take(sizeof(double) * (size_t)c->nz * c->nx);       // faceY
-    off[3] = take(sizeof(double) * N);                           // S of the previous iteration
+    off[0] = take(sizeof(double) * N * nr * nb);                 // I_r of every band
+    off[1] = take(sizeof(double) * (size_t)c->nz * c->ny * nb);  // faceX
+    off[2] = take(sizeof(double) * (size_t)c->nz * c->nx * nb);  // faceY
+    off[3] = take(sizeof(double) * N * nb);                      // S of the previous iteration
     off[4] = take(sizeof(ScatRay) * nr);
-    off[5] = take(sizeof(unsigned long long) * 2 * (size_t)std::max(niter, 1));
+    off[5] = take(sizeof(unsigned long long) * 2 * nb * (size_t)std::max(niter, 1));
     off[6] = take(sizeof(unsigned) * 4);
     return o;
 }
 
-size_t rts_scatter_workspace_bytes(rts_ctx* c, int niter)
+size_t rts_scatter_workspace_bytes(rts_ctx* c, int nbands, int niter)
 {
-    if (!c || niter < 0 || niter > 65536) return 0;
+    if (!c || nbands < 1 || nbands > 1024 || niter < 0 || niter > 65536) return 0;
     size_t off[8];
-    return scatter_layout(c, niter, off);
+    return scatter_layout(c, nbands, niter, off);
 }
 
-int rts_scatter_solve(rts_ctx* c, const float* kaprho, const float* B, const float* eps, int niter, int gauss_seidel,
+int rts_scatter_solve(rts_ctx* c, int nbands, const float* kaprho, const float* B, const float* eps, int niter, int gauss_seidel,
                       void* workspace, size_t ws_bytes, double* S, double* J, double* change_host, void* stream)
 {
     if (!c) return RTS_EINVAL;
     if (!kaprho || !B || !eps || !S || !J || !workspace) return fail(c, RTS_EINVAL, "rts_scatter_solve: null pointer");
-    if (niter < 0 || niter > 65536) return fail(c, RTS_EINVAL, "rts_scatter_solve: 0 <= niter <= 65536");
+    if (niter < 0 || niter > 65536 || nbands < 1 || nbands > 1024) return fail(c, RTS_EINVAL, "rts_scatter_solve: 0 <= niter <= 65536, 1 <= nbands <= 1024");
     size_t off[8];
-    const size_t need = scatter_layout(c, niter, off);
+    const size_t need = scatter_layout(c, nbands, niter, off);
     if (((uintptr_t)workspace & 255u) != 0 || ws_bytes < need) return fail(c, RTS_EINVAL, "rts_scatter_solve: workspace misaligned or too small");
     cudaStream_t st = as_stream(stream);
     unsigned char* ws = (unsigned char*)workspace;
@@ -1141,10 +1141,10 @@ int rts_scatter_solve(rts_ctx* c, const float* kaprho, const float* B, const flo
         c->scat_rays.push_back(q);
     }
     CUDA_TRY(c, cudaMemcpyAsync(ws + off[4], c->scat_rays.data(), sizeof(ScatRay) * c->scat_rays.size(), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(c, cudaMemsetAsync(ws + off[5], 0, sizeof(unsigned long long) * 2 * (size_t)std::max(niter, 1), st));
+    CUDA_TRY(c, cudaMemsetAsync(ws + off[5], 0, sizeof(unsigned long long) * 2 * (size_t)nbands * (size_t)std::max(niter, 1), st));
     CUDA_TRY(c, cudaMemsetAsync(ws + off[6], 0, sizeof(unsigned) * 4, st));
     ScatParams p{};
-    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nrays = (int)c->rays.size(); p.niter = niter; p.gs = gauss_seidel != 0;
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nrays = (int)c->rays.size(); p.niter = niter; p.gs = gauss_seidel != 0; p.nb = nbands;
     p.kaprho = kaprho; p.B = B; p.eps = eps;
     p.rays = (const ScatRay*)(ws + off[4]);
     p.I = (double*)(ws + off[0]); p.faceX = (double*)(ws + off[1]); p.faceY = (double*)(ws + off[2]); p.Sold = (double*)(ws + off[3]);
@@ -1154,21 +1154,21 @@ int rts_scatter_solve(rts_ctx* c, const float* kaprho, const float* B, const flo
     CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_scatter_kernel, 256, 0));
     if (occ < 1) return fail(c, RTS_ECUDA, "rts_scatter_solve: kernel does not fit on an SM");
     const size_t plane_max = (size_t)std::max(c->nx, c->ny) * std::max(std::max(c->nx, c->ny), c->nz);
-    const int grid = (int)std::max<size_t>(1, std::min<size_t>((size_t)c->sm_count * std::min(occ, 4), (plane_max + 255) / 256));
+    const int grid = (int)std::max<size_t>(1, std::min<size_t>((size_t)c->sm_count * std::min(occ, 4), (plane_max * nbands + 255) / 256));
     void* args[] = {&p};
     // cooperative launch: every CTA is resident, which the grid-wide barrier between planes relies on
     CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_scatter_kernel, dim3(grid), dim3(256), args, 0, st));
-    std::vector<unsigned long long> chg(2 * (size_t)std::max(niter, 1));
+    std::vector<unsigned long long> chg(2 * (size_t)nbands * (size_t)std::max(niter, 1));
     unsigned flags[4] = {0, 0, 0, 0};
     CUDA_TRY(c, cudaMemcpyAsync(chg.data(), ws + off[5], sizeof(unsigned long long) * chg.size(), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaMemcpyAsync(flags, ws + off[6], sizeof(flags), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaStreamSynchronize(st));
     if (flags[1] != 0) return fail(c, RTS_ETIMEOUT, "rts_scatter_solve: the grid barrier timed out");
     if (change_host)
-        for (int it = 0; it < niter; ++it) {
+        for (size_t q = 0; q < (size_t)niter * nbands; ++q) {                 // [niter][nbands]
             double e, sc;
-            std::memcpy(&e, &chg[2 * it], 8); std::memcpy(&sc, &chg[2 * it + 1], 8);
-            change_host[it] = (sc > 0.0) ? e / sc : 0.0;
+            std::memcpy(&e, &chg[2 * q], 8); std::memcpy(&sc, &chg[2 * q + 1], 8);
+            change_host[q] = (sc > 0.0) ? e / sc : 0.0;
         }
     return RTS_OK;
 }

@@ -1,7 +1,8 @@
 // Scattering source function with the source update along the ray ("a
 // Gauss-Seidel convergence scheme ... updating the source function for each point along the ray, and then using
 // the 'new' source function to integrate the intensity at the next point along the ray.  This algorithm requires a
-// combined treatment of interpolation and integration"; reading R23).  One band per call:
+// combined treatment of interpolation and integration"; reading R23).  Per band (the bands of a call are
+// independent problems that share every plane step and its barrier):
 //     S = (1 - eps) J + eps B,   J = sum_r w_r I_r,
 // the rays visited in index order, the planes of a ray along its exit-face axis in upwind order, all nodes of a plane
 // at once (they read the previous plane only), one Jacobi-seam pass of the periodic faces per iteration.
@@ -23,14 +24,14 @@ struct ScatRay {
 };
 
 struct ScatParams {
-    int nx, ny, nz, nrays, niter, gs;
-    const float* kaprho; const float* B; const float* eps;    // [N] each
+    int nx, ny, nz, nrays, niter, gs, nb;
+    const float* kaprho; const float* B; const float* eps;    // [nb][N] each
     const ScatRay* rays;
-    double* I;                         // [nrays][N]
-    double* faceX; double* faceY;      // [nz][ny], [nz][nx]
-    double* Sold;                      // [N]
-    double* S; double* J;              // [N] outputs
-    unsigned long long* chg;           // [niter][2]: bit patterns of max |S - Sold|, max |S|
+    double* I;                         // [nb][nrays][N]
+    double* faceX; double* faceY;      // [nb][nz][ny], [nb][nz][nx]
+    double* Sold;                      // [nb][N]
+    double* S; double* J;              // [nb][N] outputs
+    unsigned long long* chg;           // [niter][nb][2]: bit patterns of max |S - Sold|, max |S|
     unsigned* bar;                     // [0] arrivals (monotonic), [1] abort flag
 };
 
@@ -76,49 +77,60 @@ __device__ __forceinline__ void scat_psi(const double d, double& E, double& pu, 
 
 __global__ void __launch_bounds__(256) rts_scatter_kernel(const ScatParams p)
 {
-    const int nx = p.nx, ny = p.ny, nz = p.nz;
-    const size_t N = (size_t)nx * ny * nz;
+    const int nx = p.nx, ny = p.ny, nz = p.nz, nb = p.nb;
+    const size_t N = (size_t)nx * ny * nz, NB = N * nb;
     const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, gsz = (size_t)gridDim.x * blockDim.x;
     unsigned gen = 0;
     const int dim[3] = {nx, ny, nz};
+    const size_t fxs = (size_t)nz * ny, fys = (size_t)nz * nx;      // one band's faces
 
     // start: S = B, I_r = I(0) (S everywhere, 0 on the top plane of a downward ray), J = sum_r w_r I_r
-    for (size_t n = gtid; n < N; n += gsz) {
-        const double b = (double)p.B[n];
+    for (size_t e = gtid; e < NB; e += gsz) {
+        const size_t b = e / N, n = e - b * N;
+        const double bv = (double)p.B[e];
         const int k = (int)(n / ((size_t)nx * ny));
         double j = 0.0;
         for (int r = 0; r < p.nrays; ++r) {
             const ScatRay& q = p.rays[r];
-            const double i0 = (k == q.kdir && !q.up) ? 0.0 : b;
-            p.I[(size_t)r * N + n] = i0;
+            const double i0 = (k == q.kdir && !q.up) ? 0.0 : bv;
+            p.I[(b * p.nrays + r) * N + n] = i0;
             j += q.wq * i0;
         }
-        p.S[n] = b; p.J[n] = j;
+        p.S[e] = bv; p.J[e] = j;
     }
     if (!scat_grid_sync(p.bar, gen)) return;
 
     for (int it = 0; it < p.niter; ++it) {
-        for (size_t n = gtid; n < N; n += gsz) p.Sold[n] = p.S[n];
+        for (size_t e = gtid; e < NB; e += gsz) p.Sold[e] = p.S[e];
         for (int r = 0; r < p.nrays; ++r) {
             const ScatRay q = p.rays[r];
-            double* const X = p.I + (size_t)r * N;
             // the periodic faces of the previous iteration (Jacobi seam ghosts)
-            for (size_t e = gtid; e < (size_t)nz * (ny + nx); e += gsz) {
-                const int k = (int)(e / (size_t)(ny + nx)), t = (int)(e - (size_t)k * (ny + nx));
-                if (t < ny) p.faceX[(size_t)k * ny + t] = X[((size_t)k * ny + t) * nx + q.iface];
-                else p.faceY[(size_t)k * nx + (t - ny)] = X[((size_t)k * ny + q.jface) * nx + (t - ny)];
+            const size_t nface = (size_t)nz * (ny + nx);
+            for (size_t e = gtid; e < nface * nb; e += gsz) {
+                const size_t b = e / nface, f = e - b * nface;
+                const double* X = p.I + (b * p.nrays + r) * N;
+                const int k = (int)(f / (size_t)(ny + nx)), t = (int)(f - (size_t)k * (ny + nx));
+                if (t < ny) p.faceX[b * fxs + (size_t)k * ny + t] = X[((size_t)k * ny + t) * nx + q.iface];
+                else p.faceY[b * fys + (size_t)k * nx + (t - ny)] = X[((size_t)k * ny + q.jface) * nx + (t - ny)];
             }
             if (!scat_grid_sync(p.bar, gen)) return;
             const int as = q.as, ua = (as == 0) ? 1 : 0, va = (as == 2) ? 1 : 2;
             const int n_u = dim[ua], n_v = dim[va], n_m = dim[as];
+            const size_t npl = (size_t)n_u * n_v;
             for (int mm = 0; mm < n_m; ++mm) {
                 const int pl = (q.dir > 0) ? mm : n_m - 1 - mm;
-                for (size_t e = gtid; e < (size_t)n_u * n_v; e += gsz) {
+                for (size_t e = gtid; e < npl * nb; e += gsz) {
+                    const size_t b = e / npl, ep = e - b * npl;
+                    double* const X = p.I + (b * p.nrays + r) * N;
+                    const double* const Sb = p.S + b * N;
+                    const float* const kb = p.kaprho + b * N;
+                    const double* const fX = p.faceX + b * fxs;
+                    const double* const fY = p.faceY + b * fys;
                     int idx[3];
-                    idx[as] = pl; idx[va] = (int)(e / n_u); idx[ua] = (int)(e - (size_t)idx[va] * n_u);
+                    idx[as] = pl; idx[va] = (int)(ep / n_u); idx[ua] = (int)(ep - (size_t)idx[va] * n_u);
                     const int i = idx[0], j = idx[1], k = idx[2];
                     const size_t n = ((size_t)k * ny + j) * nx + i;
-                    const double Sn = p.S[n];
+                    const double Sn = Sb[n];
                     double Inew;
                     if (k == q.kdir) Inew = q.up ? Sn : 0.0;
                     else {
@@ -131,21 +143,22 @@ __global__ void __launch_bounds__(256) rts_scatter_kernel(const ScatParams p)
                             if (iu < 0) { iu += nx; wx = true; } else if (iu >= nx) { iu -= nx; wx = true; }
                             if (ju < 0) { ju += ny; wy = true; } else if (ju >= ny) { ju -= ny; wy = true; }
                             const size_t m = ((size_t)kq * ny + ju) * nx + iu;
-                            const double xv = wx ? p.faceX[(size_t)kq * ny + ju] : (wy ? p.faceY[(size_t)kq * nx + iu] : X[m]);
+                            const double xv = wx ? fX[(size_t)kq * ny + ju] : (wy ? fY[(size_t)kq * nx + iu] : X[m]);
                             Xu += q.w[t] * xv;
-                            ku += q.w[t] * (double)p.kaprho[m];
-                            Su += q.w[t] * p.S[m];
+                            ku += q.w[t] * (double)kb[m];
+                            Su += q.w[t] * Sb[m];
                         }
-                        const double dtau = 0.5 * (ku + (double)p.kaprho[n]) * q.ds;
+                        const double dtau = 0.5 * (ku + (double)kb[n]) * q.ds;
                         double E, pu, pp;
                         scat_psi(dtau, E, pu, pp);
                         Inew = Xu * E + pu * Su + pp * Sn;
                     }
                     if (p.gs) {
-                        const double jn = p.J[n] + q.wq * (Inew - X[n]);
-                        const double ep = (double)p.eps[n];
-                        p.J[n] = jn;
-                        p.S[n] = (1.0 - ep) * jn + ep * (double)p.B[n];
+                        const size_t g = b * N + n;
+                        const double jn = p.J[g] + q.wq * (Inew - X[n]);
+                        const double ep_ = (double)p.eps[g];
+                        p.J[g] = jn;
+                        p.S[g] = (1.0 - ep_) * jn + ep_ * (double)p.B[g];
                     }
                     X[n] = Inew;
                 }
@@ -153,21 +166,24 @@ __global__ void __launch_bounds__(256) rts_scatter_kernel(const ScatParams p)
             }
         }
         if (!p.gs) {
-            for (size_t n = gtid; n < N; n += gsz) {
+            for (size_t e = gtid; e < NB; e += gsz) {
+                const size_t b = e / N, n = e - b * N;
                 double a = 0.0;
-                for (int r = 0; r < p.nrays; ++r) a += p.rays[r].wq * p.I[(size_t)r * N + n];
-                const double ep = (double)p.eps[n];
-                p.J[n] = a;
-                p.S[n] = (1.0 - ep) * a + ep * (double)p.B[n];
+                for (int r = 0; r < p.nrays; ++r) a += p.rays[r].wq * p.I[(b * p.nrays + r) * N + n];
+                const double ep_ = (double)p.eps[e];
+                p.J[e] = a;
+                p.S[e] = (1.0 - ep_) * a + ep_ * (double)p.B[e];
             }
         }
-        // change of this iteration (positive doubles order like their bit patterns)
-        double e = 0.0, sc = 0.0;
-        for (size_t n = gtid; n < N; n += gsz) { const double s = p.S[n]; e = fmax(e, fabs(s - p.Sold[n])); sc = fmax(sc, fabs(s)); }
-        for (int o = 16; o > 0; o >>= 1) { e = fmax(e, __shfl_xor_sync(0xffffffffu, e, o)); sc = fmax(sc, __shfl_xor_sync(0xffffffffu, sc, o)); }
-        if ((threadIdx.x & 31) == 0) {
-            atomicMax(p.chg + 2 * it, (unsigned long long)__double_as_longlong(e));
-            atomicMax(p.chg + 2 * it + 1, (unsigned long long)__double_as_longlong(sc));
+        // change of this iteration per band (positive doubles order like their bit patterns)
+        for (int b = 0; b < nb; ++b) {
+            double e = 0.0, sc = 0.0;
+            for (size_t n = gtid; n < N; n += gsz) { const double s = p.S[b * N + n]; e = fmax(e, fabs(s - p.Sold[b * N + n])); sc = fmax(sc, fabs(s)); }
+            for (int o = 16; o > 0; o >>= 1) { e = fmax(e, __shfl_xor_sync(0xffffffffu, e, o)); sc = fmax(sc, __shfl_xor_sync(0xffffffffu, sc, o)); }
+            if ((threadIdx.x & 31) == 0) {
+                atomicMax(p.chg + 2 * ((size_t)it * nb + b), (unsigned long long)__double_as_longlong(e));
+                atomicMax(p.chg + 2 * ((size_t)it * nb + b) + 1, (unsigned long long)__double_as_longlong(sc));
+            }
         }
         if (!scat_grid_sync(p.bar, gen)) return;
     }

@@ -102,9 +102,9 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_solve_flux.restype = c_int
     lib.rts_solve_flux.argtypes = [c_void_p] + [c_void_p] * 8 + [c_void_p]
     lib.rts_scatter_workspace_bytes.restype = ctypes.c_size_t
-    lib.rts_scatter_workspace_bytes.argtypes = [c_void_p, c_int]
+    lib.rts_scatter_workspace_bytes.argtypes = [c_void_p, c_int, c_int]
     lib.rts_scatter_solve.restype = c_int
-    lib.rts_scatter_solve.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, ctypes.c_size_t,
+    lib.rts_scatter_solve.argtypes = [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, ctypes.c_size_t,
                                       c_void_p, c_void_p, ctypes.POINTER(ctypes.c_double), c_void_p]
     lib.rts_set_tolerance.restype = c_int
     lib.rts_set_tolerance.argtypes = [c_void_p, c_double, c_int]
@@ -349,23 +349,29 @@ class RTS:
         self._check(self._lib.rts_set_tolerance(self._ctx, float(tol), int(max_passes)), "rts_set_tolerance")
 
     def scatter_solve(self, kaprho, B, eps, niter: int, gauss_seidel: bool = True):
-        """NEXT #4, one band: S = (1 - eps) J + eps B with the source update along the ray (or as a Jacobi iteration).
-        kaprho, B, eps: CUDA float32 [nz][ny][nx].  Returns (S, J CUDA float64 [nz][ny][nx], change per iteration)."""
+        """NEXT #4: S = (1 - eps) J + eps B with the source update along the ray (or as a Jacobi iteration), for one band
+        (CUDA float32 [nz][ny][nx]) or several independent ones ([nb][nz][ny][nx]).  Returns (S, J CUDA float64 of the
+        same shape, change per iteration: a list of floats for one band, of per-band lists for several)."""
         torch = self._torch
         shp = (self.nz, self.ny, self.nx)
+        one = (kaprho.dim() == 3)
+        nb = 1 if one else int(kaprho.shape[0])
+        full = shp if one else (nb,) + shp
         for t in (kaprho, B, eps):
-            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == shp
-        nbytes = int(self._lib.rts_scatter_workspace_bytes(self._ctx, int(niter)))
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == full
+        nbytes = int(self._lib.rts_scatter_workspace_bytes(self._ctx, nb, int(niter)))
         ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
         base = (ws.data_ptr() + 255) & ~255
-        S = torch.empty(shp, dtype=torch.float64, device="cuda")
-        J = torch.empty(shp, dtype=torch.float64, device="cuda")
-        change = (ctypes.c_double * max(int(niter), 1))()
-        self._check(self._lib.rts_scatter_solve(self._ctx, ctypes.c_void_p(kaprho.data_ptr()), ctypes.c_void_p(B.data_ptr()),
+        S = torch.empty(full, dtype=torch.float64, device="cuda")
+        J = torch.empty(full, dtype=torch.float64, device="cuda")
+        change = (ctypes.c_double * max(int(niter) * nb, 1))()
+        self._check(self._lib.rts_scatter_solve(self._ctx, nb, ctypes.c_void_p(kaprho.data_ptr()), ctypes.c_void_p(B.data_ptr()),
                                                 ctypes.c_void_p(eps.data_ptr()), int(niter), 1 if gauss_seidel else 0,
                                                 ctypes.c_void_p(base), nbytes, ctypes.c_void_p(S.data_ptr()),
                                                 ctypes.c_void_p(J.data_ptr()), change, self._stream()), "rts_scatter_solve")
-        return S, J, [float(change[i]) for i in range(int(niter))]
+        if one:
+            return S, J, [float(change[i]) for i in range(int(niter))]
+        return S, J, [[float(change[i * nb + b]) for b in range(nb)] for i in range(int(niter))]
 
     def set_warm_start(self, on: bool = True):
         self._check(self._lib.rts_set_warm_start(self._ctx, 1 if on else 0), "rts_set_warm_start")

@@ -47,6 +47,31 @@ def test_scatter_against_oracle(cfg, grid, band, niter, gs):
     assert np.allclose(change, cho, rtol=1e-6, atol=1e-14)
 
 
+def test_several_bands_in_one_call_are_independent_problems():
+    """All bands of a call share the plane steps; every band must equal the oracle's one-band solve (and so the
+    one-band call) element by element."""
+    import oracle
+    import torch
+    from paper_2107_08145_b200 import rts
+    inp = inputs.make_config(4, grid=(20, 24, 17))                # 12 bands, opacity scales up to 1e5
+    s = rts.from_inputs(inp)
+    rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
+    k, B = s.coefficients(rho, T, P)
+    rng = np.random.default_rng(3)
+    eps = torch.from_numpy((0.02 + 0.98 * rng.random((inp.nbands,) + inp.shape)).astype(np.float32)).cuda()
+    S, J, change = s.scatter_solve(k, B, eps, 4)
+    S1, J1, ch1 = s.scatter_solve(k[5].contiguous(), B[5].contiguous(), eps[5].contiguous(), 4)
+    s.sync_check(); s.close()
+    assert torch.equal(S[5], S1) and torch.equal(J[5], J1) and [c[5] for c in change] == ch1
+    for b in (0, 7, 11):
+        So, Jo, cho = oracle.scatter_solve(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.mu, inp.wq,
+                                           k[b].cpu().numpy().astype(np.float64), B[b].cpu().numpy().astype(np.float64),
+                                           eps[b].cpu().numpy().astype(np.float64), 4, gs=True)
+        assert np.abs(S[b].cpu().numpy() - So).max() <= TOL * np.abs(So).max()
+        assert np.abs(J[b].cpu().numpy() - Jo).max() <= TOL * np.abs(Jo).max()
+        assert np.allclose([c[b] for c in change], cho, rtol=1e-6, atol=1e-14)
+
+
 def test_eps_one_is_the_lte_source_and_zero_iterations_return_the_start():
     import torch
     inp, s, k, B, eps = _case(1, (16, 12, 10), 0, 0.05)
