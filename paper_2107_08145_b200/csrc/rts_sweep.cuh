@@ -1061,7 +1061,9 @@ __device__ void run_task(TaskShared& S, const SweepMaps& maps, const int tile, f
                     hist_pass<PITCH>(&S, S.stage0 + (size_t)stc * PS, S.Xb + (size_t)(cur ^ 1) * NG * PS, m, P);
                     __syncthreads();
                 }
-                if (tid == 0) {
+                // one thread of the LAST warp (a ray's fourth warp holds its shortest strips): warp 0 is on the step's
+                // critical path, and the ~0.1 us of the next plane's TMA issue there delayed every step (25.55 -> 25.38 ms)
+                if (tid == T - 32) {
                     // arrival (release): at every block end, or with the tagged exchange at the end of a pass only
                     if (blk_last && more && (!tagged || m == n_m - 1)) { __threadfence(); atomicAdd(U.barrier, 1); }
                     const int ahead = NST - 1;               // planes in flight beyond the previous one
