@@ -226,6 +226,21 @@ int rts_scatter_solve(rts_ctx* ctx, int nbands, const float* kaprho_dev, const f
                       int niter, int gauss_seidel, void* workspace_dev, size_t workspace_bytes, double* S_dev,
                       double* J_dev, double* change_host, void* stream);
 
+/* The scattering solve for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same operation, kernel and results as rts_scatter_solve (PAPER.md:261,
+ * reading R23), with the scratch in a static device array of RTS_SCATTER_STATIC_BYTES bytes inside the library, which
+ * every GPU that loads the library holds until the process exits.  The call makes no cudaMalloc / cudaFree and no
+ * host heap allocation.  Arguments as rts_scatter_solve (inputs DEVICE float [nbands][nz][ny][nx], outputs DEVICE
+ * double of the same shape, change_host HOST [niter][nbands] or NULL), without the workspace pair.
+ * Limits: rts_scatter_workspace_bytes(ctx, nbands, niter) <= RTS_SCATTER_STATIC_BYTES (about 80 000 nodes x bands with
+ * 24 rays), max(niter, 1) * nbands <= 2048, at most 256 rays; beyond them RTS_EINVAL with a message that names the
+ * sizes.  The context's device must be current (RTS_ESTATE otherwise).  Every call on a device shares the one array,
+ * which keeps the last call's contents (the entry clears what must start at zero): calls that overlap on the GPU
+ * -- two streams, two contexts, two threads -- race; serialise them.  Synchronous on `stream`. */
+#define RTS_SCATTER_STATIC_BYTES (16u << 20)
+int rts_scatter_solve_static(rts_ctx* ctx, int nbands, const float* kaprho_dev, const float* B_dev, const float* eps_dev,
+                             int niter, int gauss_seidel, double* S_dev, double* J_dev, double* change_host, void* stream);
+
 /* [measurement only]
  * Per-stage device timing of the last rts_solve (CUDA events recorded on the solve stream
  * inside rts_solve).  rts_last_timing waits for the solve and fills ms4 (HOST) with

@@ -16,11 +16,19 @@
 #undef RTS_MODE_NS
 #include "rts_scatter.cuh"
 
+// Scratch of the entry point that allocates nothing (rts_scatter_solve_static): a file-scope device array, held by
+// every GPU that loads this library until the process exits.  In host code the name below is a host-side stand-in,
+// NOT a device address: host code takes the address once per device with cudaGetSymbolAddress (resolve_static_scratch,
+// called at set-up by rts_create with that device current) and hands that pointer to the kernel.
+#define RTS_SCATTER_STATIC_BYTES_IMPL (16u << 20)
+static __device__ __align__(256) unsigned char g_scatter_scratch[RTS_SCATTER_STATIC_BYTES_IMPL];
+
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -63,6 +71,9 @@ struct rts_ctx {
     double tol = 0.0;
     bool warm = false;                 // keep the seam state between solves
     int nplain = 0;                    // partial-heating buffers in the x-fastest layout (summed first by the finalize kernel)
+    int device = 0;                    // the device this context was created on
+    void* static_scratch = nullptr;    // device address of g_scatter_scratch on that device (null: static_scratch_err says why)
+    cudaError_t static_scratch_err = cudaSuccess;
     std::vector<ScatRay> scat_rays;    // ray constants of the last rts_scatter_solve (kept until its copy has run)
     int pass_counter = 0;              // passes the seam state has seen (0: cold)
     int passes_used = 0;
@@ -551,6 +562,23 @@ int launch_stage_a(rts_ctx* c, const float* rho, const float* T, const float* P,
 // =========================================================================== C-ABI
 extern "C" {
 
+// Device address of g_scatter_scratch on device `dev`, which must be current; resolved once per device.
+static cudaError_t resolve_static_scratch(int dev, void** ptr)
+{
+    static std::mutex mu;
+    static struct { bool done; cudaError_t err; void* ptr; } tab[64] = {};
+    if (dev < 0 || dev >= 64) { *ptr = nullptr; return cudaErrorInvalidDevice; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!tab[dev].done) {
+        void* q = nullptr;
+        tab[dev].err = cudaGetSymbolAddress(&q, g_scatter_scratch);
+        tab[dev].ptr = (tab[dev].err == cudaSuccess) ? q : nullptr;
+        tab[dev].done = true;
+    }
+    *ptr = tab[dev].ptr;
+    return tab[dev].err;
+}
+
 int rts_create(rts_ctx** out, int nx, int ny, int nz, double dx, double dy, double dz, int nbands)
 {
     if (!out) return RTS_EINVAL;
@@ -589,6 +617,8 @@ int rts_create(rts_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
             qres != cudaDriverEntryPointSuccess || !c->encode_fn)
             return bail("cuTensorMapEncodeTiled not available from the driver");
     }
+    c->device = dev;
+    c->static_scratch_err = resolve_static_scratch(dev, &c->static_scratch);   // reported by rts_scatter_solve_static only
     *out = c;
     return RTS_OK;
 }
@@ -1164,6 +1194,88 @@ int rts_scatter_solve(rts_ctx* c, int nbands, const float* kaprho, const float* 
     CUDA_TRY(c, cudaMemcpyAsync(flags, ws + off[6], sizeof(flags), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaStreamSynchronize(st));
     if (flags[1] != 0) return fail(c, RTS_ETIMEOUT, "rts_scatter_solve: the grid barrier timed out");
+    if (change_host)
+        for (size_t q = 0; q < (size_t)niter * nbands; ++q) {                 // [niter][nbands]
+            double e, sc;
+            std::memcpy(&e, &chg[2 * q], 8); std::memcpy(&sc, &chg[2 * q + 1], 8);
+            change_host[q] = (sc > 0.0) ? e / sc : 0.0;
+        }
+    return RTS_OK;
+}
+
+// The same solve with its scratch in the static device array: allocates nothing (no cudaMalloc / cudaFree, no host
+// heap: the ray constants and the change words live on the stack, which bounds nrays and niter * nbands).
+int rts_scatter_solve_static(rts_ctx* c, int nbands, const float* kaprho, const float* B, const float* eps, int niter,
+                             int gauss_seidel, double* S, double* J, double* change_host, void* stream)
+{
+    constexpr int MAXR = 256, MAXCHG = 2048;
+    if (!c) return RTS_EINVAL;
+    if (!kaprho || !B || !eps || !S || !J) return fail(c, RTS_EINVAL, "rts_scatter_solve_static: null pointer");
+    if (niter < 0 || nbands < 1 || (long long)std::max(niter, 1) * nbands > MAXCHG)
+        return fail(c, RTS_EINVAL, "rts_scatter_solve_static: need niter >= 0, nbands >= 1, max(niter, 1) * nbands <= 2048");
+    const int nr = (int)c->rays.size();
+    if (nr < 1 || nr > MAXR) return fail(c, RTS_EINVAL, "rts_scatter_solve_static: 1 <= rays <= 256");
+    int dev = -1;
+    CUDA_TRY(c, cudaGetDevice(&dev));
+    if (dev != c->device) return fail(c, RTS_ESTATE, "rts_scatter_solve_static: the context's device is not current");
+    if (c->static_scratch_err != cudaSuccess || !c->static_scratch)
+        return fail(c, RTS_ECUDA, std::string("rts_scatter_solve_static: cudaGetSymbolAddress of the static scratch failed at set-up: ") +
+                                      cudaGetErrorString(c->static_scratch_err));
+    size_t off[8];
+    const size_t need = scatter_layout(c, nbands, niter, off);
+    if (need > (size_t)RTS_SCATTER_STATIC_BYTES_IMPL) {
+        char buf[200];
+        snprintf(buf, sizeof buf, "rts_scatter_solve_static: this problem needs %zu bytes of scratch, the static array holds %u "
+                                  "(use rts_scatter_solve with a caller-owned workspace)", need, (unsigned)RTS_SCATTER_STATIC_BYTES_IMPL);
+        return fail(c, RTS_EINVAL, buf);
+    }
+    cudaStream_t st = as_stream(stream);
+    unsigned char* ws = (unsigned char*)c->static_scratch;       // the DEVICE address, never the symbol's name
+    ScatRay rays[MAXR];
+    for (int i = 0; i < nr; ++i) {
+        HostRay r = c->rays[i];
+        if (ray_geometry(c->h, r) != 0) return fail(c, RTS_EINVAL, "ray with mu_z == 0");
+        ScatRay q{};
+        const int as = r.march, ua = (as == 0) ? 1 : 0, va = (as == 2) ? 1 : 2;
+        q.as = as; q.dir = r.dir; q.up = r.up; q.kdir = r.up ? 0 : c->nz - 1;
+        int sg[3]; sg[as] = r.dir; sg[ua] = r.su; sg[va] = r.sv;
+        q.iface = (sg[0] > 0) ? c->nx - 1 : 0; q.jface = (sg[1] > 0) ? c->ny - 1 : 0;
+        for (int eu = 0; eu < 2; ++eu)
+            for (int ev = 0; ev < 2; ++ev) {
+                const int t = eu * 2 + ev;
+                q.off[t][0] = q.off[t][1] = q.off[t][2] = 0;
+                q.off[t][as] = -sg[as]; q.off[t][ua] = -eu * sg[ua]; q.off[t][va] = -ev * sg[va];
+                q.w[t] = (eu ? r.fu : 1.0 - r.fu) * (ev ? r.fv : 1.0 - r.fv);
+            }
+        q.ds = r.ds; q.wq = r.w;
+        rays[i] = q;
+    }
+    const size_t nchg = 2 * (size_t)nbands * (size_t)std::max(niter, 1);
+    // the array keeps the previous call's contents: the change words and the barrier words must start at zero (the
+    // kernel itself initialises I_r, J, S and rewrites the faces and S_old before it reads them)
+    CUDA_TRY(c, cudaMemcpyAsync(ws + off[4], rays, sizeof(ScatRay) * nr, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(c, cudaMemsetAsync(ws + off[5], 0, sizeof(unsigned long long) * nchg, st));
+    CUDA_TRY(c, cudaMemsetAsync(ws + off[6], 0, sizeof(unsigned) * 4, st));
+    ScatParams p{};
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nrays = nr; p.niter = niter; p.gs = gauss_seidel != 0; p.nb = nbands;
+    p.kaprho = kaprho; p.B = B; p.eps = eps;
+    p.rays = (const ScatRay*)(ws + off[4]);
+    p.I = (double*)(ws + off[0]); p.faceX = (double*)(ws + off[1]); p.faceY = (double*)(ws + off[2]); p.Sold = (double*)(ws + off[3]);
+    p.S = S; p.J = J;
+    p.chg = (unsigned long long*)(ws + off[5]); p.bar = (unsigned*)(ws + off[6]);
+    int occ = 0;
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_scatter_kernel, 256, 0));
+    if (occ < 1) return fail(c, RTS_ECUDA, "rts_scatter_solve_static: kernel does not fit on an SM");
+    const size_t plane_max = (size_t)std::max(c->nx, c->ny) * std::max(std::max(c->nx, c->ny), c->nz);
+    const int grid = (int)std::max<size_t>(1, std::min<size_t>((size_t)c->sm_count * std::min(occ, 4), (plane_max * nbands + 255) / 256));
+    void* args[] = {&p};
+    CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_scatter_kernel, dim3(grid), dim3(256), args, 0, st));
+    unsigned long long chg[2 * MAXCHG];
+    unsigned flags[4] = {0, 0, 0, 0};
+    CUDA_TRY(c, cudaMemcpyAsync(chg, ws + off[5], sizeof(unsigned long long) * nchg, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaMemcpyAsync(flags, ws + off[6], sizeof(flags), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    if (flags[1] != 0) return fail(c, RTS_ETIMEOUT, "rts_scatter_solve_static: the grid barrier timed out");
     if (change_host)
         for (size_t q = 0; q < (size_t)niter * nbands; ++q) {                 // [niter][nbands]
             double e, sc;

@@ -28,7 +28,7 @@ EXPORTS = [
     "rts_cells_to_nodes", "rts_nodes_to_cells", "rts_solve_cells", "rts_set_thick_skip", "rts_thick_levels",
     "rts_enable_flux", "rts_set_flux_blend", "rts_solve_flux", "rts_set_shard", "rts_shard_info",
     "rts_set_tolerance", "rts_set_warm_start", "rts_passes_used",
-    "rts_scatter_workspace_bytes", "rts_scatter_solve",
+    "rts_scatter_workspace_bytes", "rts_scatter_solve", "rts_scatter_solve_static",
 ]
 
 
@@ -106,6 +106,9 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.rts_scatter_solve.restype = c_int
     lib.rts_scatter_solve.argtypes = [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, ctypes.c_size_t,
                                       c_void_p, c_void_p, ctypes.POINTER(ctypes.c_double), c_void_p]
+    lib.rts_scatter_solve_static.restype = c_int
+    lib.rts_scatter_solve_static.argtypes = [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_int, c_int,
+                                             c_void_p, c_void_p, ctypes.POINTER(ctypes.c_double), c_void_p]
     lib.rts_set_tolerance.restype = c_int
     lib.rts_set_tolerance.argtypes = [c_void_p, c_double, c_int]
     lib.rts_set_warm_start.restype = c_int
@@ -369,6 +372,32 @@ class RTS:
                                                 ctypes.c_void_p(eps.data_ptr()), int(niter), 1 if gauss_seidel else 0,
                                                 ctypes.c_void_p(base), nbytes, ctypes.c_void_p(S.data_ptr()),
                                                 ctypes.c_void_p(J.data_ptr()), change, self._stream()), "rts_scatter_solve")
+        if one:
+            return S, J, [float(change[i]) for i in range(int(niter))]
+        return S, J, [[float(change[i * nb + b]) for b in range(nb)] for i in range(int(niter))]
+
+    def scatter_solve_static(self, kaprho, B, eps, niter: int, gauss_seidel: bool = True, S=None, J=None):
+        """scatter_solve with the scratch in the library's static device array: the C call allocates nothing (pass S and
+        J, CUDA float64 of the inputs' shape, to keep this wrapper from allocating them).  Small problems only
+        (rts.h: RTS_SCATTER_STATIC_BYTES); calls that overlap on the GPU race."""
+        torch = self._torch
+        shp = (self.nz, self.ny, self.nx)
+        one = (kaprho.dim() == 3)
+        nb = 1 if one else int(kaprho.shape[0])
+        full = shp if one else (nb,) + shp
+        for t in (kaprho, B, eps):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == full
+        if S is None:
+            S = torch.empty(full, dtype=torch.float64, device="cuda")
+        if J is None:
+            J = torch.empty(full, dtype=torch.float64, device="cuda")
+        for t in (S, J):
+            assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == full
+        change = (ctypes.c_double * max(int(niter) * nb, 1))()
+        self._check(self._lib.rts_scatter_solve_static(self._ctx, nb, ctypes.c_void_p(kaprho.data_ptr()), ctypes.c_void_p(B.data_ptr()),
+                                                       ctypes.c_void_p(eps.data_ptr()), int(niter), 1 if gauss_seidel else 0,
+                                                       ctypes.c_void_p(S.data_ptr()), ctypes.c_void_p(J.data_ptr()), change,
+                                                       self._stream()), "rts_scatter_solve_static")
         if one:
             return S, J, [float(change[i]) for i in range(int(niter))]
         return S, J, [[float(change[i * nb + b]) for b in range(nb)] for i in range(int(niter))]
