@@ -1180,14 +1180,17 @@ int rts_scatter_solve(rts_ctx* c, int nbands, const float* kaprho, const float* 
     p.I = (double*)(ws + off[0]); p.faceX = (double*)(ws + off[1]); p.faceY = (double*)(ws + off[2]); p.Sold = (double*)(ws + off[3]);
     p.S = S; p.J = J;
     p.chg = (unsigned long long*)(ws + off[5]); p.bar = (unsigned*)(ws + off[6]);
-    int occ = 0;
-    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_scatter_kernel, 256, 0));
-    if (occ < 1) return fail(c, RTS_ECUDA, "rts_scatter_solve: kernel does not fit on an SM");
     const size_t plane_max = (size_t)std::max(c->nx, c->ny) * std::max(std::max(c->nx, c->ny), c->nz);
+    // the variant with 3 CTAs per SM where 2 per SM would leave some threads with a second node per plane step
+    const bool big = plane_max * nbands > (size_t)c->sm_count * 2 * 256;
+    const void* kern = big ? (const void*)rts_scatter_kernel<3> : (const void*)rts_scatter_kernel<2>;
+    int occ = 0;
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, 0));
+    if (occ < 1) return fail(c, RTS_ECUDA, "rts_scatter_solve: kernel does not fit on an SM");
     const int grid = (int)std::max<size_t>(1, std::min<size_t>((size_t)c->sm_count * std::min(occ, 4), (plane_max * nbands + 255) / 256));
     void* args[] = {&p};
     // cooperative launch: every CTA is resident, which the grid-wide barrier between planes relies on
-    CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_scatter_kernel, dim3(grid), dim3(256), args, 0, st));
+    CUDA_TRY(c, cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(256), args, 0, st));
     std::vector<unsigned long long> chg(2 * (size_t)nbands * (size_t)std::max(niter, 1));
     unsigned flags[4] = {0, 0, 0, 0};
     CUDA_TRY(c, cudaMemcpyAsync(chg.data(), ws + off[5], sizeof(unsigned long long) * chg.size(), cudaMemcpyDeviceToHost, st));
@@ -1263,13 +1266,16 @@ int rts_scatter_solve_static(rts_ctx* c, int nbands, const float* kaprho, const 
     p.I = (double*)(ws + off[0]); p.faceX = (double*)(ws + off[1]); p.faceY = (double*)(ws + off[2]); p.Sold = (double*)(ws + off[3]);
     p.S = S; p.J = J;
     p.chg = (unsigned long long*)(ws + off[5]); p.bar = (unsigned*)(ws + off[6]);
-    int occ = 0;
-    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rts_scatter_kernel, 256, 0));
-    if (occ < 1) return fail(c, RTS_ECUDA, "rts_scatter_solve_static: kernel does not fit on an SM");
     const size_t plane_max = (size_t)std::max(c->nx, c->ny) * std::max(std::max(c->nx, c->ny), c->nz);
+    // the variant with 3 CTAs per SM where 2 per SM would leave some threads with a second node per plane step
+    const bool big = plane_max * nbands > (size_t)c->sm_count * 2 * 256;
+    const void* kern = big ? (const void*)rts_scatter_kernel<3> : (const void*)rts_scatter_kernel<2>;
+    int occ = 0;
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, 0));
+    if (occ < 1) return fail(c, RTS_ECUDA, "rts_scatter_solve_static: kernel does not fit on an SM");
     const int grid = (int)std::max<size_t>(1, std::min<size_t>((size_t)c->sm_count * std::min(occ, 4), (plane_max * nbands + 255) / 256));
     void* args[] = {&p};
-    CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)rts_scatter_kernel, dim3(grid), dim3(256), args, 0, st));
+    CUDA_TRY(c, cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(256), args, 0, st));
     unsigned long long chg[2 * MAXCHG];
     unsigned flags[4] = {0, 0, 0, 0};
     CUDA_TRY(c, cudaMemcpyAsync(chg, ws + off[5], sizeof(unsigned long long) * nchg, cudaMemcpyDeviceToHost, st));

@@ -75,7 +75,11 @@ __device__ __forceinline__ void scat_psi(const double d, double& E, double& pu, 
     }
 }
 
-__global__ void __launch_bounds__(256) rts_scatter_kernel(const ScatParams p)
+// MINB CTAs per SM: 2 (98 registers, no spills) for planes that 2 x 256 threads per SM cover with one node per thread,
+// 3 (80 registers, 120 bytes of spills) for larger ones, where a second node per thread doubles the dependent chain of a
+// plane step (288^3, one band: 80 -> 63 ms per iteration; 96^3: 10.5 -> 11.4 ms, hence both).
+template <int MINB>
+__global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams p)
 {
     const int nx = p.nx, ny = p.ny, nz = p.nz, nb = p.nb;
     const size_t N = (size_t)nx * ny * nz, NB = N * nb;
