@@ -72,6 +72,40 @@ def test_several_bands_in_one_call_are_independent_problems():
         assert np.allclose([c[b] for c in change], cho, rtol=1e-6, atol=1e-14)
 
 
+@pytest.mark.parametrize("rays", ["axis_parallel_and_aligned", "single", "z_face_only"])
+def test_scatter_with_other_ray_sets(rays):
+    """Rays with a zero component (f = 0), lattice-aligned rays (f = 1), one ray alone, and a set whose rays all
+    march along z: the per-ray geometry of the kernel against the oracle's."""
+    import oracle
+    import torch
+    from paper_2107_08145_b200 import rts
+    inp = inputs.make_config(1, grid=(16, 12, 14))
+    if rays == "axis_parallel_and_aligned":
+        inp.dz = inp.dx * 0.9082483 / 0.2958759
+        inp.mu = np.array([[0.0, 0.6, 0.8], [0.6, 0.0, -0.8], [0.0, 0.0, 1.0], [0.0, 0.0, -1.0],
+                           [0.2958759, 0.2958759, 0.9082483], [-0.2958759, 0.2958759, -0.9082483]])
+        inp.wq = np.full(6, 1.0 / 6.0)
+    elif rays == "single":
+        inp.mu = np.array([[0.3, -0.5, 0.81]]); inp.wq = np.array([1.0])
+    else:
+        mu, w = inputs.carlson24()
+        sel = [r for r in range(24) if r % 3 == 2]
+        inp.mu = np.ascontiguousarray(mu[sel]); inp.wq = np.full(len(sel), 1.0 / len(sel))
+    s = rts.from_inputs(inp)
+    rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
+    k, B = s.coefficients(rho, T, P)
+    rng = np.random.default_rng(5)
+    eps = torch.from_numpy((0.1 + 0.9 * rng.random(inp.shape)).astype(np.float32)).cuda()
+    S, J, change = s.scatter_solve(k[0].contiguous(), B[0].contiguous(), eps, 5)
+    s.sync_check(); s.close()
+    So, Jo, cho = oracle.scatter_solve(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.mu, inp.wq,
+                                       k[0].cpu().numpy().astype(np.float64), B[0].cpu().numpy().astype(np.float64),
+                                       eps.cpu().numpy().astype(np.float64), 5, gs=True)
+    assert np.abs(S.cpu().numpy() - So).max() <= TOL * np.abs(So).max()
+    assert np.abs(J.cpu().numpy() - Jo).max() <= TOL * np.abs(Jo).max()
+    assert np.allclose(change, cho, rtol=1e-6, atol=1e-14)
+
+
 def test_eps_one_is_the_lte_source_and_zero_iterations_return_the_start():
     import torch
     inp, s, k, B, eps = _case(1, (16, 12, 10), 0, 0.05)
