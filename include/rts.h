@@ -219,7 +219,7 @@ int rts_shard_info(rts_ctx* ctx, int* units_mine, int* units_all);
  * Outputs: S, J DEVICE double [nbands][nz][ny][nx] (this kernel computes in fp64); change_host (HOST
  * [niter][nbands], may be NULL): max|S - S_previous| / max|S| of every iteration and band.  workspace: DEVICE,
  * 256-byte aligned, at least rts_scatter_workspace_bytes(ctx, nbands, niter) bytes (one double per ray, node and
- * band: 4.6 GB per band at 288^3 with 24 rays), borrowed for the call.  Synchronous on `stream` (the host reads
+ * band, plus copies of the three inputs: 4.9 GB per band at 288^3 with 24 rays), borrowed for the call.  Synchronous on `stream` (the host reads
  * the change words).  RTS_ETIMEOUT if the grid barrier's watchdog fired; RTS_EINVAL for bad arguments. */
 size_t rts_scatter_workspace_bytes(rts_ctx* ctx, int nbands, int niter);
 int rts_scatter_solve(rts_ctx* ctx, int nbands, const float* kaprho_dev, const float* B_dev, const float* eps_dev,
@@ -232,7 +232,7 @@ int rts_scatter_solve(rts_ctx* ctx, int nbands, const float* kaprho_dev, const f
  * every GPU that loads the library holds until the process exits.  The call makes no cudaMalloc / cudaFree and no
  * host heap allocation.  Arguments as rts_scatter_solve (inputs DEVICE float [nbands][nz][ny][nx], outputs DEVICE
  * double of the same shape, change_host HOST [niter][nbands] or NULL), without the workspace pair.
- * Limits: rts_scatter_workspace_bytes(ctx, nbands, niter) <= RTS_SCATTER_STATIC_BYTES (about 80 000 nodes x bands with
+ * Limits: rts_scatter_workspace_bytes(ctx, nbands, niter) <= RTS_SCATTER_STATIC_BYTES (about 75 000 nodes x bands with
  * 24 rays), max(niter, 1) * nbands <= 2048, at most 256 rays; beyond them RTS_EINVAL with a message that names the
  * sizes.  The context's device must be current (RTS_ESTATE otherwise).  Every call on a device shares the one array,
  * which keeps the last call's contents (the entry clears what must start at zero): calls that overlap on the GPU

@@ -1130,6 +1130,7 @@ static size_t scatter_layout(const rts_ctx* c, int nbands, int niter, size_t off
     off[4] = take(sizeof(ScatRay) * nr);
     off[5] = take(sizeof(unsigned long long) * 2 * nb * (size_t)std::max(niter, 1));
     off[6] = take(sizeof(unsigned) * 4);
+    off[7] = take(sizeof(float) * 3 * N * nb);                   // y-fastest copies of kaprho, B, eps
     return o;
 }
 
@@ -1180,6 +1181,7 @@ int rts_scatter_solve(rts_ctx* c, int nbands, const float* kaprho, const float* 
     p.I = (double*)(ws + off[0]); p.faceX = (double*)(ws + off[1]); p.faceY = (double*)(ws + off[2]); p.Sold = (double*)(ws + off[3]);
     p.S = S; p.J = J;
     p.chg = (unsigned long long*)(ws + off[5]); p.bar = (unsigned*)(ws + off[6]);
+    { const size_t NBn = (size_t)c->nx * c->ny * c->nz * (size_t)nbands; p.kapT = (float*)(ws + off[7]); p.BT = p.kapT + NBn; p.epsT = p.BT + NBn; }
     const size_t plane_max = (size_t)std::max(c->nx, c->ny) * std::max(std::max(c->nx, c->ny), c->nz);
     // the variant with 3 CTAs per SM where 2 per SM would leave some threads with a second node per plane step
     const bool big = plane_max * nbands > (size_t)c->sm_count * 2 * 256;
@@ -1266,6 +1268,7 @@ int rts_scatter_solve_static(rts_ctx* c, int nbands, const float* kaprho, const 
     p.I = (double*)(ws + off[0]); p.faceX = (double*)(ws + off[1]); p.faceY = (double*)(ws + off[2]); p.Sold = (double*)(ws + off[3]);
     p.S = S; p.J = J;
     p.chg = (unsigned long long*)(ws + off[5]); p.bar = (unsigned*)(ws + off[6]);
+    { const size_t NBn = (size_t)c->nx * c->ny * c->nz * (size_t)nbands; p.kapT = (float*)(ws + off[7]); p.BT = p.kapT + NBn; p.epsT = p.BT + NBn; }
     const size_t plane_max = (size_t)std::max(c->nx, c->ny) * std::max(std::max(c->nx, c->ny), c->nz);
     // the variant with 3 CTAs per SM where 2 per SM would leave some threads with a second node per plane step
     const bool big = plane_max * nbands > (size_t)c->sm_count * 2 * 256;

@@ -26,6 +26,8 @@ struct ScatRay {
 struct ScatParams {
     int nx, ny, nz, nrays, niter, gs, nb;
     const float* kaprho; const float* B; const float* eps;    // [nb][N] each
+    float* kapT; float* BT; float* epsT;   // [nb][nz][nx][ny] (y fastest) copies of the three inputs, made by the kernel: the
+                                           // x-march rays read them with unit stride (their planes have no x extent)
     const ScatRay* rays;
     double* I;                         // [nb][nrays][N]
     double* faceX; double* faceY;      // [nb][nz][ny], [nb][nz][nx]
@@ -77,10 +79,15 @@ __device__ __forceinline__ void scat_psi(const double d, double& E, double& pu, 
 
 // MINB CTAs per SM: 2 (98 registers, no spills) for planes that 2 x 256 threads per SM cover with one node per thread,
 // 3 (80 registers, 120 bytes of spills) for larger ones, where a second node per thread doubles the dependent chain of a
-// plane step (288^3, one band: 80 -> 63 ms per iteration; 96^3: 10.5 -> 11.4 ms, hence both).
+// plane step (288^3, one band: 80 -> 63 ms per iteration; 96^3: 10.5 -> 11.4 ms, hence both).  The build for large planes
+// also keeps y-fastest copies of kaprho, B and eps, and stores I_r y-fastest, for the x-march rays, whose planes have no x extent: every access
+// of theirs is a 32-byte sector for 4 or 8 bytes, and these three arrays are 7 of their 13 strided accesses per node
+// (288^3: one band 63 -> 57 ms, four bands in one call 276 -> 206 ms; on small planes, which are latency-bound, the
+// extra index arithmetic costs more than the sectors: 144^3 18.1 -> 19.7 ms, hence not there).
 template <int MINB>
 __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams p)
 {
+    constexpr bool UT = (MINB == 3);     // the build for large planes reads y-fastest copies of the inputs on x-march rays
     const int nx = p.nx, ny = p.ny, nz = p.nz, nb = p.nb;
     const size_t N = (size_t)nx * ny * nz, NB = N * nb;
     const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, gsz = (size_t)gridDim.x * blockDim.x;
@@ -93,14 +100,17 @@ __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams
         const size_t b = e / N, n = e - b * N;
         const double bv = (double)p.B[e];
         const int k = (int)(n / ((size_t)nx * ny));
+        const int jj = (int)((n / (size_t)nx) % (size_t)ny), ii = (int)(n % (size_t)nx);
+        const size_t nT = ((size_t)k * nx + ii) * ny + jj;       // the node in a y-fastest array
         double j = 0.0;
         for (int r = 0; r < p.nrays; ++r) {
             const ScatRay& q = p.rays[r];
             const double i0 = (k == q.kdir && !q.up) ? 0.0 : bv;
-            p.I[(b * p.nrays + r) * N + n] = i0;
+            p.I[(b * p.nrays + r) * N + ((UT && q.as == 0) ? nT : n)] = i0;
             j += q.wq * i0;
         }
         p.S[e] = bv; p.J[e] = j;
+        if (UT) { p.kapT[b * N + nT] = p.kaprho[e]; p.BT[b * N + nT] = p.B[e]; p.epsT[b * N + nT] = p.eps[e]; }
     }
     if (!scat_grid_sync(p.bar, gen)) return;
 
@@ -114,8 +124,9 @@ __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams
                 const size_t b = e / nface, f = e - b * nface;
                 const double* X = p.I + (b * p.nrays + r) * N;
                 const int k = (int)(f / (size_t)(ny + nx)), t = (int)(f - (size_t)k * (ny + nx));
-                if (t < ny) p.faceX[b * fxs + (size_t)k * ny + t] = X[((size_t)k * ny + t) * nx + q.iface];
-                else p.faceY[b * fys + (size_t)k * nx + (t - ny)] = X[((size_t)k * ny + q.jface) * nx + (t - ny)];
+                const bool xt = UT && (q.as == 0);               // this ray's intensity is stored y-fastest
+                if (t < ny) p.faceX[b * fxs + (size_t)k * ny + t] = X[xt ? ((size_t)k * nx + q.iface) * ny + t : ((size_t)k * ny + t) * nx + q.iface];
+                else p.faceY[b * fys + (size_t)k * nx + (t - ny)] = X[xt ? ((size_t)k * nx + (t - ny)) * ny + q.jface : ((size_t)k * ny + q.jface) * nx + (t - ny)];
             }
             if (!scat_grid_sync(p.bar, gen)) return;
             const int as = q.as, ua = (as == 0) ? 1 : 0, va = (as == 2) ? 1 : 2;
@@ -127,13 +138,18 @@ __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams
                     const size_t b = e / npl, ep = e - b * npl;
                     double* const X = p.I + (b * p.nrays + r) * N;
                     const double* const Sb = p.S + b * N;
-                    const float* const kb = p.kaprho + b * N;
+                    // coefficient arrays: the y-fastest copies for an x-march ray
+                    const bool xm = UT && (as == 0);
+                    const float* const kb = (xm ? p.kapT : p.kaprho) + b * N;
+                    const float* const eb = (xm ? p.epsT : p.eps) + b * N;
+                    const float* const Bb = (xm ? p.BT : p.B) + b * N;
                     const double* const fX = p.faceX + b * fxs;
                     const double* const fY = p.faceY + b * fys;
                     int idx[3];
                     idx[as] = pl; idx[va] = (int)(ep / n_u); idx[ua] = (int)(ep - (size_t)idx[va] * n_u);
                     const int i = idx[0], j = idx[1], k = idx[2];
                     const size_t n = ((size_t)k * ny + j) * nx + i;
+                    const size_t nc = xm ? ((size_t)k * nx + i) * ny + j : n;       // the node in the coefficient arrays and in I_r
                     const double Sn = Sb[n];
                     double Inew;
                     if (k == q.kdir) Inew = q.up ? Sn : 0.0;
@@ -147,24 +163,25 @@ __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams
                             if (iu < 0) { iu += nx; wx = true; } else if (iu >= nx) { iu -= nx; wx = true; }
                             if (ju < 0) { ju += ny; wy = true; } else if (ju >= ny) { ju -= ny; wy = true; }
                             const size_t m = ((size_t)kq * ny + ju) * nx + iu;
-                            const double xv = wx ? fX[(size_t)kq * ny + ju] : (wy ? fY[(size_t)kq * nx + iu] : X[m]);
+                            const size_t mc = xm ? ((size_t)kq * nx + iu) * ny + ju : m;   // in the coefficient arrays and in I_r
+                            const double xv = wx ? fX[(size_t)kq * ny + ju] : (wy ? fY[(size_t)kq * nx + iu] : X[mc]);
                             Xu += q.w[t] * xv;
-                            ku += q.w[t] * (double)kb[m];
+                            ku += q.w[t] * (double)kb[mc];
                             Su += q.w[t] * Sb[m];
                         }
-                        const double dtau = 0.5 * (ku + (double)kb[n]) * q.ds;
+                        const double dtau = 0.5 * (ku + (double)kb[nc]) * q.ds;
                         double E, pu, pp;
                         scat_psi(dtau, E, pu, pp);
                         Inew = Xu * E + pu * Su + pp * Sn;
                     }
                     if (p.gs) {
                         const size_t g = b * N + n;
-                        const double jn = p.J[g] + q.wq * (Inew - X[n]);
-                        const double ep_ = (double)p.eps[g];
+                        const double jn = p.J[g] + q.wq * (Inew - X[nc]);
+                        const double ep_ = (double)eb[nc];
                         p.J[g] = jn;
-                        p.S[g] = (1.0 - ep_) * jn + ep_ * (double)p.B[g];
+                        p.S[g] = (1.0 - ep_) * jn + ep_ * (double)Bb[nc];
                     }
-                    X[n] = Inew;
+                    X[nc] = Inew;
                 }
                 if (!scat_grid_sync(p.bar, gen)) return;
             }
@@ -172,8 +189,10 @@ __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams
         if (!p.gs) {
             for (size_t e = gtid; e < NB; e += gsz) {
                 const size_t b = e / N, n = e - b * N;
+                const int kk = (int)(n / ((size_t)nx * ny)), jj = (int)((n / (size_t)nx) % (size_t)ny), ii = (int)(n % (size_t)nx);
+                const size_t nT = ((size_t)kk * nx + ii) * ny + jj;
                 double a = 0.0;
-                for (int r = 0; r < p.nrays; ++r) a += p.rays[r].wq * p.I[(b * p.nrays + r) * N + n];
+                for (int r = 0; r < p.nrays; ++r) a += p.rays[r].wq * p.I[(b * p.nrays + r) * N + ((UT && p.rays[r].as == 0) ? nT : n)];
                 const double ep_ = (double)p.eps[e];
                 p.J[e] = a;
                 p.S[e] = (1.0 - ep_) * a + ep_ * (double)p.B[e];

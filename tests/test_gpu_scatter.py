@@ -30,6 +30,8 @@ def _case(cfg, grid, band, eps_lo):
     (3, (37, 41, 30), 2, 4, True),      # ragged widths, a thick band
     (5, (30, 34, 61), 1, 3, True),
     (2, (5, 3, 2), 0, 5, True),         # two levels: every node is a Dirichlet node for half of the rays
+    (3, (288, 280, 5), 1, 3, True),     # planes beyond 2 x 256 threads per SM: the kernel build with y-fastest copies for
+    (3, (288, 280, 5), 3, 2, False),    # the x-march rays (rts_scatter.cuh), Gauss-Seidel and Jacobi
 ])
 def test_scatter_against_oracle(cfg, grid, band, niter, gs):
     import oracle
@@ -104,6 +106,28 @@ def test_scatter_with_other_ray_sets(rays):
     assert np.abs(S.cpu().numpy() - So).max() <= TOL * np.abs(So).max()
     assert np.abs(J.cpu().numpy() - Jo).max() <= TOL * np.abs(Jo).max()
     assert np.allclose(change, cho, rtol=1e-6, atol=1e-14)
+
+
+def test_many_bands_on_the_large_plane_build():
+    """12 bands x 80 x 80 nodes per plane step select the kernel build for large planes; every band against the oracle."""
+    import oracle
+    import torch
+    from paper_2107_08145_b200 import rts
+    inp = inputs.make_config(4, grid=(80, 80, 6))
+    s = rts.from_inputs(inp)
+    rho, T, P = (torch.from_numpy(a).cuda() for a in (inp.rho, inp.T, inp.P))
+    k, B = s.coefficients(rho, T, P)
+    rng = np.random.default_rng(11)
+    eps = torch.from_numpy((0.05 + 0.95 * rng.random((inp.nbands,) + inp.shape)).astype(np.float32)).cuda()
+    S, J, change = s.scatter_solve(k, B, eps, 3)
+    s.sync_check(); s.close()
+    for b in range(0, inp.nbands, 5):
+        So, Jo, cho = oracle.scatter_solve(inp.nx, inp.ny, inp.nz, inp.dx, inp.dy, inp.dz, inp.mu, inp.wq,
+                                           k[b].cpu().numpy().astype(np.float64), B[b].cpu().numpy().astype(np.float64),
+                                           eps[b].cpu().numpy().astype(np.float64), 3, gs=True)
+        assert np.abs(S[b].cpu().numpy() - So).max() <= TOL * np.abs(So).max()
+        assert np.abs(J[b].cpu().numpy() - Jo).max() <= TOL * np.abs(Jo).max()
+        assert np.allclose([c[b] for c in change], cho, rtol=1e-6, atol=1e-14)
 
 
 def test_eps_one_is_the_lte_source_and_zero_iterations_return_the_start():
