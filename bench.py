@@ -351,7 +351,7 @@ def main():
         scat = {"ms_per_iteration": t_it, "node_band_ray_updates_per_s": inp.ncells * inp.nbands * inp.nrays / (t_it * 1e-3),
                 "dtype": "f64", "bands": inp.nbands, "rays": inp.nrays, "eps": 0.1,
                 "scheme": "source update along the ray (Gauss-Seidel)", "last_change_per_band": change[-1],
-                "note": "one grid-wide barrier per plane of every ray; small grids are bound by it, 288^3 by the L2 sector traffic of the strided x-march planes"}
+                "note": "one grid-wide barrier per plane of every ray; small grids are bound by it and by the dependent loads of a plane step, 288^3 by the strided accesses that are left on the x-march rays (S and J) and by three nodes per thread with four bands (DESIGN.md 7.5)"}
         del kap, Bsrc, eps
 
     cpu = None
