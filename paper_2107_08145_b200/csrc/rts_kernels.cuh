@@ -491,17 +491,31 @@ __global__ void __launch_bounds__(256) rts_cells_to_nodes_kernel(const StaggerPa
     for (int f = 0; f < p.nf; ++f) {
         const float* __restrict__ c = p.cell[f];
         float* __restrict__ n = p.node[f];
-        auto hsum = [&](int kc) {
-            const float* q = c + (size_t)kc * plane;
-            return ((double)__ldg(q + r0 + i) + (double)__ldg(q + r0 + im)) + ((double)__ldg(q + r1 + i) + (double)__ldg(q + r1 + im));
+        // the four cells of a level around the corner column, as loaded (level clamped into the cell grid: the corner
+        // levels below / above the box repeat the edge cell level, so k = 0 and k = nz - 1 get the same sum twice)
+        auto hload = [&](int kc, float (&v)[4]) {
+            const float* q = c + (size_t)min(max(kc, 0), ncz - 1) * plane;
+            v[0] = __ldg(q + r0 + i); v[1] = __ldg(q + r0 + im); v[2] = __ldg(q + r1 + i); v[3] = __ldg(q + r1 + im);
         };
-        double below = hsum(min(max(k0 - 1, 0), ncz - 1));
-#pragma unroll 4
-        for (int k = k0; k < k1; ++k) {
-            const double above = (k <= ncz - 1) ? hsum(k) : below;   // top corner level: edge cells again
-            if (k == 0) below = above;                               // bottom corner level
-            n[(size_t)k * plane + r0 + i] = (float)((below + above) * 0.125);
-            below = above;
+        auto hsum = [](const float (&v)[4]) { return ((double)v[0] + (double)v[1]) + ((double)v[2] + (double)v[3]); };
+        float v0[4];
+        hload(k0 - 1, v0);
+        double below = hsum(v0);
+        // LB levels per turn: all their loads are issued before the first store (the compiler does not move loads
+        // across the stores of an unrolled loop by itself, and one level at a time is a chain of memory latencies)
+        constexpr int LB = 4;
+        for (int k = k0; k < k1; k += LB) {
+            float v[LB][4];
+#pragma unroll
+            for (int u = 0; u < LB; ++u) hload(k + u, v[u]);
+#pragma unroll
+            for (int u = 0; u < LB; ++u) {
+                if (k + u < k1) {
+                    const double above = hsum(v[u]);
+                    n[(size_t)(k + u) * plane + r0 + i] = (float)((below + above) * 0.125);
+                    below = above;
+                }
+            }
         }
     }
 }
