@@ -150,11 +150,17 @@ __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams
                     const int i = idx[0], j = idx[1], k = idx[2];
                     const size_t n = ((size_t)k * ny + j) * nx + i;
                     const size_t nc = xm ? ((size_t)k * nx + i) * ny + j : n;       // the node in the coefficient arrays and in I_r
+                    // every load of the node is issued before the first use: the plane step is a chain of memory latencies,
+                    // and a branch around a load (seam ghost or not; Gauss-Seidel or not) would put it behind the others
+                    const size_t g = b * N + n;
                     const double Sn = Sb[n];
+                    const double Xold = X[nc], Jold = p.J[g];
+                    const float kn = kb[nc], epn = eb[nc], Bn = Bb[nc];
                     double Inew;
                     if (k == q.kdir) Inew = q.up ? Sn : 0.0;
                     else {
-                        double Xu = 0.0, ku = 0.0, Su = 0.0;
+                        double xv[4], sv[4];
+                        float kv[4];
 #pragma unroll
                         for (int t = 0; t < 4; ++t) {
                             int iu = i + q.off[t][0], ju = j + q.off[t][1];
@@ -164,22 +170,23 @@ __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams
                             if (ju < 0) { ju += ny; wy = true; } else if (ju >= ny) { ju -= ny; wy = true; }
                             const size_t m = ((size_t)kq * ny + ju) * nx + iu;
                             const size_t mc = xm ? ((size_t)kq * nx + iu) * ny + ju : m;   // in the coefficient arrays and in I_r
-                            const double xv = wx ? fX[(size_t)kq * ny + ju] : (wy ? fY[(size_t)kq * nx + iu] : X[mc]);
-                            Xu += q.w[t] * xv;
-                            ku += q.w[t] * (double)kb[mc];
-                            Su += q.w[t] * Sb[m];
+                            // a stencil node beyond a periodic seam comes from the face of the previous iteration
+                            const double* const src = wx ? fX + ((size_t)kq * ny + ju) : (wy ? fY + ((size_t)kq * nx + iu) : X + mc);
+                            xv[t] = *src; kv[t] = kb[mc]; sv[t] = Sb[m];
                         }
-                        const double dtau = 0.5 * (ku + (double)kb[nc]) * q.ds;
+                        double Xu = 0.0, ku = 0.0, Su = 0.0;
+#pragma unroll
+                        for (int t = 0; t < 4; ++t) { Xu += q.w[t] * xv[t]; ku += q.w[t] * (double)kv[t]; Su += q.w[t] * sv[t]; }
+                        const double dtau = 0.5 * (ku + (double)kn) * q.ds;
                         double E, pu, pp;
                         scat_psi(dtau, E, pu, pp);
                         Inew = Xu * E + pu * Su + pp * Sn;
                     }
                     if (p.gs) {
-                        const size_t g = b * N + n;
-                        const double jn = p.J[g] + q.wq * (Inew - X[nc]);
-                        const double ep_ = (double)eb[nc];
+                        const double jn = Jold + q.wq * (Inew - Xold);
+                        const double ep_ = (double)epn;
                         p.J[g] = jn;
-                        p.S[g] = (1.0 - ep_) * jn + ep_ * (double)Bb[nc];
+                        p.S[g] = (1.0 - ep_) * jn + ep_ * (double)Bn;
                     }
                     X[nc] = Inew;
                 }
