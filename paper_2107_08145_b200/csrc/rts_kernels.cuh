@@ -531,16 +531,23 @@ __global__ void __launch_bounds__(256) rts_nodes_to_cells_kernel(const float* __
     const int ip = (i == nx - 1) ? 0 : i + 1, jp = (j == ny - 1) ? 0 : j + 1;
     const size_t r0 = (size_t)j * nx, r1 = (size_t)jp * nx, plane = (size_t)nx * ny;
     auto hsum = [&](int k) {
-        const float* q = qn + (size_t)k * plane;
+        const float* q = qn + (size_t)min(k, nz - 1) * plane;
         return (__ldg(q + r0 + i) + __ldg(q + r0 + ip)) + (__ldg(q + r1 + i) + __ldg(q + r1 + ip));
     };
     if (k0 >= k1) return;
     float below = hsum(k0);
-#pragma unroll 4
-    for (int k = k0; k < k1; ++k) {
-        const float above = hsum(k + 1);
-        qc[(size_t)k * plane + r0 + i] = 0.125f * (below + above);
-        below = above;
+    constexpr int LB = 4;                // levels whose loads are issued before the first store (see cells -> nodes)
+    for (int k = k0; k < k1; k += LB) {
+        float above[LB];
+#pragma unroll
+        for (int u = 0; u < LB; ++u) above[u] = hsum(k + u + 1);
+#pragma unroll
+        for (int u = 0; u < LB; ++u) {
+            if (k + u < k1) {
+                qc[(size_t)(k + u) * plane + r0 + i] = 0.125f * (below + above[u]);
+                below = above[u];
+            }
+        }
     }
 }
 
