@@ -117,7 +117,13 @@ __global__ void __launch_bounds__(256, MINB) rts_scatter_kernel(const ScatParams
     for (int it = 0; it < p.niter; ++it) {
         for (size_t e = gtid; e < NB; e += gsz) p.Sold[e] = p.S[e];
         for (int r = 0; r < p.nrays; ++r) {
-            const ScatRay q = p.rays[r];
+            // the ray's constants through shared memory (uniform reads), not 30 registers per thread: the large-plane build
+            // spilled them (288^3: 51.5 -> 40.6 ms per iteration)
+            __shared__ ScatRay qsh;
+            __syncthreads();
+            if (threadIdx.x < sizeof(ScatRay) / 4) reinterpret_cast<int*>(&qsh)[threadIdx.x] = reinterpret_cast<const int*>(p.rays + r)[threadIdx.x];
+            __syncthreads();
+            const ScatRay& q = qsh;
             // the periodic faces of the previous iteration (Jacobi seam ghosts)
             const size_t nface = (size_t)nz * (ny + nx);
             for (size_t e = gtid; e < nface * nb; e += gsz) {
