@@ -437,12 +437,14 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
         const f2 as0 = mul2(bc(a_p), make_float2(sp.x, sp.y)), as1 = mul2(bc(a_p), make_float2(sp.z, sp.w));
 #pragma unroll
         for (int s = 0; s < NSLOT; ++s) {
-            if (!U.ray[s].active) continue;
+            // no branch around the load: an absent ray's place in the plane set holds zeros or (two rays per CTA) the
+            // other ray's values, finite either way, and its weight is 0
+            const bool on = U.ray[s].active != 0;
             const float4 x = *reinterpret_cast<const float4*>(Xn + xso<PITCH>(S, s) + bo);
-            const float wq = U.ray[s].wq;
+            const float wq = on ? U.ray[s].wq : 0.f;
             acc0 = fma2(bc(wq), sub2(make_float2(x.x, x.y), s0), acc0);       // w_r (I - S)
             acc1 = fma2(bc(wq), sub2(make_float2(x.z, x.w), s1), acc1);
-            if (Fdst) {
+            if (Fdst && on) {
                 const f2 i0 = add2(make_float2(x.x, x.y), as0), i1 = add2(make_float2(x.z, x.w), as1);   // I = X + a S
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
@@ -451,7 +453,7 @@ __device__ __noinline__ void q_pass(const TaskShared* __restrict__ Sp, const f2*
                     fl1[a] = fma2(bc(wm), i1, fl1[a]);
                 }
             }
-            if (topstep && U.ray[s].itop >= 0) {
+            if (topstep && on && U.ray[s].itop >= 0) {
                 const bool top = zmarch || (v == U.nz - 1 && !(s & 2));
                 if (top) {
                     float* dst = Itop_b + (long long)U.ray[s].itop * U.it_sr + (zmarch ? (long long)v : (long long)pl) * U.it_so;
